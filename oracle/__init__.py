@@ -1,0 +1,218 @@
+"""numpy front-end of the CPU oracle (oracle/mq_oracle.cpp).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs.  It imports nothing from
+paper_2606_15652_b200 and that package imports nothing from here.
+
+Function names follow the O-steps of the .cpp header (PAPER.md citations there).
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+from typing import Optional, Tuple
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_select.restype = C.c_int64
+        _lib.orc_gemm.restype = C.c_int
+        _lib.orc_forward.restype = C.c_int
+    return _lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def quantize_row(x: np.ndarray) -> Tuple[np.ndarray, np.float32]:
+    """O1 (Eq.1)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    q = np.empty(x.shape[0], dtype=np.int8)
+    s = np.empty(1, dtype=np.float32)
+    lib().orc_quantize_row(_p(x), C.c_int64(x.shape[0]), _p(q), _p(s))
+    return q, s[0]
+
+
+def _bits16(A) -> Tuple[np.ndarray, int]:
+    """fp16 numpy array, or (uint16 bf16 bits, 'bf16') tuple -> (uint16 bits, dtype code)."""
+    if isinstance(A, tuple):
+        bits, kind = A
+        assert kind == "bf16" and bits.dtype == np.uint16
+        return np.ascontiguousarray(bits), 1
+    assert A.dtype == np.float16
+    return np.ascontiguousarray(A).view(np.uint16), 0
+
+
+def quantize_act(A) -> Tuple[np.ndarray, np.ndarray]:
+    """O2: per-token int4 quantization of fp16 (np.float16) or bf16 ((bits,'bf16')) activations."""
+    bits, code = _bits16(A)
+    M, K = bits.shape
+    qa = np.empty((M, K), dtype=np.int8)
+    sa = np.empty(M, dtype=np.float32)
+    lib().orc_quantize_act(_p(bits), C.c_int(code), C.c_int64(M), C.c_int64(K), C.c_int64(K), _p(qa), _p(sa))
+    return qa, sa
+
+
+@dataclass
+class Decomp:
+    qw: np.ndarray  # int8 [N,K]
+    sw: np.ndarray  # fp32 [N]
+    R: np.ndarray   # fp32 [N,K]
+    qr: np.ndarray  # int8 [N,K]  (whole matrix, before selection)
+    sr: np.ndarray  # fp32 [N]
+
+
+def decompose(W: np.ndarray) -> Decomp:
+    """O3 + O4 (Alg.1 line 1; Eq.4)."""
+    W = np.ascontiguousarray(W, dtype=np.float32)
+    N, K = W.shape
+    d = Decomp(np.empty((N, K), np.int8), np.empty(N, np.float32), np.empty((N, K), np.float32),
+               np.empty((N, K), np.int8), np.empty(N, np.float32))
+    lib().orc_decompose(_p(W), C.c_int64(N), C.c_int64(K), _p(d.qw), _p(d.sw), _p(d.R), _p(d.qr), _p(d.sr))
+    return d
+
+
+def hessian_diag(X: np.ndarray) -> np.ndarray:
+    """O5: binary64 h[K]."""
+    X = np.ascontiguousarray(X, dtype=np.float32)
+    h = np.empty(X.shape[1], dtype=np.float64)
+    lib().orc_hessian_diag(_p(X), C.c_int64(X.shape[0]), C.c_int64(X.shape[1]), _p(h))
+    return h
+
+
+@dataclass
+class Scores:
+    A_B: np.ndarray
+    B_B: np.ndarray
+    delta: np.ndarray
+    S: np.ndarray
+
+
+def scores(d: Decomp, h: np.ndarray, bs: int) -> Scores:
+    """O6: h is taken as fp32 (the ABI's h_host type) and promoted."""
+    h32 = np.ascontiguousarray(h, dtype=np.float32)
+    N, K = d.R.shape
+    nb = (N // bs) * (K // bs)
+    s = Scores(*(np.empty(nb, np.float64) for _ in range(4)))
+    lib().orc_scores(_p(d.R), _p(d.qr), _p(d.sr), _p(h32), C.c_int64(N), C.c_int64(K), C.c_int64(bs),
+                     _p(s.A_B), _p(s.B_B), _p(s.delta), _p(s.S))
+    return s
+
+
+def select(S: np.ndarray, budget: int) -> np.ndarray:
+    """O7: selected linear block indices, score descending."""
+    S = np.ascontiguousarray(S, dtype=np.float64)
+    sel = np.empty(max(1, min(int(budget), S.shape[0])), dtype=np.int64)
+    nnz = lib().orc_select(_p(S), C.c_int64(S.shape[0]), C.c_int64(int(budget)), _p(sel))
+    return sel[:nnz].copy()
+
+
+def gemm(qa: np.ndarray, qw: np.ndarray, qr: np.ndarray, bs: int, blk_n: np.ndarray, blk_k: np.ndarray):
+    """O8 (Eq.2, Eq.4): int64 acc0, acc1."""
+    qa = np.ascontiguousarray(qa, np.int8)
+    qw = np.ascontiguousarray(qw, np.int8)
+    qr = np.ascontiguousarray(qr, np.int8)
+    bn = np.ascontiguousarray(blk_n, np.int32)
+    bk = np.ascontiguousarray(blk_k, np.int32)
+    M, K = qa.shape
+    N = qw.shape[0]
+    acc0 = np.empty((M, N), np.int64)
+    acc1 = np.empty((M, N), np.int64)
+    rc = lib().orc_gemm(_p(qa), C.c_int64(M), C.c_int64(K), _p(qw), C.c_int64(N), _p(qr), C.c_int64(bs),
+                        C.c_int64(bn.shape[0]), _p(bn), _p(bk), _p(acc0), _p(acc1))
+    if rc != 0:
+        raise OverflowError("accumulator exceeds int32 range")
+    return acc0, acc1
+
+
+def output(acc0, acc1, sa, sw, sr, want_mag: bool = False):
+    """O9: binary64 Y_exact (and the parity rule's magnitude term)."""
+    M, N = acc0.shape
+    Y = np.empty((M, N), np.float64)
+    mag = np.empty((M, N), np.float64) if want_mag else None
+    lib().orc_output(_p(np.ascontiguousarray(acc0, np.int64)), _p(np.ascontiguousarray(acc1, np.int64)),
+                     _p(np.ascontiguousarray(sa, np.float32)), _p(np.ascontiguousarray(sw, np.float32)),
+                     _p(np.ascontiguousarray(sr, np.float32)), C.c_int64(M), C.c_int64(N), _p(Y),
+                     _p(mag) if want_mag else None)
+    return (Y, mag) if want_mag else Y
+
+
+@dataclass
+class PackedLayer:
+    """Algorithm 1's outputs for one layer: everything mq_pack_prequantized needs."""
+    N: int
+    K: int
+    bs: int
+    d: Decomp
+    sc: Optional[Scores]
+    blk_n: np.ndarray  # int32 [nnz]
+    blk_k: np.ndarray  # int32 [nnz]
+
+    @property
+    def nnz(self) -> int:
+        return int(self.blk_n.shape[0])
+
+    def qr_blocks(self) -> np.ndarray:
+        """Q(R) gathered on the selected blocks: int8 [nnz, bs, bs] (row = n, col = k)."""
+        out = np.empty((self.nnz, self.bs, self.bs), np.int8)
+        for e in range(self.nnz):
+            n0, k0 = int(self.blk_n[e]) * self.bs, int(self.blk_k[e]) * self.bs
+            out[e] = self.d.qr[n0:n0 + self.bs, k0:k0 + self.bs]
+        return out
+
+
+def algorithm1(W: np.ndarray, h: Optional[np.ndarray], bs: int, budget: int) -> PackedLayer:
+    """Algorithm 1: O3, O4, O6, O7 in order.  h None = all ones."""
+    N, K = W.shape
+    d = decompose(W)
+    if h is None:
+        h = np.ones(K, np.float32)
+    sc = scores(d, h, bs)
+    sel = select(sc.S, budget)
+    nbk = K // bs
+    return PackedLayer(N, K, bs, d, sc, (sel // nbk).astype(np.int32), (sel % nbk).astype(np.int32))
+
+
+def forward(A, L: PackedLayer):
+    """O2 + O8 + O9 for one layer; returns dict with qa, sa, acc0, acc1, Y, mag."""
+    qa, sa = quantize_act(A)
+    acc0, acc1 = gemm(qa, L.d.qw, L.d.qr, L.bs, L.blk_n, L.blk_k)
+    Y, mag = output(acc0, acc1, sa, L.d.sw, L.d.sr, want_mag=True)
+    return dict(qa=qa, sa=sa, acc0=acc0, acc1=acc1, Y=Y, mag=mag)
+
+
+def forward_timed(A, L: PackedLayer) -> np.ndarray:
+    """The same three steps through one C call (no Python between them) -- what bench.py times."""
+    bits, code = _bits16(A)
+    M, K = bits.shape
+    Y = np.empty((M, L.N), np.float64)
+    lib().orc_forward(_p(bits), C.c_int(code), C.c_int64(M), C.c_int64(K), _p(L.d.qw), _p(L.d.sw), C.c_int64(L.N),
+                      _p(L.d.qr), _p(L.d.sr), C.c_int64(L.bs), C.c_int64(L.nnz), _p(L.blk_n), _p(L.blk_k), _p(Y))
+    return Y
+
+
+def round_to_bf16(Y: np.ndarray) -> np.ndarray:
+    """RNE binary64 -> bf16, returned as float64 values (Y_ref of O9).  Double rounding via
+    fp32 is avoided: round the binary64 value directly to 8 significant bits."""
+    Y = np.asarray(Y, np.float64)
+    out = np.zeros_like(Y)
+    nz = Y != 0
+    m, e = np.frexp(Y[nz])          # Y = m * 2^e, 0.5 <= |m| < 1
+    scaled = m * 256.0              # 8 significant bits
+    r = np.rint(scaled)             # RNE
+    out[nz] = np.ldexp(r, e - 8)
+    return out
