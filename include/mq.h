@@ -1,0 +1,148 @@
+/* mq.h -- C ABI of libmq.so: the B200 (sm_100a) hot path of MosaicQuant / ZipperEngine.
+ *
+ * What the library computes (citations are lines of the paper text, "P:<line>" =
+ * /root/reference/PAPER.md, and readings "A<n>" of DESIGN.md section 3):
+ *
+ *   Y = A * W^T for one bias-free linear layer, with
+ *     A  [M,K]  activations, quantized per token to int4      (Eq.1; A5)
+ *     W  [N,K]  weights = dense int4 base  Q(W)  per output channel (A9)
+ *               + sparse int4 residual Q(R), R = W - Q(W), kept only on the top-K
+ *                 blocks of the Delta-Hessian score          (Eq.4; Alg.1)
+ *     Y[m,n] = s_a[m] * ( s_w[n] * acc0[m,n] + s_r[n] * acc1[m,n] )      (Eq.2; Eq.4)
+ *     acc0 = sum_k q_a[m,k] q_w[n,k]                (dense 4-bit component)
+ *     acc1 = sum over selected blocks containing n of sum_{k in block} q_a[m,k] q_r[n,k]
+ *   with the residual blocks' MMAs issued inside the dense K-loop of ONE kernel
+ *   (ZipperEngine, section 4.2, Fig.3).
+ *
+ * Conventions: every function returns an mq_status (0 = MQ_OK, negative = error);
+ * nothing throws, aborts or prints.  "_dev" pointers are CUDA device pointers, "_host"
+ * pointers are host pointers.  All device work is enqueued on `cuda_stream` (a
+ * cudaStream_t passed as void*; NULL = the legacy default stream) and the online calls
+ * (mq_quantize_act, mq_gemm, mq_linear) neither allocate nor synchronise with the host.
+ * The caller owns every buffer it passes in; the library owns only what an
+ * mq_weights* refers to.  There is no CPU fallback: on a machine without a
+ * compute-capability-10.0 device the compute calls return MQ_ERR_UNSUPPORTED_DEVICE.
+ */
+#ifndef MQ_H_
+#define MQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  MQ_OK = 0,
+  MQ_ERR_INVALID_ARG = -1,        /* NULL pointer, bad enum, misaligned pointer, bad block list */
+  MQ_ERR_UNSUPPORTED_SHAPE = -2,  /* N % 128, K % 128, block not in {64,128}, M < 0 ...        */
+  MQ_ERR_UNSUPPORTED_DEVICE = -3, /* current device is not compute capability 10.0             */
+  MQ_ERR_CUDA = -4,               /* a CUDA runtime / driver call failed                       */
+  MQ_ERR_OOM = -5,                /* host or device allocation failed                          */
+  MQ_ERR_ACC_OVERFLOW = -6,       /* K so large that the int32 accumulator could overflow      */
+  MQ_ERR_WORKSPACE = -7           /* workspace smaller than mq_gemm_workspace_bytes()          */
+} mq_status;
+
+typedef enum { MQ_F16 = 0, MQ_BF16 = 1 } mq_dtype;
+
+/* Opaque packed layer: immutable after packing, safe to share between streams. */
+typedef struct mq_weights mq_weights;
+
+/* Static string for a status code; never NULL, never freed. */
+const char* mq_status_string(int status);
+
+/* ------------------------------------------------------------------------------------
+ * (1) Activation quantization -- Eq.1, per token (A5), q_max = 7 (A1).
+ *
+ * Row m of A (fp16 or bf16, `lda_elems` elements between rows, 16-byte aligned rows) is
+ * converted exactly to fp32; amax = max|a|; s = amax / 7 (one IEEE binary32 division);
+ * q_k = clamp(rint(a_k / s), -7, 7) with an IEEE binary32 division and round-half-even
+ * (A3); an all-zero row gives s = 1, q = 0 (A2).
+ *
+ * Output layout (canonical, part of the ABI):
+ *   qA_dev : uint8 [M, K/2] row-major, row stride K/2 bytes; byte i of row m holds
+ *            element 2i in bits 0-3 and element 2i+1 in bits 4-7, two's-complement
+ *            nibbles.  mq_qact_bytes(M,K) = M*K/2.  Must be 16-byte aligned.
+ *   sA_dev : float [M].
+ * Requires K % 128 == 0, M >= 0 (M == 0 is a no-op).
+ */
+size_t mq_qact_bytes(int64_t M, int64_t K);
+int mq_quantize_act(const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda_elems,
+                    void* qA_dev, float* sA_dev, void* cuda_stream);
+/* Test aid: expands qA to one int8 per element, q_dev [M,K] row-major. */
+int mq_unpack_act(const void* qA_dev, int64_t M, int64_t K, int8_t* q_dev, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
+ * (2) Weight packing -- Algorithm 1 on the host, then the device layout.
+ *
+ * mq_pack_weights: W_host [N,K] fp32 row-major ([out,in], A9).  Steps, in the paper's
+ * order: base quantize per output channel (Eq.1); R = W - s_w q_w (Alg.1 line 1);
+ * Q(R) per output channel over all K, before selection (A4); Delta-Hessian score
+ * S_B = [sum_B h_k R^2 - sum_B h_k (R - Q(R))^2]_+  over aligned block x block
+ * blocks (A8), h_host [K] fp32 or NULL = all ones; global top-`budget_blocks` by score,
+ * ties to the lower linear block index bn*(K/block)+bk, zero-score blocks never selected
+ * (A6, A7).  The result is uploaded in the kernel's tiled layout (DESIGN.md
+ * section 5).  Host inputs are copied; they may be freed on return.  The call
+ * synchronises `cuda_stream` before returning.
+ *
+ * mq_pack_prequantized: layout only; the caller supplies the decomposition.
+ *   qW [N,K] int8 in [-7,7]; sW [N]; nnz selected blocks with coordinates
+ *   (blk_n[e], blk_k[e]) in units of `block`, no duplicates; qR [nnz][block][block]
+ *   int8 in [-7,7] (row = n, col = k); sR [N] (A4: per output channel).
+ *
+ * Requires N % 128 == 0, K % 128 == 0, block in {64,128}, 49*256*K < 2^31.
+ */
+int mq_pack_weights(const float* W_host, int64_t N, int64_t K, const float* h_host, int block,
+                    int64_t budget_blocks, mq_weights** out, void* cuda_stream);
+int mq_pack_prequantized(const int8_t* qW_host, const float* sW_host, int64_t N, int64_t K, int block,
+                         int64_t nnz, const int32_t* blk_n_host, const int32_t* blk_k_host,
+                         const int8_t* qR_host, const float* sR_host, mq_weights** out,
+                         void* cuda_stream);
+/* Reads the device layout back and returns the canonical arrays (any pointer may be
+ * NULL = skipped).  Blocks are returned sorted by (blk_n, blk_k).  Host call; syncs. */
+int mq_weights_export(const mq_weights* w, int8_t* qW_host, float* sW_host, int64_t* nnz,
+                      int32_t* blk_n_host, int32_t* blk_k_host, int8_t* qR_host, float* sR_host);
+int mq_weights_info(const mq_weights* w, int64_t* N, int64_t* K, int* block, int64_t* nnz,
+                    size_t* device_bytes);
+void mq_weights_free(mq_weights* w);
+
+/* ------------------------------------------------------------------------------------
+ * (3) Fused base + residual GEMM -- ZipperEngine (Eq.4).
+ *
+ *   qA_dev, sA_dev : output of mq_quantize_act for the same M and this layer's K
+ *                    (row stride K/2 bytes).
+ *   Y_dev          : [M,N] fp16/bf16 row-major, `ldy_elems` elements between rows.
+ *   dbg_acc_base_dev / dbg_acc_res_dev : optional int32 [M,N] row-major (stride N); when
+ *                    non-NULL they receive acc0 / acc1 exactly (parity hooks).
+ *   workspace_dev  : at least mq_gemm_workspace_bytes(w, M) bytes, 16-byte aligned; must be
+ *                    all-zero before the FIRST call that uses it; every call leaves it
+ *                    all-zero again (split-K partial sums and tile counters).  Calls that
+ *                    may run concurrently need distinct workspaces.
+ * M == 0 is a no-op.
+ */
+size_t mq_gemm_workspace_bytes(const mq_weights* w, int64_t M);
+int mq_gemm(const mq_weights* w, const void* qA_dev, const float* sA_dev, int64_t M, void* Y_dev,
+            mq_dtype y_dtype, int64_t ldy_elems, int32_t* dbg_acc_base_dev, int32_t* dbg_acc_res_dev,
+            void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Convenience: mq_quantize_act into the head of the workspace followed by mq_gemm on the
+ * same stream.  Workspace: mq_linear_workspace_bytes(w, M), same zero-state contract. */
+size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M);
+int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t lda_elems,
+              void* Y_dev, mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev,
+              size_t workspace_bytes, void* cuda_stream);
+
+/* Tuning / ablation knobs (process-wide, not thread-safe; for benchmarks and tests).
+ *   "split_k"   : 0 = automatic, n >= 1 = force n K-splits
+ *   "token_tile": 0 = automatic, else 16/32/64/128/256
+ *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
+ * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */
+int mq_set_option(const char* name, int64_t value);
+/* Number of kernels the last mq_gemm / mq_linear / mq_quantize_act call launched. */
+int mq_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MQ_H_ */

@@ -1,0 +1,27 @@
+"""paper_2606_15652_b200 -- B200 (sm_100a) hot path of MosaicQuant / ZipperEngine.
+
+The product is the C-ABI library `libmq.so` (include/mq.h, sources in csrc/); this package is
+its thin Python binding with the same entry-point names.  No CPU fallback exists.
+"""
+from .binding import (  # noqa: F401
+    MQ_BF16,
+    MQ_F16,
+    EXPORTS,
+    LIB_PATH,
+    MqError,
+    Weights,
+    lib,
+    mq_gemm,
+    mq_gemm_workspace_bytes,
+    mq_last_launch_count,
+    mq_linear,
+    mq_linear_workspace_bytes,
+    mq_pack_prequantized,
+    mq_pack_weights,
+    mq_qact_bytes,
+    mq_quantize_act,
+    mq_set_option,
+    mq_unpack_act,
+    new_workspace,
+    status_string,
+)

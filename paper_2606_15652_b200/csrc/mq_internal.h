@@ -1,0 +1,77 @@
+// mq_internal.h -- shared declarations of libmq.so's translation units (not installed).
+//
+// Device layout of a packed layer.  BN = 128 output channels per
+// weight tile, BK = 128 input channels per K-step.
+//
+//   base   : uint8 [N/BN][K/BK][BN rows][BK/2 bytes]   one 8 KB tile per (n-tile, K-step),
+//            contiguous, so the kernel fetches it with ONE 1-D bulk copy (TMA).
+//            Inside a row the nibble order is canonical (byte i = elements 2i | 2i+1<<4).
+//   sw, sr : float [N]  base / residual scale per output channel (A4).
+//   residual "cells": one cell per (n-tile, K-step) that holds >= 1 selected block,
+//            CSR over n-tiles (cell_ptr[N/BN + 1]), sorted by K-step inside a tile.
+//            A cell is split into four quarters q = 2*h + r  (h = k-half, r = row-half),
+//            each 64 rows x 64 k = 2 KB packed [64 rows][32 bytes].  Only present quarters
+//            are stored, in ascending q, contiguously (res_data).
+//              block = 64 : a selected block (bn,bk) is quarter (h = bk&1, r = bn&1) of
+//                           cell (bn>>1, bk>>1)
+//              block = 128: a selected block is a whole cell (mask 0xF)
+//   cell_meta : int2 {kstep | mask << 24, first quarter index into res_data (2 KB units)}
+#pragma once
+
+#include <cstddef>
+#include <cstdint>
+#include <vector>
+
+#include "../../include/mq.h"
+
+namespace mq {
+
+constexpr int BN = 128;           // output channels per tile (MMA M)
+constexpr int BK = 128;           // input channels per K-step
+constexpr int TILE_BYTES = BN * BK / 2;   // 8192
+constexpr int QUARTER_BYTES = 64 * 64 / 2;  // 2048
+
+struct CellMeta {
+  int32_t kstep_mask;  // bits 0-23: K-step index; bits 24-27: quarter-present mask
+  int32_t qoff;        // index of the cell's first stored quarter (2 KB units)
+};
+
+}  // namespace mq
+
+struct mq_weights {
+  int64_t N = 0, K = 0;
+  int block = 0;
+  int64_t nnz = 0;         // selected blocks
+  int64_t n_cells = 0;
+  int64_t n_quarters = 0;
+  // device buffers (one allocation, sub-pointers)
+  void* dev_blob = nullptr;
+  size_t dev_bytes = 0;
+  uint8_t* d_base = nullptr;
+  float* d_sw = nullptr;
+  float* d_sr = nullptr;
+  uint8_t* d_res = nullptr;
+  int32_t* d_cell_ptr = nullptr;       // [N/BN + 1]
+  mq::CellMeta* d_cell_meta = nullptr; // [n_cells]
+  // host copies of the small metadata (used by the launcher and by export)
+  std::vector<int32_t> h_cell_ptr;
+  std::vector<mq::CellMeta> h_cell_meta;
+  int max_cells_per_tile = 0;
+};
+
+namespace mq {
+
+// options (mq_set_option)
+struct Options {
+  int64_t split_k = 0;
+  int64_t token_tile = 0;
+  int64_t max_ctas = 0;
+};
+Options& options();
+void set_launch_count(int n);
+void add_launch_count(int n);
+
+int check_device();  // MQ_OK or MQ_ERR_UNSUPPORTED_DEVICE / MQ_ERR_CUDA
+int sm_count();
+
+}  // namespace mq

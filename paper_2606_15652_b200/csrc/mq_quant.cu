@@ -1,0 +1,235 @@
+// mq_quant.cu -- kernel (i): per-token int4 activation quantization (Eq.1; A1-A3, A5)
+// plus the library's small runtime (status strings, options, device check).
+//
+// One CTA per token row.  The row (fp16/bf16) is read once with 128-bit loads and kept in
+// registers (up to 32 elements per thread per pass -> K <= 8192 at 256 threads; longer rows
+// re-read from L2), |max| is reduced with warp shuffles + one shared-memory step, then each
+// thread divides, rounds half-to-even, clamps and packs 8 nibbles per 32-bit word.
+// HBM-bound: 2 B read + 0.5 B written per element.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include <cstring>
+
+#include "mq_internal.h"
+
+namespace mq {
+
+Options& options() {
+  static Options o;
+  return o;
+}
+static int g_launches = 0;
+void set_launch_count(int n) { g_launches = n; }
+void add_launch_count(int n) { g_launches += n; }
+
+static int g_dev_checked = -1;  // device ordinal for which the check passed
+static int g_sms = 0;
+int check_device() {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_UNSUPPORTED_DEVICE;
+  }
+  if (dev == g_dev_checked) return MQ_OK;
+  int major = 0, minor = 0, sms = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  if (major != 10 || minor != 0) return MQ_ERR_UNSUPPORTED_DEVICE;
+  g_dev_checked = dev;
+  g_sms = sms;
+  return MQ_OK;
+}
+int sm_count() { return g_sms; }
+
+}  // namespace mq
+
+namespace {
+
+constexpr int QT = 256;  // threads per row
+
+template <bool BF16>
+__device__ __forceinline__ void cvt8(const uint4& v, float* f) {
+  const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    if (BF16) {
+      f[2 * i] = __uint_as_float(w[i] << 16);
+      f[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+    } else {
+      __half2 h = *reinterpret_cast<const __half2*>(&w[i]);
+      float2 t = __half22float2(h);
+      f[2 * i] = t.x;
+      f[2 * i + 1] = t.y;
+    }
+  }
+}
+
+__device__ __forceinline__ uint32_t quant_pack8(const float* f, float s) {
+  uint32_t out = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    float t = __fdiv_rn(f[i], s);                 // IEEE binary32 division (A3)
+    int q = __float2int_rn(t);                    // round half to even
+    q = max(-7, min(7, q));
+    out |= (uint32_t)(q & 0xF) << (4 * i);
+  }
+  return out;
+}
+
+// CHUNKS = 16-byte chunks (8 elements) each thread keeps in registers per pass.
+template <bool BF16, int CHUNKS>
+__global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __restrict__ A, int64_t lda, int K,
+                                                             uint8_t* __restrict__ qA, float* __restrict__ sA) {
+  const int64_t m = blockIdx.x;
+  const uint4* row = reinterpret_cast<const uint4*>(A + m * lda);
+  uint32_t* qrow = reinterpret_cast<uint32_t*>(qA + m * (int64_t)(K / 2));
+  const int nchunk = K / 8;
+  __shared__ float red[QT / 32];
+
+  uint4 cache[CHUNKS];
+  float amax = 0.f;
+#pragma unroll
+  for (int c = 0; c < CHUNKS; ++c) {
+    int idx = threadIdx.x + c * QT;
+    if (idx < nchunk) {
+      cache[c] = __ldg(row + idx);
+      float f[8];
+      cvt8<BF16>(cache[c], f);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(f[i]));
+    }
+  }
+  for (int idx = threadIdx.x + CHUNKS * QT; idx < nchunk; idx += QT) {  // rows longer than the register cache
+    uint4 v = __ldg(row + idx);
+    float f[8];
+    cvt8<BF16>(v, f);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(f[i]));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = amax;
+  __syncthreads();
+  amax = red[0];
+#pragma unroll
+  for (int i = 1; i < QT / 32; ++i) amax = fmaxf(amax, red[i]);
+
+  const float s = amax == 0.f ? 1.0f : __fdiv_rn(amax, 7.0f);  // A2 / Eq.1
+  if (threadIdx.x == 0) sA[m] = s;
+
+#pragma unroll
+  for (int c = 0; c < CHUNKS; ++c) {
+    int idx = threadIdx.x + c * QT;
+    if (idx < nchunk) {
+      float f[8];
+      cvt8<BF16>(cache[c], f);
+      qrow[idx] = quant_pack8(f, s);
+    }
+  }
+  for (int idx = threadIdx.x + CHUNKS * QT; idx < nchunk; idx += QT) {
+    uint4 v = __ldg(row + idx);
+    float f[8];
+    cvt8<BF16>(v, f);
+    qrow[idx] = quant_pack8(f, s);
+  }
+}
+
+__global__ void mq_unpack_act_kernel(const uint8_t* __restrict__ qA, int64_t total_bytes, int8_t* __restrict__ q) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total_bytes) return;
+  uint8_t b = qA[i];
+  int lo = b & 0xF, hi = b >> 4;
+  q[2 * i] = (int8_t)(lo >= 8 ? lo - 16 : lo);
+  q[2 * i + 1] = (int8_t)(hi >= 8 ? hi - 16 : hi);
+}
+
+}  // namespace
+
+extern "C" const char* mq_status_string(int status) {
+  switch (status) {
+    case MQ_OK: return "ok";
+    case MQ_ERR_INVALID_ARG: return "invalid argument";
+    case MQ_ERR_UNSUPPORTED_SHAPE: return "unsupported shape";
+    case MQ_ERR_UNSUPPORTED_DEVICE: return "unsupported device (needs compute capability 10.0, sm_100a)";
+    case MQ_ERR_CUDA: return "CUDA error";
+    case MQ_ERR_OOM: return "out of memory";
+    case MQ_ERR_ACC_OVERFLOW: return "K too large for the int32 accumulator";
+    case MQ_ERR_WORKSPACE: return "workspace too small";
+    default: return "unknown status";
+  }
+}
+
+extern "C" int mq_set_option(const char* name, int64_t value) {
+  if (!name || value < 0) return MQ_ERR_INVALID_ARG;
+  mq::Options& o = mq::options();
+  if (!strcmp(name, "split_k")) {
+    o.split_k = value;
+  } else if (!strcmp(name, "token_tile")) {
+    if (value != 0 && value != 16 && value != 32 && value != 64 && value != 128 && value != 256)
+      return MQ_ERR_INVALID_ARG;
+    o.token_tile = value;
+  } else if (!strcmp(name, "max_ctas")) {
+    o.max_ctas = value;
+  } else {
+    return MQ_ERR_INVALID_ARG;
+  }
+  return MQ_OK;
+}
+
+extern "C" int mq_last_launch_count(void) { return mq::g_launches; }
+
+extern "C" size_t mq_qact_bytes(int64_t M, int64_t K) {
+  if (M < 0 || K < 0) return 0;
+  return (size_t)M * (size_t)K / 2;
+}
+
+extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda, void* qA, float* sA,
+                               void* cuda_stream) {
+  if (M < 0 || K <= 0 || K % mq::BK != 0 || K > (int64_t)1 << 30) return MQ_ERR_UNSUPPORTED_SHAPE;
+  if (a_dtype != MQ_F16 && a_dtype != MQ_BF16) return MQ_ERR_INVALID_ARG;
+  mq::set_launch_count(0);
+  if (M == 0) return MQ_OK;
+  if (!A || !qA || !sA || lda < K) return MQ_ERR_INVALID_ARG;
+  if (((uintptr_t)A & 15) || ((uintptr_t)qA & 15) || (lda % 8) != 0 || ((uintptr_t)sA & 3)) return MQ_ERR_INVALID_ARG;
+  if (M > 2147483647LL) return MQ_ERR_UNSUPPORTED_SHAPE;
+  int rc = mq::check_device();
+  if (rc != MQ_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const uint16_t* a = (const uint16_t*)A;
+  dim3 grid((unsigned)M), blk(QT);
+  const int nchunk_per_thread = (int)((K / 8 + QT - 1) / QT);
+  if (a_dtype == MQ_BF16) {
+    if (nchunk_per_thread <= 2)
+      mq_quantize_act_kernel<true, 2><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+    else
+      mq_quantize_act_kernel<true, 4><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+  } else {
+    if (nchunk_per_thread <= 2)
+      mq_quantize_act_kernel<false, 2><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+    else
+      mq_quantize_act_kernel<false, 4><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+  }
+  mq::set_launch_count(1);
+  if (cudaGetLastError() != cudaSuccess) return MQ_ERR_CUDA;
+  return MQ_OK;
+}
+
+extern "C" int mq_unpack_act(const void* qA, int64_t M, int64_t K, int8_t* q, void* cuda_stream) {
+  if (M < 0 || K <= 0 || K % 2 != 0) return MQ_ERR_UNSUPPORTED_SHAPE;
+  if (M == 0) return MQ_OK;
+  if (!qA || !q) return MQ_ERR_INVALID_ARG;
+  int rc = mq::check_device();
+  if (rc != MQ_OK) return rc;
+  int64_t total = M * K / 2;
+  int64_t blocks = (total + 255) / 256;
+  if (blocks > 2147483647LL) return MQ_ERR_UNSUPPORTED_SHAPE;
+  mq_unpack_act_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const uint8_t*)qA, total, q);
+  if (cudaGetLastError() != cudaSuccess) return MQ_ERR_CUDA;
+  return MQ_OK;
+}

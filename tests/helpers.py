@@ -1,0 +1,109 @@
+"""Shared helpers of the parity tests: build a seeded case with the ORACLE, run the CUDA path
+through the C ABI, compare.  The oracle and the CUDA path meet only here (and in smoke/bench).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+import oracle
+import synth
+
+# north_star tolerance: max relative error 2e-3 on Y (bf16 RNE alone is 2^-9 = 1.95e-3), plus an
+# absolute term for the fp32 epilogue's cancellation between the base and residual terms.
+Y_RTOL = 2e-3
+Y_MAG_TOL = 1e-6
+
+
+@dataclass
+class Case:
+    M: int
+    K: int
+    N: int
+    bs: int
+    W: np.ndarray
+    h: Optional[np.ndarray]
+    A16: np.ndarray          # np.float16, or uint16 bf16 bits
+    a_dtype: str             # "f16" | "bf16"
+    L: "oracle.PackedLayer"
+
+
+def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """RNE fp32 -> bf16 bit patterns (uint16); inputs are finite."""
+    u = np.ascontiguousarray(x, np.float32).view(np.uint32).astype(np.uint64)
+    r = (u + 0x7FFF + ((u >> 16) & 1)) >> 16
+    return r.astype(np.uint16)
+
+
+def make_case(seed: int, M: int, K: int, N: int, bs: int = 64, rho: Optional[float] = 0.05,
+              budget: Optional[int] = None, a_dtype: str = "f16", calib_tokens: int = 64,
+              n_outlier_ch: Optional[int] = None) -> Case:
+    W = synth.gen_weight(seed, N, K)
+    if a_dtype == "f16":
+        A16 = synth.gen_act(seed, M, K, n_outlier_ch=n_outlier_ch)
+    else:
+        A16 = f32_to_bf16_bits(synth.gen_act(seed, M, K, n_outlier_ch=n_outlier_ch, dtype="f32"))
+    X = synth.gen_calib(seed, K, calib_tokens, n_outlier_ch=n_outlier_ch)
+    h = oracle.hessian_diag(X).astype(np.float32)
+    if budget is None:
+        budget = synth.budget_from_density(rho, N, K, bs)
+    L = oracle.algorithm1(W, h, bs, budget)
+    return Case(M, K, N, bs, W, h, A16, a_dtype, L)
+
+
+def oracle_act(case: Case):
+    return oracle.quantize_act(case.A16 if case.a_dtype == "f16" else (case.A16, "bf16"))
+
+
+def oracle_forward(case: Case, rows: Optional[np.ndarray] = None):
+    """O2 + O8 + O9 (optionally on a subset of token rows)."""
+    qa, sa = oracle_act(case)
+    if rows is not None:
+        qa, sa = qa[rows], sa[rows]
+    acc0, acc1 = oracle.gemm(qa, case.L.d.qw, case.L.d.qr, case.L.bs, case.L.blk_n, case.L.blk_k)
+    Y, mag = oracle.output(acc0, acc1, sa, case.L.d.sw, case.L.d.sr, want_mag=True)
+    return dict(qa=qa, sa=sa, acc0=acc0, acc1=acc1, Y=Y, mag=mag)
+
+
+# ---------------------------------------------------------------------------------- CUDA side
+def to_device_act(case: Case):
+    import torch
+    if case.a_dtype == "f16":
+        return torch.from_numpy(case.A16).cuda()
+    return torch.from_numpy(case.A16.view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def pack_from_oracle(case: Case):
+    """mq_pack_prequantized on the oracle's decomposition (isolates GEMM parity from selection)."""
+    import paper_2606_15652_b200 as mq
+    L = case.L
+    return mq.mq_pack_prequantized(L.d.qw, L.d.sw, L.bs, L.blk_n, L.blk_k, L.qr_blocks(), L.d.sr)
+
+
+def run_cuda(case: Case, w=None, out_dtype="bf16", workspace=None):
+    import torch
+    import paper_2606_15652_b200 as mq
+    if w is None:
+        w = pack_from_oracle(case)
+    A = to_device_act(case)
+    qA, sA = mq.mq_quantize_act(A)
+    Y, d0, d1 = mq.mq_gemm(w, qA, sA, case.M, out_dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float16,
+                           dbg=True, workspace=workspace)
+    torch.cuda.synchronize()
+    q = mq.mq_unpack_act(qA, case.M, case.K)
+    return dict(qa=q.cpu().numpy(), sa=sA.cpu().numpy(), acc0=d0.cpu().numpy(), acc1=d1.cpu().numpy(),
+                Y=Y.float().cpu().numpy().astype(np.float64), w=w)
+
+
+def assert_parity(got: dict, want: dict, rows: Optional[np.ndarray] = None, what: str = ""):
+    g = {k: (v[rows] if rows is not None and isinstance(v, np.ndarray) and k != "w" else v) for k, v in got.items()}
+    assert np.array_equal(g["sa"].view(np.uint32), want["sa"].view(np.uint32)), f"{what}: activation scales differ"
+    assert np.array_equal(g["qa"], want["qa"]), f"{what}: activation ints differ"
+    assert np.array_equal(g["acc0"].astype(np.int64), want["acc0"]), f"{what}: base accumulator not bit-exact"
+    assert np.array_equal(g["acc1"].astype(np.int64), want["acc1"]), f"{what}: residual accumulator not bit-exact"
+    err = np.abs(g["Y"] - want["Y"])
+    tol = Y_RTOL * np.abs(want["Y"]) + Y_MAG_TOL * want["mag"]
+    bad = err > tol
+    assert not bad.any(), f"{what}: Y out of tolerance at {int(bad.sum())} of {bad.size} (max excess {float((err - tol).max()):.3e})"

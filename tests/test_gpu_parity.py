@@ -1,0 +1,294 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Bars (north_star): activation ints/scales and both int32
+accumulators bit-exact; Y within 2e-3 relative (helpers.assert_parity).
+
+Run with:  python -m pytest tests -m gpu
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from helpers import (Case, assert_parity, f32_to_bf16_bits, make_case, oracle_act, oracle_forward, pack_from_oracle,
+                     run_cuda, to_device_act)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mq():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    assert torch.cuda.get_device_capability() == (10, 0), "libmq targets sm_100a (B200) only"
+    import paper_2606_15652_b200 as m
+    m.lib()  # raises if the extension is missing: no fallback
+    yield m
+    m.mq_set_option("split_k", 0)
+    m.mq_set_option("token_tile", 0)
+    m.mq_set_option("max_ctas", 0)
+
+
+# ------------------------------------------------------------------ kernel (i): activation quantize
+@pytest.mark.parametrize("M,K,dt", [(1, 128, "f16"), (16, 256, "f16"), (37, 4096, "f16"), (5, 14336, "f16"),
+                                    (3, 28672, "bf16"), (130, 1024, "bf16"), (1, 4096, "bf16")])
+def test_quantize_act_bit_exact(mq, M, K, dt):
+    import torch
+    case = make_case(7 + M, M, K, 128, rho=0.0, a_dtype=dt, calib_tokens=4)
+    want_q, want_s = oracle_act(case)
+    A = to_device_act(case)
+    qA, sA = mq.mq_quantize_act(A)
+    got_q = mq.mq_unpack_act(qA, M, K).cpu().numpy()
+    torch.cuda.synchronize()
+    assert np.array_equal(sA.cpu().numpy().view(np.uint32), want_s.view(np.uint32))
+    assert np.array_equal(got_q, want_q)
+    # canonical nibble packing (include/mq.h): byte i = element 2i | element 2i+1 << 4
+    raw = qA.cpu().numpy()
+    lo = (want_q[:, 0::2].astype(np.int16) & 0xF).astype(np.uint8)
+    hi = (want_q[:, 1::2].astype(np.int16) & 0xF).astype(np.uint8)
+    assert np.array_equal(raw, lo | (hi << 4))
+
+
+def test_quantize_act_edge_rows(mq):
+    """all-zero row (A2), exact ties on the fp16 grid (A3: half to even), +-amax, strided input."""
+    import torch
+    K = 256
+    A = np.zeros((4, K), np.float16)
+    A[1, :9] = [7, -7, 3.5, 2.5, 1.5, 0.5, -0.5, -2.5, 0]       # tests/golden/o1_hand_vector.txt
+    A[2, :] = np.float16(-3.0)
+    A[3, ::2] = np.float16(6.5e4)
+    A[3, 1::2] = np.float16(6e-8)                                 # fp16 subnormal
+    want_q, want_s = oracle.quantize_act(A)
+    big = torch.zeros((4, K + 64), dtype=torch.float16, device="cuda")
+    big[:, :K] = torch.from_numpy(A).cuda()
+    qA, sA = mq.mq_quantize_act(big[:, :K])                       # lda = K + 64
+    got = mq.mq_unpack_act(qA, 4, K).cpu().numpy()
+    assert np.array_equal(got, want_q)
+    assert np.array_equal(sA.cpu().numpy().view(np.uint32), want_s.view(np.uint32))
+    assert want_s[0] == 1.0 and not want_q[0].any()
+    assert want_q[1, :9].tolist() == [7, -7, 4, 2, 2, 0, 0, -2, 0]
+
+
+# ------------------------------------------------------------------ packing
+@pytest.mark.parametrize("bs", [64, 128])
+def test_pack_prequantized_roundtrip(mq, bs):
+    case = make_case(11, 4, 512, 384, bs=bs, rho=0.25)
+    w = pack_from_oracle(case)
+    e = w.export()
+    L = case.L
+    assert np.array_equal(e["qW"], L.d.qw)
+    assert np.array_equal(e["sW"].view(np.uint32), L.d.sw.view(np.uint32))
+    assert np.array_equal(e["sR"].view(np.uint32), L.d.sr.view(np.uint32))
+    order = np.lexsort((L.blk_k, L.blk_n))
+    assert e["nnz"] == L.nnz
+    assert np.array_equal(e["blk_n"], L.blk_n[order]) and np.array_equal(e["blk_k"], L.blk_k[order])
+    assert np.array_equal(e["qR"], L.qr_blocks()[order])
+    info = w.info()
+    assert (info["N"], info["K"], info["block"], info["nnz"]) == (384, 512, bs, L.nnz)
+
+
+@pytest.mark.parametrize("N,K,bs,rho", [(256, 256, 64, 2 / 16), (384, 1024, 64, 0.05), (256, 512, 128, 0.25),
+                                        (1024, 2048, 64, 0.10)])
+def test_pack_weights_matches_algorithm1(mq, N, K, bs, rho):
+    """mq_pack_weights (the library's own Algorithm 1) against the oracle's: same base ints and
+    scales, same residual scales, same selected set, same Q(R) on it."""
+    seed = 0 if N == 256 and K == 256 else 21
+    case = make_case(seed, 16, K, N, bs=bs, rho=rho, n_outlier_ch=2 if seed == 0 else None)
+    budget = synth.budget_from_density(rho, N, K, bs)
+    w = mq.mq_pack_weights(case.W, case.h, bs, budget)
+    e = w.export()
+    L = case.L
+    assert np.array_equal(e["qW"], L.d.qw)
+    assert np.array_equal(e["sW"].view(np.uint32), L.d.sw.view(np.uint32))
+    assert np.array_equal(e["sR"].view(np.uint32), L.d.sr.view(np.uint32))
+    order = np.lexsort((L.blk_k, L.blk_n))
+    assert e["nnz"] == L.nnz and L.nnz > 0
+    assert np.array_equal(e["blk_n"], L.blk_n[order]) and np.array_equal(e["blk_k"], L.blk_k[order])
+    assert np.array_equal(e["qR"], L.qr_blocks()[order])
+
+
+def test_pack_weights_zero_h_columns_and_null_h(mq):
+    """blocks whose score is zero are never selected (nnz < budget); h = NULL means all ones."""
+    N, K, bs = 256, 512, 64
+    W = synth.gen_weight(5, N, K)
+    h = np.ones(K, np.float32)
+    h[128:] = 0.0                       # only block-columns 0,1 can score
+    w = mq.mq_pack_weights(W, h, bs, 1000)
+    L = oracle.algorithm1(W, h, bs, 1000)
+    e = w.export()
+    assert e["nnz"] == L.nnz == 8 and set(e["blk_k"].tolist()) == {0, 1}
+    w1 = mq.mq_pack_weights(W, None, bs, 5)
+    L1 = oracle.algorithm1(W, None, bs, 5)
+    e1 = w1.export()
+    order = np.lexsort((L1.blk_k, L1.blk_n))
+    assert np.array_equal(e1["blk_n"], L1.blk_n[order]) and np.array_equal(e1["blk_k"], L1.blk_k[order])
+
+
+def test_pack_rejects_bad_input(mq):
+    qW = np.zeros((128, 128), np.int8)
+    s = np.ones(128, np.float32)
+    qW[3, 3] = -8                                                  # A1: code -8 is rejected
+    with pytest.raises(mq.MqError):
+        mq.mq_pack_prequantized(qW, s, 64, np.zeros(0, np.int32), np.zeros(0, np.int32), np.zeros((0, 64, 64), np.int8), s)
+    qW[3, 3] = 0
+    bn = np.array([0, 0], np.int32)
+    bk = np.array([1, 1], np.int32)                               # duplicate block
+    with pytest.raises(mq.MqError):
+        mq.mq_pack_prequantized(qW, s, 64, bn, bk, np.zeros((2, 64, 64), np.int8), s)
+    with pytest.raises(mq.MqError):
+        mq.mq_pack_prequantized(qW, s, 64, np.array([5], np.int32), np.array([0], np.int32),
+                                np.zeros((1, 64, 64), np.int8), s)  # out of range
+
+
+# ------------------------------------------------------------------ fused GEMM
+def test_config1_tiny(mq):
+    """BASELINE.json configs[0]: M=16, K=N=256, 64x64 blocks, top-2 of 16, seed 0."""
+    W = synth.gen_weight(0, 256, 256)
+    A = synth.gen_act(0, 16, 256, n_outlier_ch=2)
+    h = oracle.hessian_diag(A.astype(np.float32)).astype(np.float32)
+    L = oracle.algorithm1(W, h, 64, 2)
+    case = Case(16, 256, 256, 64, W, h, A, "f16", L)
+    want = oracle_forward(case)
+    w = mq.mq_pack_weights(W, h, 64, 2)                           # the library's own Algorithm 1
+    got = run_cuda(case, w=w)
+    assert_parity(got, want, what="config1")
+    assert np.abs(want["acc1"]).sum() > 0
+
+
+SHAPES = [
+    # M, K, N, bs, rho, dtype
+    (1, 512, 256, 64, 0.10, "f16"),
+    (8, 1024, 384, 64, 0.05, "f16"),
+    (17, 640, 256, 64, 0.20, "bf16"),       # ragged M, K-steps = 5
+    (33, 1024, 512, 128, 0.25, "f16"),
+    (100, 512, 384, 64, 0.10, "bf16"),
+    (128, 768, 256, 64, 0.10, "f16"),
+    (130, 512, 256, 128, 0.50, "f16"),      # two token tiles, ragged tail of 2
+    (300, 1024, 640, 64, 0.05, "bf16"),     # several tiles both ways
+]
+
+
+@pytest.mark.parametrize("M,K,N,bs,rho,dt", SHAPES)
+def test_gemm_parity_small(mq, M, K, N, bs, rho, dt):
+    case = make_case(100 + M, M, K, N, bs=bs, rho=rho, a_dtype=dt)
+    want = oracle_forward(case)
+    got = run_cuda(case)
+    assert_parity(got, want, what=f"M{M} K{K} N{N} bs{bs}")
+
+
+@pytest.mark.parametrize("bt", [16, 32, 64, 128, 256])
+def test_gemm_every_token_tile(mq, bt):
+    """Each template instantiation (token tile) on a shape with a ragged token tail."""
+    M = {16: 40, 32: 70, 64: 150, 128: 260, 256: 300}[bt]
+    case = make_case(200 + bt, M, 768, 384, bs=64, rho=0.15)
+    want = oracle_forward(case)
+    mq.mq_set_option("token_tile", bt)
+    try:
+        got = run_cuda(case)
+    finally:
+        mq.mq_set_option("token_tile", 0)
+    assert_parity(got, want, what=f"token_tile {bt}")
+
+
+@pytest.mark.parametrize("S", [2, 3, 8])
+def test_gemm_split_k_exact_and_workspace_clean(mq, S):
+    """Split-K partial sums are int32 adds, so the accumulators stay bit-exact; the workspace
+    must come back all-zero (include/mq.h contract) and be reusable."""
+    import torch
+    case = make_case(300 + S, 24, 2048, 384, bs=64, rho=0.10)
+    want = oracle_forward(case)
+    w = pack_from_oracle(case)
+    mq.mq_set_option("split_k", S)
+    try:
+        ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, case.M))
+        assert ws is not None
+        for rep in range(2):
+            got = run_cuda(case, w=w, workspace=ws)
+            assert_parity(got, want, what=f"split_k {S} rep {rep}")
+            torch.cuda.synchronize()
+            assert int(ws.count_nonzero().item()) == 0
+    finally:
+        mq.mq_set_option("split_k", 0)
+
+
+def test_gemm_budget_zero_equals_dense_w4a4(mq):
+    """north_star invariant: K=0 blocks == the dense-only W4A4 GEMM (acc1 == 0)."""
+    case = make_case(41, 20, 1024, 256, bs=64, budget=0)
+    want = oracle_forward(case)
+    got = run_cuda(case)
+    assert_parity(got, want, what="budget 0")
+    assert not got["acc1"].any()
+    dense = want["sa"][:, None].astype(np.float64) * (want["acc0"] * case.L.d.sw[None, :].astype(np.float64))
+    assert np.allclose(got["Y"], dense, rtol=2.5e-3, atol=1e-6)
+
+
+@pytest.mark.parametrize("bs", [64, 128])
+def test_gemm_all_blocks_equals_two_level_dequant(mq, bs):
+    """north_star invariant: selecting every block == the two-level dequantized weight."""
+    N, K, M = 256, 512, 12
+    case = make_case(43, M, K, N, bs=bs, budget=(N // bs) * (K // bs))
+    L = case.L
+    assert L.nnz == (N // bs) * (K // bs)
+    want = oracle_forward(case)
+    got = run_cuda(case)
+    assert_parity(got, want, what="all blocks")
+    W2 = L.d.sw[:, None].astype(np.float64) * L.d.qw + L.d.sr[:, None].astype(np.float64) * L.d.qr
+    Aq = want["sa"][:, None].astype(np.float64) * want["qa"]
+    assert np.allclose(got["Y"], Aq @ W2.T, rtol=2.5e-3, atol=1e-5)
+
+
+def test_gemm_extreme_values(mq):
+    """all +-7 operands: |acc0| = 49 K exactly (int32 head-room of the x16 unpack)."""
+    import torch
+    M, K, N = 8, 4096, 128
+    qw = np.full((N, K), 7, np.int8)
+    qw[1::2] = -7
+    s1 = np.ones(N, np.float32)
+    bn = np.array([0, 1], np.int32)
+    bk = np.array([0, K // 64 - 1], np.int32)
+    qr = np.full((2, 64, 64), -7, np.int8)
+    w = mq.mq_pack_prequantized(qw, s1, 64, bn, bk, qr, s1)
+    A = torch.full((M, K), 7.0, dtype=torch.float16, device="cuda")
+    qA, sA = mq.mq_quantize_act(A)
+    Y, d0, d1 = mq.mq_gemm(w, qA, sA, M, dbg=True)
+    d0, d1 = d0.cpu().numpy(), d1.cpu().numpy()
+    assert (d0[:, 0::2] == 49 * K).all() and (d0[:, 1::2] == -49 * K).all()
+    assert (d1 == -49 * 64).all()
+    assert np.allclose(sA.cpu().numpy(), 1.0)
+
+
+def test_gemm_fp16_output_and_strided_y(mq):
+    import torch
+    case = make_case(47, 9, 512, 256, bs=64, rho=0.10)
+    want = oracle_forward(case)
+    w = pack_from_oracle(case)
+    A = to_device_act(case)
+    qA, sA = mq.mq_quantize_act(A)
+    big = torch.full((9, 256 + 32), 123.0, dtype=torch.float16, device="cuda")
+    mq.mq_gemm(w, qA, sA, 9, Y=big[:, :256])
+    got = big.float().cpu().numpy().astype(np.float64)
+    assert (got[:, 256:] == 123.0).all()
+    err = np.abs(got[:, :256] - want["Y"])
+    assert (err <= 1e-3 * np.abs(want["Y"]) + 1e-6 * want["mag"]).all()
+
+
+def test_linear_matches_two_calls(mq):
+    import torch
+    case = make_case(49, 40, 1024, 384, bs=64, rho=0.05)
+    w = pack_from_oracle(case)
+    A = to_device_act(case)
+    qA, sA = mq.mq_quantize_act(A)
+    Y2 = mq.mq_gemm(w, qA, sA, case.M)
+    Y1 = mq.mq_linear(w, A)
+    torch.cuda.synchronize()
+    assert torch.equal(Y1, Y2)
+    assert mq.mq_last_launch_count() == 2
+
+
+def test_m_zero_is_noop(mq):
+    import torch
+    case = make_case(51, 1, 256, 128, rho=0.0)
+    w = pack_from_oracle(case)
+    L = mq.lib()
+    assert L.mq_gemm(w.handle, None, None, 0, None, 1, 128, None, None, None, 0, None) == 0
+    assert L.mq_quantize_act(None, 0, 0, 256, 256, None, None, None) == 0
+    torch.cuda.synchronize()
