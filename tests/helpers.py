@@ -11,10 +11,22 @@ import numpy as np
 import oracle
 import synth
 
-# north_star tolerance: max relative error 2e-3 on Y (bf16 RNE alone is 2^-9 = 1.95e-3), plus an
-# absolute term for the fp32 epilogue's cancellation between the base and residual terms.
+# Tolerance on Y (reading A17).  north_star: "within max relative error 2e-3
+# (fp32 epilogue, bf16 output rounding)".  fp16 output: exactly that bound.  bf16 output: a bf16
+# has 8 significant bits, so even the CORRECTLY ROUNDED result is up to 2^-8 = 3.9e-3 away (first
+# GPU run: exact -5.13993 -> nearest bf16 -5.125, 2.9e-3); the bound used is therefore the
+# tightest one any implementation can meet: half a bf16 ulp of the exact value.  Both carry an
+# absolute term for the fp32 epilogue (cancellation between the base and residual terms).
 Y_RTOL = 2e-3
 Y_MAG_TOL = 1e-6
+
+
+def y_tolerance(Y_exact: np.ndarray, mag: np.ndarray, out_dtype: str) -> np.ndarray:
+    if out_dtype == "f16":
+        return Y_RTOL * np.abs(Y_exact) + Y_MAG_TOL * mag
+    _, e = np.frexp(Y_exact)                      # |Y| in [2^(e-1), 2^e)
+    half_ulp = np.where(Y_exact == 0, 0.0, np.ldexp(1.0, e - 1 - 7 - 1))   # ulp = 2^(e-1) * 2^-7
+    return half_ulp + Y_MAG_TOL * mag
 
 
 @dataclass
@@ -94,16 +106,17 @@ def run_cuda(case: Case, w=None, out_dtype="bf16", workspace=None):
     torch.cuda.synchronize()
     q = mq.mq_unpack_act(qA, case.M, case.K)
     return dict(qa=q.cpu().numpy(), sa=sA.cpu().numpy(), acc0=d0.cpu().numpy(), acc1=d1.cpu().numpy(),
-                Y=Y.float().cpu().numpy().astype(np.float64), w=w)
+                Y=Y.float().cpu().numpy().astype(np.float64), w=w, out_dtype=out_dtype)
 
 
 def assert_parity(got: dict, want: dict, rows: Optional[np.ndarray] = None, what: str = ""):
-    g = {k: (v[rows] if rows is not None and isinstance(v, np.ndarray) and k != "w" else v) for k, v in got.items()}
+    g = {k: (v[rows] if rows is not None and isinstance(v, np.ndarray) else v) for k, v in got.items()}
     assert np.array_equal(g["sa"].view(np.uint32), want["sa"].view(np.uint32)), f"{what}: activation scales differ"
     assert np.array_equal(g["qa"], want["qa"]), f"{what}: activation ints differ"
     assert np.array_equal(g["acc0"].astype(np.int64), want["acc0"]), f"{what}: base accumulator not bit-exact"
     assert np.array_equal(g["acc1"].astype(np.int64), want["acc1"]), f"{what}: residual accumulator not bit-exact"
     err = np.abs(g["Y"] - want["Y"])
-    tol = Y_RTOL * np.abs(want["Y"]) + Y_MAG_TOL * want["mag"]
+    tol = y_tolerance(want["Y"], want["mag"], got.get("out_dtype", "bf16"))
+    assert (tol <= 2.0 ** -8 * np.abs(want["Y"]) + Y_MAG_TOL * want["mag"] + 1e-300).all()
     bad = err > tol
     assert not bad.any(), f"{what}: Y out of tolerance at {int(bad.sum())} of {bad.size} (max excess {float((err - tol).max()):.3e})"

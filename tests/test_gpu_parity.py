@@ -167,12 +167,13 @@ SHAPES = [
 ]
 
 
+@pytest.mark.parametrize("out_dtype", ["bf16", "f16"])
 @pytest.mark.parametrize("M,K,N,bs,rho,dt", SHAPES)
-def test_gemm_parity_small(mq, M, K, N, bs, rho, dt):
+def test_gemm_parity_small(mq, M, K, N, bs, rho, dt, out_dtype):
     case = make_case(100 + M, M, K, N, bs=bs, rho=rho, a_dtype=dt)
     want = oracle_forward(case)
-    got = run_cuda(case)
-    assert_parity(got, want, what=f"M{M} K{K} N{N} bs{bs}")
+    got = run_cuda(case, out_dtype=out_dtype)      # f16: north_star's 2e-3; bf16: half an ulp
+    assert_parity(got, want, what=f"M{M} K{K} N{N} bs{bs} {out_dtype}")
 
 
 @pytest.mark.parametrize("bt", [16, 32, 64, 128, 256])
@@ -218,7 +219,7 @@ def test_gemm_budget_zero_equals_dense_w4a4(mq):
     assert_parity(got, want, what="budget 0")
     assert not got["acc1"].any()
     dense = want["sa"][:, None].astype(np.float64) * (want["acc0"] * case.L.d.sw[None, :].astype(np.float64))
-    assert np.allclose(got["Y"], dense, rtol=2.5e-3, atol=1e-6)
+    assert np.allclose(got["Y"], dense, rtol=4e-3, atol=1e-6)
 
 
 @pytest.mark.parametrize("bs", [64, 128])
@@ -233,7 +234,7 @@ def test_gemm_all_blocks_equals_two_level_dequant(mq, bs):
     assert_parity(got, want, what="all blocks")
     W2 = L.d.sw[:, None].astype(np.float64) * L.d.qw + L.d.sr[:, None].astype(np.float64) * L.d.qr
     Aq = want["sa"][:, None].astype(np.float64) * want["qa"]
-    assert np.allclose(got["Y"], Aq @ W2.T, rtol=2.5e-3, atol=1e-5)
+    assert np.allclose(got["Y"], Aq @ W2.T, rtol=4e-3, atol=1e-5)
 
 
 def test_gemm_extreme_values(mq):
