@@ -1,0 +1,418 @@
+#!/usr/bin/env python
+"""bench.py -- the headline benchmark of the MosaicQuant / ZipperEngine hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+Workload (default): BASELINE.json configs[1], "LLaMA3-8B-shaped decode layers":
+M in {1, 8, 32} tokens x {qkv 4096x6144, o 4096x4096, gate_up 4096x28672, down 14336x4096},
+W ~ N(0, 0.02) + 0.5% block-clustered x20 outliers, 64x64 residual blocks at 5% density chosen by
+the Delta-Hessian score (mq_pack_weights = Algorithm 1), fp16 activations, bf16 output.
+One STEP = the whole hot path once over one batch for every (M, projection):
+mq_quantize_act + mq_gemm, 12 pairs = 24 kernel launches, replayed from a CUDA graph.
+Every call reads a weight copy that was last touched > 3x L2 ago (4 rotating copies, 460 MB).
+
+Prints ONE JSON line (see the keys at the bottom).  `--impl reference` times the CPU oracle
+(this tier's reference arm) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fused W4A4+residual GEMM TOPS & frac of INT8/HBM roofline; tokens/s vs W16A16"
+RHO, BS = 0.05, 64
+N_COPIES = 4
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d["bf16_tflops"]),
+                    bf16_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+def workload_shapes(name: str):
+    import synth
+    cfg = synth.CONFIGS[name]
+    return cfg, [(m, l) for m in cfg["Ms"] for l in cfg["layers"]]
+
+
+def algo_bytes(M, K, N, nnz, bs):
+    """SURVEY 8(d) algorithmic bytes of one mq_gemm launch: packed base + residual blocks + block
+    metadata + scales + packed activations (+ their scales) in, 16-bit Y out."""
+    return N * K // 2 + nnz * bs * bs // 2 + 8 * nnz + 8 * N + M * K // 2 + 4 * M + 2 * M * N
+
+
+def algo_ops(M, K, N, nnz, bs):
+    return 2 * M * N * K + 2 * M * nnz * bs * bs
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                pw.append(float(r[2]))
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                pass
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                    samples=len(sm), reasons=sorted(reasons))
+
+
+class Layer:
+    """One projection: host tensors, N_COPIES packed device copies, per-M device buffers."""
+
+    def __init__(self, mq, torch, synth, seed, shape, Ms, n_copies):
+        self.name, self.K, self.N = shape.name, shape.K, shape.N
+        t0 = time.time()
+        self.W = synth.gen_weight(seed, self.N, self.K)
+        X = synth.gen_calib(seed, self.K, 256)
+        self.h = (2.0 / X.shape[0] * (X.astype(np.float64) ** 2).sum(0)).astype(np.float32)   # calibration input
+        self.budget = synth.budget_from_density(RHO, self.N, self.K, BS)
+        w0 = mq.mq_pack_weights(self.W, self.h, BS, self.budget)
+        self.copies = [w0] + [w0.clone() for _ in range(n_copies - 1)]
+        self.nnz = w0.info()["nnz"]
+        self.pack_s = time.time() - t0
+        self.A_host, self.A, self.qA, self.sA, self.Y, self.ws = {}, {}, {}, {}, {}, {}
+        for m in Ms:
+            a = synth.gen_act(seed + m, m, self.K)
+            self.A_host[m] = torch.from_numpy(a).pin_memory()
+            self.A[m] = self.A_host[m].cuda()
+            self.qA[m] = torch.empty((m, self.K // 2), dtype=torch.uint8, device="cuda")
+            self.sA[m] = torch.empty((m,), dtype=torch.float32, device="cuda")
+            self.Y[m] = torch.empty((m, self.N), dtype=torch.bfloat16, device="cuda")
+            self.ws[m] = mq.new_workspace(mq.mq_gemm_workspace_bytes(w0, m))
+
+
+def run_ours(args, rank, world):
+    import torch
+    import synth
+    import paper_2606_15652_b200 as mq
+
+    mq.lib()  # no fallback: raises if libmq.so is missing
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    assert torch.cuda.get_device_capability() == (10, 0), "bench.py needs a B200 (sm_100a)"
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = load_peaks()
+    cfg, shapes = workload_shapes(args.workload)
+    Ms, layers_cfg = cfg["Ms"], cfg["layers"]
+    layers = [Layer(mq, torch, synth, cfg["seed"] + i, l, Ms, N_COPIES) for i, l in enumerate(layers_cfg)]
+    calls = [(m, L) for m in Ms for L in layers]           # one step, in order
+
+    def step(si: int, only_gemm: bool = False):
+        for ci, (m, L) in enumerate(calls):
+            w = L.copies[(si * len(Ms) + ci // len(layers)) % N_COPIES]
+            if not only_gemm:
+                mq.mq_quantize_act(L.A[m], L.qA[m], L.sA[m])
+            mq.mq_gemm(w, L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+
+    stream = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        step(0)                                                  # first-call setup outside capture
+        stream.synchronize()
+        graphs = []
+        for si in range(N_COPIES):                               # pattern of copies repeats every 4 steps
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                step(si)
+            graphs.append(g)
+
+        def barrier():
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+
+        for i in range(args.warmup):
+            graphs[i % N_COPIES].replay()
+        barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        time.sleep(0.25)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(args.steps):
+            graphs[(args.warmup + i) % N_COPIES].replay()
+        e1.record(stream)
+        barrier()
+        ms_total = e0.elapsed_time(e1)
+        clocks = sampler.stop()
+
+        # ---- roofline of the dominant kernel (mq_gemm_kernel), timed alone: graphs of GEMM launches only
+        reps = 8
+        per_shape = []
+        for (m, L) in calls:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                for r in range(reps):
+                    mq.mq_gemm(L.copies[r % N_COPIES], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+            for _ in range(3):
+                g.replay()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            best = 1e30
+            for _ in range(5):
+                # other layers' traffic between repetitions keeps this layer's 4 copies cold in L2
+                graphs[0].replay()
+                a0.record(stream)
+                g.replay()
+                a1.record(stream)
+                stream.synchronize()
+                best = min(best, a0.elapsed_time(a1) / reps)
+            per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3,
+                                  bytes=algo_bytes(m, L.K, L.N, L.nnz, BS), ops=algo_ops(m, L.K, L.N, L.nnz, BS)))
+
+        # ---- W16A16 comparator: cuBLAS bf16 on the same shapes, same rotation
+        w16 = {L.name: [torch.randn((L.N, L.K), device="cuda", dtype=torch.bfloat16) * 0.02 for _ in range(2)]
+               for L in layers}
+        a16 = {(m, L.name): L.A[m].to(torch.bfloat16) for (m, L) in calls}
+
+        def step16(si):
+            for ci, (m, L) in enumerate(calls):
+                torch.matmul(a16[(m, L.name)], w16[L.name][(si + ci // len(layers)) % 2].t())
+        step16(0)
+        stream.synchronize()
+        g16 = []
+        for si in range(2):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=stream):
+                step16(si)
+            g16.append(g)
+        for i in range(3):
+            g16[i % 2].replay()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
+        for i in range(args.steps):
+            g16[i % 2].replay()
+        c1.record(stream)
+        stream.synchronize()
+        ms16 = c0.elapsed_time(c1) / args.steps
+        del w16, g16
+
+        # ---- e2e: host buffers through the C ABI (mq_linear), H2D + D2H inside the timed region
+        Yh = {(m, L.name): torch.empty((m, L.N), dtype=torch.bfloat16).pin_memory() for (m, L) in calls}
+        Ad = {(m, L.name): torch.empty_like(L.A[m]) for (m, L) in calls}
+        lws = {(m, L.name): mq.new_workspace(mq.mq_linear_workspace_bytes(L.copies[0], m)) for (m, L) in calls}
+
+        def step_e2e(si):
+            for ci, (m, L) in enumerate(calls):
+                k = (m, L.name)
+                Ad[k].copy_(L.A_host[m], non_blocking=True)
+                mq.mq_linear(L.copies[(si * len(Ms) + ci // len(layers)) % N_COPIES], Ad[k], Y=L.Y[m], workspace=lws[k])
+                Yh[k].copy_(L.Y[m], non_blocking=True)
+            stream.synchronize()                                 # the caller reads the result
+
+        for i in range(3):
+            step_e2e(i)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            step_e2e(i)
+        torch.cuda.synchronize()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+
+    ms_step = ms_total / args.steps
+    if world > 1:
+        t = torch.tensor([ms_step, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, e2e_ms = float(t[0]), float(t[1])
+    ops_step = sum(algo_ops(m, L.K, L.N, L.nnz, BS) for (m, L) in calls)
+    bytes_step = sum(algo_bytes(m, L.K, L.N, L.nnz, BS) for (m, L) in calls)
+    tokens_step = sum(Ms)
+    gemm_us = sum(s["us"] for s in per_shape)
+    gemm_bytes = sum(s["bytes"] for s in per_shape)
+    achieved = gemm_bytes / (gemm_us * 1e-6) / 1e9
+    h2d = sum(L.A_host[m].numel() * 2 for (m, L) in calls)
+    d2h = sum(m * L.N * 2 for (m, L) in calls)
+    out = {
+        "metric": METRIC, "value": world * ops_step / (ms_step * 1e-3) / 1e12, "unit": "TOPS",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int4 storage / int8 MMA / int32 acc",
+        "data": "synthetic",
+        "config": {"workload": f"{args.workload}: M in {Ms} x {[l.name for l in layers_cfg]} (K,N)="
+                               f"{[(l.K, l.N) for l in layers_cfg]}, rho={RHO}, block={BS}, fp16 in, bf16 out",
+                   "step": "mq_quantize_act + mq_gemm for each of the 12 (M, projection) pairs, CUDA-graph replay",
+                   "l2": f"{N_COPIES} rotating weight copies per layer ({N_COPIES * bytes_step / len(Ms) / 1e6:.0f} MB > 3x L2)",
+                   "parallelism": "replicas (no collective on the path)" if world > 1 else "single GPU"},
+        "tokens_per_s": world * tokens_step / (ms_step * 1e-3),
+        "hbm_gbs_step": bytes_step / (ms_step * 1e-3) / 1e9,
+        "w16a16_cublas_bf16": {"ms_per_step": ms16, "speedup_vs_w16a16": ms16 / ms_step,
+                               "paper_context": "up to 1.24x over W16A16 on RTX 4090 (P:43)"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                     "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+                     "kernel": "mq_gemm_kernel (12 launches of the step, timed alone, cold weights)",
+                     "per_shape": [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3),
+                                        gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
+                                        tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in per_shape]},
+        "e2e": {"value": world * ops_step / (e2e_ms * 1e-3) / 1e12, "unit": "TOPS", "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "mq_linear (C ABI) with pinned host buffers"},
+        "gpu_launches": args.steps * 2 * len(calls),
+        "clocks": clocks,
+        "pack_seconds": round(sum(L.pack_s for L in layers), 2),
+    }
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(args.workload, budget_s=20.0)
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
+# ------------------------------------------------------------------------------------------
+_ORACLE_GMACS = 1.0   # rough int64 MAC/ns of the plain oracle on ~8 cores; only sizes the sample
+
+
+def _oracle_layers(workload):
+    import oracle
+    import synth
+    cfg, _ = workload_shapes(workload)
+    out = []
+    for i, l in enumerate(cfg["layers"]):
+        seed = cfg["seed"] + i
+        W = synth.gen_weight(seed, l.N, l.K)
+        X = synth.gen_calib(seed, l.K, 256)
+        h = oracle.hessian_diag(X).astype(np.float32)
+        out.append((seed, l, oracle.algorithm1(W, h, BS, synth.budget_from_density(RHO, l.N, l.K, BS))))
+        del W
+    return cfg, out
+
+
+def _oracle_sample_rows(cfg, layers, seconds_per_step):
+    """Largest token count m_s (<= max M of the workload) whose pass over all projections is
+    estimated to fit in `seconds_per_step`."""
+    macs_per_token = sum(l.N * l.K * (1 + RHO) for (_, l, _) in layers)
+    m = max(cfg["Ms"])
+    while m > 1 and m * macs_per_token / (_ORACLE_GMACS * 1e9) > seconds_per_step:
+        m //= 2
+    return m
+
+
+def _oracle_step(layers, acts):
+    import oracle
+    for (_, l, L), A in zip(layers, acts):
+        oracle.forward_timed(A, L)
+
+
+def cpu_baseline(workload, budget_s=20.0, steps=2):
+    import oracle
+    import synth
+    cfg, layers = _oracle_layers(workload)
+    m = _oracle_sample_rows(cfg, layers, budget_s / steps)
+    acts = [synth.gen_act(seed + m, m, l.K) for (seed, l, _) in layers]
+    best = 1e30
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        _oracle_step(layers, acts)
+        best = min(best, time.perf_counter() - t0)
+    ops = sum(algo_ops(m, l.K, l.N, L.nnz, BS) for (_, l, L) in layers)
+    return {"value": ops / best / 1e12, "unit": "TOPS", "cores": min(oracle.num_threads(), m), "kind": "oracle",
+            "threads_available": oracle.num_threads(), "seconds": round(best, 3),
+            "sample": f"oracle O2+O8+O9 on M={m} tokens x all {len(layers)} projections of {workload} "
+                      f"(best of {steps}; the oracle parallelises over tokens only)"}
+
+
+def run_reference(args, rank, world):
+    """This tier's reference arm: the CPU oracle, as it stands, on the host cores."""
+    if rank != 0:
+        return
+    import oracle
+    import synth
+    total = max(1, args.steps + args.warmup)
+    cfg, layers = _oracle_layers(args.workload)
+    m = _oracle_sample_rows(cfg, layers, 150.0 / total)
+    acts = [synth.gen_act(seed + m, m, l.K) for (seed, l, _) in layers]
+    for _ in range(args.warmup):
+        _oracle_step(layers, acts)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _oracle_step(layers, acts)
+    dt = (time.perf_counter() - t0) / args.steps
+    ops = sum(algo_ops(m, l.K, l.N, L.nnz, BS) for (_, l, L) in layers)
+    tops = ops / dt / 1e12
+    sample = (f"oracle O2+O8+O9 on M={m} tokens x all {len(layers)} projections of {args.workload} per step "
+              f"(bounded sample of the workload)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": tops, "unit": "TOPS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int8 values / int64 acc / f64 output", "data": "synthetic",
+        "config": {"workload": f"{args.workload} (CPU oracle, sample: {sample})"},
+        "cpu_baseline": {"value": tops, "unit": "TOPS", "cores": min(oracle.num_threads(), m), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": tops, "unit": "TOPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="llama3_8b_decode")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -103,6 +103,9 @@ int mq_pack_prequantized(const int8_t* qW_host, const float* sW_host, int64_t N,
  * NULL = skipped).  Blocks are returned sorted by (blk_n, blk_k).  Host call; syncs. */
 int mq_weights_export(const mq_weights* w, int8_t* qW_host, float* sW_host, int64_t* nnz,
                       int32_t* blk_n_host, int32_t* blk_k_host, int8_t* qR_host, float* sR_host);
+/* Device-to-device copy of a packed layer into a fresh allocation (benchmarks rotate several
+ * copies so that every timed call reads its weights from HBM, not from L2).  Syncs the stream. */
+int mq_weights_clone(const mq_weights* w, mq_weights** out, void* cuda_stream);
 int mq_weights_info(const mq_weights* w, int64_t* N, int64_t* K, int* block, int64_t* nnz,
                     size_t* device_bytes);
 void mq_weights_free(mq_weights* w);

@@ -20,7 +20,7 @@ MQ_F16, MQ_BF16 = 0, 1
 
 EXPORTS = [
     "mq_status_string", "mq_qact_bytes", "mq_quantize_act", "mq_unpack_act", "mq_pack_weights",
-    "mq_pack_prequantized", "mq_weights_export", "mq_weights_info", "mq_weights_free",
+    "mq_pack_prequantized", "mq_weights_export", "mq_weights_clone", "mq_weights_info", "mq_weights_free",
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_set_option",
     "mq_last_launch_count",
 ]
@@ -59,6 +59,8 @@ def lib() -> C.CDLL:
     L.mq_pack_prequantized.argtypes = [vp, vp, i64, i64, i32, i64, vp, vp, vp, vp, C.POINTER(vp), vp]
     L.mq_weights_export.restype = i32
     L.mq_weights_export.argtypes = [vp, vp, vp, C.POINTER(i64), vp, vp, vp, vp]
+    L.mq_weights_clone.restype = i32
+    L.mq_weights_clone.argtypes = [vp, C.POINTER(vp), vp]
     L.mq_weights_info.restype = i32
     L.mq_weights_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), C.POINTER(i32), C.POINTER(i64), C.POINTER(sz)]
     L.mq_weights_free.restype = None
@@ -171,6 +173,11 @@ class Weights:
         _check(lib().mq_weights_export(self.handle, _np_ptr(qW), _np_ptr(sW), C.byref(n), _np_ptr(bn), _np_ptr(bk),
                                        _np_ptr(qR), _np_ptr(sR)), "mq_weights_export")
         return dict(qW=qW, sW=sW, sR=sR, blk_n=bn[:nnz], blk_k=bk[:nnz], qR=qR[:nnz], nnz=int(n.value))
+
+    def clone(self) -> "Weights":
+        out = C.c_void_p()
+        _check(lib().mq_weights_clone(self.handle, C.byref(out), _stream()), "mq_weights_clone")
+        return Weights(out.value)
 
     def free(self) -> None:
         if self._h:

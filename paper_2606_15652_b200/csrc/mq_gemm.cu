@@ -64,7 +64,7 @@ struct Cfg {
   static constexpr int OFF_BAR = OFF_RP + RSTAGES * RP_BYTES;
   static constexpr int NUM_BARS = 2 * PSTAGES + 2 * USTAGES + 4 * RSTAGES + 4;
   static constexpr int OFF_META = OFF_BAR + NUM_BARS * 8;
-  static constexpr int OFF_END = OFF_META + (PSTAGES + USTAGES + 4) * 4;
+  static constexpr int OFF_END = OFF_META + (PSTAGES + USTAGES + 8) * 4;
   static constexpr int SMEM_BYTES = OFF_END + 1024;  // slack for the 1024-byte alignment
 };
 
@@ -144,6 +144,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   volatile int32_t* meta_u = meta_p + C::PSTAGES;
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(meta_u + C::USTAGES);
   volatile int32_t* flag_slot = reinterpret_cast<volatile int32_t*>(tmem_slot + 1);
+  volatile int32_t* acc_flag = flag_slot + 1;  // [2]: did this accumulator stage receive residual MMAs?
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -164,7 +165,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       mbar_init(bar(B_EMPTY_RU + i), 1);
     }
     for (int i = 0; i < 2; ++i) {
-      mbar_init(bar(B_TFULL + i), 1);
+      mbar_init(bar(B_TFULL + i), 2);
       mbar_init(bar(B_TEMPTY + i), 4);
     }
     fence_mbar_init();
@@ -275,7 +276,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           tc_commit(bar(B_EMPTY_U + ru.stage));
           ru.next<C::USTAGES>();
         }
-        tc_commit(bar(B_TFULL + a));
+        acc_flag[a] = (int32_t)acc1_on;
+        mbar_arrive(bar(B_TFULL + a));   // release: publishes acc_flag to the epilogue warps
+        tc_commit(bar(B_TFULL + a));     // completes the phase when the MMAs have finished
       }
     }
   } else if (warp >= FIRST_UNPACK_WARP) {
@@ -355,22 +358,6 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       const int s = item % p.S, nt = (item / p.S) % p.NT, tt = item / (p.S * p.NT);
       int k0, k1;
       split_range(p.KS, p.S, s, k0, k1);
-      // does this (tile, split) own a residual cell?  (acc1 is undefined otherwise)
-      bool has_res = false;
-      {
-        const int cb = p.cell_ptr[nt], ce = p.cell_ptr[nt + 1];
-        if (p.S == 1) {
-          has_res = ce > cb;
-        } else {
-          for (int c = cb; c < ce; ++c) {
-            const int kc = p.cell_meta[c].kstep_mask & 0xFFFFFF;
-            if (kc >= k0 && kc < k1) {
-              has_res = true;
-              break;
-            }
-          }
-        }
-      }
       const int a = C::ACC_STAGES == 2 ? (it & 1) : 0;
       const uint32_t aphase = C::ACC_STAGES == 2 ? ((it >> 1) & 1) : (it & 1);
       const int n_loc = lq * 32 + lane;
@@ -381,6 +368,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 
       mbar_wait(bar(B_TFULL + a), aphase);
       tc_fence_after();
+      const bool has_res = acc_flag[a] != 0;  // acc1 is undefined when no residual MMA was issued
       const uint32_t t0addr = tmem_base + ((uint32_t)(lq * 32) << 16) + (uint32_t)(a * 2 * BT);
       const int tile_id = tt * p.NT + nt;
       int32_t* ws0 = p.ws_acc + (size_t)tile_id * (2 * BT * BN);

@@ -423,6 +423,38 @@ extern "C" int mq_weights_export(const mq_weights* w, int8_t* qW, float* sW, int
   return MQ_OK;
 }
 
+extern "C" int mq_weights_clone(const mq_weights* w, mq_weights** out, void* cuda_stream) {
+  if (!w || !out) return MQ_ERR_INVALID_ARG;
+  *out = nullptr;
+  mq_weights* c = new (std::nothrow) mq_weights(*w);
+  if (!c) return MQ_ERR_OOM;
+  void* blob = nullptr;
+  cudaError_t ce = cudaMalloc(&blob, w->dev_bytes);
+  if (ce != cudaSuccess) {
+    cudaGetLastError();
+    delete c;
+    return ce == cudaErrorMemoryAllocation ? MQ_ERR_OOM : MQ_ERR_CUDA;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaMemcpyAsync(blob, w->dev_blob, w->dev_bytes, cudaMemcpyDeviceToDevice, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(blob);
+    delete c;
+    return MQ_ERR_CUDA;
+  }
+  const ptrdiff_t d = (uint8_t*)blob - (uint8_t*)w->dev_blob;
+  c->dev_blob = blob;
+  c->d_base = w->d_base + d;
+  c->d_sw = (float*)((uint8_t*)w->d_sw + d);
+  c->d_sr = (float*)((uint8_t*)w->d_sr + d);
+  c->d_res = w->d_res + d;
+  c->d_cell_ptr = (int32_t*)((uint8_t*)w->d_cell_ptr + d);
+  c->d_cell_meta = (CellMeta*)((uint8_t*)w->d_cell_meta + d);
+  *out = c;
+  return MQ_OK;
+}
+
 extern "C" int mq_weights_info(const mq_weights* w, int64_t* N, int64_t* K, int* block, int64_t* nnz,
                                size_t* device_bytes) {
   if (!w) return MQ_ERR_INVALID_ARG;

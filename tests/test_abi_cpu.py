@@ -35,7 +35,7 @@ def test_header_symbols_all_exported(mqlib):
 
 def test_binding_has_same_names(mqlib):
     for n in _declared_symbols():
-        if n in ("mq_status_string", "mq_weights_export", "mq_weights_info", "mq_weights_free"):
+        if n in ("mq_status_string", "mq_weights_export", "mq_weights_info", "mq_weights_free", "mq_weights_clone"):
             continue  # exposed as status_string / Weights methods
         assert hasattr(mqlib, n), n
 
