@@ -119,9 +119,11 @@ void mq_weights_free(mq_weights* w);
  *   dbg_acc_base_dev / dbg_acc_res_dev : optional int32 [M,N] row-major (stride N); when
  *                    non-NULL they receive acc0 / acc1 exactly (parity hooks).
  *   workspace_dev  : at least mq_gemm_workspace_bytes(w, M) bytes, 16-byte aligned; must be
- *                    all-zero before the FIRST call that uses it; every call leaves it
- *                    all-zero again (split-K partial sums and tile counters).  Calls that
- *                    may run concurrently need distinct workspaces.
+ *                    all-zero before the FIRST call that uses it; afterwards its contents are
+ *                    library-private and stay valid from call to call (tile arrival counters,
+ *                    which every call returns to zero, and int32 partial tiles of the
+ *                    stream-K fix-up).  Calls that may run concurrently need distinct
+ *                    workspaces.
  * M == 0 is a no-op.
  */
 size_t mq_gemm_workspace_bytes(const mq_weights* w, int64_t M);
@@ -137,8 +139,9 @@ int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t 
               size_t workspace_bytes, void* cuda_stream);
 
 /* Tuning / ablation knobs (process-wide, not thread-safe; for benchmarks and tests).
- *   "split_k"   : 0 = automatic, n >= 1 = force n K-splits
- *   "token_tile": 0 = automatic, else 16/32/64/128/256
+ *   "split_k"   : 0 = automatic, 1 = whole output tiles per CTA, >= 2 = stream-K (the K-steps of
+ *                 all tiles cut into equal per-CTA ranges, shared tiles finished by the last arriver)
+ *   "token_tile": 0 = automatic, else 16/32/64/128
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */
 int mq_set_option(const char* name, int64_t value);

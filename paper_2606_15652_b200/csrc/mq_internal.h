@@ -3,19 +3,24 @@
 // Device layout of a packed layer.  BN = 128 output channels per
 // weight tile, BK = 128 input channels per K-step.
 //
-//   base   : uint8 [N/BN][K/BK][BN rows][BK/2 bytes]   one 8 KB tile per (n-tile, K-step),
-//            contiguous, so the kernel fetches it with ONE 1-D bulk copy (TMA).
-//            Inside a row the nibble order is canonical (byte i = elements 2i | 2i+1<<4).
+//   base   : uint8 [N/BN][K/BK][4 chunks][BN rows][16 bytes]   one 8 KB tile per (n-tile, K-step),
+//            contiguous, so the kernel fetches it with ONE 1-D bulk copy (TMA).  Chunk c of a
+//            row holds its 32 input channels 32c .. 32c+31 (one tcgen05.mma K slice) in the
+//            canonical nibble order (byte i = elements 2i | 2i+1<<4); rows are 16 bytes apart
+//            so that "one thread per output channel" reads shared memory without bank conflicts.
 //   sw, sr : float [N]  base / residual scale per output channel (A4).
 //   residual "cells": one cell per (n-tile, K-step) that holds >= 1 selected block,
 //            CSR over n-tiles (cell_ptr[N/BN + 1]), sorted by K-step inside a tile.
 //            A cell is split into four quarters q = 2*h + r  (h = k-half, r = row-half),
-//            each 64 rows x 64 k = 2 KB packed [64 rows][32 bytes].  Only present quarters
+//            each 64 rows x 64 k = 2 KB packed [2 chunks of 32 k][64 rows][16 bytes].  Only present quarters
 //            are stored, in ascending q, contiguously (res_data).
 //              block = 64 : a selected block (bn,bk) is quarter (h = bk&1, r = bn&1) of
 //                           cell (bn>>1, bk>>1)
 //              block = 128: a selected block is a whole cell (mask 0xF)
 //   cell_meta : int2 {kstep | mask << 24, first quarter index into res_data (2 KB units)}
+//   unit_meta : int2 [N/BN][K/BK] {mask, first quarter index}: the same cells indexed densely by
+//            (n-tile, K-step), so that the producer warp fetches the metadata of 32 consecutive
+//            K-steps with one coalesced load (mask 0 = the K-step has no residual cell)
 #pragma once
 
 #include <cstddef>
@@ -53,6 +58,7 @@ struct mq_weights {
   uint8_t* d_res = nullptr;
   int32_t* d_cell_ptr = nullptr;       // [N/BN + 1]
   mq::CellMeta* d_cell_meta = nullptr; // [n_cells]
+  int32_t* d_unit_meta = nullptr;      // [N/BN][K/BK][2] dense index of the cells: {quarter mask, first quarter}
   // host copies of the small metadata (used by the launcher and by export)
   std::vector<int32_t> h_cell_ptr;
   std::vector<mq::CellMeta> h_cell_meta;

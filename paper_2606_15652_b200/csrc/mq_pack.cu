@@ -75,8 +75,13 @@ struct HostLayer {
 
 inline size_t base_offset(int64_t n, int64_t k, int64_t K) {
   int64_t tile = (n / BN) * (K / BK) + k / BK;
-  return (size_t)tile * TILE_BYTES + (size_t)(n % BN) * (BK / 2) + (size_t)((k % BK) >> 1);
+  // inside a tile: [chunk c = (k % BK) / 32][row n % BN][16 bytes] (mq_internal.h)
+  return (size_t)tile * TILE_BYTES + (size_t)((k % BK) >> 5) * (BN * 16) + (size_t)(n % BN) * 16 +
+         (size_t)((k & 31) >> 1);
 }
+
+// byte of element (row, c) inside a 2 KB residual quarter: [chunk c / 32][row 0..63][16 bytes]
+inline size_t quarter_offset(int row, int c) { return (size_t)(c >> 5) * 1024 + (size_t)row * 16 + (size_t)((c & 31) >> 1); }
 
 inline void put_nibble(uint8_t* byte, int hi, int v) {
   uint8_t nib = (uint8_t)(v & 0xF);
@@ -153,7 +158,7 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
     for (int row = 0; row < 64; ++row)
       for (int c = 0; c < 64; ++c) {
         int v = e.b->q[(size_t)(e.sub_r * 64 + row) * bs + (size_t)(e.sub_h * 64 + c)];
-        put_nibble(dst + row * 32 + (c >> 1), c & 1, v);
+        put_nibble(dst + quarter_offset(row, c), c & 1, v);
       }
   }
   w->n_cells = (int64_t)w->h_cell_meta.size();
@@ -169,7 +174,17 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   size_t o_res = align_up(o_sr + (size_t)L.N * 4, 256);
   size_t o_cptr = align_up(o_res + std::max<size_t>(res.size(), 16), 256);
   size_t o_cmeta = align_up(o_cptr + ((size_t)NT + 1) * 4, 256);
-  size_t total = align_up(o_cmeta + std::max<size_t>((size_t)w->n_cells, 1) * sizeof(CellMeta), 256);
+  size_t o_umeta = align_up(o_cmeta + std::max<size_t>((size_t)w->n_cells, 1) * sizeof(CellMeta), 256);
+  size_t total = align_up(o_umeta + (size_t)NT * KS * 8, 256);
+  // dense per-(n-tile, K-step) lookup of the CSR cells: {quarter mask, first quarter index}
+  std::vector<int32_t> umeta((size_t)NT * KS * 2, 0);
+  for (int64_t t = 0; t < NT; ++t)
+    for (int32_t c = w->h_cell_ptr[(size_t)t]; c < w->h_cell_ptr[(size_t)t + 1]; ++c) {
+      const CellMeta& m = w->h_cell_meta[(size_t)c];
+      const size_t u = (size_t)t * KS + (size_t)(m.kstep_mask & 0xFFFFFF);
+      umeta[2 * u] = (m.kstep_mask >> 24) & 0xF;
+      umeta[2 * u + 1] = m.qoff;
+    }
   void* blob = nullptr;
   cudaError_t ce = cudaMalloc(&blob, total);
   if (ce != cudaSuccess) {
@@ -189,6 +204,7 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   if (w->n_cells)
     ok &= cudaMemcpyAsync(p + o_cmeta, w->h_cell_meta.data(), (size_t)w->n_cells * sizeof(CellMeta),
                           cudaMemcpyHostToDevice, stream) == cudaSuccess;
+  ok &= cudaMemcpyAsync(p + o_umeta, umeta.data(), umeta.size() * 4, cudaMemcpyHostToDevice, stream) == cudaSuccess;
   ok &= cudaStreamSynchronize(stream) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
@@ -204,6 +220,7 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   w->d_res = p + o_res;
   w->d_cell_ptr = (int32_t*)(p + o_cptr);
   w->d_cell_meta = (CellMeta*)(p + o_cmeta);
+  w->d_unit_meta = (int32_t*)(p + o_umeta);
   *out = w;
   return MQ_OK;
 }
@@ -416,7 +433,7 @@ extern "C" int mq_weights_export(const mq_weights* w, int8_t* qW, float* sW, int
         const uint8_t* src = res.data() + (size_t)outs[e].qidx[p] * QUARTER_BYTES;
         for (int row = 0; row < 64; ++row)
           for (int c = 0; c < 64; ++c)
-            dst[(size_t)(r * 64 + row) * bs + (size_t)(h * 64 + c)] = (int8_t)get_nibble(src[row * 32 + (c >> 1)], c & 1);
+            dst[(size_t)(r * 64 + row) * bs + (size_t)(h * 64 + c)] = (int8_t)get_nibble(src[quarter_offset(row, c)], c & 1);
       }
     }
   }
@@ -451,6 +468,7 @@ extern "C" int mq_weights_clone(const mq_weights* w, mq_weights** out, void* cud
   c->d_res = w->d_res + d;
   c->d_cell_ptr = (int32_t*)((uint8_t*)w->d_cell_ptr + d);
   c->d_cell_meta = (CellMeta*)((uint8_t*)w->d_cell_meta + d);
+  c->d_unit_meta = (int32_t*)((uint8_t*)w->d_unit_meta + d);
   *out = c;
   return MQ_OK;
 }

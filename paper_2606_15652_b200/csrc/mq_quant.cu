@@ -171,7 +171,7 @@ extern "C" int mq_set_option(const char* name, int64_t value) {
   if (!strcmp(name, "split_k")) {
     o.split_k = value;
   } else if (!strcmp(name, "token_tile")) {
-    if (value != 0 && value != 16 && value != 32 && value != 64 && value != 128 && value != 256)
+    if (value != 0 && value != 16 && value != 32 && value != 64 && value != 128)
       return MQ_ERR_INVALID_ARG;
     o.token_tile = value;
   } else if (!strcmp(name, "max_ctas")) {
