@@ -99,7 +99,18 @@ struct GemmParams {
   int gran;           // range boundaries are multiples of gran (1 = stream-K, KS = whole tiles)
   int M, N, KS, NT, TT;
   int y_bf16;
+#ifdef MQ_TRACE
+  long long* trace;  // [grid][64] clock64 stamps (development builds only)
+#endif
 };
+
+#ifdef MQ_TRACE
+#define MQ_STAMP(slot) do { p.trace[(size_t)blockIdx.x * 64 + (slot)] = clock64(); } while (0)
+#define MQ_STAMP_IF(cond, slot) do { if (cond) MQ_STAMP(slot); } while (0)
+#else
+#define MQ_STAMP(slot) do { } while (0)
+#define MQ_STAMP_IF(cond, slot) do { } while (0)
+#endif
 
 // first unit of CTA c's range
 __device__ __forceinline__ long long range_begin(const GemmParams& p, int c) {
@@ -166,6 +177,14 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   volatile int32_t* acc_flag = flag_slot + 1;  // [2]: did this accumulator stage receive residual MMAs?
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#ifdef MQ_TRACE
+  if (threadIdx.x == 0) {
+    unsigned long long gt;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
+    p.trace[(size_t)blockIdx.x * 64 + 12] = (long long)gt;
+    MQ_STAMP(0);
+  }
+#endif
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmap_a);
@@ -197,6 +216,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  MQ_STAMP_IF(threadIdx.x == 0, 1);
 
   const long long u_beg = range_begin(p, (int)blockIdx.x);
   const long long u_end = blockIdx.x + 1 == gridDim.x ? p.units : range_begin(p, (int)blockIdx.x + 1);
@@ -228,6 +248,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         const int c1 = __shfl_sync(0xffffffffu, l_c1, j);
         if (lane == 0) {
           mbar_wait(bar(B_EMPTY_P + ps), pphase ^ 1);
+          MQ_STAMP_IF(i0 + j == 0, 2);
+          MQ_STAMP_IF(i0 + j < 16, 48 + i0 + j);
+          MQ_STAMP_IF(i0 + j == n_units - 1, 3);
           meta_p[ps] = mask | (rseq << 8);
           const uint32_t dst = sP + ps * C::P_STAGE;
           mbar_arrive_expect_tx(bar(B_FULL_P + ps), C::P_STAGE);
@@ -273,6 +296,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         for (int ks = k0; ks < k1; ++ks) {
           mbar_wait(bar(B_FULL_U + as), aphase_u);
           tc_fence_after();
+#ifdef MQ_TRACE
+          { const int ui = (int)(g - (k1 - k0) - u_beg) + (ks - k0); MQ_STAMP_IF(ui == 0, 7); MQ_STAMP_IF(ui < 16, 32 + ui); }
+#endif
           const int meta = meta_u[as];
           const int mask = meta & 0xF;
           const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + as * A_COLS);
@@ -307,6 +333,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         acc_flag[a] = (int32_t)acc1_on;
         mbar_arrive(bar(B_TFULL + a));   // release: publishes acc_flag to the epilogue warps
         tc_commit(bar(B_TFULL + a));     // completes the phase when the MMAs have finished
+        MQ_STAMP(8);
       }
     }
   } else if (warp >= FIRST_UNPACK_WARP) {
@@ -320,6 +347,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     for (int i = gi; i < n_units; i += NUM_UNPACK_GROUPS) {
       const int ps = i % C::PSTAGES, as = i % C::ASTAGES;
       mbar_wait(bar(B_FULL_P + ps), (uint32_t)(i / C::PSTAGES) & 1);
+      MQ_STAMP_IF(i == 0 && gtid == 0, 4);
       const int meta = meta_p[ps];
       const uint32_t pw = sP + ps * C::P_STAGE;
       uint4 v[4];
@@ -347,6 +375,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) {
+        MQ_STAMP_IF(i == 0 && gtid == 0, 5);
+        MQ_STAMP_IF(gi == 0 && gtid == 0 && i < 32, 16 + i / 2);
+        MQ_STAMP_IF(gi == 0 && gtid == 0, 6);
         if (wq == 0) meta_u[as] = meta;
         mbar_arrive(bar(B_FULL_U + as));
         mbar_arrive(bar(B_EMPTY_P + ps));
@@ -419,6 +450,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 
       mbar_wait(bar(B_TFULL + a), aphase);
       tc_fence_after();
+      MQ_STAMP_IF(et == 0 && it == 1, 9);
       const bool has_res = acc_flag[a] != 0;  // acc1 is undefined when no residual MMA was issued
       const uint32_t t0addr = tmem_base + ((uint32_t)(lq * 32) << 16) + (uint32_t)(a * 2 * BT);
       const bool whole = (k0 == 0 && k1 == p.KS);
@@ -496,12 +528,15 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           if (et == 0) p.ws_cnt[tile] = 0;
         }
       }
+      MQ_STAMP_IF(et == 0, 10);
     }
   }
 
-  // teardown
+  // teardown (single-lane roles re-converge first: bar.sync must be reached warp-convergent)
+  __syncwarp();
   tc_fence_before();
   __syncthreads();
+  MQ_STAMP_IF(threadIdx.x == 0, 11);
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc(tmem_base, C::TMEM_COLS);
@@ -590,6 +625,11 @@ int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t
 
 }  // namespace
 
+#ifdef MQ_TRACE
+static long long* g_trace = nullptr;
+extern "C" void mq_debug_set_trace(long long* dev_buf) { g_trace = dev_buf; }
+#endif
+
 extern "C" size_t mq_gemm_workspace_bytes(const mq_weights* w, int64_t M) {
   if (!w || M <= 0) return 0;
   if (mq::check_device() != MQ_OK) return 0;
@@ -651,6 +691,10 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   gp.ws_cnt = (int32_t*)ws;
   gp.ws_flag = (int32_t*)(ws + pl.off_flag);
   gp.ws_part = (int32_t*)(ws + pl.off_part);
+#ifdef MQ_TRACE
+  gp.trace = g_trace;
+  if (!g_trace) return MQ_ERR_INVALID_ARG;
+#endif
 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   switch (pl.BT) {
