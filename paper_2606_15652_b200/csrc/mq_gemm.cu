@@ -11,20 +11,27 @@
 // into TENSOR MEMORY (tcgen05.st), from where tcgen05.mma reads it as its A operand.  Shared
 // memory therefore carries 0.5 B (TMA write) + 0.5 B (read) per weight instead of 3 B.
 //
-// Warp roles (448 threads, one persistent CTA per SM):
-//   warp 0      producer : TMA.  Per K-step one 8 KB 1-D bulk copy of the pre-tiled packed
-//                          base-weight tile + one 2-D tensor copy of the packed token tile
-//                          into the "packed" ring; for K-steps that own a residual cell also
-//                          the cell's present 2 KB quarters.
-//   warps 6-9, 10-13       two unpack groups, alternating K-steps: int4 -> int8 (value x16:
+// Granularity.  A K-STEP is 128 input channels (one 8 KB packed weight tile).  The single-thread
+// roles pay a fixed instruction cost per hand-off, so hand-offs are coarser than a K-step:
+//   P stage  = SK consecutive K-steps of one output tile: ONE 1-D bulk copy of SK*8 KB packed
+//              weights (the device layout keeps a tile's K-steps contiguous) + ONE 2-D tensor
+//              copy of the packed token tile [BT][SK*64 B];
+//   U stage  = UK K-steps unpacked: 32*UK TMEM columns (weights, MMA A operand) + UK token
+//              sub-tiles [BT][128 B] in the K-major SWIZZLE_128B layout (MMA B operand).
+// Decode (BT <= 32): SK = UK = 4 (32 KB per hand-off).  Prefill (BT = 128): SK = 2, UK = 1,
+// because two accumulators of 128 columns, the base one double-buffered, leave 128 TMEM
+// columns for the operand rings.
+//
+// Warp roles (448 threads, one persistent CTA per SM), control flow warp-uniform, single
+// instructions issued by an elected lane:
+//   warp 0      producer : TMA.  Also loads the residual metadata of its K-steps (one stage
+//                          ahead) and, for K-steps that own a residual cell, the cell's 2 KB quarters.
+//   warps 6-9, 10-13       two unpack groups, alternating U stages: int4 -> int8 (value x16:
 //                          nibble moved to the high half of a byte, two logic ops per 8
-//                          elements).  Weights -> TMEM (A operand), tokens -> shared memory in
-//                          the K-major SWIZZLE_128B layout (B operand).  Both operands use the
-//                          same within-32-byte element order, so dot products are unchanged;
-//                          accumulators are 256 x the true value.
-//   warp 1      MMA      : one thread issues tcgen05.mma kind::i8 (4 per K-step for the base,
-//                          2 per present k-half of a residual cell, re-using the SAME token
-//                          tile) and commits to the rings' empty barriers.
+//                          elements; both operands use the same element order inside 32 bytes, so
+//                          dot products are unchanged and accumulators are 256 x the true value).
+//   warp 1      MMA      : tcgen05.mma kind::i8, A from TMEM: 4 per K-step for the base, 2 per
+//                          present k-half of a residual cell re-using the SAME token tile.
 //   warps 2-5   epilogue : tcgen05.ld both accumulators, y = s_a * (s_w*acc0 + s_r*acc1) in
 //                          fp32, bf16/fp16 store.
 //
@@ -52,33 +59,50 @@ constexpr int FIRST_EPI_WARP = 2;
 constexpr int FIRST_UNPACK_WARP = 6;
 constexpr int NUM_UNPACK_GROUPS = 2;
 constexpr int NUM_THREADS = 32 * (FIRST_UNPACK_WARP + 4 * NUM_UNPACK_GROUPS);  // 448
-constexpr int RSTAGES = 2;
-constexpr int A_COLS = BK / 4;               // 32 TMEM columns hold 128 int8 per lane
-constexpr int RP_BYTES = 4 * QUARTER_BYTES;  // 8 KB packed residual cell slot
+constexpr int A_COLS = BK / 4;               // 32 TMEM columns hold 128 int8 per lane (one K-step)
+
+// per-K-step metadata word handed from the producer to the unpack groups and the MMA warp
+constexpr int META_VALID = (int)0x80000000;  // the K-step exists (a P stage may hold fewer than SK)
+constexpr int META_FIRST = 1 << 30;          // first K-step of this CTA's segment of a tile
+constexpr int META_LAST = 1 << 29;           // last K-step of the segment: accumulators complete
+// bits 0-3: residual quarter mask; bits 4-11: sequence number of the residual cell in this CTA
+// (mod 256); bits 12-27: sequence number of the cell's first stored quarter (mod 65536)
 
 template <int BT>
 struct Cfg {
-  static constexpr int PSTAGES = BT <= 32 ? 10 : (BT == 64 ? 8 : 6);
-  static constexpr int ASTAGES = BT <= 64 ? 4 : 3;
-  static constexpr int P_TOK = BT * (BK / 2);
-  static constexpr int P_STAGE = TILE_BYTES + P_TOK;
-  static constexpr int U_TOK = BT * BK;
-  static constexpr int ACC_STAGES = BT <= 64 ? 2 : 1;
-  static constexpr int ACC_COLS = ACC_STAGES * 2 * BT;
-  static constexpr int A_COL0 = ACC_COLS;
-  static constexpr int R_COL0 = A_COL0 + ASTAGES * A_COLS;
+  static constexpr int SK = BT <= 32 ? 4 : 2;                    // K-steps per P stage
+  static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // K-steps per U stage (item)
+  static constexpr int IPS = SK / UK;                            // items per P stage
+  static constexpr int PSTAGES = BT <= 32 ? 4 : (BT == 64 ? 6 : 4);
+  static constexpr int USTAGES = BT <= 64 ? 2 : 3;
+  static constexpr int RSTAGES = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // unpacked residual cells (TMEM)
+  static constexpr int NQ = BT == 16 ? 16 : 8;                        // packed residual quarter slots (2 KB each)
+  static constexpr int ACC0_STAGES = 2;
+  static constexpr int ACC1_STAGES = BT <= 64 ? 2 : 1;
+  static constexpr int P_W = SK * TILE_BYTES;
+  static constexpr int P_TOK = BT * SK * (BK / 2);
+  static constexpr int P_STAGE = P_W + P_TOK;
+  static constexpr int U_SUB = BT * BK;                          // one int8 token sub-tile
+  static constexpr int U_STAGE = UK * U_SUB;
+  // tensor memory columns
+  static constexpr int ACC1_COL0 = ACC0_STAGES * BT;
+  static constexpr int A_COL0 = ACC1_COL0 + ACC1_STAGES * BT;
+  static constexpr int R_COL0 = A_COL0 + USTAGES * UK * A_COLS;
   static constexpr int TMEM_NEED = R_COL0 + RSTAGES * A_COLS;
   static constexpr int TMEM_COLS = TMEM_NEED <= 32 ? 32 : (TMEM_NEED <= 64 ? 64 : (TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512)));
   static_assert(TMEM_NEED <= 512, "tensor memory budget");
   // shared memory map (offsets from a 1024-aligned base)
   static constexpr int OFF_U = 0;
-  static constexpr int OFF_P = OFF_U + ASTAGES * U_TOK;
+  static constexpr int OFF_P = OFF_U + USTAGES * U_STAGE;
   static constexpr int OFF_RP = OFF_P + PSTAGES * P_STAGE;
-  static constexpr int OFF_BAR = OFF_RP + RSTAGES * RP_BYTES;
-  static constexpr int NUM_BARS = 2 * PSTAGES + 2 * ASTAGES + 4 * RSTAGES + 4;
+  static constexpr int OFF_BAR = OFF_RP + NQ * QUARTER_BYTES;
+  static constexpr int NUM_BARS = 2 * PSTAGES + 2 * USTAGES + 2 * NQ + 2 * RSTAGES + 2 + ACC0_STAGES + ACC1_STAGES;
   static constexpr int OFF_META = OFF_BAR + NUM_BARS * 8;
-  static constexpr int OFF_END = OFF_META + (PSTAGES + ASTAGES + 8) * 4;
+  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 8;
+  static constexpr int OFF_END = OFF_META + META_WORDS * 4;
   static constexpr int SMEM_BYTES = OFF_END + 1024;  // slack for the 1024-byte alignment
+  static_assert(SMEM_BYTES <= 232448, "shared memory budget");
+  static_assert(P_STAGE % 1024 == 0 && U_SUB % 1024 == 0, "swizzle atoms need 1024-byte alignment");
 };
 
 struct GemmParams {
@@ -95,8 +119,9 @@ struct GemmParams {
   int32_t* ws_flag;   // [grid][2] did this partial receive residual MMAs?
   int32_t* ws_part;   // [grid][2 slots][2 accs][BT][128] int32 partial tiles
   int64_t ldy;
-  long long units;    // NT*TT*KS
-  int gran;           // range boundaries are multiples of gran (1 = stream-K, KS = whole tiles)
+  uint32_t units;     // NT*TT*KS (< 2^31, checked by the host)
+  uint32_t gran;      // range boundaries are multiples of gran (1 = stream-K, KS = whole tiles)
+  uint32_t upg_q, upg_r;  // (units / gran) = upg_q * gridDim.x + upg_r
   int M, N, KS, NT, TT;
   int y_bf16;
 #ifdef MQ_TRACE
@@ -112,16 +137,63 @@ struct GemmParams {
 #define MQ_STAMP_IF(cond, slot) do { } while (0)
 #endif
 
-// first unit of CTA c's range
-__device__ __forceinline__ long long range_begin(const GemmParams& p, int c) {
-  return (long long)p.gran * (((p.units / p.gran) * (long long)c) / (long long)gridDim.x);
+// All index arithmetic is 32-bit unsigned: a 64-bit division costs a single-thread role ~400 cycles.
+// first unit of CTA c's range: gran * floor((units / gran) * c / grid)
+__device__ __forceinline__ uint32_t range_begin(const GemmParams& p, uint32_t c) {
+  return p.gran * (p.upg_q * c + (p.upg_r * c) / gridDim.x);
 }
 // the CTA whose range holds unit x
-__device__ __forceinline__ int owner_of(const GemmParams& p, long long x) {
-  int c = (int)((x * (long long)gridDim.x) / p.units);
-  while (c + 1 < (int)gridDim.x && range_begin(p, c + 1) <= x) ++c;
-  while (c > 0 && range_begin(p, c) > x) --c;
+__device__ __forceinline__ int owner_of(const GemmParams& p, uint32_t x) {
+  int c = (int)((float)(x / p.gran) * (float)gridDim.x / (float)(p.upg_q * gridDim.x + p.upg_r));
+  c = max(0, min(c, (int)gridDim.x - 1));
+  while (c + 1 < (int)gridDim.x && range_begin(p, (uint32_t)c + 1) <= x) ++c;
+  while (c > 0 && range_begin(p, (uint32_t)c) > x) --c;
   return c;
+}
+
+// One P stage of a CTA's work: up to SK consecutive K-steps of one (n-tile, token-tile).
+struct Stage {
+  int nt, tt, ks, nks;
+  bool first, last;   // first / last stage of this CTA's segment of the tile
+};
+// Walks a CTA's unit range [g, u_end) segment by segment (segment = this CTA's K-steps of one
+// tile) and, inside a segment, in P stages of up to SK K-steps.
+struct StageIter {
+  uint32_t g, u_end;
+  int KS, TT, k1, ks, nt, tt;
+  __device__ StageIter(uint32_t u_beg, uint32_t u_end_, int KS_, int TT_)
+      : g(u_beg), u_end(u_end_), KS(KS_), TT(TT_), k1(0), ks(0), nt(0), tt(0) {}
+  template <int SK>
+  __device__ bool next(Stage& s) {
+    s.first = false;
+    if (ks >= k1) {
+      if (g >= u_end) return false;
+      const uint32_t tile = g / (uint32_t)KS;
+      ks = (int)(g - tile * (uint32_t)KS);
+      k1 = (int)min((uint32_t)KS, (uint32_t)ks + (u_end - g));
+      g += (uint32_t)(k1 - ks);
+      nt = (int)(tile / (uint32_t)TT);
+      tt = (int)(tile - (uint32_t)nt * (uint32_t)TT);
+      s.first = true;
+    }
+    s.nt = nt;
+    s.tt = tt;
+    s.ks = ks;
+    s.nks = min(SK, k1 - ks);
+    ks += s.nks;
+    s.last = ks >= k1;
+    return true;
+  }
+};
+
+// number of P stages of the range [u_beg, u_end): closed form of StageIter
+__device__ __forceinline__ int count_stages(uint32_t u_beg, uint32_t u_end, uint32_t KS, uint32_t SK) {
+  if (u_end <= u_beg) return 0;
+  const uint32_t n = u_end - u_beg;
+  const uint32_t head = KS - u_beg % KS;
+  if (n <= head) return (int)((n + SK - 1) / SK);
+  const uint32_t rem = n - head;
+  return (int)((head + SK - 1) / SK + (rem / KS) * ((KS + SK - 1) / SK) + (rem % KS + SK - 1) / SK);
 }
 
 // 32 packed nibbles (16 B) -> 32 int8 = 16 x value.  Output element order inside the 32
@@ -146,6 +218,14 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
 __device__ __forceinline__ void sts128(uint32_t addr, const uint32_t* v) {
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
 }
+__device__ __forceinline__ int lds32(uint32_t addr) {
+  int v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, int v) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
 
 template <bool BF16>
 __device__ __forceinline__ void store_y(void* Y, size_t o, float y) {
@@ -159,22 +239,25 @@ template <int BT>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   using C = Cfg<BT>;
+  constexpr int SK = C::SK, UK = C::UK, IPS = C::IPS;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
 
   const uint32_t sU = smem_base + C::OFF_U, sP = smem_base + C::OFF_P, sRP = smem_base + C::OFF_RP,
                  sBar = smem_base + C::OFF_BAR;
   auto bar = [&](int i) { return sBar + 8u * (uint32_t)i; };
-  constexpr int B_FULL_P = 0, B_EMPTY_P = C::PSTAGES, B_FULL_U = 2 * C::PSTAGES, B_EMPTY_U = B_FULL_U + C::ASTAGES,
-                B_FULL_RP = B_EMPTY_U + C::ASTAGES, B_EMPTY_RP = B_FULL_RP + RSTAGES, B_FULL_RU = B_EMPTY_RP + RSTAGES,
-                B_EMPTY_RU = B_FULL_RU + RSTAGES, B_TFULL = B_EMPTY_RU + RSTAGES, B_TEMPTY = B_TFULL + 2;
-  // meta words: bits 0-3 quarter mask, bits 8.. sequence number of the residual cell in this CTA
-  volatile int32_t* meta_p = reinterpret_cast<volatile int32_t*>(smem_gen + C::OFF_META);
-  volatile int32_t* meta_u = meta_p + C::PSTAGES;
-  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(meta_u + C::ASTAGES);
-  volatile int32_t* flag_slot = reinterpret_cast<volatile int32_t*>(tmem_slot + 1);
-  volatile int32_t* acc_flag = flag_slot + 1;  // [2]: did this accumulator stage receive residual MMAs?
+  constexpr int B_FULL_P = 0, B_EMPTY_P = C::PSTAGES, B_FULL_U = 2 * C::PSTAGES, B_EMPTY_U = B_FULL_U + C::USTAGES,
+                B_FULL_Q = B_EMPTY_U + C::USTAGES, B_EMPTY_Q = B_FULL_Q + C::NQ,
+                B_FULL_RU = B_EMPTY_Q + C::NQ, B_EMPTY_RU = B_FULL_RU + C::RSTAGES,
+                B_TFULL = B_EMPTY_RU + C::RSTAGES, B_A0E = B_TFULL + 2, B_A1E = B_A0E + C::ACC0_STAGES;
+  static_assert(B_A1E + C::ACC1_STAGES == C::NUM_BARS, "barrier map");
+  // small shared words: metadata rings, TMEM base, fix-up flags
+  const uint32_t sMetaP = smem_base + C::OFF_META;              // [PSTAGES][SK]
+  const uint32_t sMetaU = sMetaP + 4u * C::PSTAGES * SK;        // [USTAGES][UK]
+  const uint32_t sMisc = sMetaU + 4u * C::USTAGES * UK;         // [0] tmem base, [1..5] fix-up, [6..7] acc_flag
+  volatile int32_t* misc = reinterpret_cast<volatile int32_t*>(smem_raw + (sMisc - smem_u32(smem_raw)));
+  volatile int32_t* flag_slot = misc + 1;
+  volatile int32_t* acc_flag = misc + 6;  // [2]: did this base-accumulator stage's segment get residual MMAs?
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #ifdef MQ_TRACE
@@ -189,229 +272,310 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmap_a);
     for (int i = 0; i < C::PSTAGES; ++i) {
-      mbar_init(bar(B_FULL_P + i), 1);
-      mbar_init(bar(B_EMPTY_P + i), 4);
+      mbar_init(bar(B_FULL_P + i), 2);          // TMA issue (expect_tx) + metadata published
+      mbar_init(bar(B_EMPTY_P + i), 4 * IPS);   // one arrival per unpack warp per item
     }
-    for (int i = 0; i < C::ASTAGES; ++i) {
+    for (int i = 0; i < C::USTAGES; ++i) {
       mbar_init(bar(B_FULL_U + i), 4);
       mbar_init(bar(B_EMPTY_U + i), 1);
     }
-    for (int i = 0; i < RSTAGES; ++i) {
-      mbar_init(bar(B_FULL_RP + i), 1);
-      mbar_init(bar(B_EMPTY_RP + i), 4);
+    for (int i = 0; i < C::NQ; ++i) {
+      mbar_init(bar(B_FULL_Q + i), 1);
+      mbar_init(bar(B_EMPTY_Q + i), 2);         // the two unpack warps that own the quarter's 64 rows
+    }
+    for (int i = 0; i < C::RSTAGES; ++i) {
       mbar_init(bar(B_FULL_RU + i), 4);
       mbar_init(bar(B_EMPTY_RU + i), 1);
     }
-    for (int i = 0; i < 2; ++i) {
-      mbar_init(bar(B_TFULL + i), 2);
-      mbar_init(bar(B_TEMPTY + i), 4);
-    }
+    for (int i = 0; i < 2; ++i) mbar_init(bar(B_TFULL + i), 2);
+    for (int i = 0; i < C::ACC0_STAGES; ++i) mbar_init(bar(B_A0E + i), 4);
+    for (int i = 0; i < C::ACC1_STAGES; ++i) mbar_init(bar(B_A1E + i), 4);
     fence_mbar_init();
   }
   if (warp == 1) {
-    tmem_alloc(smem_u32((const void*)tmem_slot), C::TMEM_COLS);
+    tmem_alloc(sMisc, C::TMEM_COLS);
     tmem_relinquish();
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_base = (uint32_t)misc[0];
   MQ_STAMP_IF(threadIdx.x == 0, 1);
 
-  const long long u_beg = range_begin(p, (int)blockIdx.x);
-  const long long u_end = blockIdx.x + 1 == gridDim.x ? p.units : range_begin(p, (int)blockIdx.x + 1);
-  const int n_units = (int)(u_end - u_beg);
+  const uint32_t u_beg = range_begin(p, blockIdx.x);
+  const uint32_t u_end = blockIdx.x + 1 == gridDim.x ? p.units : range_begin(p, blockIdx.x + 1);
+  const int n_stages = count_stages(u_beg, u_end, (uint32_t)p.KS, SK);
+  const int n_items = n_stages * IPS;
 
   if (warp == 0) {
-    // ===================== producer (TMA) =====================
-    int ps = 0, rseq = 0;
+    // ===================== producer (TMA); all lanes run the loop, one elected lane issues =====================
+    StageIter it(u_beg, u_end, p.KS, p.TT);
+    Stage cur, nxt;
+    auto load_meta = [&](const Stage& s) {
+      // lane j < nks: {quarter mask, first quarter} of the stage's K-step j
+      return lane < s.nks ? __ldg(p.unit_meta + (size_t)s.nt * p.KS + s.ks + lane) : make_int2(0, 0);
+    };
+    bool have = it.next<SK>(cur);
+    int2 um = make_int2(0, 0);
+    if (have) um = load_meta(cur);
+    int ps = 0, rseq = 0, qseq = 0, si = 0;
     uint32_t pphase = 0;
-    for (int i0 = 0; i0 < n_units; i0 += 32) {
-      // each lane looks up one unit of the batch: tile = nt * TT + tt, unit = tile * KS + ks
-      int2 um = make_int2(0, 0);
-      int l_wi = 0, l_c0 = 0, l_c1 = 0;
-      if (i0 + lane < n_units) {
-        const long long u = u_beg + i0 + lane;
-        const long long tile = u / p.KS;
-        const int ks = (int)(u - tile * p.KS);
-        l_wi = (int)(tile / p.TT) * p.KS + ks;     // index of the base tile and of unit_meta
-        l_c0 = ks * (BK / 2);                      // tensor-map coordinates of the token tile
-        l_c1 = (int)(tile % p.TT) * BT;
-        um = __ldg(p.unit_meta + l_wi);
+    while (have) {
+      const bool have_n = it.next<SK>(nxt);
+      int2 um_n = make_int2(0, 0);
+      if (have_n) um_n = load_meta(nxt);   // one stage ahead: its latency hides behind this stage's issue
+      mbar_wait(bar(B_EMPTY_P + ps), pphase ^ 1);
+      __syncwarp();
+      const uint32_t dst = sP + ps * C::P_STAGE;
+      if (elect_one()) {
+        MQ_STAMP_IF(si == 0, 2);
+        MQ_STAMP_IF(si < 16, 48 + si);
+        MQ_STAMP_IF(si == n_stages - 1, 3);
+        const uint32_t fb = bar(B_FULL_P + ps);
+        mbar_arrive_expect_tx(fb, (uint32_t)cur.nks * (TILE_BYTES + BT * (BK / 2)));
+        tma_load_1d(dst, p.base + ((size_t)cur.nt * p.KS + cur.ks) * TILE_BYTES, (uint32_t)cur.nks * TILE_BYTES, fb);
+        for (int j = 0; j < cur.nks; ++j)
+          tma_load_2d(dst + C::P_W + j * (BT * (BK / 2)), &tmap_a, (cur.ks + j) * (BK / 2), cur.tt * BT, fb);
       }
-      const int nb = min(32, n_units - i0);
-      for (int j = 0; j < nb; ++j) {
-        const int mask = __shfl_sync(0xffffffffu, um.x, j);
-        const int qoff = __shfl_sync(0xffffffffu, um.y, j);
-        const int wi = __shfl_sync(0xffffffffu, l_wi, j);
-        const int c0 = __shfl_sync(0xffffffffu, l_c0, j);
-        const int c1 = __shfl_sync(0xffffffffu, l_c1, j);
-        if (lane == 0) {
-          mbar_wait(bar(B_EMPTY_P + ps), pphase ^ 1);
-          MQ_STAMP_IF(i0 + j == 0, 2);
-          MQ_STAMP_IF(i0 + j < 16, 48 + i0 + j);
-          MQ_STAMP_IF(i0 + j == n_units - 1, 3);
-          meta_p[ps] = mask | (rseq << 8);
-          const uint32_t dst = sP + ps * C::P_STAGE;
-          mbar_arrive_expect_tx(bar(B_FULL_P + ps), C::P_STAGE);
-          tma_load_1d(dst, p.base + (size_t)wi * TILE_BYTES, TILE_BYTES, bar(B_FULL_P + ps));
-          tma_load_2d(dst + TILE_BYTES, &tmap_a, c0, c1, bar(B_FULL_P + ps));
-          if (mask) {
-            const int rs = rseq % RSTAGES;
-            mbar_wait(bar(B_EMPTY_RP + rs), (((uint32_t)rseq / RSTAGES) & 1) ^ 1);
-            mbar_arrive_expect_tx(bar(B_FULL_RP + rs), (uint32_t)__popc(mask) * QUARTER_BYTES);
-            const uint8_t* rsrc = p.res + (size_t)qoff * QUARTER_BYTES;
-            for (int q = 0; q < 4; ++q)
-              if (mask & (1 << q)) {
-                tma_load_1d(sRP + rs * RP_BYTES + q * QUARTER_BYTES, rsrc, QUARTER_BYTES, bar(B_FULL_RP + rs));
-                rsrc += QUARTER_BYTES;
-              }
+      // metadata words of the stage (lane j writes K-step j), then the second arrival publishes them.
+      // The empty asm pins the first USE of the prefetched metadata behind the TMA issue above.
+      asm volatile("" : "+r"(um.x), "+r"(um.y));
+      const int mask = lane < cur.nks ? (um.x & 0xF) : 0;
+      const uint32_t nz = __ballot_sync(0xffffffffu, mask != 0);
+      // quarters stored by the cells of the lanes below this one (inclusive scan of popc(mask))
+      int qbefore = __popc(mask);
+#pragma unroll
+      for (int d = 1; d < SK; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, qbefore, d);
+        if (lane >= d) qbefore += o;
+      }
+      const int qtotal = __shfl_sync(0xffffffffu, qbefore, SK - 1);
+      qbefore -= __popc(mask);
+      if (lane < SK) {
+        int word = 0;
+        if (lane < cur.nks) {
+          word = META_VALID | mask | (((rseq + __popc(nz & ((1u << lane) - 1u))) & 0xFF) << 4) |
+                 (((qseq + qbefore) & 0xFFFF) << 12);
+          if (cur.first && lane == 0) word |= META_FIRST;
+          if (cur.last && lane == cur.nks - 1) word |= META_LAST;
+        }
+        sts32(sMetaP + 4u * (uint32_t)(ps * SK + lane), word);
+      }
+      __syncwarp();
+      if (elect_one()) mbar_arrive(bar(B_FULL_P + ps));
+      // residual cells of the stage: each present quarter is one 2 KB bulk copy into the quarter ring
+      uint32_t todo = nz;
+      while (todo) {
+        const int j = __ffs((int)todo) - 1;
+        todo &= todo - 1;
+        const int m = __shfl_sync(0xffffffffu, mask, j);
+        const uint8_t* rsrc = p.res + (size_t)__shfl_sync(0xffffffffu, um.y, j) * QUARTER_BYTES;
+        for (int q = 0; q < __popc(m); ++q) {
+          const int slot = (qseq + q) % C::NQ;
+          mbar_wait(bar(B_EMPTY_Q + slot), (((uint32_t)(qseq + q) / C::NQ) & 1) ^ 1);
+          __syncwarp();
+          if (elect_one()) {
+            const uint32_t rb = bar(B_FULL_Q + slot);
+            mbar_arrive_expect_tx(rb, QUARTER_BYTES);
+            tma_load_1d(sRP + slot * QUARTER_BYTES, rsrc + (size_t)q * QUARTER_BYTES, QUARTER_BYTES, rb);
           }
         }
-        if (mask) ++rseq;
-        if (++ps == C::PSTAGES) {
-          ps = 0;
-          pphase ^= 1;
-        }
+        qseq += __popc(m);
       }
+      rseq += __popc(nz);
+      (void)qtotal;
+      if (++ps == C::PSTAGES) {
+        ps = 0;
+        pphase ^= 1;
+      }
+      ++si;
+      cur = nxt;
+      um = um_n;
+      have = have_n;
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    if (lane == 0) {
-      constexpr uint32_t IDESC = make_idesc_i8(BN, BT);
-      int as = 0, it = 0;
-      uint32_t aphase_u = 0;
-      long long g = u_beg;
-      while (g < u_end) {
-        const int k0 = (int)(g % p.KS);
-        const int k1 = (int)min((long long)p.KS, k0 + (u_end - g));
-        g += k1 - k0;
-        const int a = C::ACC_STAGES == 2 ? (it & 1) : 0;
-        const uint32_t aphase = C::ACC_STAGES == 2 ? ((it >> 1) & 1) : (it & 1);
-        ++it;
-        mbar_wait(bar(B_TEMPTY + a), aphase ^ 1);
-        tc_fence_after();
-        const uint32_t d0 = tmem_base + (uint32_t)(a * 2 * BT), d1 = d0 + BT;
-        uint32_t acc0_on = 0, acc1_on = 0;
-        for (int ks = k0; ks < k1; ++ks) {
-          mbar_wait(bar(B_FULL_U + as), aphase_u);
-          tc_fence_after();
-#ifdef MQ_TRACE
-          { const int ui = (int)(g - (k1 - k0) - u_beg) + (ks - k0); MQ_STAMP_IF(ui == 0, 7); MQ_STAMP_IF(ui < 16, 32 + ui); }
-#endif
-          const int meta = meta_u[as];
-          const int mask = meta & 0xF;
-          const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + as * A_COLS);
-          const uint64_t dt = make_desc_sw128(sU + as * C::U_TOK);
+    // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
+    constexpr uint32_t IDESC = make_idesc_i8(BN, BT);
+    int seg = 0;                 // index of the current segment (selects the accumulator stages)
+    uint32_t acc0_on = 0, acc1_on = 0;
+    uint32_t d0 = 0, d1 = 0;
+    int a0s = 0, a1s = 0;
+    for (int item = 0; item < n_items; ++item) {
+      const int us = item % C::USTAGES;
+      mbar_wait(bar(B_FULL_U + us), ((uint32_t)item / C::USTAGES) & 1);
+      tc_fence_after();
+      __syncwarp();
+      MQ_STAMP_IF(item == 0 && lane == 0, 7);
+      MQ_STAMP_IF(item < 16 && lane == 0, 32 + item);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, acc0_on);
-            acc0_on = 1;
-          }
-          if (mask) {
-            const int rseq = meta >> 8, rs = rseq % RSTAGES;
-            mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / RSTAGES) & 1);
+      for (int j = 0; j < UK; ++j) {
+        const int m = lds32(sMetaU + 4u * (uint32_t)(us * UK + j));
+        if (!(m & META_VALID)) break;   // the valid K-steps of an item are a prefix
+        if (m & META_FIRST) {
+          a0s = seg % C::ACC0_STAGES;
+          a1s = seg % C::ACC1_STAGES;
+          mbar_wait(bar(B_A0E + a0s), (((uint32_t)seg / C::ACC0_STAGES) & 1) ^ 1);
+          tc_fence_after();
+          d0 = tmem_base + (uint32_t)(a0s * BT);
+          d1 = tmem_base + (uint32_t)(C::ACC1_COL0 + a1s * BT);
+          acc0_on = 0;
+          acc1_on = 0;
+        }
+        const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + (us * UK + j) * A_COLS);
+        const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE + j * C::U_SUB);
+        if (elect_one()) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? acc0_on : 1u);
+        }
+        acc0_on = 1;
+        const int mask = m & 0xF;
+        if (mask) {
+          if (!acc1_on) {
+            // first residual MMA of the segment: the epilogue must have drained this acc1 stage
+            mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
             tc_fence_after();
-            const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + rs * A_COLS);
+          }
+          const int rseq = (m >> 4) & 0xFF, rs = rseq % C::RSTAGES;
+          mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RSTAGES) & 1);
+          tc_fence_after();
+          __syncwarp();
+          const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + rs * A_COLS);
+          if (elect_one()) {
+            uint32_t on = acc1_on;
 #pragma unroll
             for (int h = 0; h < 2; ++h)
               if (mask & (3 << (2 * h))) {
 #pragma unroll
                 for (int k = 2 * h; k < 2 * h + 2; ++k) {
-                  mma_i8_ts(d1, rt + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, acc1_on);
-                  acc1_on = 1;
+                  mma_i8_ts(d1, rt + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
+                  on = 1;
                 }
               }
             tc_commit(bar(B_EMPTY_RU + rs));
           }
-          tc_commit(bar(B_EMPTY_U + as));
-          if (++as == C::ASTAGES) {
-            as = 0;
-            aphase_u ^= 1;
-          }
+          acc1_on = 1;
         }
-        acc_flag[a] = (int32_t)acc1_on;
-        mbar_arrive(bar(B_TFULL + a));   // release: publishes acc_flag to the epilogue warps
-        tc_commit(bar(B_TFULL + a));     // completes the phase when the MMAs have finished
-        MQ_STAMP(8);
+        if (m & META_LAST) {
+          if (!acc1_on) {
+            // keep the acc1 ring's phases in step: the epilogue releases it once per segment
+            mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
+          }
+          __syncwarp();
+          if (elect_one()) {
+            acc_flag[a0s] = (int32_t)acc1_on;
+            mbar_arrive(bar(B_TFULL + a0s));   // release: publishes acc_flag to the epilogue warps
+            tc_commit(bar(B_TFULL + a0s));     // completes the phase when the MMAs have finished
+            MQ_STAMP(8);
+          }
+          ++seg;
+        }
       }
+      __syncwarp();
+      if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
     }
   } else if (warp >= FIRST_UNPACK_WARP) {
     // ============ unpack groups: int4 -> int8 (x16); weights -> TMEM, tokens -> smem ============
-    const int gi = (warp - FIRST_UNPACK_WARP) >> 2;               // group: takes units i = gi (mod 2)
+    const int gi = (warp - FIRST_UNPACK_WARP) >> 2;               // group: takes items i = gi (mod 2)
     const int wq = warp & 3;                                      // TMEM lane quadrant of this warp
     const uint32_t row = (uint32_t)(wq * 32 + lane);              // output channel inside the tile
     const uint32_t gtid = (uint32_t)(((warp - FIRST_UNPACK_WARP) & 3) * 32 + lane);
     const uint32_t lane_addr = tmem_base + ((uint32_t)(wq * 32) << 16);
     const int rhalf = wq >> 1;                                    // row half of a residual cell
-    for (int i = gi; i < n_units; i += NUM_UNPACK_GROUPS) {
-      const int ps = i % C::PSTAGES, as = i % C::ASTAGES;
-      mbar_wait(bar(B_FULL_P + ps), (uint32_t)(i / C::PSTAGES) & 1);
-      MQ_STAMP_IF(i == 0 && gtid == 0, 4);
-      const int meta = meta_p[ps];
-      const uint32_t pw = sP + ps * C::P_STAGE;
+    for (int item = gi; item < n_items; item += NUM_UNPACK_GROUPS) {
+      const int stage = item / IPS, sub = item - stage * IPS;
+      const int ps = stage % C::PSTAGES, us = item % C::USTAGES;
+      mbar_wait(bar(B_FULL_P + ps), ((uint32_t)stage / C::PSTAGES) & 1);
+      MQ_STAMP_IF(item == 0 && gtid == 0, 4);
+      int mw[UK];
+#pragma unroll
+      for (int j = 0; j < UK; ++j) mw[j] = lds32(sMetaP + 4u * (uint32_t)(ps * SK + sub * UK + j));
+      const uint32_t pw = sP + ps * C::P_STAGE + sub * UK * TILE_BYTES;
+      // the first K-step's packed weights are fetched before the U stage is known to be free
       uint4 v[4];
 #pragma unroll
       for (int c = 0; c < 4; ++c) v[c] = lds128(pw + c * (BN * 16) + row * 16);
-      mbar_wait(bar(B_EMPTY_U + as), ((uint32_t)(i / C::ASTAGES) & 1) ^ 1);
+      mbar_wait(bar(B_EMPTY_U + us), (((uint32_t)item / C::USTAGES) & 1) ^ 1);
       tc_fence_after();
-      uint32_t o[32];
+      int nk = 0;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) unpack16(v[c], o + 8 * c);
-      tmem_st32(lane_addr + (uint32_t)(C::A_COL0 + as * A_COLS), o);
-      // tokens: packed [BT][64 B] row-major -> [BT][128 B] K-major SWIZZLE_128B
-      const uint32_t pt = pw + TILE_BYTES, ut = sU + as * C::U_TOK;
+      for (int j = 0; j < UK; ++j) {
+        if (mw[j] & META_VALID) {
+          ++nk;
+          uint32_t o[32];
 #pragma unroll
-      for (uint32_t idx = gtid; idx < (uint32_t)(BT * 4); idx += 128) {
-        const uint32_t t = idx >> 2, j = idx & 3;
-        const uint4 tv = lds128(pt + idx * 16);
-        uint32_t w8[8];
-        unpack16(tv, w8);
-        sts128(ut + t * 128 + (((2 * j) ^ (t & 7)) << 4), w8);
-        sts128(ut + t * 128 + (((2 * j + 1) ^ (t & 7)) << 4), w8 + 4);
+          for (int c = 0; c < 4; ++c) unpack16(v[c], o + 8 * c);
+          if (j + 1 < UK && (mw[j + 1] & META_VALID)) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) v[c] = lds128(pw + (j + 1) * TILE_BYTES + c * (BN * 16) + row * 16);
+          }
+          tmem_st32(lane_addr + (uint32_t)(C::A_COL0 + (us * UK + j) * A_COLS), o);
+        }
+      }
+      // tokens: packed [UK][BT][64 B] -> UK sub-tiles [BT][128 B] K-major SWIZZLE_128B
+      const uint32_t pt = sP + ps * C::P_STAGE + C::P_W + sub * UK * (BT * (BK / 2)), ut = sU + us * C::U_STAGE;
+#pragma unroll
+      for (uint32_t idx = gtid; idx < (uint32_t)(UK * BT * 4); idx += 128) {
+        const uint32_t jj = idx / (BT * 4), rem = idx % (BT * 4), t = rem >> 2, c = rem & 3;
+        if ((int)jj < nk) {
+          const uint4 tv = lds128(pt + idx * 16);
+          uint32_t w8[8];
+          unpack16(tv, w8);
+          const uint32_t dst = ut + jj * C::U_SUB + t * 128;
+          sts128(dst + (((2 * c) ^ (t & 7)) << 4), w8);
+          sts128(dst + (((2 * c + 1) ^ (t & 7)) << 4), w8 + 4);
+        }
       }
       tmem_st_wait();
       tc_fence_before();
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) {
-        MQ_STAMP_IF(i == 0 && gtid == 0, 5);
-        MQ_STAMP_IF(gi == 0 && gtid == 0 && i < 32, 16 + i / 2);
+        MQ_STAMP_IF(item == 0 && gtid == 0, 5);
+        MQ_STAMP_IF(gi == 0 && gtid == 0 && item < 32, 16 + item / 2);
         MQ_STAMP_IF(gi == 0 && gtid == 0, 6);
-        if (wq == 0) meta_u[as] = meta;
-        mbar_arrive(bar(B_FULL_U + as));
+        if (wq == 0) {
+#pragma unroll
+          for (int j = 0; j < UK; ++j) sts32(sMetaU + 4u * (uint32_t)(us * UK + j), mw[j]);
+        }
+        mbar_arrive(bar(B_FULL_U + us));
         mbar_arrive(bar(B_EMPTY_P + ps));
       }
-      const int mask = meta & 0xF;
-      if (mask) {
-        const int rseq = meta >> 8, rs = rseq % RSTAGES;
-        const uint32_t rphase = ((uint32_t)rseq / RSTAGES) & 1;
-        mbar_wait(bar(B_FULL_RP + rs), rphase);
-        mbar_wait(bar(B_EMPTY_RU + rs), rphase ^ 1);
-        tc_fence_after();
-        const uint32_t rp = sRP + rs * RP_BYTES;
+      // residual cells of this item's K-steps
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          if (!(mask & (3 << (2 * h)))) continue;   // k-half without any block: never read by the MMA
-          const int q = 2 * h + rhalf;
-          uint32_t ro[16];
-          if (mask & (1 << q)) {
-            const uint4 r0 = lds128(rp + q * QUARTER_BYTES + (row & 63) * 16);
-            const uint4 r1 = lds128(rp + q * QUARTER_BYTES + 1024 + (row & 63) * 16);
-            unpack16(r0, ro);
-            unpack16(r1, ro + 8);
-          } else {
+      for (int j = 0; j < UK; ++j) {
+        const int mask = (mw[j] & META_VALID) ? (mw[j] & 0xF) : 0;
+        if (mask) {
+          const int rseq = (mw[j] >> 4) & 0xFF, rs = rseq % C::RSTAGES;
+          const int qseq0 = (mw[j] >> 12) & 0xFFFF;
+          mbar_wait(bar(B_EMPTY_RU + rs), (((uint32_t)rseq / C::RSTAGES) & 1) ^ 1);
+          tc_fence_after();
 #pragma unroll
-            for (int z = 0; z < 16; ++z) ro[z] = 0;
+          for (int h = 0; h < 2; ++h) {
+            if (!(mask & (3 << (2 * h)))) continue;   // k-half without any block: never read by the MMA
+            const int q = 2 * h + rhalf;
+            uint32_t ro[16];
+            if (mask & (1 << q)) {
+              // the cell's present quarters sit in consecutive ring slots in ascending q
+              const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
+              const int slot = qs % C::NQ;
+              mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::NQ) & 1);
+              const uint32_t rp = sRP + slot * QUARTER_BYTES;
+              const uint4 r0 = lds128(rp + (row & 63) * 16);
+              const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
+              unpack16(r0, ro);
+              unpack16(r1, ro + 8);
+              __syncwarp();
+              if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot));
+            } else {
+#pragma unroll
+              for (int z = 0; z < 16; ++z) ro[z] = 0;
+            }
+            tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + rs * A_COLS + 16 * h), ro);
           }
-          tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + rs * A_COLS + 16 * h), ro);
-        }
-        tmem_st_wait();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) {
-          mbar_arrive(bar(B_FULL_RU + rs));
-          mbar_arrive(bar(B_EMPTY_RP + rs));
+          tmem_st_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar(B_FULL_RU + rs));
         }
       }
     }
@@ -420,19 +584,19 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     const int lq = warp & 3;  // TMEM lane quadrant this warp may access
     const int et = (warp - FIRST_EPI_WARP) * 32 + lane;  // 0..127 within the epilogue group
     const int n_loc = lq * 32 + lane;
-    const long long my_first_tile = u_beg / p.KS;
+    const uint32_t my_first_tile = u_beg / (uint32_t)p.KS;
     constexpr int PART = BT * BN;  // int32 elements of one partial accumulator
-    int it = 0;
-    long long g = u_beg;
+    int seg = 0;
+    uint32_t g = u_beg;
     while (g < u_end) {
-      const long long tile = g / p.KS;
-      const int k0 = (int)(g % p.KS);
-      const int k1 = (int)min((long long)p.KS, k0 + (u_end - g));
-      g += k1 - k0;
-      const int nt = (int)(tile / p.TT), tt = (int)(tile % p.TT);
-      const int a = C::ACC_STAGES == 2 ? (it & 1) : 0;
-      const uint32_t aphase = C::ACC_STAGES == 2 ? ((it >> 1) & 1) : (it & 1);
-      ++it;
+      const uint32_t tile = g / (uint32_t)p.KS;
+      const int k0 = (int)(g - tile * (uint32_t)p.KS);
+      const int k1 = (int)min((uint32_t)p.KS, (uint32_t)k0 + (u_end - g));
+      g += (uint32_t)(k1 - k0);
+      const int nt = (int)(tile / (uint32_t)p.TT), tt = (int)(tile - (uint32_t)nt * (uint32_t)p.TT);
+      const int a0s = seg % C::ACC0_STAGES, a1s = seg % C::ACC1_STAGES;
+      const uint32_t aphase = ((uint32_t)seg / C::ACC0_STAGES) & 1;
+      ++seg;
       const int n = nt * BN + n_loc;
       const int t_base = tt * BT;
       const int t_cnt = min(BT, p.M - t_base);
@@ -448,11 +612,13 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (p.dbg1) p.dbg1[(size_t)(t_base + t) * p.N + n] = a1 >> 8;
       };
 
-      mbar_wait(bar(B_TFULL + a), aphase);
+      mbar_wait(bar(B_TFULL + a0s), aphase);
       tc_fence_after();
-      MQ_STAMP_IF(et == 0 && it == 1, 9);
-      const bool has_res = acc_flag[a] != 0;  // acc1 is undefined when no residual MMA was issued
-      const uint32_t t0addr = tmem_base + ((uint32_t)(lq * 32) << 16) + (uint32_t)(a * 2 * BT);
+      MQ_STAMP_IF(et == 0 && seg == 1, 9);
+      const bool has_res = acc_flag[a0s] != 0;  // acc1 is undefined when no residual MMA was issued
+      const uint32_t lane_off = (uint32_t)(lq * 32) << 16;
+      const uint32_t t0addr = tmem_base + lane_off + (uint32_t)(a0s * BT);
+      const uint32_t t1addr = tmem_base + lane_off + (uint32_t)(C::ACC1_COL0 + a1s * BT);
       const bool whole = (k0 == 0 && k1 == p.KS);
       const int slot = tile == my_first_tile ? 0 : 1;
       int32_t* part0 = p.ws_part + ((size_t)blockIdx.x * 2 + slot) * (2 * PART);
@@ -462,7 +628,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         uint32_t v0[16], v1[16];
         tmem_ld16(t0addr + c0, v0);
         if (has_res) {
-          tmem_ld16(t0addr + BT + c0, v1);
+          tmem_ld16(t1addr + c0, v1);
         } else {
 #pragma unroll
           for (int i = 0; i < 16; ++i) v1[i] = 0;
@@ -481,10 +647,13 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             }
         }
       }
-      // accumulator stage drained: hand it back to the MMA warp
+      // accumulator stages drained: hand them back to the MMA warp
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(B_TEMPTY + a));
+      if (lane == 0) {
+        mbar_arrive(bar(B_A1E + a1s));
+        mbar_arrive(bar(B_A0E + a0s));
+      }
 
       if (!whole) {
         // stream-K fix-up: the last CTA to arrive for this tile sums all partials and finishes it
@@ -492,33 +661,42 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         __threadfence();
         named_bar_sync(1, 128);
         if (et == 0) {
-          const int c_lo = owner_of(p, tile * p.KS), c_hi = owner_of(p, (tile + 1) * p.KS - 1);
+          const int c_lo = owner_of(p, tile * (uint32_t)p.KS), c_hi = owner_of(p, (tile + 1) * (uint32_t)p.KS - 1);
           const int old = atomicAdd(p.ws_cnt + tile, 1);
           flag_slot[0] = (old == c_hi - c_lo);
+          flag_slot[2] = (range_begin(p, (uint32_t)c_lo) / (uint32_t)p.KS == tile) ? 0 : 1;  // slot of c_lo's partial
           flag_slot[3] = c_lo;
           flag_slot[4] = c_hi;
         }
         named_bar_sync(1, 128);
         const bool last = flag_slot[0] != 0;
-        const int c_lo = flag_slot[3], c_hi = flag_slot[4];
+        const int lo_slot = flag_slot[2], c_lo = flag_slot[3], c_hi = flag_slot[4];
         named_bar_sync(1, 128);  // flag_slot may be rewritten by the next segment
         if (last) {
           __threadfence();
+          // every contributor but the first started this tile at its range begin: slot 0
           for (int c0 = 0; c0 < t_cnt; c0 += 16) {
             int32_t s0[16], s1[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) s0[i] = s1[i] = 0;
-            for (int c = c_lo; c <= c_hi; ++c) {
-              const int cs = (range_begin(p, c) / p.KS == tile) ? 0 : 1;
-              const int32_t* q0 = p.ws_part + ((size_t)c * 2 + cs) * (2 * PART) + n_loc;
-              const bool cres = __ldcg(p.ws_flag + c * 2 + cs) != 0;
-#pragma unroll
-              for (int i = 0; i < 16; ++i)
-                if (c0 + i < t_cnt) s0[i] += __ldcg(q0 + (c0 + i) * BN);
-              if (cres) {
+            for (int cb = c_lo; cb <= c_hi; cb += 32) {
+              // residual flags of up to 32 contributors at once (lane L: contributor cb + L)
+              const int cl = cb + lane;
+              int f = 0;
+              if (cl <= c_hi) f = __ldcg(p.ws_flag + cl * 2 + (cl == c_lo ? lo_slot : 0));
+              const uint32_t fm = __ballot_sync(0xffffffffu, f != 0);
+              const int ce = min(c_hi, cb + 31);
+#pragma unroll 4
+              for (int c = cb; c <= ce; ++c) {
+                const int32_t* q0 = p.ws_part + ((size_t)c * 2 + (c == c_lo ? lo_slot : 0)) * (2 * PART) + n_loc;
 #pragma unroll
                 for (int i = 0; i < 16; ++i)
-                  if (c0 + i < t_cnt) s1[i] += __ldcg(q0 + PART + (c0 + i) * BN);
+                  if (c0 + i < t_cnt) s0[i] += __ldcg(q0 + (c0 + i) * BN);
+                if ((fm >> (c - cb)) & 1u) {
+#pragma unroll
+                  for (int i = 0; i < 16; ++i)
+                    if (c0 + i < t_cnt) s1[i] += __ldcg(q0 + PART + (c0 + i) * BN);
+                }
               }
             }
 #pragma unroll
@@ -532,7 +710,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     }
   }
 
-  // teardown (single-lane roles re-converge first: bar.sync must be reached warp-convergent)
+  // teardown (single-lane regions re-converge first: bar.sync must be reached warp-convergent)
   __syncwarp();
   tc_fence_before();
   __syncthreads();
@@ -574,7 +752,7 @@ size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 
 struct Plan {
   int BT = 16, TT = 1, grid = 1, gran = 1;
-  long long units = 0;
+  int64_t units = 0;   // K-steps of all tiles; the kernel indexes them with 32 bits
   size_t off_flag = 0, off_part = 0, ws_bytes = 0;
 };
 
@@ -652,6 +830,7 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   if (!enc) return MQ_ERR_CUDA;
 
   const Plan pl = make_plan(w, M);
+  if (pl.units >= (int64_t)1 << 31) return MQ_ERR_UNSUPPORTED_SHAPE;
   if (pl.ws_bytes > 0) {
     if (!workspace || workspace_bytes < pl.ws_bytes) return MQ_ERR_WORKSPACE;
     if ((uintptr_t)workspace & 15) return MQ_ERR_INVALID_ARG;
@@ -684,8 +863,10 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   gp.KS = (int)(w->K / BK);
   gp.NT = (int)(w->N / BN);
   gp.TT = pl.TT;
-  gp.units = pl.units;
-  gp.gran = pl.gran;
+  gp.units = (uint32_t)pl.units;
+  gp.gran = (uint32_t)pl.gran;
+  gp.upg_q = (uint32_t)((pl.units / pl.gran) / pl.grid);
+  gp.upg_r = (uint32_t)((pl.units / pl.gran) % pl.grid);
   gp.y_bf16 = y_dtype == MQ_BF16;
   uint8_t* ws = (uint8_t*)workspace;
   gp.ws_cnt = (int32_t*)ws;
