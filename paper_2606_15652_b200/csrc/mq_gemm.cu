@@ -65,8 +65,9 @@ constexpr int A_COLS = BK / 4;               // 32 TMEM columns hold 128 int8 pe
 constexpr int META_VALID = (int)0x80000000;  // the K-step exists (a P stage may hold fewer than SK)
 constexpr int META_FIRST = 1 << 30;          // first K-step of this CTA's segment of a tile
 constexpr int META_LAST = 1 << 29;           // last K-step of the segment: accumulators complete
-// bits 0-3: residual quarter mask; bits 4-11: sequence number of the residual cell in this CTA
-// (mod 256); bits 12-27: sequence number of the cell's first stored quarter (mod 65536)
+// bits 0-3: residual quarter mask; bits 4-11: sequence number of the residual cell among the cells
+// of its unpack group in this CTA (mod 256); bits 12-27: sequence number of the cell's first
+// stored quarter among the quarters of its unpack group (mod 65536)
 
 template <int BT>
 struct Cfg {
@@ -74,9 +75,14 @@ struct Cfg {
   static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // K-steps per U stage (item)
   static constexpr int IPS = SK / UK;                            // items per P stage
   static constexpr int PSTAGES = BT <= 32 ? 4 : (BT == 64 ? 6 : 4);
-  static constexpr int USTAGES = BT <= 64 ? 2 : 3;
-  static constexpr int RSTAGES = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // unpacked residual cells (TMEM)
-  static constexpr int NQ = BT == 16 ? 16 : 8;                        // packed residual quarter slots (2 KB each)
+  static constexpr int USTAGES = 2;                                   // one per unpack group
+  // Unpacked residual cells (TMEM): every unpack group owns a private ring of RG stages.  A ring
+  // shared between the groups would be unsafe: mbarrier parity waits cannot tell "my turn" from
+  // "two phases early", and cells fall on the groups irregularly.
+  static constexpr int RG = BT <= 32 ? 2 : 1;
+  static constexpr int RSTAGES = NUM_UNPACK_GROUPS * RG;
+  static constexpr int QG = BT == 16 ? 8 : 4;                         // packed residual quarter slots (2 KB) per group,
+  static constexpr int NQ = NUM_UNPACK_GROUPS * QG;                   // private for the same reason
   static constexpr int ACC0_STAGES = 2;
   static constexpr int ACC1_STAGES = BT <= 64 ? 2 : 1;
   static constexpr int P_W = SK * TILE_BYTES;
@@ -91,6 +97,7 @@ struct Cfg {
   static constexpr int TMEM_NEED = R_COL0 + RSTAGES * A_COLS;
   static constexpr int TMEM_COLS = TMEM_NEED <= 32 ? 32 : (TMEM_NEED <= 64 ? 64 : (TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512)));
   static_assert(TMEM_NEED <= 512, "tensor memory budget");
+  static_assert(NUM_UNPACK_GROUPS == 2 && USTAGES >= NUM_UNPACK_GROUPS, "ring safety: groups <= stages");
   // shared memory map (offsets from a 1024-aligned base)
   static constexpr int OFF_U = 0;
   static constexpr int OFF_P = OFF_U + USTAGES * U_STAGE;
@@ -318,7 +325,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     bool have = it.next<SK>(cur);
     int2 um = make_int2(0, 0);
     if (have) um = load_meta(cur);
-    int ps = 0, rseq = 0, qseq = 0, si = 0;
+    int ps = 0, si = 0;
+    int qseq_g0 = 0, qseq_g1 = 0;   // residual quarters handed to unpack group 0 / 1 so far
+    int rseq_g0 = 0, rseq_g1 = 0;   // residual cells handed to unpack group 0 / 1 so far
     uint32_t pphase = 0;
     while (have) {
       const bool have_n = it.next<SK>(nxt);
@@ -342,20 +351,23 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       asm volatile("" : "+r"(um.x), "+r"(um.y));
       const int mask = lane < cur.nks ? (um.x & 0xF) : 0;
       const uint32_t nz = __ballot_sync(0xffffffffu, mask != 0);
-      // quarters stored by the cells of the lanes below this one (inclusive scan of popc(mask))
-      int qbefore = __popc(mask);
+      // the unpack group that will handle K-step `lane` of this stage: item index mod 2
+      const int my_group = (si * IPS + (lane < SK ? lane : 0) / UK) & (NUM_UNPACK_GROUPS - 1);
+      const uint32_t g1_lanes = __ballot_sync(0xffffffffu, my_group != 0);
+      // quarters stored by the cells of the lower lanes of the same group (SK <= 4: plain loop)
+      int qbefore = 0;
 #pragma unroll
-      for (int d = 1; d < SK; d <<= 1) {
-        const int o = __shfl_up_sync(0xffffffffu, qbefore, d);
-        if (lane >= d) qbefore += o;
+      for (int j = 0; j < SK; ++j) {
+        const int mj = __shfl_sync(0xffffffffu, mask, j);
+        const int gj = __shfl_sync(0xffffffffu, my_group, j);
+        if (j < lane && gj == my_group) qbefore += __popc(mj);
       }
-      const int qtotal = __shfl_sync(0xffffffffu, qbefore, SK - 1);
-      qbefore -= __popc(mask);
       if (lane < SK) {
         int word = 0;
         if (lane < cur.nks) {
-          word = META_VALID | mask | (((rseq + __popc(nz & ((1u << lane) - 1u))) & 0xFF) << 4) |
-                 (((qseq + qbefore) & 0xFFFF) << 12);
+          const int my_rseq = (my_group ? rseq_g1 : rseq_g0) + __popc(nz & (my_group ? g1_lanes : ~g1_lanes) & ((1u << lane) - 1u));
+          word = META_VALID | mask | ((my_rseq & 0xFF) << 4) |
+                 ((((my_group ? qseq_g1 : qseq_g0) + qbefore) & 0xFFFF) << 12);
           if (cur.first && lane == 0) word |= META_FIRST;
           if (cur.last && lane == cur.nks - 1) word |= META_LAST;
         }
@@ -369,10 +381,12 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         const int j = __ffs((int)todo) - 1;
         todo &= todo - 1;
         const int m = __shfl_sync(0xffffffffu, mask, j);
+        const int gj = __shfl_sync(0xffffffffu, my_group, j);
         const uint8_t* rsrc = p.res + (size_t)__shfl_sync(0xffffffffu, um.y, j) * QUARTER_BYTES;
+        const int q0 = gj ? qseq_g1 : qseq_g0;
         for (int q = 0; q < __popc(m); ++q) {
-          const int slot = (qseq + q) % C::NQ;
-          mbar_wait(bar(B_EMPTY_Q + slot), (((uint32_t)(qseq + q) / C::NQ) & 1) ^ 1);
+          const int slot = gj * C::QG + (q0 + q) % C::QG;
+          mbar_wait(bar(B_EMPTY_Q + slot), (((uint32_t)(q0 + q) / C::QG) & 1) ^ 1);
           __syncwarp();
           if (elect_one()) {
             const uint32_t rb = bar(B_FULL_Q + slot);
@@ -380,10 +394,13 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             tma_load_1d(sRP + slot * QUARTER_BYTES, rsrc + (size_t)q * QUARTER_BYTES, QUARTER_BYTES, rb);
           }
         }
-        qseq += __popc(m);
+        if (gj)
+          qseq_g1 += __popc(m);
+        else
+          qseq_g0 += __popc(m);
       }
-      rseq += __popc(nz);
-      (void)qtotal;
+      rseq_g0 += __popc(nz & ~g1_lanes);
+      rseq_g1 += __popc(nz & g1_lanes);
       if (++ps == C::PSTAGES) {
         ps = 0;
         pphase ^= 1;
@@ -435,8 +452,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
             tc_fence_after();
           }
-          const int rseq = (m >> 4) & 0xFF, rs = rseq % C::RSTAGES;
-          mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RSTAGES) & 1);
+          const int rseq = (m >> 4) & 0xFF, rs = (item & (NUM_UNPACK_GROUPS - 1)) * C::RG + rseq % C::RG;
+          mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RG) & 1);
           tc_fence_after();
           __syncwarp();
           const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + rs * A_COLS);
@@ -545,9 +562,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       for (int j = 0; j < UK; ++j) {
         const int mask = (mw[j] & META_VALID) ? (mw[j] & 0xF) : 0;
         if (mask) {
-          const int rseq = (mw[j] >> 4) & 0xFF, rs = rseq % C::RSTAGES;
+          const int rseq = (mw[j] >> 4) & 0xFF, rs = gi * C::RG + rseq % C::RG;
           const int qseq0 = (mw[j] >> 12) & 0xFFFF;
-          mbar_wait(bar(B_EMPTY_RU + rs), (((uint32_t)rseq / C::RSTAGES) & 1) ^ 1);
+          mbar_wait(bar(B_EMPTY_RU + rs), (((uint32_t)rseq / C::RG) & 1) ^ 1);
           tc_fence_after();
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
@@ -557,8 +574,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             if (mask & (1 << q)) {
               // the cell's present quarters sit in consecutive ring slots in ascending q
               const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
-              const int slot = qs % C::NQ;
-              mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::NQ) & 1);
+              const int slot = gi * C::QG + qs % C::QG;
+              mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::QG) & 1);
               const uint32_t rp = sRP + slot * QUARTER_BYTES;
               const uint4 r0 = lds128(rp + (row & 63) * 16);
               const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);

@@ -3,6 +3,7 @@
 // commit, ld, fences).  No logic lives here.
 #pragma once
 #include <cstdint>
+#include <cstdio>
 
 namespace mq {
 namespace ptx {
@@ -41,7 +42,14 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
+#ifdef MQ_TRACE
+    if (++spins > (1u << 22)) {
+      printf("mq watchdog: block %d thread %d bar smem 0x%x parity %u\n", (int)blockIdx.x, (int)threadIdx.x, bar, parity);
+      __trap();
+    }
+#else
     if (++spins > (1u << 26)) __trap();
+#endif
   }
 }
 
