@@ -116,11 +116,11 @@ void mq_weights_free(mq_weights* w);
  *   qA_dev, sA_dev : output of mq_quantize_act for the same M and this layer's K
  *                    (row stride K/2 bytes).
  *   Y_dev          : [M,N] fp16/bf16 row-major, `ldy_elems` elements between rows.
- *   dbg_acc_base_dev / dbg_acc_res_dev : optional int32 [M,N] row-major (stride N); when
- *                    non-NULL they receive acc0 / acc1 exactly (parity hooks).
+ *   dbg_acc_base_dev / dbg_acc_res_dev : optional int32 [M,N] row-major (stride N), 16-byte
+ *                    aligned; when non-NULL they receive acc0 / acc1 exactly (parity hooks).
  *   workspace_dev  : at least mq_gemm_workspace_bytes(w, M) bytes, 16-byte aligned; must be
  *                    all-zero before the FIRST call that uses it; afterwards its contents are
- *                    library-private and stay valid from call to call (tile arrival counters,
+ *                    library-private and stay valid from call to call (per-tile counters,
  *                    which every call returns to zero, and int32 partial tiles of the
  *                    stream-K fix-up).  Calls that may run concurrently need distinct
  *                    workspaces.
@@ -143,6 +143,8 @@ int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t 
  *                 all tiles cut into equal per-CTA ranges, shared tiles finished by the last arriver)
  *   "token_tile": 0 = automatic, else 16/32/64/128
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
+ *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
+ *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */
 int mq_set_option(const char* name, int64_t value);
 /* Number of kernels the last mq_gemm / mq_linear / mq_quantize_act call launched. */

@@ -105,7 +105,7 @@ struct Cfg {
   static constexpr int OFF_BAR = OFF_RP + NQ * QUARTER_BYTES;
   static constexpr int NUM_BARS = 2 * PSTAGES + 2 * USTAGES + 2 * NQ + 2 * RSTAGES + 2 + ACC0_STAGES + ACC1_STAGES;
   static constexpr int OFF_META = OFF_BAR + NUM_BARS * 8;
-  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 8;
+  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 12;
   static constexpr int OFF_END = OFF_META + META_WORDS * 4;
   static constexpr int SMEM_BYTES = OFF_END + 1024;  // slack for the 1024-byte alignment
   static_assert(SMEM_BYTES <= 232448, "shared memory budget");
@@ -122,7 +122,8 @@ struct GemmParams {
   void* Y;
   int32_t* dbg0;
   int32_t* dbg1;
-  int32_t* ws_cnt;    // [tiles] arrival counters (zero between calls)
+  int32_t* ws_cnt;    // [tiles] partials published (zero between calls)
+  int32_t* ws_done;   // [tiles] contributors finished (zero between calls)
   int32_t* ws_flag;   // [grid][2] did this partial receive residual MMAs?
   int32_t* ws_part;   // [grid][2 slots][2 accs][BT][128] int32 partial tiles
   int64_t ldy;
@@ -160,6 +161,7 @@ __device__ __forceinline__ int owner_of(const GemmParams& p, uint32_t x) {
 
 // One P stage of a CTA's work: up to SK consecutive K-steps of one (n-tile, token-tile).
 struct Stage {
+  uint32_t u;         // index of the stage's first K-step in the CTA-independent unit sequence
   int nt, tt, ks, nks;
   bool first, last;   // first / last stage of this CTA's segment of the tile
 };
@@ -183,6 +185,7 @@ struct StageIter {
       tt = (int)(tile - (uint32_t)nt * (uint32_t)TT);
       s.first = true;
     }
+    s.u = g - (uint32_t)(k1 - ks);
     s.nt = nt;
     s.tt = tt;
     s.ks = ks;
@@ -263,8 +266,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   const uint32_t sMetaU = sMetaP + 4u * C::PSTAGES * SK;        // [USTAGES][UK]
   const uint32_t sMisc = sMetaU + 4u * C::USTAGES * UK;         // [0] tmem base, [1..5] fix-up, [6..7] acc_flag
   volatile int32_t* misc = reinterpret_cast<volatile int32_t*>(smem_raw + (sMisc - smem_u32(smem_raw)));
-  volatile int32_t* flag_slot = misc + 1;
-  volatile int32_t* acc_flag = misc + 6;  // [2]: did this base-accumulator stage's segment get residual MMAs?
+  volatile int32_t* pend = misc + 1;      // [2][4] partial tiles awaiting the fix-up: tile, c_lo, c_hi, lo_slot
+  volatile int32_t* acc_flag = misc + 9;  // [2]: did this base-accumulator stage's segment get residual MMAs?
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #ifdef MQ_TRACE
@@ -308,6 +311,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)misc[0];
   MQ_STAMP_IF(threadIdx.x == 0, 1);
+  // PDL: the next kernel in the stream may start its prologue as this grid's CTAs retire
+  griddep_launch();
 
   const uint32_t u_beg = range_begin(p, blockIdx.x);
   const uint32_t u_end = blockIdx.x + 1 == gridDim.x ? p.units : range_begin(p, blockIdx.x + 1);
@@ -318,37 +323,76 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     // ===================== producer (TMA); all lanes run the loop, one elected lane issues =====================
     StageIter it(u_beg, u_end, p.KS, p.TT);
     Stage cur, nxt;
-    auto load_meta = [&](const Stage& s) {
-      // lane j < nks: {quarter mask, first quarter} of the stage's K-step j
-      return lane < s.nks ? __ldg(p.unit_meta + (size_t)s.nt * p.KS + s.ks + lane) : make_int2(0, 0);
+    // Residual metadata {quarter mask, first quarter} is fetched 32 K-steps at a time (lane L: unit
+    // ub + L) and two batches ahead, so that the producer never waits on global memory per stage.
+    auto load_batch = [&](uint32_t ub) {
+      const uint32_t u = ub + (uint32_t)lane;
+      int2 v = make_int2(0, 0);
+      if (u < u_end) {
+        const uint32_t tile = u / (uint32_t)p.KS;
+        v = __ldg(p.unit_meta + (size_t)(tile / (uint32_t)p.TT) * p.KS + (u - tile * (uint32_t)p.KS));
+      }
+      return v;
     };
+    uint32_t ubA = u_beg;
+    int2 umA = load_batch(ubA), umB = load_batch(ubA + 32);
+    // PDL prologue: the packed weights are static, so the first ring-full of weight copies is issued
+    // BEFORE waiting for the previous kernel (which produces the quantized activations).
+    int pre = 0;
+    {
+      StageIter itp = it;
+      Stage s;
+      for (; pre < C::PSTAGES && itp.next<SK>(s); ++pre) {
+        if (elect_one()) {
+          MQ_STAMP_IF(pre == 0, 2);
+          const uint32_t fb = bar(B_FULL_P + pre);
+          mbar_arrive_expect_tx(fb, (uint32_t)s.nks * (TILE_BYTES + BT * (BK / 2)));
+          tma_load_1d(sP + pre * C::P_STAGE, p.base + ((size_t)s.nt * p.KS + s.ks) * TILE_BYTES,
+                      (uint32_t)s.nks * TILE_BYTES, fb);
+        }
+        __syncwarp();
+      }
+    }
+    griddep_wait();
     bool have = it.next<SK>(cur);
-    int2 um = make_int2(0, 0);
-    if (have) um = load_meta(cur);
     int ps = 0, si = 0;
     int qseq_g0 = 0, qseq_g1 = 0;   // residual quarters handed to unpack group 0 / 1 so far
     int rseq_g0 = 0, rseq_g1 = 0;   // residual cells handed to unpack group 0 / 1 so far
     uint32_t pphase = 0;
     while (have) {
       const bool have_n = it.next<SK>(nxt);
-      int2 um_n = make_int2(0, 0);
-      if (have_n) um_n = load_meta(nxt);   // one stage ahead: its latency hides behind this stage's issue
       mbar_wait(bar(B_EMPTY_P + ps), pphase ^ 1);
       __syncwarp();
       const uint32_t dst = sP + ps * C::P_STAGE;
       if (elect_one()) {
-        MQ_STAMP_IF(si == 0, 2);
         MQ_STAMP_IF(si < 16, 48 + si);
         MQ_STAMP_IF(si == n_stages - 1, 3);
         const uint32_t fb = bar(B_FULL_P + ps);
-        mbar_arrive_expect_tx(fb, (uint32_t)cur.nks * (TILE_BYTES + BT * (BK / 2)));
-        tma_load_1d(dst, p.base + ((size_t)cur.nt * p.KS + cur.ks) * TILE_BYTES, (uint32_t)cur.nks * TILE_BYTES, fb);
+        if (si >= pre) {   // the prologue already issued the weights of the first `pre` stages
+          mbar_arrive_expect_tx(fb, (uint32_t)cur.nks * (TILE_BYTES + BT * (BK / 2)));
+          tma_load_1d(dst, p.base + ((size_t)cur.nt * p.KS + cur.ks) * TILE_BYTES, (uint32_t)cur.nks * TILE_BYTES, fb);
+        }
         for (int j = 0; j < cur.nks; ++j)
           tma_load_2d(dst + C::P_W + j * (BT * (BK / 2)), &tmap_a, (cur.ks + j) * (BK / 2), cur.tt * BT, fb);
       }
       // metadata words of the stage (lane j writes K-step j), then the second arrival publishes them.
       // The empty asm pins the first USE of the prefetched metadata behind the TMA issue above.
-      asm volatile("" : "+r"(um.x), "+r"(um.y));
+      asm volatile("" : "+r"(umA.x), "+r"(umA.y));
+      if (cur.u - ubA >= 32) {          // rotate: batch B was requested >= 32 K-steps ago
+        umA = umB;
+        ubA += 32;
+        umB = load_batch(ubA + 32);
+      }
+      int2 um;
+      {
+        const uint32_t rel = cur.u - ubA + (uint32_t)(lane < SK ? lane : 0);   // < 64
+        um.x = __shfl_sync(0xffffffffu, umA.x, rel & 31);
+        um.y = __shfl_sync(0xffffffffu, umA.y, rel & 31);
+        if (cur.u - ubA + SK > 32) {     // warp-uniform: the stage straddles into batch B (loaded long ago)
+          const int bx = __shfl_sync(0xffffffffu, umB.x, rel & 31), by = __shfl_sync(0xffffffffu, umB.y, rel & 31);
+          if (rel >= 32) um = make_int2(bx, by);
+        }
+      }
       const int mask = lane < cur.nks ? (um.x & 0xF) : 0;
       const uint32_t nz = __ballot_sync(0xffffffffu, mask != 0);
       // the unpack group that will handle K-step `lane` of this stage: item index mod 2
@@ -407,7 +451,6 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       }
       ++si;
       cur = nxt;
-      um = um_n;
       have = have_n;
     }
   } else if (warp == 1) {
@@ -598,12 +641,14 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     }
   } else {
     // ===================== epilogue warps (2..5) =====================
+    griddep_wait();   // s_a, Y, the workspace: ordered after the previous kernel in the stream
     const int lq = warp & 3;  // TMEM lane quadrant this warp may access
     const int et = (warp - FIRST_EPI_WARP) * 32 + lane;  // 0..127 within the epilogue group
     const int n_loc = lq * 32 + lane;
     const uint32_t my_first_tile = u_beg / (uint32_t)p.KS;
     constexpr int PART = BT * BN;  // int32 elements of one partial accumulator
-    int seg = 0;
+    int seg = 0, npend = 0;      // npend: partial tiles published by this CTA (at most 2)
+    constexpr bool kBothParts = BT <= 32;
     uint32_t g = u_beg;
     while (g < u_end) {
       const uint32_t tile = g / (uint32_t)p.KS;
@@ -633,6 +678,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       tc_fence_after();
       MQ_STAMP_IF(et == 0 && seg == 1, 9);
       const bool has_res = acc_flag[a0s] != 0;  // acc1 is undefined when no residual MMA was issued
+      // small token tiles (kBothParts): partial tiles always carry both accumulators (zeros when
+      // there was no residual MMA), which takes the flag round trip out of the fix-up's latency chain
       const uint32_t lane_off = (uint32_t)(lq * 32) << 16;
       const uint32_t t0addr = tmem_base + lane_off + (uint32_t)(a0s * BT);
       const uint32_t t1addr = tmem_base + lane_off + (uint32_t)(C::ACC1_COL0 + a1s * BT);
@@ -660,7 +707,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           for (int i = 0; i < 16; ++i)
             if (c0 + i < t_cnt) {
               __stcg(part0 + (c0 + i) * BN + n_loc, (int32_t)v0[i]);
-              if (has_res) __stcg(part1 + (c0 + i) * BN + n_loc, (int32_t)v1[i]);
+              if (kBothParts || has_res) __stcg(part1 + (c0 + i) * BN + n_loc, (int32_t)v1[i]);
             }
         }
       }
@@ -673,57 +720,110 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       }
 
       if (!whole) {
-        // stream-K fix-up: the last CTA to arrive for this tile sums all partials and finishes it
-        if (et == 0) p.ws_flag[blockIdx.x * 2 + slot] = has_res ? 1 : 0;
+        // stream-K fix-up, part 1: publish this partial (release) and count the arrival.  Nothing
+        // waits here; a CTA waits only after ALL of its partials are published (part 2), so the
+        // contributors of different tiles cannot wait on each other in a cycle.
+        if (!kBothParts && et == 0) p.ws_flag[blockIdx.x * 2 + slot] = has_res ? 1 : 0;
         __threadfence();
         named_bar_sync(1, 128);
         if (et == 0) {
           const int c_lo = owner_of(p, tile * (uint32_t)p.KS), c_hi = owner_of(p, (tile + 1) * (uint32_t)p.KS - 1);
-          const int old = atomicAdd(p.ws_cnt + tile, 1);
-          flag_slot[0] = (old == c_hi - c_lo);
-          flag_slot[2] = (range_begin(p, (uint32_t)c_lo) / (uint32_t)p.KS == tile) ? 0 : 1;  // slot of c_lo's partial
-          flag_slot[3] = c_lo;
-          flag_slot[4] = c_hi;
+          atomicAdd(p.ws_cnt + tile, 1);
+          int32_t* pd = const_cast<int32_t*>(pend) + npend * 4;
+          pd[0] = (int32_t)tile;
+          pd[1] = c_lo;
+          pd[2] = c_hi;
+          pd[3] = (range_begin(p, (uint32_t)c_lo) / (uint32_t)p.KS == tile) ? 0 : 1;  // slot of c_lo's partial
         }
-        named_bar_sync(1, 128);
-        const bool last = flag_slot[0] != 0;
-        const int lo_slot = flag_slot[2], c_lo = flag_slot[3], c_hi = flag_slot[4];
-        named_bar_sync(1, 128);  // flag_slot may be rewritten by the next segment
-        if (last) {
-          __threadfence();
-          // every contributor but the first started this tile at its range begin: slot 0
-          for (int c0 = 0; c0 < t_cnt; c0 += 16) {
-            int32_t s0[16], s1[16];
-#pragma unroll
-            for (int i = 0; i < 16; ++i) s0[i] = s1[i] = 0;
-            for (int cb = c_lo; cb <= c_hi; cb += 32) {
-              // residual flags of up to 32 contributors at once (lane L: contributor cb + L)
-              const int cl = cb + lane;
-              int f = 0;
-              if (cl <= c_hi) f = __ldcg(p.ws_flag + cl * 2 + (cl == c_lo ? lo_slot : 0));
-              const uint32_t fm = __ballot_sync(0xffffffffu, f != 0);
-              const int ce = min(c_hi, cb + 31);
-#pragma unroll 4
-              for (int c = cb; c <= ce; ++c) {
-                const int32_t* q0 = p.ws_part + ((size_t)c * 2 + (c == c_lo ? lo_slot : 0)) * (2 * PART) + n_loc;
-#pragma unroll
-                for (int i = 0; i < 16; ++i)
-                  if (c0 + i < t_cnt) s0[i] += __ldcg(q0 + (c0 + i) * BN);
-                if ((fm >> (c - cb)) & 1u) {
-#pragma unroll
-                  for (int i = 0; i < 16; ++i)
-                    if (c0 + i < t_cnt) s1[i] += __ldcg(q0 + PART + (c0 + i) * BN);
-                }
-              }
-            }
-#pragma unroll
-            for (int i = 0; i < 16; ++i)
-              if (c0 + i < t_cnt) emit(c0 + i, s0[i], s1[i]);
-          }
-          if (et == 0) p.ws_cnt[tile] = 0;
-        }
+        ++npend;
       }
       MQ_STAMP_IF(et == 0, 10);
+    }
+
+    // stream-K fix-up, part 2: the S contributors of a tile wait until all S partials are visible,
+    // then EACH reduces and finishes 1/S of the tile (16-byte loads, all contributors in flight).
+    // All CTAs of the grid are resident (grid <= SM count, one CTA per SM), so the wait terminates.
+    if (npend) named_bar_sync(1, 128);   // pend[] written by thread et == 0
+    for (int pi = 0; pi < npend; ++pi) {
+      const uint32_t tile = (uint32_t)pend[pi * 4 + 0];
+      const int c_lo = pend[pi * 4 + 1], c_hi = pend[pi * 4 + 2], lo_slot = pend[pi * 4 + 3];
+      const int S = c_hi - c_lo + 1, r = (int)blockIdx.x - c_lo;
+      const int nt = (int)(tile / (uint32_t)p.TT), tt = (int)(tile - (uint32_t)nt * (uint32_t)p.TT);
+      const int t_base = tt * BT;
+      const int t_cnt = min(BT, p.M - t_base);
+      {
+        uint32_t spins = 0;
+        int seen;
+        do {
+          asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.ws_cnt + tile) : "memory");
+          if (++spins > (1u << 24)) __trap();
+        } while (seen < S);
+      }
+      // residual flags of the contributors (bit c - c_lo); S <= 32 in practice, else treat all as set
+      uint32_t fm = 0xffffffffu;
+      if (!kBothParts && S <= 32) {
+        int f = 0;
+        if (lane < S) f = __ldcg(p.ws_flag + (c_lo + lane) * 2 + (lane == 0 ? lo_slot : 0));
+        fm = __ballot_sync(0xffffffffu, f != 0);
+      }
+      const int E4 = t_cnt * (BN / 4);                       // 16-byte units of one accumulator
+      const int e_lo = (int)(((long long)E4 * r) / S), e_hi = (int)(((long long)E4 * (r + 1)) / S);
+      const bool y_vec = ((reinterpret_cast<uintptr_t>(p.Y) | (uintptr_t)(p.ldy * 2)) & 7) == 0;
+      for (int e = e_lo + et; e < e_hi; e += 128) {
+        const int t = e / (BN / 4), n0 = (e - t * (BN / 4)) * 4;
+        int4 s0 = make_int4(0, 0, 0, 0), s1 = make_int4(0, 0, 0, 0);
+#pragma unroll 4
+        for (int c = c_lo; c <= c_hi; ++c) {
+          const int32_t* q0 = p.ws_part + ((size_t)c * 2 + (c == c_lo ? lo_slot : 0)) * (2 * PART) + t * BN + n0;
+          const int4 a = __ldcg(reinterpret_cast<const int4*>(q0));
+          int4 b = make_int4(0, 0, 0, 0);
+          if (kBothParts || ((fm >> ((c - c_lo) & 31)) & 1u)) b = __ldcg(reinterpret_cast<const int4*>(q0 + PART));
+          s0.x += a.x; s0.y += a.y; s0.z += a.z; s0.w += a.w;
+          s1.x += b.x; s1.y += b.y; s1.z += b.z; s1.w += b.w;
+        }
+        const int n = nt * BN + n0;
+        const float4 sw4 = *reinterpret_cast<const float4*>(p.sw + n), sr4 = *reinterpret_cast<const float4*>(p.sr + n);
+        const float sat = p.sa[t_base + t] * 0.00390625f;    // / 256: accumulators are x256
+        float y[4];
+        y[0] = sat * ((float)s0.x * sw4.x + (float)s1.x * sr4.x);
+        y[1] = sat * ((float)s0.y * sw4.y + (float)s1.y * sr4.y);
+        y[2] = sat * ((float)s0.z * sw4.z + (float)s1.z * sr4.z);
+        y[3] = sat * ((float)s0.w * sw4.w + (float)s1.w * sr4.w);
+        const size_t o = (size_t)(t_base + t) * p.ldy + n;
+        if (y_vec) {
+          uint2 pk;
+          if (p.y_bf16) {
+            __nv_bfloat162 lo = __floats2bfloat162_rn(y[0], y[1]), hi = __floats2bfloat162_rn(y[2], y[3]);
+            pk.x = *reinterpret_cast<uint32_t*>(&lo);
+            pk.y = *reinterpret_cast<uint32_t*>(&hi);
+          } else {
+            __half2 lo = __floats2half2_rn(y[0], y[1]), hi = __floats2half2_rn(y[2], y[3]);
+            pk.x = *reinterpret_cast<uint32_t*>(&lo);
+            pk.y = *reinterpret_cast<uint32_t*>(&hi);
+          }
+          *reinterpret_cast<uint2*>(reinterpret_cast<uint16_t*>(p.Y) + o) = pk;
+        } else {
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            if (p.y_bf16)
+              store_y<true>(p.Y, o + i, y[i]);
+            else
+              store_y<false>(p.Y, o + i, y[i]);
+          }
+        }
+        const size_t od = (size_t)(t_base + t) * p.N + n;
+        if (p.dbg0) *reinterpret_cast<int4*>(p.dbg0 + od) = make_int4(s0.x >> 8, s0.y >> 8, s0.z >> 8, s0.w >> 8);
+        if (p.dbg1) *reinterpret_cast<int4*>(p.dbg1 + od) = make_int4(s1.x >> 8, s1.y >> 8, s1.z >> 8, s1.w >> 8);
+      }
+      // the last contributor to finish returns the tile's counters to zero for the next call
+      named_bar_sync(1, 128);
+      if (et == 0) {
+        const int old = atomicAdd(p.ws_done + tile, 1);
+        if (old == S - 1) {
+          p.ws_cnt[tile] = 0;
+          p.ws_done[tile] = 0;
+        }
+      }
     }
   }
 
@@ -770,7 +870,7 @@ size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 struct Plan {
   int BT = 16, TT = 1, grid = 1, gran = 1;
   int64_t units = 0;   // K-steps of all tiles; the kernel indexes them with 32 bits
-  size_t off_flag = 0, off_part = 0, ws_bytes = 0;
+  size_t off_done = 0, off_flag = 0, off_part = 0, ws_bytes = 0;
 };
 
 Plan make_plan(const mq_weights* w, int64_t M) {
@@ -794,8 +894,15 @@ Plan make_plan(const mq_weights* w, int64_t M) {
   if (o.split_k >= 2) stream_k = true;
   pl.gran = stream_k ? 1 : KS;
   pl.grid = (int)std::min<int64_t>(G, pl.units / pl.gran);
+  // Few tiles: cut every tile into the same S parts (grid = tiles * S makes the stream-K ranges
+  // tile-aligned), so that each CTA owns ONE partial segment and pays the fix-up latency once.
+  if (stream_k && o.split_k == 0 && tiles * 2 <= G) {
+    const int64_t S = std::min<int64_t>(G / tiles, KS);
+    pl.grid = (int)(tiles * S);
+  }
   if (stream_k) {
-    pl.off_flag = align256((size_t)tiles * 4);
+    pl.off_done = align256((size_t)tiles * 4);
+    pl.off_flag = pl.off_done + align256((size_t)tiles * 4);
     pl.off_part = pl.off_flag + align256((size_t)pl.grid * 2 * 4);
     pl.ws_bytes = pl.off_part + (size_t)pl.grid * 2 * 2 * bt * BN * 4;
   }
@@ -814,8 +921,21 @@ int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t
     }
     attr_set = true;
   }
-  mq_gemm_kernel<BT><<<grid, NUM_THREADS, C::SMEM_BYTES, st>>>(tmap, gp);
-  return cudaGetLastError() == cudaSuccess ? MQ_OK : MQ_ERR_CUDA;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(NUM_THREADS);
+  cfg.dynamicSmemBytes = C::SMEM_BYTES;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = options().pdl ? 1 : 0;
+  if (cudaLaunchKernelEx(&cfg, mq_gemm_kernel<BT>, tmap, gp) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  return MQ_OK;
 }
 
 }  // namespace
@@ -841,6 +961,7 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   if (M == 0) return MQ_OK;
   if (!qA || !sA || !Y || ldy < w->N) return MQ_ERR_INVALID_ARG;
   if (((uintptr_t)qA & 15) || ((uintptr_t)Y & 1) || ((uintptr_t)sA & 3)) return MQ_ERR_INVALID_ARG;
+  if (((uintptr_t)dbg0 & 15) || ((uintptr_t)dbg1 & 15)) return MQ_ERR_INVALID_ARG;
   int rc = mq::check_device();
   if (rc != MQ_OK) return rc;
   EncodeTiledFn enc = get_encode_fn();
@@ -887,6 +1008,7 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   gp.y_bf16 = y_dtype == MQ_BF16;
   uint8_t* ws = (uint8_t*)workspace;
   gp.ws_cnt = (int32_t*)ws;
+  gp.ws_done = (int32_t*)(ws + pl.off_done);
   gp.ws_flag = (int32_t*)(ws + pl.off_flag);
   gp.ws_part = (int32_t*)(ws + pl.off_part);
 #ifdef MQ_TRACE

@@ -72,6 +72,7 @@ struct Options {
   int64_t split_k = 0;
   int64_t token_tile = 0;
   int64_t max_ctas = 0;
+  int64_t pdl = 1;   // launch kernels as programmatic dependents of their predecessor in the stream
 };
 Options& options();
 void set_launch_count(int n);

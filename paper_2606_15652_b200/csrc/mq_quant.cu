@@ -13,6 +13,7 @@
 #include <cstring>
 
 #include "mq_internal.h"
+#include "mq_ptx.cuh"
 
 namespace mq {
 
@@ -86,6 +87,10 @@ __device__ __forceinline__ uint32_t quant_pack8(const float* f, float s) {
 template <bool BF16, int CHUNKS>
 __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __restrict__ A, int64_t lda, int K,
                                                              uint8_t* __restrict__ qA, float* __restrict__ sA) {
+  // PDL: the next kernel (mq_gemm) may start its prologue and weight prefetch now; A may have been
+  // written by the previous kernel, so wait for it before the first load.
+  mq::ptx::griddep_launch();
+  mq::ptx::griddep_wait();
   const int64_t m = blockIdx.x;
   const uint4* row = reinterpret_cast<const uint4*>(A + m * lda);
   uint32_t* qrow = reinterpret_cast<uint32_t*>(qA + m * (int64_t)(K / 2));
@@ -176,6 +181,9 @@ extern "C" int mq_set_option(const char* name, int64_t value) {
     o.token_tile = value;
   } else if (!strcmp(name, "max_ctas")) {
     o.max_ctas = value;
+  } else if (!strcmp(name, "pdl")) {
+    if (value > 1) return MQ_ERR_INVALID_ARG;
+    o.pdl = value;
   } else {
     return MQ_ERR_INVALID_ARG;
   }
@@ -204,16 +212,33 @@ extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64
   const uint16_t* a = (const uint16_t*)A;
   dim3 grid((unsigned)M), blk(QT);
   const int nchunk_per_thread = (int)((K / 8 + QT - 1) / QT);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = blk;
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = mq::options().pdl ? 1 : 0;
+  const int Ki = (int)K;
+  uint8_t* q8 = (uint8_t*)qA;
+  cudaError_t le;
   if (a_dtype == MQ_BF16) {
     if (nchunk_per_thread <= 2)
-      mq_quantize_act_kernel<true, 2><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 2>, a, lda, Ki, q8, sA);
     else
-      mq_quantize_act_kernel<true, 4><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 4>, a, lda, Ki, q8, sA);
   } else {
     if (nchunk_per_thread <= 2)
-      mq_quantize_act_kernel<false, 2><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 2>, a, lda, Ki, q8, sA);
     else
-      mq_quantize_act_kernel<false, 4><<<grid, blk, 0, st>>>(a, lda, (int)K, (uint8_t*)qA, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 4>, a, lda, Ki, q8, sA);
+  }
+  if (le != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
   }
   mq::set_launch_count(1);
   if (cudaGetLastError() != cudaSuccess) return MQ_ERR_CUDA;
