@@ -57,8 +57,6 @@ using namespace mq::ptx;
 
 constexpr int FIRST_EPI_WARP = 2;
 constexpr int FIRST_UNPACK_WARP = 6;
-constexpr int NUM_UNPACK_GROUPS = 2;
-constexpr int NUM_THREADS = 32 * (FIRST_UNPACK_WARP + 4 * NUM_UNPACK_GROUPS);  // 448
 constexpr int A_COLS = BK / 4;               // 32 TMEM columns hold 128 int8 per lane (one K-step)
 
 // per-K-step metadata word handed from the producer to the unpack groups and the MMA warp
@@ -71,19 +69,25 @@ constexpr int META_LAST = 1 << 29;           // last K-step of the segment: accu
 
 template <int BT>
 struct Cfg {
+  // Unpack groups (4 warps each).  An item costs a group ~1000 cycles of mostly latency (loads,
+  // TMEM/shared stores, proxy fences), so prefill runs four groups side by side.
+  static constexpr int G = BT == 128 ? 4 : 2;
+  static constexpr int NUM_THREADS = 32 * (FIRST_UNPACK_WARP + 4 * G);
   static constexpr int SK = BT <= 32 ? 4 : 2;                    // K-steps per P stage
   static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // K-steps per U stage (item)
   static constexpr int IPS = SK / UK;                            // items per P stage
   static constexpr int PSTAGES = BT <= 32 ? 4 : (BT == 64 ? 6 : 4);
-  static constexpr int USTAGES = 2;                                   // one per unpack group
+  static constexpr int USTAGES = G;                                   // one per unpack group
   // Unpacked residual cells (TMEM): every unpack group owns a private ring of RG stages.  A ring
   // shared between the groups would be unsafe: mbarrier parity waits cannot tell "my turn" from
   // "two phases early", and cells fall on the groups irregularly.
   static constexpr int RG = BT <= 32 ? 2 : 1;
-  static constexpr int RSTAGES = NUM_UNPACK_GROUPS * RG;
-  static constexpr int QG = BT == 16 ? 8 : 4;                         // packed residual quarter slots (2 KB) per group,
-  static constexpr int NQ = NUM_UNPACK_GROUPS * QG;                   // private for the same reason
-  static constexpr int ACC0_STAGES = 2;
+  static constexpr int RSTAGES = G * RG;
+  static constexpr int QG = BT == 16 ? 8 : (BT == 128 ? 2 : 4);       // packed residual quarter slots (2 KB) per group,
+  static constexpr int NQ = G * QG;                   // private for the same reason
+  // BT = 128: two 128-column accumulators + four operand stages fill the 512 TMEM columns, so the
+  // base accumulator is single-buffered there (the epilogue of a tile is not overlapped).
+  static constexpr int ACC0_STAGES = BT == 128 ? 1 : 2;
   static constexpr int ACC1_STAGES = BT <= 64 ? 2 : 1;
   static constexpr int P_W = SK * TILE_BYTES;
   static constexpr int P_TOK = BT * SK * (BK / 2);
@@ -97,7 +101,7 @@ struct Cfg {
   static constexpr int TMEM_NEED = R_COL0 + RSTAGES * A_COLS;
   static constexpr int TMEM_COLS = TMEM_NEED <= 32 ? 32 : (TMEM_NEED <= 64 ? 64 : (TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512)));
   static_assert(TMEM_NEED <= 512, "tensor memory budget");
-  static_assert(NUM_UNPACK_GROUPS == 2 && USTAGES >= NUM_UNPACK_GROUPS, "ring safety: groups <= stages");
+  static_assert((G & (G - 1)) == 0 && USTAGES >= G, "ring safety: groups <= stages");
   // shared memory map (offsets from a 1024-aligned base)
   static constexpr int OFF_U = 0;
   static constexpr int OFF_P = OFF_U + USTAGES * U_STAGE;
@@ -246,7 +250,7 @@ __device__ __forceinline__ void store_y(void* Y, size_t o, float y) {
 }
 
 template <int BT>
-__global__ void __launch_bounds__(NUM_THREADS, 1)
+__global__ void __launch_bounds__(Cfg<BT>::NUM_THREADS, 1)
 mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   using C = Cfg<BT>;
   constexpr int SK = C::SK, UK = C::UK, IPS = C::IPS;
@@ -356,8 +360,15 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     griddep_wait();
     bool have = it.next<SK>(cur);
     int ps = 0, si = 0;
-    int qseq_g0 = 0, qseq_g1 = 0;   // residual quarters handed to unpack group 0 / 1 so far
-    int rseq_g0 = 0, rseq_g1 = 0;   // residual cells handed to unpack group 0 / 1 so far
+    int qseq_g[C::G], rseq_g[C::G];   // residual quarters / cells handed to each unpack group so far
+#pragma unroll
+    for (int g2 = 0; g2 < C::G; ++g2) qseq_g[g2] = rseq_g[g2] = 0;
+    auto pick = [&](const int* a, int g2) {   // a[g2] without dynamic register indexing
+      int v = a[0];
+#pragma unroll
+      for (int i = 1; i < C::G; ++i) v = g2 == i ? a[i] : v;
+      return v;
+    };
     uint32_t pphase = 0;
     while (have) {
       const bool have_n = it.next<SK>(nxt);
@@ -396,22 +407,24 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       const int mask = lane < cur.nks ? (um.x & 0xF) : 0;
       const uint32_t nz = __ballot_sync(0xffffffffu, mask != 0);
       // the unpack group that will handle K-step `lane` of this stage: item index mod 2
-      const int my_group = (si * IPS + (lane < SK ? lane : 0) / UK) & (NUM_UNPACK_GROUPS - 1);
-      const uint32_t g1_lanes = __ballot_sync(0xffffffffu, my_group != 0);
+      const int my_group = (si * IPS + (lane < SK ? lane : 0) / UK) & (C::G - 1);
       // quarters stored by the cells of the lower lanes of the same group (SK <= 4: plain loop)
-      int qbefore = 0;
+      int qbefore = 0, cbefore = 0;   // ... and cells
 #pragma unroll
       for (int j = 0; j < SK; ++j) {
         const int mj = __shfl_sync(0xffffffffu, mask, j);
         const int gj = __shfl_sync(0xffffffffu, my_group, j);
-        if (j < lane && gj == my_group) qbefore += __popc(mj);
+        if (j < lane && gj == my_group) {
+          qbefore += __popc(mj);
+          cbefore += mj != 0;
+        }
       }
       if (lane < SK) {
         int word = 0;
         if (lane < cur.nks) {
-          const int my_rseq = (my_group ? rseq_g1 : rseq_g0) + __popc(nz & (my_group ? g1_lanes : ~g1_lanes) & ((1u << lane) - 1u));
+          const int my_rseq = pick(rseq_g, my_group) + cbefore;
           word = META_VALID | mask | ((my_rseq & 0xFF) << 4) |
-                 ((((my_group ? qseq_g1 : qseq_g0) + qbefore) & 0xFFFF) << 12);
+                 (((pick(qseq_g, my_group) + qbefore) & 0xFFFF) << 12);
           if (cur.first && lane == 0) word |= META_FIRST;
           if (cur.last && lane == cur.nks - 1) word |= META_LAST;
         }
@@ -427,7 +440,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         const int m = __shfl_sync(0xffffffffu, mask, j);
         const int gj = __shfl_sync(0xffffffffu, my_group, j);
         const uint8_t* rsrc = p.res + (size_t)__shfl_sync(0xffffffffu, um.y, j) * QUARTER_BYTES;
-        const int q0 = gj ? qseq_g1 : qseq_g0;
+        const int q0 = pick(qseq_g, gj);
         for (int q = 0; q < __popc(m); ++q) {
           const int slot = gj * C::QG + (q0 + q) % C::QG;
           mbar_wait(bar(B_EMPTY_Q + slot), (((uint32_t)(q0 + q) / C::QG) & 1) ^ 1);
@@ -438,13 +451,13 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             tma_load_1d(sRP + slot * QUARTER_BYTES, rsrc + (size_t)q * QUARTER_BYTES, QUARTER_BYTES, rb);
           }
         }
-        if (gj)
-          qseq_g1 += __popc(m);
-        else
-          qseq_g0 += __popc(m);
+#pragma unroll
+        for (int g2 = 0; g2 < C::G; ++g2)
+          if (gj == g2) {
+            qseq_g[g2] += __popc(m);
+            rseq_g[g2] += 1;
+          }
       }
-      rseq_g0 += __popc(nz & ~g1_lanes);
-      rseq_g1 += __popc(nz & g1_lanes);
       if (++ps == C::PSTAGES) {
         ps = 0;
         pphase ^= 1;
@@ -495,9 +508,12 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
             tc_fence_after();
           }
-          const int rseq = (m >> 4) & 0xFF, rs = (item & (NUM_UNPACK_GROUPS - 1)) * C::RG + rseq % C::RG;
-          mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RG) & 1);
-          tc_fence_after();
+          const int rseq = (m >> 4) & 0xFF;
+          const int rs = UK == 1 ? us : (item & (C::G - 1)) * C::RG + rseq % C::RG;
+          if constexpr (UK != 1) {   // UK == 1: the cell was published together with its U stage
+            mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RG) & 1);
+            tc_fence_after();
+          }
           __syncwarp();
           const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + rs * A_COLS);
           if (elect_one()) {
@@ -511,7 +527,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
                   on = 1;
                 }
               }
-            tc_commit(bar(B_EMPTY_RU + rs));
+            if constexpr (UK != 1) tc_commit(bar(B_EMPTY_RU + rs));
           }
           acc1_on = 1;
         }
@@ -541,7 +557,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     const uint32_t gtid = (uint32_t)(((warp - FIRST_UNPACK_WARP) & 3) * 32 + lane);
     const uint32_t lane_addr = tmem_base + ((uint32_t)(wq * 32) << 16);
     const int rhalf = wq >> 1;                                    // row half of a residual cell
-    for (int item = gi; item < n_items; item += NUM_UNPACK_GROUPS) {
+    for (int item = gi; item < n_items; item += C::G) {
       const int stage = item / IPS, sub = item - stage * IPS;
       const int ps = stage % C::PSTAGES, us = item % C::USTAGES;
       mbar_wait(bar(B_FULL_P + ps), ((uint32_t)stage / C::PSTAGES) & 1);
@@ -550,6 +566,89 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 #pragma unroll
       for (int j = 0; j < UK; ++j) mw[j] = lds32(sMetaP + 4u * (uint32_t)(ps * SK + sub * UK + j));
       const uint32_t pw = sP + ps * C::P_STAGE + sub * UK * TILE_BYTES;
+      if constexpr (UK == 1) {
+        // Prefill path: the packed operands are loaded into registers BEFORE waiting for the U stage,
+        // so that the stage's turnaround (MMA done -> next item published) is the int4 -> int8
+        // expansion (2 logic ops per 8 elements), the stores and the fences.  The cell's unpacked weights ride in the U stage's own residual columns
+        // (R stage = U stage), so FULL_U / EMPTY_U cover them and no separate hand-off is needed.
+        static_assert(UK != 1 || (BT * 4) % 128 == 0, "token chunks per thread");
+        constexpr int TCH = BT * 4 / 128;   // 16-byte packed token chunks per thread
+        const int m = mw[0];
+        const bool valid = (m & META_VALID) != 0;
+        const int mask = valid ? (m & 0xF) : 0;
+        uint4 v4[4], t4[TCH];   // packed operands stay packed (32 registers) across the wait
+        if (valid) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) v4[c] = lds128(pw + c * (BN * 16) + row * 16);
+          const uint32_t pt1 = sP + ps * C::P_STAGE + C::P_W + sub * (BT * (BK / 2));
+#pragma unroll
+          for (int i = 0; i < TCH; ++i) t4[i] = lds128(pt1 + (gtid + 128u * i) * 16);
+          // the loads must have landed before the P stage is handed back
+          asm volatile("" ::"r"(v4[0].x), "r"(v4[1].x), "r"(v4[2].x), "r"(v4[3].x));
+#pragma unroll
+          for (int i = 0; i < TCH; ++i) asm volatile("" ::"r"(t4[i].x));
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(B_EMPTY_P + ps));   // this warp's reads of the P stage are done
+        mbar_wait(bar(B_EMPTY_U + us), (((uint32_t)item / C::USTAGES) & 1) ^ 1);
+        tc_fence_after();
+        if (valid) {
+          {
+            uint32_t o[32];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) unpack16(v4[c], o + 8 * c);
+            tmem_st32(lane_addr + (uint32_t)(C::A_COL0 + us * A_COLS), o);
+          }
+          if (mask) {
+            // residual cell (about one item in five): expanded after the base columns are on their
+            // way, so that its registers do not add to the hot path's pressure
+            const int qseq0 = (m >> 12) & 0xFFFF;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              if (!(mask & (3 << (2 * h)))) continue;   // k-half without any block: never read by the MMA
+              const int q = 2 * h + rhalf;
+              uint32_t ro[16];
+              if (mask & (1 << q)) {
+                const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
+                const int slot = gi * C::QG + qs % C::QG;
+                mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::QG) & 1);
+                const uint32_t rp = sRP + slot * QUARTER_BYTES;
+                const uint4 r0 = lds128(rp + (row & 63) * 16);
+                const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
+                unpack16(r0, ro);
+                unpack16(r1, ro + 8);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot));
+              } else {
+#pragma unroll
+                for (int z = 0; z < 16; ++z) ro[z] = 0;
+              }
+              tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + us * A_COLS + 16 * h), ro);
+            }
+          }
+          const uint32_t ut1 = sU + us * C::U_STAGE;
+#pragma unroll
+          for (int i = 0; i < TCH; ++i) {
+            const uint32_t idx = gtid + 128u * i, t = idx >> 2, c = idx & 3;
+            uint32_t tw[8];
+            unpack16(t4[i], tw);
+            sts128(ut1 + t * 128 + (((2 * c) ^ (t & 7)) << 4), tw);
+            sts128(ut1 + t * 128 + (((2 * c + 1) ^ (t & 7)) << 4), tw + 4);
+          }
+        }
+        tmem_st_wait();
+        tc_fence_before();
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          MQ_STAMP_IF(item == 0 && gtid == 0, 5);
+          MQ_STAMP_IF(gi == 0 && gtid == 0 && item < 32, 16 + item / 2);
+          MQ_STAMP_IF(gi == 0 && gtid == 0, 6);
+          if (wq == 0) sts32(sMetaU + 4u * (uint32_t)us, m);
+          mbar_arrive(bar(B_FULL_U + us));
+        }
+        continue;
+      }
       // the first K-step's packed weights are fetched before the U stage is known to be free
       uint4 v[4];
 #pragma unroll
@@ -662,9 +761,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       const int n = nt * BN + n_loc;
       const int t_base = tt * BT;
       const int t_cnt = min(BT, p.M - t_base);
-      const float swn = p.sw[n] * 0.00390625f, srn = p.sr[n] * 0.00390625f;  // / 256: accumulators are x256
-      auto emit = [&](int t, int32_t a0, int32_t a1) {
-        const float y = p.sa[t_base + t] * ((float)a0 * swn + (float)a1 * srn);
+      const float swn = __ldg(p.sw + n) * 0.00390625f, srn = __ldg(p.sr + n) * 0.00390625f;  // / 256: accumulators are x256
+      auto emit = [&](int t, float sat, int32_t a0, int32_t a1) {
+        const float y = sat * ((float)a0 * swn + (float)a1 * srn);
         const size_t o = (size_t)(t_base + t) * p.ldy + n;
         if (p.y_bf16)
           store_y<true>(p.Y, o, y);
@@ -690,6 +789,12 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 
       for (int c0 = 0; c0 < t_cnt; c0 += 16) {
         uint32_t v0[16], v1[16];
+        float sav[16];   // token scales of the chunk, fetched up front (read-only path: one L2 round trip
+                         // per chunk instead of one per token behind the stores)
+        if (whole) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) sav[i] = c0 + i < t_cnt ? __ldg(p.sa + t_base + c0 + i) : 0.f;
+        }
         tmem_ld16(t0addr + c0, v0);
         if (has_res) {
           tmem_ld16(t1addr + c0, v1);
@@ -701,7 +806,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (whole) {
 #pragma unroll
           for (int i = 0; i < 16; ++i)
-            if (c0 + i < t_cnt) emit(c0 + i, (int32_t)v0[i], (int32_t)v1[i]);
+            if (c0 + i < t_cnt) emit(c0 + i, sav[i], (int32_t)v0[i], (int32_t)v1[i]);
         } else {
 #pragma unroll
           for (int i = 0; i < 16; ++i)
@@ -783,7 +888,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
         const int n = nt * BN + n0;
         const float4 sw4 = *reinterpret_cast<const float4*>(p.sw + n), sr4 = *reinterpret_cast<const float4*>(p.sr + n);
-        const float sat = p.sa[t_base + t] * 0.00390625f;    // / 256: accumulators are x256
+        const float sat = __ldg(p.sa + t_base + t) * 0.00390625f;    // / 256: accumulators are x256
         float y[4];
         y[0] = sat * ((float)s0.x * sw4.x + (float)s1.x * sr4.x);
         y[1] = sat * ((float)s0.y * sw4.y + (float)s1.y * sr4.y);
@@ -923,7 +1028,7 @@ int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
-  cfg.blockDim = dim3(NUM_THREADS);
+  cfg.blockDim = dim3(C::NUM_THREADS);
   cfg.dynamicSmemBytes = C::SMEM_BYTES;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
