@@ -295,7 +295,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     }
     for (int i = 0; i < C::NQ; ++i) {
       mbar_init(bar(B_FULL_Q + i), 1);
-      mbar_init(bar(B_EMPTY_Q + i), 2);         // the two unpack warps that own the quarter's 64 rows
+      mbar_init(bar(B_EMPTY_Q + i), 4);         // every warp of the owning unpack group
     }
     for (int i = 0; i < C::RSTAGES; ++i) {
       mbar_init(bar(B_FULL_RU + i), 4);
@@ -606,22 +606,28 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
               if (!(mask & (3 << (2 * h)))) continue;   // k-half without any block: never read by the MMA
-              const int q = 2 * h + rhalf;
               uint32_t ro[16];
-              if (mask & (1 << q)) {
+#pragma unroll
+              for (int z = 0; z < 16; ++z) ro[z] = 0;
+              // EVERY warp of the group passes through every present quarter's barrier, in ring
+              // order, whether or not the quarter holds its rows: a parity wait is only sound for a
+              // waiter that has seen the slot's previous phase.
+#pragma unroll
+              for (int r = 0; r < 2; ++r) {
+                const int q = 2 * h + r;
+                if (!(mask & (1 << q))) continue;
                 const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
                 const int slot = gi * C::QG + qs % C::QG;
                 mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::QG) & 1);
-                const uint32_t rp = sRP + slot * QUARTER_BYTES;
-                const uint4 r0 = lds128(rp + (row & 63) * 16);
-                const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
-                unpack16(r0, ro);
-                unpack16(r1, ro + 8);
+                if (r == rhalf) {
+                  const uint32_t rp = sRP + slot * QUARTER_BYTES;
+                  const uint4 r0 = lds128(rp + (row & 63) * 16);
+                  const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
+                  unpack16(r0, ro);
+                  unpack16(r1, ro + 8);
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot));
-              } else {
-#pragma unroll
-                for (int z = 0; z < 16; ++z) ro[z] = 0;
               }
               tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + us * A_COLS + 16 * h), ro);
             }
@@ -711,23 +717,29 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
             if (!(mask & (3 << (2 * h)))) continue;   // k-half without any block: never read by the MMA
-            const int q = 2 * h + rhalf;
             uint32_t ro[16];
-            if (mask & (1 << q)) {
-              // the cell's present quarters sit in consecutive ring slots in ascending q
+#pragma unroll
+            for (int z = 0; z < 16; ++z) ro[z] = 0;
+            // the cell's present quarters sit in consecutive ring slots in ascending q; EVERY warp of
+            // the group passes through every present quarter's barrier, in ring order, whether or not
+            // the quarter holds its rows (a parity wait is only sound for a waiter that has seen the
+            // slot's previous phase)
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+              const int q = 2 * h + r;
+              if (!(mask & (1 << q))) continue;
               const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
               const int slot = gi * C::QG + qs % C::QG;
               mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::QG) & 1);
-              const uint32_t rp = sRP + slot * QUARTER_BYTES;
-              const uint4 r0 = lds128(rp + (row & 63) * 16);
-              const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
-              unpack16(r0, ro);
-              unpack16(r1, ro + 8);
+              if (r == rhalf) {
+                const uint32_t rp = sRP + slot * QUARTER_BYTES;
+                const uint4 r0 = lds128(rp + (row & 63) * 16);
+                const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
+                unpack16(r0, ro);
+                unpack16(r1, ro + 8);
+              }
               __syncwarp();
               if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot));
-            } else {
-#pragma unroll
-              for (int z = 0; z < 16; ++z) ro[z] = 0;
             }
             tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + rs * A_COLS + 16 * h), ro);
           }
@@ -803,7 +815,25 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           for (int i = 0; i < 16; ++i) v1[i] = 0;
         }
         tmem_ld_wait();
-        if (whole) {
+        if (whole && !p.dbg0 && !p.dbg1 && c0 + 16 <= t_cnt) {
+          // hot path (full chunk, no parity hooks): branch-free, one pointer bump per token
+          uint16_t* yp = reinterpret_cast<uint16_t*>(p.Y) + (size_t)(t_base + c0) * p.ldy + n;
+          if (p.y_bf16) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              const float y = sav[i] * ((float)(int32_t)v0[i] * swn + (float)(int32_t)v1[i] * srn);
+              *yp = __bfloat16_as_ushort(__float2bfloat16_rn(y));
+              yp += p.ldy;
+            }
+          } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              const float y = sav[i] * ((float)(int32_t)v0[i] * swn + (float)(int32_t)v1[i] * srn);
+              *yp = __half_as_ushort(__float2half_rn(y));
+              yp += p.ldy;
+            }
+          }
+        } else if (whole) {
 #pragma unroll
           for (int i = 0; i < 16; ++i)
             if (c0 + i < t_cnt) emit(c0 + i, sav[i], (int32_t)v0[i], (int32_t)v1[i]);
