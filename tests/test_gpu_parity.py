@@ -309,3 +309,57 @@ def test_m_zero_is_noop(mq):
     assert L.mq_gemm(w.handle, None, None, 0, None, 1, 128, None, None, None, 0, None) == 0
     assert L.mq_quantize_act(None, 0, 0, 256, 256, None, None, None) == 0
     torch.cuda.synchronize()
+
+
+def _random_block_case(seed, M, K, N, bs, rho):
+    """A case whose selected set is a seeded uniform-random block set (control pattern (u) of
+    DESIGN.md section 4) instead of the Delta-score top-K: it produces residual cells with every
+    quarter mask, including three and four 64x64 blocks inside one 128x128 cell."""
+    import dataclasses
+    case = make_case(seed, M, K, N, bs=bs, budget=0)
+    nb = (N // bs) * (K // bs)
+    rng = np.random.default_rng(seed)
+    sel = np.sort(rng.choice(nb, size=int(rho * nb + 0.5), replace=False))
+    L = dataclasses.replace(case.L, blk_n=(sel // (K // bs)).astype(np.int32), blk_k=(sel % (K // bs)).astype(np.int32))
+    return dataclasses.replace(case, L=L)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("M,K,N,rho,mode", [
+    (8, 2048, 512, 0.35, 0), (32, 2048, 512, 0.6, 0), (200, 2048, 512, 0.35, 1), (200, 2048, 512, 0.6, 2),
+    (300, 1024, 1024, 1.0, 1),
+])
+def test_gemm_irregular_dense_residual_cells(mq, M, K, N, rho, mode):
+    """Residual cells of every shape (1-4 quarters), many per tile, through every ring of the kernel:
+    decode tiles, prefill tiles with whole tiles (mode 1) and with stream-K partial tiles (mode 2).
+    Repeated calls on one workspace must stay bit-identical (ring/phase bookkeeping, counters)."""
+    case = _random_block_case(77 + M, M, K, N, 64, rho)
+    want = oracle_forward(case)
+    try:
+        mq.mq_set_option("split_k", mode)
+        w = pack_from_oracle(case)
+        ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+        for rep in range(3):
+            got = run_cuda(case, w=w, workspace=ws)
+            assert_parity(got, want, what=f"irregular residual M{M} rho{rho} mode{mode} rep{rep}")
+    finally:
+        mq.mq_set_option("split_k", 0)
+
+
+@pytest.mark.gpu
+def test_gemm_no_hooks_path_matches_hooked_path(mq):
+    """The epilogue's hot path (no parity hooks) and the hooked path must give the same Y bits;
+    back-to-back launches exercise programmatic dependent launch on one workspace."""
+    import torch
+    for (M, K, N) in [(4, 1024, 384), (160, 1024, 384), (260, 2048, 256)]:
+        case = _random_block_case(5 + M, M, K, N, 64, 0.2)
+        w = pack_from_oracle(case)
+        A = to_device_act(case)
+        qA, sA = mq.mq_quantize_act(A)
+        ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+        Yh, _, _ = mq.mq_gemm(w, qA, sA, M, out_dtype=torch.bfloat16, dbg=True, workspace=ws)
+        Y = torch.empty_like(Yh)
+        for _ in range(4):
+            mq.mq_gemm(w, qA, sA, M, Y=Y, workspace=ws)
+        torch.cuda.synchronize()
+        assert torch.equal(Y.view(torch.int16), Yh.view(torch.int16)), (M, K, N)
