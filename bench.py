@@ -133,30 +133,24 @@ class Layer:
             self.ws[m] = mq.new_workspace(mq.mq_gemm_workspace_bytes(w0, m))
 
 
-def run_ours(args, rank, world):
-    import torch
-    import synth
-    import paper_2606_15652_b200 as mq
-
-    mq.lib()  # no fallback: raises if libmq.so is missing
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    assert torch.cuda.get_device_capability() == (10, 0), "bench.py needs a B200 (sm_100a)"
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    peaks = load_peaks()
-    cfg, shapes = workload_shapes(args.workload)
+def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_e2e=True):
+    """Times one workload (BASELINE.json config): the whole step, the GEMM kernels alone (roofline),
+    the cuBLAS bf16 comparator and the end-to-end path through mq_linear with host buffers."""
+    cfg, _ = workload_shapes(workload)
     Ms, layers_cfg = cfg["Ms"], cfg["layers"]
     layers = [Layer(mq, torch, synth, cfg["seed"] + i, l, Ms, N_COPIES) for i, l in enumerate(layers_cfg)]
     calls = [(m, L) for m in Ms for L in layers]           # one step, in order
 
-    def step(si: int, only_gemm: bool = False):
+    def step(si: int):
         for ci, (m, L) in enumerate(calls):
             w = L.copies[(si * len(Ms) + ci // len(layers)) % N_COPIES]
-            if not only_gemm:
-                mq.mq_quantize_act(L.A[m], L.qA[m], L.sA[m])
+            mq.mq_quantize_act(L.A[m], L.qA[m], L.sA[m])
             mq.mq_gemm(w, L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
 
     stream = torch.cuda.Stream()
     torch.cuda.synchronize()
@@ -169,13 +163,7 @@ def run_ours(args, rank, world):
             with torch.cuda.graph(g, stream=stream):
                 step(si)
             graphs.append(g)
-
-        def barrier():
-            if world > 1:
-                dist.barrier()
-            torch.cuda.synchronize()
-
-        for i in range(args.warmup):
+        for i in range(warmup):
             graphs[i % N_COPIES].replay()
         barrier()
         sampler = ClockSampler(local)
@@ -183,11 +171,11 @@ def run_ours(args, rank, world):
         time.sleep(0.25)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        for i in range(args.steps):
-            graphs[(args.warmup + i) % N_COPIES].replay()
+        for i in range(steps):
+            graphs[(warmup + i) % N_COPIES].replay()
         e1.record(stream)
         barrier()
-        ms_total = e0.elapsed_time(e1)
+        ms_step = e0.elapsed_time(e1) / steps
         clocks = sampler.stop()
 
         # ---- roofline of the dominant kernel (mq_gemm_kernel), timed alone: graphs of GEMM launches only
@@ -233,81 +221,139 @@ def run_ours(args, rank, world):
             g16[i % 2].replay()
         c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         c0.record(stream)
-        for i in range(args.steps):
+        for i in range(steps):
             g16[i % 2].replay()
         c1.record(stream)
         stream.synchronize()
-        ms16 = c0.elapsed_time(c1) / args.steps
-        del w16, g16
+        ms16 = c0.elapsed_time(c1) / steps
+        del w16, g16, a16
 
         # ---- e2e: host buffers through the C ABI (mq_linear), H2D + D2H inside the timed region
-        Yh = {(m, L.name): torch.empty((m, L.N), dtype=torch.bfloat16).pin_memory() for (m, L) in calls}
-        Ad = {(m, L.name): torch.empty_like(L.A[m]) for (m, L) in calls}
-        lws = {(m, L.name): mq.new_workspace(mq.mq_linear_workspace_bytes(L.copies[0], m)) for (m, L) in calls}
+        e2e_ms = None
+        if with_e2e:
+            Yh = {(m, L.name): torch.empty((m, L.N), dtype=torch.bfloat16).pin_memory() for (m, L) in calls}
+            Ad = {(m, L.name): torch.empty_like(L.A[m]) for (m, L) in calls}
+            lws = {(m, L.name): mq.new_workspace(mq.mq_linear_workspace_bytes(L.copies[0], m)) for (m, L) in calls}
 
-        def step_e2e(si):
-            for ci, (m, L) in enumerate(calls):
-                k = (m, L.name)
-                Ad[k].copy_(L.A_host[m], non_blocking=True)
-                mq.mq_linear(L.copies[(si * len(Ms) + ci // len(layers)) % N_COPIES], Ad[k], Y=L.Y[m], workspace=lws[k])
-                Yh[k].copy_(L.Y[m], non_blocking=True)
-            stream.synchronize()                                 # the caller reads the result
+            def step_e2e(si):
+                for ci, (m, L) in enumerate(calls):
+                    k = (m, L.name)
+                    Ad[k].copy_(L.A_host[m], non_blocking=True)
+                    mq.mq_linear(L.copies[(si * len(Ms) + ci // len(layers)) % N_COPIES], Ad[k], Y=L.Y[m], workspace=lws[k])
+                    Yh[k].copy_(L.Y[m], non_blocking=True)
+                stream.synchronize()                                 # the caller reads the result
 
-        for i in range(3):
-            step_e2e(i)
-        barrier()
-        t0 = time.perf_counter()
-        for i in range(args.steps):
-            step_e2e(i)
-        torch.cuda.synchronize()
-        e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+            for i in range(3):
+                step_e2e(i)
+            barrier()
+            t0 = time.perf_counter()
+            for i in range(steps):
+                step_e2e(i)
+            torch.cuda.synchronize()
+            e2e_ms = (time.perf_counter() - t0) * 1e3 / steps
 
-    ms_step = ms_total / args.steps
     if world > 1:
-        t = torch.tensor([ms_step, e2e_ms], device="cuda", dtype=torch.float64)
+        t = torch.tensor([ms_step, e2e_ms or 0.0], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step, e2e_ms = float(t[0]), float(t[1])
-    ops_step = sum(algo_ops(m, L.K, L.N, L.nnz, BS) for (m, L) in calls)
-    bytes_step = sum(algo_bytes(m, L.K, L.N, L.nnz, BS) for (m, L) in calls)
-    tokens_step = sum(Ms)
-    gemm_us = sum(s["us"] for s in per_shape)
-    gemm_bytes = sum(s["bytes"] for s in per_shape)
-    achieved = gemm_bytes / (gemm_us * 1e-6) / 1e9
-    h2d = sum(L.A_host[m].numel() * 2 for (m, L) in calls)
-    d2h = sum(m * L.N * 2 for (m, L) in calls)
+        ms_step, e2e_ms = float(t[0]), (float(t[1]) if with_e2e else None)
+    return dict(cfg=cfg, Ms=Ms, layers_cfg=layers_cfg, layers=layers, calls=calls, ms_step=ms_step, clocks=clocks,
+                per_shape=per_shape, ms16=ms16, e2e_ms=e2e_ms,
+                ops_step=sum(algo_ops(m, L.K, L.N, L.nnz, BS) for (m, L) in calls),
+                bytes_step=sum(algo_bytes(m, L.K, L.N, L.nnz, BS) for (m, L) in calls),
+                h2d=sum(L.A_host[m].numel() * 2 for (m, L) in calls), d2h=sum(m * L.N * 2 for (m, L) in calls),
+                pack_s=sum(L.pack_s for L in layers))
+
+
+def roofline_of(r, peaks, traffic):
+    """Roofline object of the dominant kernel (mq_gemm_kernel, the launches of one step timed alone).
+    Decode-shaped workloads are bound by HBM (algorithmic bytes), prefill-shaped ones by
+    the INT8 tensor pipe; which one is decided by the slower of the two ideal times."""
+    us = sum(s["us"] for s in r["per_shape"])
+    by = sum(s["bytes"] for s in r["per_shape"])
+    ops = sum(s["ops"] for s in r["per_shape"])
+    int8_peak = 2.0 * peaks["bf16_tflops"]          # kind::i8 runs at twice the bf16 rate (nominal 4.5 vs 2.25 PF)
+    t_hbm, t_tensor = by / (peaks["hbm_gbs"] * 1e9), ops / (int8_peak * 1e12)
+    per_shape = [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3),
+                      gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
+                      tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in r["per_shape"]]
+    kern = f"mq_gemm_kernel ({len(r['per_shape'])} launches of the step, timed alone, cold weights)"
+    if t_hbm >= t_tensor:
+        a = by / (us * 1e-6) / 1e9
+        return {"bound": "hbm", "achieved": a, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": a / peaks["hbm_gbs"],
+                "traffic": traffic, "peak_source": peaks["source"], "kernel": kern, "per_shape": per_shape}
+    a = ops / (us * 1e-6) / 1e12
+    return {"bound": "tensor", "achieved": a, "peak": int8_peak, "unit": "TFLOP/s", "frac": a / int8_peak,
+            "traffic": traffic, "peak_source": peaks["source"] + " bf16 burst x 2 (int8 : bf16 nominal ratio)",
+            "kernel": kern, "per_shape": per_shape}
+
+
+def load_traffic(workload):
+    """dram__bytes_read + dram__bytes_write of the dominant kernel per step, from the committed ncu
+    summary (profiles/traffic.json, written by hand from an `ncu --set full` capture); None if absent."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(workload)
+    return None
+
+
+def run_ours(args, rank, world):
+    import torch
+    import synth
+    import paper_2606_15652_b200 as mq
+
+    mq.lib()  # no fallback: raises if libmq.so is missing
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    assert torch.cuda.get_device_capability() == (10, 0), "bench.py needs a B200 (sm_100a)"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = load_peaks()
+    r = measure(args.workload, args.steps, args.warmup, torch, mq, synth, world, dist, local)
+    Ms, layers_cfg, calls = r["Ms"], r["layers_cfg"], r["calls"]
+    ms_step, e2e_ms = r["ms_step"], r["e2e_ms"]
     out = {
-        "metric": METRIC, "value": world * ops_step / (ms_step * 1e-3) / 1e12, "unit": "TOPS",
+        "metric": METRIC, "value": world * r["ops_step"] / (ms_step * 1e-3) / 1e12, "unit": "TOPS",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int4 storage / int8 MMA / int32 acc",
         "data": "synthetic",
         "config": {"workload": f"{args.workload}: M in {Ms} x {[l.name for l in layers_cfg]} (K,N)="
                                f"{[(l.K, l.N) for l in layers_cfg]}, rho={RHO}, block={BS}, fp16 in, bf16 out",
-                   "step": "mq_quantize_act + mq_gemm for each of the 12 (M, projection) pairs, CUDA-graph replay",
-                   "l2": f"{N_COPIES} rotating weight copies per layer ({N_COPIES * bytes_step / len(Ms) / 1e6:.0f} MB > 3x L2)",
+                   "step": f"mq_quantize_act + mq_gemm for each of the {len(calls)} (M, projection) pairs, CUDA-graph "
+                           "replay, kernels chained by programmatic dependent launch",
+                   "l2": f"{N_COPIES} rotating weight copies per layer ({N_COPIES * r['bytes_step'] / len(Ms) / 1e6:.0f} MB > 3x L2)",
                    "parallelism": "replicas (no collective on the path)" if world > 1 else "single GPU"},
-        "tokens_per_s": world * tokens_step / (ms_step * 1e-3),
-        "hbm_gbs_step": bytes_step / (ms_step * 1e-3) / 1e9,
-        "w16a16_cublas_bf16": {"ms_per_step": ms16, "speedup_vs_w16a16": ms16 / ms_step,
+        "tokens_per_s": world * sum(Ms) / (ms_step * 1e-3),
+        "hbm_gbs_step": r["bytes_step"] / (ms_step * 1e-3) / 1e9,
+        "w16a16_cublas_bf16": {"ms_per_step": r["ms16"], "speedup_vs_w16a16": r["ms16"] / ms_step,
                                "paper_context": "up to 1.24x over W16A16 on RTX 4090 (P:43)"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                     "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
-                     "kernel": "mq_gemm_kernel (12 launches of the step, timed alone, cold weights)",
-                     "per_shape": [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3),
-                                        gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
-                                        tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in per_shape]},
-        "e2e": {"value": world * ops_step / (e2e_ms * 1e-3) / 1e12, "unit": "TOPS", "ms_per_step": e2e_ms,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "api": "mq_linear (C ABI) with pinned host buffers"},
+        "roofline": roofline_of(r, peaks, load_traffic(args.workload)),
+        "e2e": {"value": world * r["ops_step"] / (e2e_ms * 1e-3) / 1e12, "unit": "TOPS", "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"],
+                "api": "mq_linear (C ABI) with pinned host buffers"},
         "gpu_launches": args.steps * 2 * len(calls),
-        "clocks": clocks,
-        "pack_seconds": round(sum(L.pack_s for L in layers), 2),
+        "clocks": r["clocks"],
+        "pack_seconds": round(r["pack_s"], 2),
     }
+    del r
+    if rank == 0 and world == 1 and args.also and args.also != args.workload:
+        # the other regime of the north star (prefill: tensor-bound), same protocol, fewer steps
+        torch.cuda.empty_cache()
+        r2 = measure(args.also, max(3, args.steps // 4), 3, torch, mq, synth, world, dist, local, with_e2e=False)
+        rf = roofline_of(r2, peaks, load_traffic(args.also))
+        out["also"] = {"workload": args.also, "ms_per_step": r2["ms_step"],
+                       "value": r2["ops_step"] / (r2["ms_step"] * 1e-3) / 1e12, "unit": "TOPS",
+                       "tokens_per_s": sum(r2["Ms"]) / (r2["ms_step"] * 1e-3),
+                       "w16a16_cublas_bf16": {"ms_per_step": r2["ms16"], "speedup_vs_w16a16": r2["ms16"] / r2["ms_step"]},
+                       "roofline": rf, "clocks": r2["clocks"]}
+        del r2
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(args.workload, budget_s=20.0)
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
-
 
 # ------------------------------------------------------------------------------------------
 # CPU oracle legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
@@ -404,6 +450,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llama3_8b_decode")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--also", default="llama3_8b_prefill",
+                    help="second workload reported under \"also\" (N=1 only); empty string = skip")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))

@@ -1024,7 +1024,9 @@ Plan make_plan(const mq_weights* w, int64_t M) {
   const int64_t tiles = (int64_t)NT * pl.TT;
   pl.units = tiles * KS;
   // stream-K (ranges cut at K-step granularity) unless there are enough tiles to balance whole ones
-  bool stream_k = tiles < 8LL * G;
+  // Large token tiles pay 128 KB per partial tile in the fix-up, so they split K only when most SMs
+  // would otherwise idle; small (decode) tiles split whenever whole tiles would not balance.
+  bool stream_k = bt <= 32 ? tiles < 8LL * G : tiles * 2 <= G;
   if (o.split_k == 1) stream_k = false;
   if (o.split_k >= 2) stream_k = true;
   pl.gran = stream_k ? 1 : KS;
