@@ -473,11 +473,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     uint32_t acc0_on = 0, acc1_on = 0;
     uint32_t d0 = 0, d1 = 0;
     int a0s = 0, a1s = 0;
-    for (int item = 0; item < n_items; ++item) {
-      const int us = item % C::USTAGES;
-      mbar_wait(bar(B_FULL_U + us), ((uint32_t)item / C::USTAGES) & 1);
+    auto mma_item = [&](const int us, const int item, const uint32_t uphase) {
+      mbar_wait(bar(B_FULL_U + us), uphase);
       tc_fence_after();
-      __syncwarp();
       MQ_STAMP_IF(item == 0 && lane == 0, 7);
       MQ_STAMP_IF(item < 16 && lane == 0, 32 + item);
 #pragma unroll
@@ -548,6 +546,21 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       }
       __syncwarp();
       if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
+    };
+    if constexpr (UK == 1) {
+      // Prefill: the U stages are visited in a fixed rotation and the loop is unrolled over them, so
+      // that every barrier address, TMEM column and shared-memory descriptor of the hot path is a
+      // constant offset (this warp's instruction count per K-step is what paces prefill).
+      for (int item0 = 0; item0 < n_items; item0 += C::USTAGES) {
+        const uint32_t uphase = ((uint32_t)item0 / C::USTAGES) & 1;
+#pragma unroll
+        for (int us = 0; us < C::USTAGES; ++us)
+          if (item0 + us < n_items) mma_item(us, item0 + us, uphase);
+      }
+    } else {
+      // Decode kernels are short: code size (cold instruction cache) matters more than the arithmetic.
+      for (int item = 0; item < n_items; ++item)
+        mma_item(item % C::USTAGES, item, ((uint32_t)item / C::USTAGES) & 1);
     }
   } else if (warp >= FIRST_UNPACK_WARP) {
     // ============ unpack groups: int4 -> int8 (x16); weights -> TMEM, tokens -> smem ============
