@@ -121,6 +121,9 @@ class Layer:
         w0 = mq.mq_pack_weights(self.W, self.h, BS, self.budget)
         self.copies = [w0] + [w0.clone() for _ in range(n_copies - 1)]
         self.nnz = w0.info()["nnz"]
+        # the same layer with budget 0 (dense-only W4A4): the zero-residual baseline of the same kernel
+        z0 = mq.mq_pack_weights(self.W, self.h, BS, 0)
+        self.dense = [z0] + [z0.clone() for _ in range(n_copies - 1)]
         self.pack_s = time.time() - t0
         self.A_host, self.A, self.qA, self.sA, self.Y, self.ws = {}, {}, {}, {}, {}, {}
         for m in Ms:
@@ -198,7 +201,22 @@ def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_
                 a1.record(stream)
                 stream.synchronize()
                 best = min(best, a0.elapsed_time(a1) / reps)
-            per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3,
+            # the zero-residual baseline: same kernel, same protocol, the budget-0 packing of the same W
+            gz = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gz, stream=stream):
+                for r in range(reps):
+                    mq.mq_gemm(L.dense[r % N_COPIES], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+            for _ in range(3):
+                gz.replay()
+            best0 = 1e30
+            for _ in range(5):
+                graphs[0].replay()
+                a0.record(stream)
+                gz.replay()
+                a1.record(stream)
+                stream.synchronize()
+                best0 = min(best0, a0.elapsed_time(a1) / reps)
+            per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3, us_dense=best0 * 1e3,
                                   bytes=algo_bytes(m, L.K, L.N, L.nnz, BS), ops=algo_ops(m, L.K, L.N, L.nnz, BS)))
 
         # ---- W16A16 comparator: cuBLAS bf16 on the same shapes, same rotation
@@ -273,18 +291,22 @@ def roofline_of(r, peaks, traffic):
     ops = sum(s["ops"] for s in r["per_shape"])
     int8_peak = 2.0 * peaks["bf16_tflops"]          # kind::i8 runs at twice the bf16 rate (nominal 4.5 vs 2.25 PF)
     t_hbm, t_tensor = by / (peaks["hbm_gbs"] * 1e9), ops / (int8_peak * 1e12)
-    per_shape = [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3),
+    per_shape = [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3), us_dense_only=round(s["us_dense"], 3),
                       gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
                       tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in r["per_shape"]]
     kern = f"mq_gemm_kernel ({len(r['per_shape'])} launches of the step, timed alone, cold weights)"
+    us0 = sum(s["us_dense"] for s in r["per_shape"])
+    extra = {"residual_overhead": us / us0 - 1.0,
+             "residual_overhead_note": f"time of the {len(r['per_shape'])} launches at rho={RHO} over the same launches on the "
+                                       "budget-0 packing of the same weights (floor = rho: the residual adds rho x bytes and ops)"}
     if t_hbm >= t_tensor:
         a = by / (us * 1e-6) / 1e9
         return {"bound": "hbm", "achieved": a, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": a / peaks["hbm_gbs"],
-                "traffic": traffic, "peak_source": peaks["source"], "kernel": kern, "per_shape": per_shape}
+                "traffic": traffic, "peak_source": peaks["source"], "kernel": kern, **extra, "per_shape": per_shape}
     a = ops / (us * 1e-6) / 1e12
     return {"bound": "tensor", "achieved": a, "peak": int8_peak, "unit": "TFLOP/s", "frac": a / int8_peak,
             "traffic": traffic, "peak_source": peaks["source"] + " bf16 burst x 2 (int8 : bf16 nominal ratio)",
-            "kernel": kern, "per_shape": per_shape}
+            "kernel": kern, **extra, "per_shape": per_shape}
 
 
 def load_traffic(workload):

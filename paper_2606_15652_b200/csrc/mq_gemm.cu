@@ -116,6 +116,16 @@ struct Cfg {
   static_assert(P_STAGE % 1024 == 0 && U_SUB % 1024 == 0, "swizzle atoms need 1024-byte alignment");
 };
 
+// Exact division of n < 2^31 by a run-time constant d: q = umulhi(n, mul) >> shr with
+// l = ceil(log2 d), mul = floor(2^(31+l) / d) + 1, shr = l - 1 (d = 1: mul = 0 marks the identity).
+// A hardware 32-bit division costs a single-warp role ~100 cycles, this costs ~10.
+struct FastDiv {
+  uint32_t mul, shr, d;
+};
+__device__ __forceinline__ uint32_t fdiv(uint32_t n, const FastDiv& f) {
+  return f.mul ? (__umulhi(n, f.mul) >> f.shr) : n;
+}
+
 struct GemmParams {
   const uint8_t* base;
   const float* sw;
@@ -134,6 +144,7 @@ struct GemmParams {
   uint32_t units;     // NT*TT*KS (< 2^31, checked by the host)
   uint32_t gran;      // range boundaries are multiples of gran (1 = stream-K, KS = whole tiles)
   uint32_t upg_q, upg_r;  // (units / gran) = upg_q * gridDim.x + upg_r
+  FastDiv dKS, dTT, dGrid;
   int M, N, KS, NT, TT;
   int y_bf16;
 #ifdef MQ_TRACE
@@ -152,7 +163,7 @@ struct GemmParams {
 // All index arithmetic is 32-bit unsigned: a 64-bit division costs a single-thread role ~400 cycles.
 // first unit of CTA c's range: gran * floor((units / gran) * c / grid)
 __device__ __forceinline__ uint32_t range_begin(const GemmParams& p, uint32_t c) {
-  return p.gran * (p.upg_q * c + (p.upg_r * c) / gridDim.x);
+  return p.gran * (p.upg_q * c + fdiv(p.upg_r * c, p.dGrid));
 }
 // the CTA whose range holds unit x
 __device__ __forceinline__ int owner_of(const GemmParams& p, uint32_t x) {
@@ -173,19 +184,20 @@ struct Stage {
 // tile) and, inside a segment, in P stages of up to SK K-steps.
 struct StageIter {
   uint32_t g, u_end;
+  FastDiv dKS, dTT;
   int KS, TT, k1, ks, nt, tt;
-  __device__ StageIter(uint32_t u_beg, uint32_t u_end_, int KS_, int TT_)
-      : g(u_beg), u_end(u_end_), KS(KS_), TT(TT_), k1(0), ks(0), nt(0), tt(0) {}
+  __device__ StageIter(uint32_t u_beg, uint32_t u_end_, const FastDiv& dKS_, const FastDiv& dTT_)
+      : g(u_beg), u_end(u_end_), dKS(dKS_), dTT(dTT_), KS((int)dKS_.d), TT((int)dTT_.d), k1(0), ks(0), nt(0), tt(0) {}
   template <int SK>
   __device__ bool next(Stage& s) {
     s.first = false;
     if (ks >= k1) {
       if (g >= u_end) return false;
-      const uint32_t tile = g / (uint32_t)KS;
+      const uint32_t tile = fdiv(g, dKS);
       ks = (int)(g - tile * (uint32_t)KS);
       k1 = (int)min((uint32_t)KS, (uint32_t)ks + (u_end - g));
       g += (uint32_t)(k1 - ks);
-      nt = (int)(tile / (uint32_t)TT);
+      nt = (int)fdiv(tile, dTT);
       tt = (int)(tile - (uint32_t)nt * (uint32_t)TT);
       s.first = true;
     }
@@ -201,13 +213,13 @@ struct StageIter {
 };
 
 // number of P stages of the range [u_beg, u_end): closed form of StageIter
-__device__ __forceinline__ int count_stages(uint32_t u_beg, uint32_t u_end, uint32_t KS, uint32_t SK) {
+__device__ __forceinline__ int count_stages(uint32_t u_beg, uint32_t u_end, const FastDiv& dKS, uint32_t SK) {
   if (u_end <= u_beg) return 0;
-  const uint32_t n = u_end - u_beg;
-  const uint32_t head = KS - u_beg % KS;
+  const uint32_t KS = dKS.d, n = u_end - u_beg;
+  const uint32_t head = KS - (u_beg - fdiv(u_beg, dKS) * KS);
   if (n <= head) return (int)((n + SK - 1) / SK);
-  const uint32_t rem = n - head;
-  return (int)((head + SK - 1) / SK + (rem / KS) * ((KS + SK - 1) / SK) + (rem % KS + SK - 1) / SK);
+  const uint32_t rem = n - head, whole = fdiv(rem, dKS);
+  return (int)((head + SK - 1) / SK + whole * ((KS + SK - 1) / SK) + (rem - whole * KS + SK - 1) / SK);
 }
 
 // 32 packed nibbles (16 B) -> 32 int8 = 16 x value.  Output element order inside the 32
@@ -320,12 +332,12 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
 
   const uint32_t u_beg = range_begin(p, blockIdx.x);
   const uint32_t u_end = blockIdx.x + 1 == gridDim.x ? p.units : range_begin(p, blockIdx.x + 1);
-  const int n_stages = count_stages(u_beg, u_end, (uint32_t)p.KS, SK);
+  const int n_stages = count_stages(u_beg, u_end, p.dKS, SK);
   const int n_items = n_stages * IPS;
 
   if (warp == 0) {
     // ===================== producer (TMA); all lanes run the loop, one elected lane issues =====================
-    StageIter it(u_beg, u_end, p.KS, p.TT);
+    StageIter it(u_beg, u_end, p.dKS, p.dTT);
     Stage cur, nxt;
     // Residual metadata {quarter mask, first quarter} is fetched 32 K-steps at a time (lane L: unit
     // ub + L) and two batches ahead, so that the producer never waits on global memory per stage.
@@ -333,8 +345,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       const uint32_t u = ub + (uint32_t)lane;
       int2 v = make_int2(0, 0);
       if (u < u_end) {
-        const uint32_t tile = u / (uint32_t)p.KS;
-        v = __ldg(p.unit_meta + (size_t)(tile / (uint32_t)p.TT) * p.KS + (u - tile * (uint32_t)p.KS));
+        const uint32_t tile = fdiv(u, p.dKS);
+        v = __ldg(p.unit_meta + (size_t)fdiv(tile, p.dTT) * p.KS + (u - tile * (uint32_t)p.KS));
       }
       return v;
     };
@@ -769,17 +781,17 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     const int lq = warp & 3;  // TMEM lane quadrant this warp may access
     const int et = (warp - FIRST_EPI_WARP) * 32 + lane;  // 0..127 within the epilogue group
     const int n_loc = lq * 32 + lane;
-    const uint32_t my_first_tile = u_beg / (uint32_t)p.KS;
+    const uint32_t my_first_tile = fdiv(u_beg, p.dKS);
     constexpr int PART = BT * BN;  // int32 elements of one partial accumulator
     int seg = 0, npend = 0;      // npend: partial tiles published by this CTA (at most 2)
     constexpr bool kBothParts = BT <= 32;
     uint32_t g = u_beg;
     while (g < u_end) {
-      const uint32_t tile = g / (uint32_t)p.KS;
+      const uint32_t tile = fdiv(g, p.dKS);
       const int k0 = (int)(g - tile * (uint32_t)p.KS);
       const int k1 = (int)min((uint32_t)p.KS, (uint32_t)k0 + (u_end - g));
       g += (uint32_t)(k1 - k0);
-      const int nt = (int)(tile / (uint32_t)p.TT), tt = (int)(tile - (uint32_t)nt * (uint32_t)p.TT);
+      const int nt = (int)fdiv(tile, p.dTT), tt = (int)(tile - (uint32_t)nt * (uint32_t)p.TT);
       const int a0s = seg % C::ACC0_STAGES, a1s = seg % C::ACC1_STAGES;
       const uint32_t aphase = ((uint32_t)seg / C::ACC0_STAGES) & 1;
       ++seg;
@@ -881,7 +893,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           pd[0] = (int32_t)tile;
           pd[1] = c_lo;
           pd[2] = c_hi;
-          pd[3] = (range_begin(p, (uint32_t)c_lo) / (uint32_t)p.KS == tile) ? 0 : 1;  // slot of c_lo's partial
+          pd[3] = (fdiv(range_begin(p, (uint32_t)c_lo), p.dKS) == tile) ? 0 : 1;  // slot of c_lo's partial
         }
         ++npend;
       }
@@ -896,7 +908,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       const uint32_t tile = (uint32_t)pend[pi * 4 + 0];
       const int c_lo = pend[pi * 4 + 1], c_hi = pend[pi * 4 + 2], lo_slot = pend[pi * 4 + 3];
       const int S = c_hi - c_lo + 1, r = (int)blockIdx.x - c_lo;
-      const int nt = (int)(tile / (uint32_t)p.TT), tt = (int)(tile - (uint32_t)nt * (uint32_t)p.TT);
+      const int nt = (int)fdiv(tile, p.dTT), tt = (int)(tile - (uint32_t)nt * (uint32_t)p.TT);
       const int t_base = tt * BT;
       const int t_cnt = min(BT, p.M - t_base);
       {
@@ -1014,6 +1026,20 @@ EncodeTiledFn get_encode_fn() {
 }
 
 size_t align256(size_t x) { return (x + 255) / 256 * 256; }
+
+FastDiv make_fastdiv(uint32_t d) {
+  FastDiv f;
+  f.d = d;
+  f.mul = 0;
+  f.shr = 0;
+  if (d > 1) {
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;
+    f.mul = (uint32_t)(((1ull << (31 + l)) / d) + 1);
+    f.shr = l - 1;
+  }
+  return f;
+}
 
 struct Plan {
   int BT = 16, TT = 1, grid = 1, gran = 1;
@@ -1155,6 +1181,9 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   gp.gran = (uint32_t)pl.gran;
   gp.upg_q = (uint32_t)((pl.units / pl.gran) / pl.grid);
   gp.upg_r = (uint32_t)((pl.units / pl.gran) % pl.grid);
+  gp.dKS = make_fastdiv((uint32_t)gp.KS);
+  gp.dTT = make_fastdiv((uint32_t)gp.TT);
+  gp.dGrid = make_fastdiv((uint32_t)pl.grid);
   gp.y_bf16 = y_dtype == MQ_BF16;
   uint8_t* ws = (uint8_t*)workspace;
   gp.ws_cnt = (int32_t*)ws;
