@@ -485,25 +485,111 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     uint32_t acc0_on = 0, acc1_on = 0;
     uint32_t d0 = 0, d1 = 0;
     int a0s = 0, a1s = 0;
+    auto seg_first = [&]() {   // first K-step of a segment: claim the accumulator stages
+      a0s = seg % C::ACC0_STAGES;
+      a1s = seg % C::ACC1_STAGES;
+      mbar_wait(bar(B_A0E + a0s), (((uint32_t)seg / C::ACC0_STAGES) & 1) ^ 1);
+      tc_fence_after();
+      d0 = tmem_base + (uint32_t)(a0s * BT);
+      d1 = tmem_base + (uint32_t)(C::ACC1_COL0 + a1s * BT);
+      acc0_on = 0;
+      acc1_on = 0;
+    };
+    auto seg_last = [&]() {    // last K-step of a segment: hand the accumulators to the epilogue
+      if (!acc1_on) {
+        // keep the acc1 ring's phases in step: the epilogue releases it once per segment
+        mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
+      }
+      __syncwarp();
+      if (elect_one()) {
+        acc_flag[a0s] = (int32_t)acc1_on;
+        mbar_arrive(bar(B_TFULL + a0s));   // release: publishes acc_flag to the epilogue warps
+        tc_commit(bar(B_TFULL + a0s));     // completes the phase when the MMAs have finished
+        MQ_STAMP(8);
+      }
+      ++seg;
+    };
     auto mma_item = [&](const int us, const int item, const uint32_t uphase) {
       mbar_wait(bar(B_FULL_U + us), uphase);
       tc_fence_after();
       MQ_STAMP_IF(item == 0 && lane == 0, 7);
       MQ_STAMP_IF(item < 16 && lane == 0, 32 + item);
+      if constexpr (UK > 1) {
+        // Decode path: all base MMAs of the item (up to 4*UK) go out as ONE elected block, then the
+        // item's residual cells follow (acc0 and acc1 are separate accumulators, so their MMAs may be
+        // reordered; the token sub-tiles stay valid until EMPTY_U is committed).  A segment's FIRST
+        // flag can only sit on an item's first K-step, LAST on its last valid one.  Issuing K-step by
+        // K-step costs ~60 dependent instructions per K-step, which is the latency of a short
+        // kernel's tail and, with residual cells in half of the items, of the steady state too.
+        int mw[UK], nk = 0;
+#pragma unroll
+        for (int j = 0; j < UK; ++j) mw[j] = lds32(sMetaU + 4u * (uint32_t)(us * UK + j));
+#pragma unroll
+        for (int j = 0; j < UK; ++j)
+          if (mw[j] & META_VALID) ++nk;
+        if (nk > 0) {
+          if (mw[0] & META_FIRST) seg_first();
+          int last = 0;
+#pragma unroll
+          for (int j = 0; j < UK; ++j)
+            if (j == nk - 1) last = mw[j] & META_LAST;
+          const uint64_t dt0 = make_desc_sw128(sU + us * C::U_STAGE);
+          __syncwarp();
+          if (elect_one()) {
+            const uint32_t at0 = tmem_base + (uint32_t)(C::A_COL0 + us * UK * A_COLS);
+#pragma unroll
+            for (int j = 0; j < UK; ++j)
+              if (j < nk) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                  mma_i8_ts(d0, at0 + (uint32_t)(j * A_COLS + k * 8), dt0 + (uint64_t)(j * (C::U_SUB >> 4) + k * 2), IDESC,
+                            (j == 0 && k == 0) ? acc0_on : 1u);
+              }
+          }
+          acc0_on = 1;
+#pragma unroll
+          for (int j = 0; j < UK; ++j) {
+            const int mask = j < nk ? (mw[j] & 0xF) : 0;
+            if (mask) {
+              if (!acc1_on) {
+                // first residual MMA of the segment: the epilogue must have drained this acc1 stage
+                mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
+                tc_fence_after();
+              }
+              const int rseq = (mw[j] >> 4) & 0xFF;
+              const int rs = (item & (C::G - 1)) * C::RG + rseq % C::RG;
+              mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RG) & 1);
+              tc_fence_after();
+              __syncwarp();
+              if (elect_one()) {
+                const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + rs * A_COLS);
+                const uint64_t dt = dt0 + (uint64_t)(j * (C::U_SUB >> 4));
+                uint32_t on = acc1_on;
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                  if (mask & (3 << (2 * h))) {
+#pragma unroll
+                    for (int k = 2 * h; k < 2 * h + 2; ++k) {
+                      mma_i8_ts(d1, rt + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
+                      on = 1;
+                    }
+                  }
+                tc_commit(bar(B_EMPTY_RU + rs));
+              }
+              acc1_on = 1;
+            }
+          }
+          if (last) seg_last();
+        }
+        __syncwarp();
+        if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
+        return;
+      }
 #pragma unroll
       for (int j = 0; j < UK; ++j) {
         const int m = lds32(sMetaU + 4u * (uint32_t)(us * UK + j));
         if (!(m & META_VALID)) break;   // the valid K-steps of an item are a prefix
-        if (m & META_FIRST) {
-          a0s = seg % C::ACC0_STAGES;
-          a1s = seg % C::ACC1_STAGES;
-          mbar_wait(bar(B_A0E + a0s), (((uint32_t)seg / C::ACC0_STAGES) & 1) ^ 1);
-          tc_fence_after();
-          d0 = tmem_base + (uint32_t)(a0s * BT);
-          d1 = tmem_base + (uint32_t)(C::ACC1_COL0 + a1s * BT);
-          acc0_on = 0;
-          acc1_on = 0;
-        }
+        if (m & META_FIRST) seg_first();
         const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + (us * UK + j) * A_COLS);
         const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE + j * C::U_SUB);
         if (elect_one()) {
@@ -541,20 +627,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           }
           acc1_on = 1;
         }
-        if (m & META_LAST) {
-          if (!acc1_on) {
-            // keep the acc1 ring's phases in step: the epilogue releases it once per segment
-            mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
-          }
-          __syncwarp();
-          if (elect_one()) {
-            acc_flag[a0s] = (int32_t)acc1_on;
-            mbar_arrive(bar(B_TFULL + a0s));   // release: publishes acc_flag to the epilogue warps
-            tc_commit(bar(B_TFULL + a0s));     // completes the phase when the MMAs have finished
-            MQ_STAMP(8);
-          }
-          ++seg;
-        }
+        if (m & META_LAST) seg_last();
       }
       __syncwarp();
       if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
