@@ -22,11 +22,12 @@
 // because two accumulators of 128 columns, the base one double-buffered, leave 128 TMEM
 // columns for the operand rings.
 //
-// Warp roles (448 threads, one persistent CTA per SM), control flow warp-uniform, single
-// instructions issued by an elected lane:
-//   warp 0      producer : TMA.  Also loads the residual metadata of its K-steps (one stage
-//                          ahead) and, for K-steps that own a residual cell, the cell's 2 KB quarters.
-//   warps 6-9, 10-13       two unpack groups, alternating U stages: int4 -> int8 (value x16:
+// Warp roles (6 + 4G warps, one persistent CTA per SM; G = 2 unpack groups, 4 for BT = 128), control
+// flow warp-uniform, single instructions issued by an elected lane:
+//   warp 0      producer : TMA.  Also fetches the residual metadata of its K-steps (32 K-steps per
+//                          load, two batches ahead), writes the per-K-step metadata words and, for
+//                          K-steps that own a residual cell, loads the cell's 2 KB quarters.
+//   warps 6..   unpack groups of 4 warps, taking U stages in rotation: int4 -> int8 (value x16:
 //                          nibble moved to the high half of a byte, two logic ops per 8
 //                          elements; both operands use the same element order inside 32 bytes, so
 //                          dot products are unchanged and accumulators are 256 x the true value).
