@@ -225,16 +225,21 @@ extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64
   const int Ki = (int)K;
   uint8_t* q8 = (uint8_t*)qA;
   cudaError_t le;
+  // the whole row stays in registers for K <= 16384 (one pass over global memory, all loads in flight)
   if (a_dtype == MQ_BF16) {
     if (nchunk_per_thread <= 2)
       le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 2>, a, lda, Ki, q8, sA);
-    else
+    else if (nchunk_per_thread <= 4)
       le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 4>, a, lda, Ki, q8, sA);
+    else
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 8>, a, lda, Ki, q8, sA);
   } else {
     if (nchunk_per_thread <= 2)
       le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 2>, a, lda, Ki, q8, sA);
-    else
+    else if (nchunk_per_thread <= 4)
       le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 4>, a, lda, Ki, q8, sA);
+    else
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 8>, a, lda, Ki, q8, sA);
   }
   if (le != cudaSuccess) {
     cudaGetLastError();
