@@ -14,13 +14,13 @@
 // Granularity.  A K-STEP is 128 input channels (one 8 KB packed weight tile).  The single-thread
 // roles pay a fixed instruction cost per hand-off, so hand-offs are coarser than a K-step:
 //   P stage  = SK consecutive K-steps of one output tile: ONE 1-D bulk copy of SK*8 KB packed
-//              weights (the device layout keeps a tile's K-steps contiguous) + ONE 2-D tensor
-//              copy of the packed token tile [BT][SK*64 B];
+//              weights (the device layout keeps a tile's K-steps contiguous) + SK 2-D tensor
+//              copies of the packed token tile, [BT][64 B] per K-step;
 //   U stage  = UK K-steps unpacked: 32*UK TMEM columns (weights, MMA A operand) + UK token
 //              sub-tiles [BT][128 B] in the K-major SWIZZLE_128B layout (MMA B operand).
-// Decode (BT <= 32): SK = UK = 4 (32 KB per hand-off).  Prefill (BT = 128): SK = 2, UK = 1,
-// because two accumulators of 128 columns, the base one double-buffered, leave 128 TMEM
-// columns for the operand rings.
+// Decode (BT <= 32): SK = UK = 4 (32 KB per hand-off), two unpack groups.  Prefill (BT = 128):
+// SK = 2, UK = 1, four unpack groups; its 512 TMEM columns hold two 128-column accumulators (the
+// base one single-buffered) and four operand stages of 32 weight + 32 residual-cell columns.
 //
 // Warp roles (6 + 4G warps, one persistent CTA per SM; G = 2 unpack groups, 4 for BT = 128), control
 // flow warp-uniform, single instructions issued by an elected lane:
