@@ -363,3 +363,39 @@ def test_gemm_no_hooks_path_matches_hooked_path(mq):
             mq.mq_gemm(w, qA, sA, M, Y=Y, workspace=ws)
         torch.cuda.synchronize()
         assert torch.equal(Y.view(torch.int16), Yh.view(torch.int16)), (M, K, N)
+
+
+def test_gemm_seeded_fuzz_against_oracle(mq):
+    """40 seeded random combinations of shape, block size, density (uniform-random block pattern) and
+    launch options (token tile, split-K mode, CTA cap, PDL on/off): accumulators bit-exact and Y in
+    tolerance against the oracle; the hot epilogue path must reproduce the hooked path's Y bits."""
+    import torch
+    rng = np.random.default_rng(2026)
+    try:
+        for ci in range(40):
+            bs = int(rng.choice([64, 128]))
+            K = int(rng.choice([128, 256, 640, 1024, 2048]))
+            N = int(rng.choice([128, 256, 384, 512]))
+            M = int(rng.choice([1, 2, 7, 16, 17, 32, 33, 64, 65, 100, 128, 129, 200, 300]))
+            rho = float(rng.choice([0.0, 0.05, 0.1, 0.3, 0.6, 1.0]))
+            opts = dict(split_k=int(rng.choice([0, 0, 1, 2])), max_ctas=int(rng.choice([0, 0, 7, 33])),
+                        pdl=int(rng.choice([1, 1, 0])), token_tile=int(rng.choice([0, 0, 16, 32, 64, 128])))
+            for k, v in opts.items():
+                mq.mq_set_option(k, v)
+            case = _random_block_case(3000 + ci, M, K, N, bs, rho)
+            want = oracle_forward(case)
+            w = pack_from_oracle(case)
+            ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+            got = run_cuda(case, w=w, workspace=ws)
+            assert_parity(got, want, what=f"fuzz {ci}: M{M} K{K} N{N} bs{bs} rho{rho} {opts}")
+            A = to_device_act(case)
+            qA, sA = mq.mq_quantize_act(A)
+            Y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+            for _ in range(2):
+                mq.mq_gemm(w, qA, sA, M, Y=Y, workspace=ws)
+            torch.cuda.synchronize()
+            assert np.array_equal(Y.float().cpu().numpy().astype(np.float64), got["Y"]), f"fuzz {ci}: hot path differs"
+    finally:
+        for k in ("split_k", "max_ctas", "token_tile"):
+            mq.mq_set_option(k, 0)
+        mq.mq_set_option("pdl", 1)
