@@ -131,8 +131,14 @@ int mq_gemm(const mq_weights* w, const void* qA_dev, const float* sA_dev, int64_
             mq_dtype y_dtype, int64_t ldy_elems, int32_t* dbg_acc_base_dev, int32_t* dbg_acc_res_dev,
             void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
-/* Convenience: mq_quantize_act into the head of the workspace followed by mq_gemm on the
- * same stream.  Workspace: mq_linear_workspace_bytes(w, M), same zero-state contract. */
+/* One linear layer from raw activations: A_dev fp16/bf16 [M, K] (rows 16-byte aligned, lda_elems % 8 == 0).
+ * Default: mq_quantize_act into the workspace followed by mq_gemm on the same stream (two launches
+ * chained by programmatic dependent launch).  With option "fused_quant" = 1 and M <= 8 the quantizer runs
+ * inside the GEMM kernel (north_star (i) "optionally fused into the GEMM prologue"): one
+ * launch, bit-identical Y; the per-token absmax is found with a grid-wide atomic max, the tokens of each
+ * K-step are quantized from a TMA-staged raw tile.  Workspace: mq_linear_workspace_bytes(w, M), all-zero
+ * before the first call (it carries the GEMM's counters and the fused path's absmax control block, which
+ * every call returns to zero). */
 size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M);
 int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t lda_elems,
               void* Y_dev, mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev,
@@ -143,6 +149,7 @@ int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t 
  *                 all tiles cut into equal per-CTA ranges, shared tiles finished by the last arriver)
  *   "token_tile": 0 = automatic, else 16/32/64/128
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
+ *   "fused_quant": 0 (default) / 1: see mq_linear
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
  *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */

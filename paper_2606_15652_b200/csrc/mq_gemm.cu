@@ -47,6 +47,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstring>
 
 #include "mq_internal.h"
 #include "mq_ptx.cuh"
@@ -68,7 +69,7 @@ constexpr int META_LAST = 1 << 29;           // last K-step of the segment: accu
 // of its unpack group in this CTA (mod 256); bits 12-27: sequence number of the cell's first
 // stored quarter among the quarters of its unpack group (mod 65536)
 
-template <int BT>
+template <int BT, bool FUSED = false>
 struct Cfg {
   // Unpack groups (4 warps each).  An item costs a group ~1000 cycles of mostly latency (loads,
   // TMEM/shared stores, proxy fences), so prefill runs four groups side by side.
@@ -91,7 +92,10 @@ struct Cfg {
   static constexpr int ACC0_STAGES = BT == 128 ? 1 : 2;
   static constexpr int ACC1_STAGES = BT <= 64 ? 2 : 1;
   static constexpr int P_W = SK * TILE_BYTES;
-  static constexpr int P_TOK = BT * SK * (BK / 2);
+  // token area of a P stage: packed int4 tokens [SK][BT][64 B], or (FUSED) raw 16-bit activations
+  // [SK][8 rows][256 B] fetched by a tensor map over A itself
+  static constexpr int TOK_KSTEP = FUSED ? 8 * BK * 2 : BT * (BK / 2);
+  static constexpr int P_TOK = SK * TOK_KSTEP;
   static constexpr int P_STAGE = P_W + P_TOK;
   static constexpr int U_SUB = BT * BK;                          // one int8 token sub-tile
   static constexpr int U_STAGE = UK * U_SUB;
@@ -108,9 +112,9 @@ struct Cfg {
   static constexpr int OFF_P = OFF_U + USTAGES * U_STAGE;
   static constexpr int OFF_RP = OFF_P + PSTAGES * P_STAGE;
   static constexpr int OFF_BAR = OFF_RP + NQ * QUARTER_BYTES;
-  static constexpr int NUM_BARS = 2 * PSTAGES + 2 * USTAGES + 2 * NQ + 2 * RSTAGES + 2 + ACC0_STAGES + ACC1_STAGES;
+  static constexpr int NUM_BARS = 2 * PSTAGES + 2 * USTAGES + 2 * NQ + 2 * RSTAGES + 2 + ACC0_STAGES + ACC1_STAGES + 1;
   static constexpr int OFF_META = OFF_BAR + NUM_BARS * 8;
-  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 12;
+  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 12 + 16;   // + token scales (FUSED)
   static constexpr int OFF_END = OFF_META + META_WORDS * 4;
   static constexpr int SMEM_BYTES = OFF_END + 1024;  // slack for the 1024-byte alignment
   static_assert(SMEM_BYTES <= 232448, "shared memory budget");
@@ -148,6 +152,13 @@ struct GemmParams {
   FastDiv dKS, dTT, dGrid;
   int M, N, KS, NT, TT;
   int y_bf16;
+  // fused activation quantization (mq_linear, M <= 8; kernel template FUSED): the raw activations and a
+  // zero-state control block {amax bits [16], arrived, finished}
+  const uint16_t* A;
+  int64_t lda;
+  int a_bf16;
+  uint32_t* fz_ctrl;
+  FastDiv dRowChunks;   // K / 8: 16-byte chunks per activation row
 #ifdef MQ_TRACE
   long long* trace;  // [grid][64] clock64 stamps (development builds only)
 #endif
@@ -254,6 +265,31 @@ __device__ __forceinline__ void sts32(uint32_t addr, int v) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
+// FUSED path: 8 consecutive fp16/bf16 activations (one 16-byte load) -> the two int8 words the unpack
+// of their packed int4 form would give: evens [e0,e2,e4,e6] and odds [e1,e3,e5,e7], each byte = 16 x q.
+// The arithmetic is mq_quantize_act's, operation for operation (Eq.1; A1-A3): exact conversion to
+// fp32, quant1() = IEEE division by the token scale, round half to even, clamp to [-7, 7].
+__device__ __forceinline__ void quant8_i8x16(const uint4& raw, float s, float inv_s, bool bf16, uint32_t& ev, uint32_t& od) {
+  const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+  ev = 0;
+  od = 0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float f0, f1;
+    if (bf16) {
+      f0 = __uint_as_float(w[i] << 16);
+      f1 = __uint_as_float(w[i] & 0xFFFF0000u);
+    } else {
+      const float2 t = __half22float2(*reinterpret_cast<const __half2*>(&w[i]));
+      f0 = t.x;
+      f1 = t.y;
+    }
+    const int q0 = quant1(f0, s, inv_s), q1 = quant1(f1, s, inv_s);
+    ev |= ((uint32_t)(q0 & 0xF) << 4) << (8 * i);
+    od |= ((uint32_t)(q1 & 0xF) << 4) << (8 * i);
+  }
+}
+
 template <bool BF16>
 __device__ __forceinline__ void store_y(void* Y, size_t o, float y) {
   if (BF16)
@@ -262,10 +298,15 @@ __device__ __forceinline__ void store_y(void* Y, size_t o, float y) {
     reinterpret_cast<__half*>(Y)[o] = __float2half_rn(y);
 }
 
-template <int BT>
-__global__ void __launch_bounds__(Cfg<BT>::NUM_THREADS, 1)
+// FUSED (BT = 16 only): the activation quantizer runs inside this kernel (north_star (i)
+// "optionally fused into the GEMM prologue"): the epilogue warps find the per-token absmax together with
+// all other CTAs (atomic max + grid-wide arrival count, hidden behind the first weight stage's HBM
+// latency), and the unpack groups quantize the fp16/bf16 tokens of their K-steps straight into the int8
+// operand tile -- no packed activations, no second kernel.
+template <int BT, bool FUSED>
+__global__ void __launch_bounds__(Cfg<BT, FUSED>::NUM_THREADS, 1)
 mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
-  using C = Cfg<BT>;
+  using C = Cfg<BT, FUSED>;
   constexpr int SK = C::SK, UK = C::UK, IPS = C::IPS;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -276,15 +317,17 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   constexpr int B_FULL_P = 0, B_EMPTY_P = C::PSTAGES, B_FULL_U = 2 * C::PSTAGES, B_EMPTY_U = B_FULL_U + C::USTAGES,
                 B_FULL_Q = B_EMPTY_U + C::USTAGES, B_EMPTY_Q = B_FULL_Q + C::NQ,
                 B_FULL_RU = B_EMPTY_Q + C::NQ, B_EMPTY_RU = B_FULL_RU + C::RSTAGES,
-                B_TFULL = B_EMPTY_RU + C::RSTAGES, B_A0E = B_TFULL + 2, B_A1E = B_A0E + C::ACC0_STAGES;
-  static_assert(B_A1E + C::ACC1_STAGES == C::NUM_BARS, "barrier map");
+                B_TFULL = B_EMPTY_RU + C::RSTAGES, B_A0E = B_TFULL + 2, B_A1E = B_A0E + C::ACC0_STAGES,
+                B_SA = B_A1E + C::ACC1_STAGES;   // FUSED: token scales are in shared memory
+  static_assert(B_SA + 1 == C::NUM_BARS, "barrier map");
   // small shared words: metadata rings, TMEM base, fix-up flags
   const uint32_t sMetaP = smem_base + C::OFF_META;              // [PSTAGES][SK]
   const uint32_t sMetaU = sMetaP + 4u * C::PSTAGES * SK;        // [USTAGES][UK]
   const uint32_t sMisc = sMetaU + 4u * C::USTAGES * UK;         // [0] tmem base, [1..5] fix-up, [6..7] acc_flag
   volatile int32_t* misc = reinterpret_cast<volatile int32_t*>(smem_raw + (sMisc - smem_u32(smem_raw)));
   volatile int32_t* pend = misc + 1;      // [2][4] partial tiles awaiting the fix-up: tile, c_lo, c_hi, lo_slot
-  volatile int32_t* acc_flag = misc + 9;  // [2]: did this base-accumulator stage's segment get residual MMAs?
+  volatile int32_t* acc_flag = misc + 9;
+  volatile float* sa_s = reinterpret_cast<volatile float*>(misc + 12);   // [16] FUSED: token scales
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #ifdef MQ_TRACE
@@ -317,6 +360,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     for (int i = 0; i < 2; ++i) mbar_init(bar(B_TFULL + i), 2);
     for (int i = 0; i < C::ACC0_STAGES; ++i) mbar_init(bar(B_A0E + i), 4);
     for (int i = 0; i < C::ACC1_STAGES; ++i) mbar_init(bar(B_A1E + i), 4);
+    mbar_init(bar(B_SA), 1);
     fence_mbar_init();
   }
   if (warp == 1) {
@@ -363,7 +407,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (elect_one()) {
           MQ_STAMP_IF(pre == 0, 2);
           const uint32_t fb = bar(B_FULL_P + pre);
-          mbar_arrive_expect_tx(fb, (uint32_t)s.nks * (TILE_BYTES + BT * (BK / 2)));
+          mbar_arrive_expect_tx(fb, (uint32_t)s.nks * (TILE_BYTES + C::TOK_KSTEP));
           tma_load_1d(sP + pre * C::P_STAGE, p.base + ((size_t)s.nt * p.KS + s.ks) * TILE_BYTES,
                       (uint32_t)s.nks * TILE_BYTES, fb);
         }
@@ -393,11 +437,15 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         MQ_STAMP_IF(si == n_stages - 1, 3);
         const uint32_t fb = bar(B_FULL_P + ps);
         if (si >= pre) {   // the prologue already issued the weights of the first `pre` stages
-          mbar_arrive_expect_tx(fb, (uint32_t)cur.nks * (TILE_BYTES + BT * (BK / 2)));
+          mbar_arrive_expect_tx(fb, (uint32_t)cur.nks * (TILE_BYTES + C::TOK_KSTEP));
           tma_load_1d(dst, p.base + ((size_t)cur.nt * p.KS + cur.ks) * TILE_BYTES, (uint32_t)cur.nks * TILE_BYTES, fb);
         }
-        for (int j = 0; j < cur.nks; ++j)
-          tma_load_2d(dst + C::P_W + j * (BT * (BK / 2)), &tmap_a, (cur.ks + j) * (BK / 2), cur.tt * BT, fb);
+        for (int j = 0; j < cur.nks; ++j) {
+          if constexpr (FUSED)   // raw activations: box {128 elements, 8 rows} of the 16-bit tensor map over A
+            tma_load_2d(dst + C::P_W + j * C::TOK_KSTEP, &tmap_a, (cur.ks + j) * BK, 0, fb);
+          else
+            tma_load_2d(dst + C::P_W + j * C::TOK_KSTEP, &tmap_a, (cur.ks + j) * (BK / 2), cur.tt * BT, fb);
+        }
       }
       // metadata words of the stage (lane j writes K-step j), then the second arrival publishes them.
       // The empty asm pins the first USE of the prefetched metadata behind the TMA issue above.
@@ -656,6 +704,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     const uint32_t gtid = (uint32_t)(((warp - FIRST_UNPACK_WARP) & 3) * 32 + lane);
     const uint32_t lane_addr = tmem_base + ((uint32_t)(wq * 32) << 16);
     const int rhalf = wq >> 1;                                    // row half of a residual cell
+    bool sa_ready = false;                                        // FUSED: token scales observed
     for (int item = gi; item < n_items; item += C::G) {
       const int stage = item / IPS, sub = item - stage * IPS;
       const int ps = stage % C::PSTAGES, us = item % C::USTAGES;
@@ -776,17 +825,39 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
       }
       // tokens: packed [UK][BT][64 B] -> UK sub-tiles [BT][128 B] K-major SWIZZLE_128B
-      const uint32_t pt = sP + ps * C::P_STAGE + C::P_W + sub * UK * (BT * (BK / 2)), ut = sU + us * C::U_STAGE;
+      const uint32_t pt = sP + ps * C::P_STAGE + C::P_W + sub * UK * C::TOK_KSTEP, ut = sU + us * C::U_STAGE;
+      if constexpr (FUSED) {
+        // Units of 8 activations (one 16-byte piece of the stage's raw tile [UK][8 rows][256 B]) are
+        // dealt round-robin to the group's 128 threads: M * 64 units per item.  A unit becomes the
+        // two int8 words (even / odd elements) the packed form's expansion would give, i.e. 8 bytes
+        // of a swizzled 16-byte chunk of the operand tile.
+        static_assert(!FUSED || (BT == 16 && UK == 4), "fused activation quantization: BT = 16 only");
+        if (!sa_ready) {
+          mbar_wait(bar(B_SA), 0);
+          sa_ready = true;
+        }
+        for (uint32_t u = gtid; u < (uint32_t)p.M * 64u; u += 128) {
+          const uint32_t t = u >> 6, jj = (u >> 4) & 3, c8 = u & 15;
+          if ((int)jj < nk) {
+            const float s = sa_s[t], inv_s = quant_inv_scale(s);
+            uint32_t ev, od;
+            quant8_i8x16(lds128(pt + jj * C::TOK_KSTEP + t * (BK * 2) + c8 * 16), s, inv_s, p.a_bf16 != 0, ev, od);
+            const uint32_t dst = ut + jj * C::U_SUB + t * 128 + ((((c8 >> 1)) ^ (t & 7)) << 4) + (c8 & 1) * 8;
+            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst), "r"(ev), "r"(od) : "memory");
+          }
+        }
+      } else {
 #pragma unroll
-      for (uint32_t idx = gtid; idx < (uint32_t)(UK * BT * 4); idx += 128) {
-        const uint32_t jj = idx / (BT * 4), rem = idx % (BT * 4), t = rem >> 2, c = rem & 3;
-        if ((int)jj < nk) {
-          const uint4 tv = lds128(pt + idx * 16);
-          uint32_t w8[8];
-          unpack16(tv, w8);
-          const uint32_t dst = ut + jj * C::U_SUB + t * 128;
-          sts128(dst + (((2 * c) ^ (t & 7)) << 4), w8);
-          sts128(dst + (((2 * c + 1) ^ (t & 7)) << 4), w8 + 4);
+        for (uint32_t idx = gtid; idx < (uint32_t)(UK * BT * 4); idx += 128) {
+          const uint32_t jj = idx / (BT * 4), rem = idx % (BT * 4), t = rem >> 2, c = rem & 3;
+          if ((int)jj < nk) {
+            const uint4 tv = lds128(pt + idx * 16);
+            uint32_t w8[8];
+            unpack16(tv, w8);
+            const uint32_t dst = ut + jj * C::U_SUB + t * 128;
+            sts128(dst + (((2 * c) ^ (t & 7)) << 4), w8);
+            sts128(dst + (((2 * c + 1) ^ (t & 7)) << 4), w8 + 4);
+          }
         }
       }
       tmem_st_wait();
@@ -857,6 +928,65 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     const int n_loc = lq * 32 + lane;
     const uint32_t my_first_tile = fdiv(u_beg, p.dKS);
     constexpr int PART = BT * BN;  // int32 elements of one partial accumulator
+    if constexpr (FUSED) {
+      // ---- per-token absmax over the whole row, found together with all CTAs of the grid --------
+      // fz_ctrl: [0..15] absmax as fp32 bits (non-negative floats order like unsigned integers),
+      // [16] CTAs arrived, [17] CTAs finished; all zero between calls.  Every CTA looks at one
+      // 16-byte chunk per epilogue thread (M * K / 8 chunks <= grid * 128 for the shapes this path
+      // takes), warp-reduces, and issues one atomic max per warp and row.
+      const uint32_t total = (uint32_t)p.M * p.dRowChunks.d;
+      for (uint32_t eb = blockIdx.x * 128u + (uint32_t)(et & ~31); eb < total; eb += gridDim.x * 128u) {   // warp-uniform
+        const uint32_t e = eb + (uint32_t)lane;
+        float am = 0.f;
+        uint32_t rowi = 0xffffffffu;
+        if (e < total) {
+          rowi = fdiv(e, p.dRowChunks);
+          const uint4 v = __ldcg(reinterpret_cast<const uint4*>(p.A + (size_t)rowi * p.lda) + (e - rowi * p.dRowChunks.d));
+          const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            float f0, f1;
+            if (p.a_bf16) {
+              f0 = __uint_as_float(w[i] << 16);
+              f1 = __uint_as_float(w[i] & 0xFFFF0000u);
+            } else {
+              const float2 t2 = __half22float2(*reinterpret_cast<const __half2*>(&w[i]));
+              f0 = t2.x;
+              f1 = t2.y;
+            }
+            am = fmaxf(am, fmaxf(fabsf(f0), fabsf(f1)));
+          }
+        }
+        // lanes of a warp hold consecutive chunks: at most two rows per warp
+        const uint32_t row_lo = __shfl_sync(0xffffffffu, rowi, 0);
+        float a_lo = rowi == row_lo ? am : 0.f, a_hi = (rowi != row_lo && rowi != 0xffffffffu) ? am : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          a_lo = fmaxf(a_lo, __shfl_xor_sync(0xffffffffu, a_lo, o));
+          a_hi = fmaxf(a_hi, __shfl_xor_sync(0xffffffffu, a_hi, o));
+        }
+        const uint32_t row_hi = __shfl_sync(0xffffffffu, rowi, 31);
+        if (lane == 0 && row_lo != 0xffffffffu && a_lo > 0.f) atomicMax(p.fz_ctrl + row_lo, __float_as_uint(a_lo));
+        if (lane == 0 && row_hi != 0xffffffffu && row_hi != row_lo && a_hi > 0.f) atomicMax(p.fz_ctrl + row_hi, __float_as_uint(a_hi));
+      }
+      __threadfence();
+      named_bar_sync(1, 128);
+      if (et == 0) {
+        atomicAdd(p.fz_ctrl + 16, 1u);
+        uint32_t spins = 0, seen;
+        do {   // all CTAs are resident (grid <= SM count, one CTA per SM), so this terminates
+          asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(p.fz_ctrl + 16) : "memory");
+          if (++spins > (1u << 24)) __trap();
+        } while (seen < gridDim.x);
+      }
+      named_bar_sync(1, 128);
+      if (et < 16) {
+        const float a = et < p.M ? __uint_as_float(__ldcg(p.fz_ctrl + et)) : 0.f;
+        sa_s[et] = a == 0.f ? 1.0f : __fdiv_rn(a, 7.0f);   // Eq.1 with q_max = 7; all-zero row: s = 1 (A2)
+      }
+      named_bar_sync(1, 128);
+      if (et == 0) mbar_arrive(bar(B_SA));   // release: the unpack groups may read the token scales
+    }
     int seg = 0, npend = 0;      // npend: partial tiles published by this CTA (at most 2)
     constexpr bool kBothParts = BT <= 32;
     uint32_t g = u_beg;
@@ -904,7 +1034,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
                          // per chunk instead of one per token behind the stores)
         if (whole) {
 #pragma unroll
-          for (int i = 0; i < 16; ++i) sav[i] = c0 + i < t_cnt ? __ldg(p.sa + t_base + c0 + i) : 0.f;
+          for (int i = 0; i < 16; ++i) sav[i] = c0 + i < t_cnt ? (FUSED ? sa_s[c0 + i] : __ldg(p.sa + t_base + c0 + i)) : 0.f;
         }
         tmem_ld16(t0addr + c0, v0);
         if (has_res) {
@@ -1017,7 +1147,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
         const int n = nt * BN + n0;
         const float4 sw4 = *reinterpret_cast<const float4*>(p.sw + n), sr4 = *reinterpret_cast<const float4*>(p.sr + n);
-        const float sat = __ldg(p.sa + t_base + t) * 0.00390625f;    // / 256: accumulators are x256
+        const float sat = (FUSED ? sa_s[t] : __ldg(p.sa + t_base + t)) * 0.00390625f;    // / 256: accumulators are x256
         float y[4];
         y[0] = sat * ((float)s0.x * sw4.x + (float)s1.x * sr4.x);
         y[1] = sat * ((float)s0.y * sw4.y + (float)s1.y * sr4.y);
@@ -1056,6 +1186,15 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (old == S - 1) {
           p.ws_cnt[tile] = 0;
           p.ws_done[tile] = 0;
+        }
+      }
+    }
+    if constexpr (FUSED) {
+      // the last CTA to finish returns the absmax control block to zero for the next call
+      if (et == 0) {
+        const uint32_t old = atomicAdd(p.fz_ctrl + 17, 1u);
+        if (old == gridDim.x - 1) {
+          for (int i = 0; i < 18; ++i) p.fz_ctrl[i] = 0;
         }
       }
     }
@@ -1159,12 +1298,12 @@ Plan make_plan(const mq_weights* w, int64_t M) {
   return pl;
 }
 
-template <int BT>
+template <int BT, bool FUSED = false>
 int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t st) {
-  using C = Cfg<BT>;
+  using C = Cfg<BT, FUSED>;
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(mq_gemm_kernel<BT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) !=
+    if (cudaFuncSetAttribute(mq_gemm_kernel<BT, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) !=
         cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
@@ -1181,7 +1320,7 @@ int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = options().pdl ? 1 : 0;
-  if (cudaLaunchKernelEx(&cfg, mq_gemm_kernel<BT>, tmap, gp) != cudaSuccess) {
+  if (cudaLaunchKernelEx(&cfg, mq_gemm_kernel<BT, FUSED>, tmap, gp) != cudaSuccess) {
     cudaGetLastError();
     return MQ_ERR_CUDA;
   }
@@ -1201,16 +1340,24 @@ extern "C" size_t mq_gemm_workspace_bytes(const mq_weights* w, int64_t M) {
   return make_plan(w, M).ws_bytes;
 }
 
-extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
-                       int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
-                       void* cuda_stream) {
+namespace {
+
+// mq_gemm proper; with fused_A != NULL the kernel quantizes the raw activations itself (mq_linear, M <= 8)
+// and qA / sA are unused.
+int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+              int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes, void* cuda_stream,
+              const void* fused_A, mq_dtype a_dtype, int64_t lda, uint32_t* fz_ctrl) {
+  const bool fused = fused_A != nullptr;
   if (!w) return MQ_ERR_INVALID_ARG;
   if (M < 0 || M > (1 << 30)) return MQ_ERR_UNSUPPORTED_SHAPE;
   if (y_dtype != MQ_F16 && y_dtype != MQ_BF16) return MQ_ERR_INVALID_ARG;
   mq::set_launch_count(0);
   if (M == 0) return MQ_OK;
-  if (!qA || !sA || !Y || ldy < w->N) return MQ_ERR_INVALID_ARG;
-  if (((uintptr_t)qA & 15) || ((uintptr_t)Y & 1) || ((uintptr_t)sA & 3)) return MQ_ERR_INVALID_ARG;
+  if (!Y || ldy < w->N || ((uintptr_t)Y & 1)) return MQ_ERR_INVALID_ARG;
+  if (!fused) {
+    if (!qA || !sA) return MQ_ERR_INVALID_ARG;
+    if (((uintptr_t)qA & 15) || ((uintptr_t)sA & 3)) return MQ_ERR_INVALID_ARG;
+  }
   if (((uintptr_t)dbg0 & 15) || ((uintptr_t)dbg1 & 15)) return MQ_ERR_INVALID_ARG;
   int rc = mq::check_device();
   if (rc != MQ_OK) return rc;
@@ -1226,14 +1373,26 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
 
   // 2-D tensor map over the canonical packed activations: [M rows][K/2 bytes]
   CUtensorMap tmap;
+  memset(&tmap, 0, sizeof(tmap));
+  if (fused && pl.BT != 16) return MQ_ERR_INVALID_ARG;
   const cuuint64_t gdim[2] = {(cuuint64_t)(w->K / 2), (cuuint64_t)M};
   const cuuint64_t gstride[1] = {(cuuint64_t)(w->K / 2)};
   const cuuint32_t box[2] = {(cuuint32_t)(BK / 2), (cuuint32_t)pl.BT};
   const cuuint32_t estr[2] = {1, 1};
-  if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(qA), gdim, gstride, box, estr,
-          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+  if (!fused && enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(qA), gdim, gstride, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
     return MQ_ERR_CUDA;
+  if (fused) {
+    // 2-D tensor map over the raw 16-bit activations [M rows][K elements], box {128 elements, 8 rows}
+    const cuuint64_t fdim[2] = {(cuuint64_t)w->K, (cuuint64_t)M};
+    const cuuint64_t fstride[1] = {(cuuint64_t)lda * 2};
+    const cuuint32_t fbox[2] = {(cuuint32_t)BK, 8};
+    if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, const_cast<void*>(fused_A), fdim, fstride, fbox, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return MQ_ERR_CUDA;
+  }
 
   GemmParams gp;
   gp.base = w->d_base;
@@ -1259,6 +1418,11 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   gp.dTT = make_fastdiv((uint32_t)gp.TT);
   gp.dGrid = make_fastdiv((uint32_t)pl.grid);
   gp.y_bf16 = y_dtype == MQ_BF16;
+  gp.A = (const uint16_t*)fused_A;
+  gp.lda = lda;
+  gp.a_bf16 = a_dtype == MQ_BF16;
+  gp.fz_ctrl = fz_ctrl;
+  gp.dRowChunks = make_fastdiv((uint32_t)(w->K / 8));
   uint8_t* ws = (uint8_t*)workspace;
   gp.ws_cnt = (int32_t*)ws;
   gp.ws_done = (int32_t*)(ws + pl.off_done);
@@ -1271,7 +1435,7 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   switch (pl.BT) {
-    case 16: rc = launch<16>(tmap, gp, pl.grid, st); break;
+    case 16: rc = fused ? launch<16, true>(tmap, gp, pl.grid, st) : launch<16>(tmap, gp, pl.grid, st); break;
     case 32: rc = launch<32>(tmap, gp, pl.grid, st); break;
     case 64: rc = launch<64>(tmap, gp, pl.grid, st); break;
     case 128: rc = launch<128>(tmap, gp, pl.grid, st); break;
@@ -1281,11 +1445,20 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
   return rc;
 }
 
+}  // namespace
+
+extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
+                       int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
+                       void* cuda_stream) {
+  return gemm_impl(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, nullptr, MQ_F16, 0,
+                   nullptr);
+}
+
 extern "C" size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M) {
   if (!w || M <= 0) return 0;
   size_t q = (mq_qact_bytes(M, w->K) + 255) / 256 * 256;
   size_t s = ((size_t)M * 4 + 255) / 256 * 256;
-  return q + s + align256(mq_gemm_workspace_bytes(w, M));
+  return align256(mq_gemm_workspace_bytes(w, M)) + 256 /* fused-quantization control block */ + q + s;
 }
 
 extern "C" int mq_linear(const mq_weights* w, const void* A, mq_dtype a_dtype, int64_t M, int64_t lda, void* Y,
@@ -1293,16 +1466,25 @@ extern "C" int mq_linear(const mq_weights* w, const void* A, mq_dtype a_dtype, i
   if (!w) return MQ_ERR_INVALID_ARG;
   if (M == 0) return MQ_OK;
   if (M < 0) return MQ_ERR_UNSUPPORTED_SHAPE;
+  if (a_dtype != MQ_F16 && a_dtype != MQ_BF16) return MQ_ERR_INVALID_ARG;
+  if (!A || lda < w->K || (lda % 8) != 0 || ((uintptr_t)A & 15)) return MQ_ERR_INVALID_ARG;
   if (!workspace || ((uintptr_t)workspace & 255)) return MQ_ERR_INVALID_ARG;
   const size_t need = mq_linear_workspace_bytes(w, M);
   if (workspace_bytes < need) return MQ_ERR_WORKSPACE;
-  // the GEMM's zero-state region comes first so that the caller's one-time memset covers it
+  // zero-state regions first (the GEMM's counters, the fused path's control block), so that the
+  // caller's one-time memset covers them; then the packed activations and their scales
   const size_t g = mq_gemm_workspace_bytes(w, M);
   const size_t g_al = align256(g);
   uint8_t* base = (uint8_t*)workspace;
-  uint8_t* qa = base + g_al;
+  uint32_t* ctrl = (uint32_t*)(base + g_al);
+  uint8_t* qa = base + g_al + 256;
   float* sa = (float*)(qa + (mq_qact_bytes(M, w->K) + 255) / 256 * 256);
   if ((size_t)((uint8_t*)sa + (size_t)M * 4 - base) > workspace_bytes) return MQ_ERR_WORKSPACE;
+  // Decode-sized calls (M <= 8): ONE kernel, the activation quantizer runs inside the GEMM.
+  // Larger M: the quantizer as its own kernel (chained by programmatic dependent launch).
+  const Options& o = options();
+  if (o.fused_quant && M <= 8 && w->K >= 256 && (o.token_tile == 0 || o.token_tile == 16))
+    return gemm_impl(w, nullptr, nullptr, M, Y, y_dtype, ldy, nullptr, nullptr, base, g, cuda_stream, A, a_dtype, lda, ctrl);
   int rc = mq_quantize_act(A, a_dtype, M, w->K, lda, qa, sa, cuda_stream);
   if (rc != MQ_OK) return rc;
   rc = mq_gemm(w, qa, sa, M, Y, y_dtype, ldy, nullptr, nullptr, base, g, cuda_stream);

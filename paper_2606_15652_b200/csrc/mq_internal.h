@@ -72,6 +72,8 @@ struct Options {
   int64_t split_k = 0;
   int64_t token_tile = 0;
   int64_t max_ctas = 0;
+  int64_t fused_quant = 0;   // mq_linear with M <= 8: quantize the activations inside the GEMM kernel (slower than
+                             // the PDL-chained two-kernel path on B200; off by default)
   int64_t pdl = 1;   // launch kernels as programmatic dependents of their predecessor in the stream
 };
 Options& options();

@@ -151,6 +151,23 @@ __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wa
 // launch_dependents: lets the next kernel in the stream start its CTAs as resources free up.
 __device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// ---- Eq.1 for one element, bit-exact and cheap ---------------------------------------------------
+// The result q = clamp(rint(x / s)) is DEFINED with an IEEE binary32 division and round-half-even
+// (A3).  The division costs ~12 instructions; x * (1/s) costs one, and differs from the
+// exact quotient by at most 3 * 2^-24 * |t| < 1.4e-6 for |t| <= 7.5, so rint() of the two can only
+// differ when the product lies within that distance of a half-integer.  Only then (rare; exact ties
+// do occur on fp16 grids) is the division performed.  `inv_s` must be 0 when 1/s is not usable
+// (tiny scales), which forces the division.
+__device__ __forceinline__ int quant1(float x, float s, float inv_s) {
+  const float tp = x * inv_s;
+  float r = rintf(tp);
+  const float d = fabsf(fabsf(tp - r) - 0.5f);   // distance of tp from the nearest half-integer
+  if (inv_s == 0.f || !(d > 4e-6f)) r = rintf(__fdiv_rn(x, s));
+  const int q = (int)r;
+  return max(-7, min(7, q));
+}
+__device__ __forceinline__ float quant_inv_scale(float s) { return s > 1e-30f ? __frcp_rn(s) : 0.f; }
+
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }

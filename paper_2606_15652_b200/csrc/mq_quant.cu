@@ -71,13 +71,11 @@ __device__ __forceinline__ void cvt8(const uint4& v, float* f) {
   }
 }
 
-__device__ __forceinline__ uint32_t quant_pack8(const float* f, float s) {
+__device__ __forceinline__ uint32_t quant_pack8(const float* f, float s, float inv_s) {
   uint32_t out = 0;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    float t = __fdiv_rn(f[i], s);                 // IEEE binary32 division (A3)
-    int q = __float2int_rn(t);                    // round half to even
-    q = max(-7, min(7, q));
+    const int q = mq::ptx::quant1(f[i], s, inv_s);   // == clamp(rint(IEEE f / s)), see mq_ptx.cuh (A3)
     out |= (uint32_t)(q & 0xF) << (4 * i);
   }
   return out;
@@ -127,6 +125,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
 
   const float s = amax == 0.f ? 1.0f : __fdiv_rn(amax, 7.0f);  // A2 / Eq.1
   if (threadIdx.x == 0) sA[m] = s;
+  const float inv_s = mq::ptx::quant_inv_scale(s);
 
 #pragma unroll
   for (int c = 0; c < CHUNKS; ++c) {
@@ -134,14 +133,14 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
     if (idx < nchunk) {
       float f[8];
       cvt8<BF16>(cache[c], f);
-      qrow[idx] = quant_pack8(f, s);
+      qrow[idx] = quant_pack8(f, s, inv_s);
     }
   }
   for (int idx = threadIdx.x + CHUNKS * QT; idx < nchunk; idx += QT) {
     uint4 v = __ldg(row + idx);
     float f[8];
     cvt8<BF16>(v, f);
-    qrow[idx] = quant_pack8(f, s);
+    qrow[idx] = quant_pack8(f, s, inv_s);
   }
 }
 
@@ -184,6 +183,9 @@ extern "C" int mq_set_option(const char* name, int64_t value) {
   } else if (!strcmp(name, "pdl")) {
     if (value > 1) return MQ_ERR_INVALID_ARG;
     o.pdl = value;
+  } else if (!strcmp(name, "fused_quant")) {
+    if (value > 1) return MQ_ERR_INVALID_ARG;
+    o.fused_quant = value;
   } else {
     return MQ_ERR_INVALID_ARG;
   }

@@ -301,6 +301,36 @@ def test_linear_matches_two_calls(mq):
     assert mq.mq_last_launch_count() == 2
 
 
+@pytest.mark.parametrize("dt", ["f16", "bf16"])
+@pytest.mark.parametrize("M,K,N,rho", [(1, 256, 128, 0.5), (3, 1024, 384, 0.1), (8, 2048, 512, 0.3), (8, 4096, 4096, 0.05),
+                                       (5, 14336, 1024, 0.05)])
+def test_linear_fused_quantization_small_m(mq, M, K, N, rho, dt):
+    """mq_linear with M <= 8 and option fused_quant = 1 runs the activation quantizer INSIDE the GEMM kernel
+    (one launch, SURVEY 8(f)-1): Y must be bit-identical to mq_quantize_act + mq_gemm, which is checked against the oracle;
+    repeated calls on one workspace (grid-wide absmax control block returns to zero) stay identical."""
+    import torch
+    case = make_case(600 + M + K, M, K, N, bs=64, rho=rho, a_dtype=dt)
+    want = oracle_forward(case)
+    w = pack_from_oracle(case)
+    got = run_cuda(case, w=w)
+    assert_parity(got, want, what=f"two-call path M{M} K{K}")
+    A = to_device_act(case)
+    ws = mq.new_workspace(mq.mq_linear_workspace_bytes(w, M))
+    try:
+        mq.mq_set_option("fused_quant", 1)
+        for rep in range(3):
+            Y1 = mq.mq_linear(w, A, workspace=ws)
+            torch.cuda.synchronize()
+            assert mq.mq_last_launch_count() == 1
+            assert np.array_equal(Y1.float().cpu().numpy().astype(np.float64), got["Y"]), f"fused path differs (rep {rep})"
+        mq.mq_set_option("fused_quant", 0)
+        Y2 = mq.mq_linear(w, A, workspace=ws)
+        torch.cuda.synchronize()
+        assert mq.mq_last_launch_count() == 2 and torch.equal(Y1, Y2)
+    finally:
+        mq.mq_set_option("fused_quant", 0)
+
+
 def test_m_zero_is_noop(mq):
     import torch
     case = make_case(51, 1, 256, 128, rho=0.0)
