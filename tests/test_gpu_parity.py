@@ -68,6 +68,53 @@ def test_quantize_act_edge_rows(mq):
     assert want_q[1, :9].tolist() == [7, -7, 4, 2, 2, 0, 0, -2, 0]
 
 
+@pytest.mark.parametrize("dt", ["f16", "bf16"])
+def test_quantize_act_near_ties_bit_exact(mq, dt):
+    """The kernels multiply by 1/s and divide only near half-integers (A3): rows made of the
+    16-bit neighbours of (k + 1/2) * s, for power-of-two scales (exact ties) and for scales that are not
+    representable nicely, plus tiny-scale rows (reciprocal unusable), must quantize exactly like the
+    oracle's IEEE division (the fused mq_linear path shares quant1() and is checked against the two-call path)."""
+    import torch
+    rng = np.random.default_rng(5)
+    K, rows = 512, []
+    amaxes = [7.0, 3.5, 56.0, 1.0, 5.0, 0.3, 1234.0, 6.0e-5, 2.2]
+    if dt == "bf16":
+        amaxes += [3.0e-38, 1.0e-30, 1.7e38]
+    for amax in amaxes:
+        amax16 = np.float32(np.float16(amax)) if dt == "f16" else None
+        if dt == "bf16":
+            amax16 = (np.array([amax], np.float32).view(np.uint32) & 0xFFFF0000).view(np.float32)[0]
+        s = np.float32(amax16) / np.float32(7.0)
+        x = np.zeros(K, np.float32)
+        ks = rng.integers(-7, 7, size=K).astype(np.float32) + np.float32(0.5)
+        x[:] = ks * s                                            # near a tie; snapped to the 16-bit grid below
+        x[0] = amax16
+        if dt == "f16":
+            base = x.astype(np.float16)
+            nb = base.view(np.int16) + rng.integers(-2, 3, size=K).astype(np.int16)   # neighbours on the grid
+            row = nb.view(np.float16)
+            row[0] = np.float16(amax16)
+            row = np.where(np.isfinite(row) & (np.abs(row.astype(np.float32)) <= amax16), row, np.float16(0))
+        else:
+            bits = (x.view(np.uint32) >> 16).astype(np.uint16) + rng.integers(0, 3, size=K).astype(np.uint16)
+            row = bits
+            row[0] = np.uint16(np.array([amax16], np.float32).view(np.uint32)[0] >> 16)
+            f = (row.astype(np.uint32) << 16).view(np.float32)
+            row = np.where(np.isfinite(f) & (np.abs(f) <= amax16), row, np.uint16(0))
+        rows.append(row)
+    A16 = np.stack(rows)
+    want_q, want_s = oracle.quantize_act(A16 if dt == "f16" else (A16, "bf16"))
+    if dt == "f16":
+        A = torch.from_numpy(A16).cuda()
+    else:
+        A = torch.from_numpy(A16.view(np.int16)).cuda().view(torch.bfloat16)
+    qA, sA = mq.mq_quantize_act(A)
+    got = mq.mq_unpack_act(qA, A.shape[0], K).cpu().numpy()
+    assert np.array_equal(sA.cpu().numpy().view(np.uint32), want_s.view(np.uint32))
+    assert np.array_equal(got, want_q), f"{int((got != want_q).sum())} codes differ"
+    assert (np.abs(want_q) == 7).any(axis=1).all()
+
+
 # ------------------------------------------------------------------ packing
 @pytest.mark.parametrize("bs", [64, 128])
 def test_pack_prequantized_roundtrip(mq, bs):
