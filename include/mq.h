@@ -144,6 +144,17 @@ int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t 
               void* Y_dev, mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev,
               size_t workspace_bytes, void* cuda_stream);
 
+/* The same layer with HOST buffers (end-to-end entry): A_host fp16/bf16 [M, K] dense (row stride K) is
+ * copied to the device, mq_linear runs, and Y [M, N] dense is copied back to Y_host, all enqueued on
+ * `cuda_stream`; the caller synchronises the stream before reading Y_host.  Host buffers should be pinned
+ * (page-locked) for the copies to be asynchronous; pageable memory works but blocks.  staging_dev: device
+ * scratch of at least mq_linear_host_staging_bytes(w, M) bytes (A and Y images), 256-byte aligned;
+ * workspace_dev as for mq_linear. */
+size_t mq_linear_host_staging_bytes(const mq_weights* w, int64_t M);
+int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, int64_t M, void* Y_host,
+                   mq_dtype y_dtype, void* staging_dev, size_t staging_bytes, void* workspace_dev,
+                   size_t workspace_bytes, void* cuda_stream);
+
 /* Tuning / ablation knobs (process-wide, not thread-safe; for benchmarks and tests).
  *   "split_k"   : 0 = automatic, 1 = whole output tiles per CTA, >= 2 = stream-K (the K-steps of
  *                 all tiles cut into equal per-CTA ranges, shared tiles finished by the last arriver)

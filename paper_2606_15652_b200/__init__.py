@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     mq_gemm_workspace_bytes,
     mq_last_launch_count,
     mq_linear,
+    mq_linear_host,
+    mq_linear_host_staging_bytes,
     mq_linear_workspace_bytes,
     mq_pack_prequantized,
     mq_pack_weights,

@@ -21,7 +21,8 @@ MQ_F16, MQ_BF16 = 0, 1
 EXPORTS = [
     "mq_status_string", "mq_qact_bytes", "mq_quantize_act", "mq_unpack_act", "mq_pack_weights",
     "mq_pack_prequantized", "mq_weights_export", "mq_weights_clone", "mq_weights_info", "mq_weights_free",
-    "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_set_option",
+    "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
+    "mq_linear_host", "mq_set_option",
     "mq_last_launch_count",
 ]
 
@@ -73,6 +74,10 @@ def lib() -> C.CDLL:
     L.mq_linear_workspace_bytes.argtypes = [vp, i64]
     L.mq_linear.restype = i32
     L.mq_linear.argtypes = [vp, vp, i32, i64, i64, vp, i32, i64, vp, sz, vp]
+    L.mq_linear_host_staging_bytes.restype = sz
+    L.mq_linear_host_staging_bytes.argtypes = [vp, i64]
+    L.mq_linear_host.restype = i32
+    L.mq_linear_host.argtypes = [vp, vp, i32, i64, vp, i32, vp, sz, vp, sz, vp]
     L.mq_set_option.restype = i32
     L.mq_set_option.argtypes = [C.c_char_p, i64]
     L.mq_last_launch_count.restype = i32
@@ -268,3 +273,19 @@ def mq_linear(w: Weights, A: torch.Tensor, Y: Optional[torch.Tensor] = None, out
     _check(lib().mq_linear(w.handle, A.data_ptr(), _dtype_code(A.dtype), M, lda, Y.data_ptr(), _dtype_code(Y.dtype),
                            ldy, workspace.data_ptr(), workspace.numel(), _stream()), "mq_linear")
     return Y
+
+
+def mq_linear_host_staging_bytes(w: Weights, M: int) -> int:
+    return int(lib().mq_linear_host_staging_bytes(w.handle, M))
+
+
+def mq_linear_host(w: Weights, A_host: torch.Tensor, Y_host: torch.Tensor, staging: torch.Tensor,
+                   workspace: torch.Tensor) -> torch.Tensor:
+    """End-to-end entry with HOST tensors (pinned for asynchronous copies): enqueues H2D copy, mq_linear and
+    D2H copy on the current stream; the caller synchronises before reading Y_host."""
+    M, K = A_host.shape
+    assert A_host.is_contiguous() and Y_host.is_contiguous() and not A_host.is_cuda and not Y_host.is_cuda
+    _check(lib().mq_linear_host(w.handle, A_host.data_ptr(), _dtype_code(A_host.dtype), M, Y_host.data_ptr(),
+                                _dtype_code(Y_host.dtype), staging.data_ptr(), staging.numel(), workspace.data_ptr(),
+                                workspace.numel(), _stream()), "mq_linear_host")
+    return Y_host

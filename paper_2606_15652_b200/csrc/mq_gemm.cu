@@ -1491,3 +1491,34 @@ extern "C" int mq_linear(const mq_weights* w, const void* A, mq_dtype a_dtype, i
   if (rc == MQ_OK) mq::set_launch_count(2);
   return rc;
 }
+
+extern "C" size_t mq_linear_host_staging_bytes(const mq_weights* w, int64_t M) {
+  if (!w || M <= 0) return 0;
+  return align256((size_t)M * (size_t)w->K * 2) + align256((size_t)M * (size_t)w->N * 2);
+}
+
+extern "C" int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, int64_t M, void* Y_host,
+                              mq_dtype y_dtype, void* staging, size_t staging_bytes, void* workspace,
+                              size_t workspace_bytes, void* cuda_stream) {
+  if (!w) return MQ_ERR_INVALID_ARG;
+  if (M == 0) return MQ_OK;
+  if (M < 0) return MQ_ERR_UNSUPPORTED_SHAPE;
+  if (!A_host || !Y_host || !staging || ((uintptr_t)staging & 255)) return MQ_ERR_INVALID_ARG;
+  if (staging_bytes < mq_linear_host_staging_bytes(w, M)) return MQ_ERR_WORKSPACE;
+  int rc = mq::check_device();
+  if (rc != MQ_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  uint8_t* a_dev = (uint8_t*)staging;
+  uint8_t* y_dev = a_dev + align256((size_t)M * (size_t)w->K * 2);
+  if (cudaMemcpyAsync(a_dev, A_host, (size_t)M * (size_t)w->K * 2, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  rc = mq_linear(w, a_dev, a_dtype, M, w->K, y_dev, y_dtype, w->N, workspace, workspace_bytes, cuda_stream);
+  if (rc != MQ_OK) return rc;
+  if (cudaMemcpyAsync(Y_host, y_dev, (size_t)M * (size_t)w->N * 2, cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  return MQ_OK;
+}

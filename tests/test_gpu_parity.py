@@ -378,6 +378,23 @@ def test_linear_fused_quantization_small_m(mq, M, K, N, rho, dt):
         mq.mq_set_option("fused_quant", 0)
 
 
+def test_linear_host_buffers_end_to_end(mq):
+    """mq_linear_host: host pointers in and out (the e2e entry bench.py times) equals the device path."""
+    import torch
+    for M in (3, 40):
+        case = make_case(71 + M, M, 1024, 384, bs=64, rho=0.1)
+        w = pack_from_oracle(case)
+        got = run_cuda(case, w=w)
+        A_host = torch.from_numpy(case.A16).pin_memory()
+        Y_host = torch.empty((M, 384), dtype=torch.bfloat16).pin_memory()
+        stg = torch.empty(mq.mq_linear_host_staging_bytes(w, M), dtype=torch.uint8, device="cuda")
+        ws = mq.new_workspace(mq.mq_linear_workspace_bytes(w, M))
+        for _ in range(2):
+            mq.mq_linear_host(w, A_host, Y_host, stg, ws)
+            torch.cuda.synchronize()
+            assert np.array_equal(Y_host.float().numpy().astype(np.float64), got["Y"])
+
+
 def test_m_zero_is_noop(mq):
     import torch
     case = make_case(51, 1, 256, 128, rho=0.0)
