@@ -1263,22 +1263,35 @@ struct Plan {
 Plan make_plan(const mq_weights* w, int64_t M) {
   Plan pl;
   const Options& o = options();
-  int bt;
-  if (o.token_tile)
-    bt = (int)o.token_tile;
-  else
-    bt = M <= 16 ? 16 : (M <= 32 ? 32 : (M <= 64 ? 64 : 128));
-  pl.BT = bt;
-  pl.TT = (int)((M + bt - 1) / bt);
   const int NT = (int)(w->N / BN), KS = (int)(w->K / BK);
   int G = sm_count() > 0 ? sm_count() : 148;
   if (o.max_ctas > 0) G = (int)std::min<int64_t>(G, o.max_ctas);
+  int bt;
+  if (o.token_tile) {
+    bt = (int)o.token_tile;
+  } else if (M <= 32) {
+    bt = M <= 16 ? 16 : 32;
+  } else {
+    // Mid-size M: the smallest token tile whose tile count still fits one wave (most CTAs busy with
+    // whole tiles, no split-K fix-up); if even 128-token tiles need several waves, the tile that
+    // wastes least (M <= 64: 64, else 128).
+    bt = M <= 64 ? 64 : 128;
+    for (int cand = 32; cand <= 128; cand *= 2)
+      if ((int64_t)NT * ((M + cand - 1) / cand) <= G) {
+        bt = cand;
+        break;
+      }
+  }
+  pl.BT = bt;
+  pl.TT = (int)((M + bt - 1) / bt);
   const int64_t tiles = (int64_t)NT * pl.TT;
   pl.units = tiles * KS;
-  // stream-K (ranges cut at K-step granularity) unless there are enough tiles to balance whole ones
-  // Large token tiles pay 128 KB per partial tile in the fix-up, so they split K only when most SMs
-  // would otherwise idle; small (decode) tiles split whenever whole tiles would not balance.
-  bool stream_k = bt <= 32 ? tiles < 8LL * G : tiles * 2 <= G;
+  // Decode (M <= 32) streams weights and needs every SM pulling: split K whenever whole tiles would not
+  // balance.  Beyond that a partial tile costs BT x 128 x 8 bytes in the fix-up, so K is split only when
+  // most SMs would otherwise idle.
+  bool stream_k = M <= 32 ? tiles < 8LL * G
+                          : (bt <= 32 ? tiles * 2 <= G && (tiles * 3 <= G || KS >= 64)   // cheap fix-up: long K pays
+                                      : tiles * 2 <= G);
   if (o.split_k == 1) stream_k = false;
   if (o.split_k >= 2) stream_k = true;
   pl.gran = stream_k ? 1 : KS;
