@@ -57,3 +57,24 @@ def test_full_size_sampled_rows(mq, name, M, K, N):
     for rep in range(2):
         got = run_cuda(case, w=w, workspace=ws)
         assert_parity(got, want, rows=rows, what=f"{name} rep {rep}")
+
+
+# BASELINE.json configs[3]: the Qwen3-8B density / block-size sweep (0 %, 1 %, 5 %, 10 %; 64 and 128)
+SWEEP = [(1, 4096, 6144, 64, 0.0), (1, 4096, 6144, 64, 0.01), (128, 4096, 4096, 64, 0.10), (1, 12288, 4096, 128, 0.05),
+         (128, 4096, 6144, 128, 0.10), (4096, 4096, 4096, 128, 0.01)]
+
+
+@pytest.mark.parametrize("M,K,N,bs,rho", SWEEP)
+def test_qwen3_density_and_block_sweep(mq, M, K, N, bs, rho):
+    case = make_case(9500 + M + N + bs, M, K, N, bs=bs, rho=rho, calib_tokens=64)
+    budget = synth.budget_from_density(rho, N, K, bs)
+    w = mq.mq_pack_weights(case.W, case.h, bs, budget)
+    ex = w.export()
+    assert sorted(zip(ex["blk_n"].tolist(), ex["blk_k"].tolist())) == sorted(zip(case.L.blk_n.tolist(), case.L.blk_k.tolist()))
+    rng = np.random.default_rng(M + N + bs)
+    rows = np.arange(M) if M <= 64 else np.sort(rng.choice(M, size=64, replace=False))
+    want = oracle_forward(case, rows=rows)
+    got = run_cuda(case, w=w)
+    assert_parity(got, want, rows=rows, what=f"qwen3 sweep M{M} K{K} N{N} bs{bs} rho{rho}")
+    if rho == 0.0:
+        assert not got["acc1"].any()
