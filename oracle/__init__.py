@@ -38,12 +38,12 @@ def num_threads() -> int:
     return int(lib().orc_num_threads())
 
 
-def quantize_row(x: np.ndarray) -> Tuple[np.ndarray, np.float32]:
-    """O1 (Eq.1, P:77)."""
+def quantize_row(x: np.ndarray, bits: int = 4) -> Tuple[np.ndarray, np.float32]:
+    """O1 (Eq.1); bits = 4 (q_max 7) or 8 (q_max 127: the W4A8 activations)."""
     x = np.ascontiguousarray(x, dtype=np.float32)
     q = np.empty(x.shape[0], dtype=np.int8)
     s = np.empty(1, dtype=np.float32)
-    lib().orc_quantize_row(_p(x), C.c_int64(x.shape[0]), _p(q), _p(s))
+    lib().orc_quantize_row_bits(_p(x), C.c_int64(x.shape[0]), C.c_int(bits), _p(q), _p(s))
     return q, s[0]
 
 
@@ -57,13 +57,13 @@ def _bits16(A) -> Tuple[np.ndarray, int]:
     return np.ascontiguousarray(A).view(np.uint16), 0
 
 
-def quantize_act(A) -> Tuple[np.ndarray, np.ndarray]:
-    """O2: per-token int4 quantization of fp16 (np.float16) or bf16 ((bits,'bf16')) activations."""
-    bits, code = _bits16(A)
-    M, K = bits.shape
+def quantize_act(A, bits: int = 4) -> Tuple[np.ndarray, np.ndarray]:
+    """O2: per-token int4 (or int8, W4A8) quantization of fp16 (np.float16) or bf16 ((bits,'bf16')) activations."""
+    b16, code = _bits16(A)
+    M, K = b16.shape
     qa = np.empty((M, K), dtype=np.int8)
     sa = np.empty(M, dtype=np.float32)
-    lib().orc_quantize_act(_p(bits), C.c_int(code), C.c_int64(M), C.c_int64(K), C.c_int64(K), _p(qa), _p(sa))
+    lib().orc_quantize_act_bits(_p(b16), C.c_int(code), C.c_int64(M), C.c_int64(K), C.c_int64(K), C.c_int(bits), _p(qa), _p(sa))
     return qa, sa
 
 

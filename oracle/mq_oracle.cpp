@@ -9,8 +9,9 @@
 // paper's order and notation.  Citations are PAPER.md lines ("P:<line>") of
 // /root/reference/PAPER.md; "A<n>" are the readings listed in DESIGN.md section 3.
 //
-//   O1 quantize_row      Eq.1  P:75-80   uniform symmetric quantizer, q_max = 7 (A1-A3)
-//   O2 activation        P:439-441       per-token dynamic quantization (A5)
+//   O1 quantize_row      Eq.1  P:75-80   uniform symmetric quantizer, q_max = 7 (A1-A3); q_max = 127 for the
+//                                        8-bit activations of the W4A8 variant (Table 1 W4A8 rows)
+//   O2 activation        P:439-441       per-token dynamic quantization (A5), 4-bit or 8-bit
 //   O3 base weight + R   Alg.1 line 1    P:124, per output channel (A9)
 //   O4 residual Q(R)     Alg.1 / Eq.4    P:106,124, per output channel over all K (A4)
 //   O5 h_j               Alg.1 line 2
@@ -72,10 +73,10 @@ float bf16_bits_to_float(uint16_t b) {
   return f;
 }
 
-// O1 -- Eq.1: Q_X = round(X / s_X), s_X = max|X| / q_max, q_max = 7 (A1).
-// One binary32 division for s, one binary32 division per element, round half to
-// even (A3).  All-zero row: s = 1, q = 0 (A2).
-void quantize_row(const float* x, int64_t L, int8_t* q, float* s_out) {
+// O1 -- Eq.1: Q_X = round(X / s_X), s_X = max|X| / q_max; q_max = 2^(b-1) - 1: 7 for the 4-bit
+// operands (A1), 127 for the 8-bit activations of W4A8.  One binary32 division for s, one
+// binary32 division per element, round half to even (A3).  All-zero row: s = 1, q = 0 (A2).
+void quantize_row(const float* x, int64_t L, int8_t* q, float* s_out, int qmax = 7) {
   float amax = 0.0f;
   for (int64_t i = 0; i < L; ++i) {
     float a = std::fabs(x[i]);
@@ -86,13 +87,13 @@ void quantize_row(const float* x, int64_t L, int8_t* q, float* s_out) {
     for (int64_t i = 0; i < L; ++i) q[i] = 0;
     return;
   }
-  volatile float s = amax / 7.0f;
+  volatile float s = amax / (float)qmax;
   for (int64_t i = 0; i < L; ++i) {
     volatile float t = x[i] / s;
     float r = std::nearbyintf(t);  // default rounding mode: round half to even
     int v = (int)r;
-    if (v > 7) v = 7;
-    if (v < -7) v = -7;
+    if (v > qmax) v = qmax;
+    if (v < -qmax) v = -qmax;
     q[i] = (int8_t)v;
   }
   *s_out = s;
@@ -112,12 +113,23 @@ int orc_num_threads() {
 
 // O1 exposed for pins.
 void orc_quantize_row(const float* x, int64_t L, int8_t* q, float* s) { quantize_row(x, L, q, s); }
+void orc_quantize_row_bits(const float* x, int64_t L, int bits, int8_t* q, float* s) {
+  quantize_row(x, L, q, s, bits == 8 ? 127 : 7);
+}
 
 // O2 -- per-token activation quantization ("per-token dynamic activation
 // quantization"; A5).  A is fp16 (dtype 0) or bf16 (dtype 1) bits, row stride lda
 // elements; each row is converted exactly to fp32 and quantized by O1 over all K.
+void orc_quantize_act_bits(const uint16_t* A_bits, int dtype, int64_t M, int64_t K, int64_t lda, int bits,
+                           int8_t* qa /*[M,K]*/, float* sa /*[M]*/);
 void orc_quantize_act(const uint16_t* A_bits, int dtype, int64_t M, int64_t K, int64_t lda,
                       int8_t* qa /*[M,K]*/, float* sa /*[M]*/) {
+  orc_quantize_act_bits(A_bits, dtype, M, K, lda, 4, qa, sa);
+}
+// O2 with the activation width as a parameter: 4 bits (W4A4) or 8 bits (W4A8)
+void orc_quantize_act_bits(const uint16_t* A_bits, int dtype, int64_t M, int64_t K, int64_t lda, int bits,
+                           int8_t* qa /*[M,K]*/, float* sa /*[M]*/) {
+  const int qmax = bits == 8 ? 127 : 7;
 #pragma omp parallel
   {
     std::vector<float> row((size_t)K);
@@ -126,7 +138,7 @@ void orc_quantize_act(const uint16_t* A_bits, int dtype, int64_t M, int64_t K, i
       const uint16_t* src = A_bits + m * lda;
       for (int64_t k = 0; k < K; ++k)
         row[(size_t)k] = dtype == 0 ? half_bits_to_float(src[k]) : bf16_bits_to_float(src[k]);
-      quantize_row(row.data(), K, qa + m * K, sa + m);
+      quantize_row(row.data(), K, qa + m * K, sa + m, qmax);
     }
   }
 }

@@ -76,6 +76,49 @@ def test_o1_ties_on_fp16_grid_round_half_even():
     assert q.tolist() == want
 
 
+def test_o1_8bit_activations_w4a8():
+    """The W4A8 variant (Table 1 W4A8 rows): the same quantizer with q_max = 127.  Hand vector
+    (tests/golden/o1_hand_vector_8bit.txt), correctly rounded scale, nearest code, no clipping, symmetry,
+    power-of-two scaling, exact ties, and the per-token activation path on 16-bit inputs."""
+    rows = [l.split() for l in open(__file__.replace("test_oracle_pins.py", "golden/o1_hand_vector_8bit.txt"))
+            if l.strip() and not l.startswith("#")]
+    x = np.array([float(r[0]) for r in rows], np.float32)
+    q, s = oracle.quantize_row(x, bits=8)
+    assert s == np.float32(1.0) and q.tolist() == [int(r[1]) for r in rows]
+    rng = np.random.default_rng(8)
+    for trial in range(10):
+        x = (rng.standard_normal(300) * 10 ** rng.uniform(-3, 3)).astype(np.float32)
+        q, s = oracle.quantize_row(x, bits=8)
+        exact = Fraction(float(np.abs(x).max())) / 127
+        sf = Fraction(float(s))
+        lo = Fraction(float(np.nextafter(s, np.float32(0))))
+        hi = Fraction(float(np.nextafter(s, np.float32(np.inf))))
+        assert abs(sf - exact) <= abs(lo - exact) and abs(sf - exact) <= abs(hi - exact)
+        for xi, qi in zip(x, q):
+            t = Fraction(float(xi)) / sf
+            assert abs(t - int(qi)) <= Fraction(1, 2) + abs(t) * Fraction(1, 2 ** 23)
+        i = int(np.abs(x).argmax())
+        assert abs(int(q[i])) == 127 and np.sign(q[i]) == np.sign(x[i]) and np.abs(q.astype(np.int32)).max() <= 127
+        assert np.all(np.abs(x.astype(np.float64) - float(s) * q) <= float(s) / 2 * (1 + 2 ** -20))
+        qn, sn = oracle.quantize_row(-x, bits=8)
+        assert sn == s and np.array_equal(qn, -q)
+        q2, s2 = oracle.quantize_row(np.ldexp(x, 5).astype(np.float32), bits=8)
+        assert np.array_equal(q2, q) and s2 == np.float32(np.ldexp(np.float64(s), 5))
+    # exact ties on the fp16 grid: amax = 127 * 2^-4 -> s = 2^-4; x = (n + 1/2) * 2^-4
+    n = np.arange(-126, 127, 7)
+    x = np.concatenate([[127 / 16], (n + 0.5) / 16]).astype(np.float16).astype(np.float32)
+    q, s = oracle.quantize_row(x, bits=8)
+    assert s == np.float32(1 / 16) and q.tolist() == [127] + [int(2 * round((k + 0.5) / 2)) for k in n]
+    # O2 at 8 bits: per token, row by row equal to O1 on the exactly converted fp16 row
+    A = (rng.standard_normal((5, 64)) * 3).astype(np.float16)
+    qa, sa = oracle.quantize_act(A, bits=8)
+    for m in range(5):
+        qr, sr = oracle.quantize_row(A[m].astype(np.float32), bits=8)
+        assert np.array_equal(qa[m], qr) and sa[m] == sr
+    qz, sz = oracle.quantize_row(np.zeros(9, np.float32), bits=8)
+    assert sz == np.float32(1.0) and not qz.any()
+
+
 def test_o2_fp16_bf16_conversion_exact_and_per_token():
     rng = np.random.default_rng(3)
     A = (rng.standard_normal((9, 128)) * 3).astype(np.float16)
