@@ -131,6 +131,19 @@ int mq_gemm(const mq_weights* w, const void* qA_dev, const float* sA_dev, int64_
             mq_dtype y_dtype, int64_t ldy_elems, int32_t* dbg_acc_base_dev, int32_t* dbg_acc_res_dev,
             void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------
+ * (3b) W4A8 variant -- the paper's other reported precision ("per-token ... activation quantization",
+ * Table 1 W4A8 rows): per-token int8 activations (Eq.1 with q_max = 127) against the same packed int4
+ * base + residual weights.  mq_quantize_act8 writes qA8_dev int8 [M, K] row-major (canonical order,
+ * 16-byte aligned) and sA_dev float [M]; mq_gemm_a8 is mq_gemm on those (same arguments, workspace,
+ * parity hooks and tolerances; acc0 / acc1 are the exact integer dot products of the int8 activations).
+ * Requires 127*7*16*K < 2^31. */
+int mq_quantize_act8(const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda_elems,
+                     int8_t* qA8_dev, float* sA_dev, void* cuda_stream);
+int mq_gemm_a8(const mq_weights* w, const int8_t* qA8_dev, const float* sA_dev, int64_t M, void* Y_dev,
+               mq_dtype y_dtype, int64_t ldy_elems, int32_t* dbg_acc_base_dev, int32_t* dbg_acc_res_dev,
+               void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
 /* One linear layer from raw activations: A_dev fp16/bf16 [M, K] (rows 16-byte aligned, lda_elems % 8 == 0).
  * Default: mq_quantize_act into the workspace followed by mq_gemm on the same stream (two launches
  * chained by programmatic dependent launch).  With option "fused_quant" = 1 and M <= 8 the quantizer runs

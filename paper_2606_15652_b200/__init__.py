@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     Weights,
     lib,
     mq_gemm,
+    mq_gemm_a8,
     mq_gemm_workspace_bytes,
     mq_last_launch_count,
     mq_linear,
@@ -22,6 +23,7 @@ from .binding import (  # noqa: F401
     mq_pack_weights,
     mq_qact_bytes,
     mq_quantize_act,
+    mq_quantize_act8,
     mq_set_option,
     mq_unpack_act,
     new_workspace,

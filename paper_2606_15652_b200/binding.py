@@ -22,7 +22,7 @@ EXPORTS = [
     "mq_status_string", "mq_qact_bytes", "mq_quantize_act", "mq_unpack_act", "mq_pack_weights",
     "mq_pack_prequantized", "mq_weights_export", "mq_weights_clone", "mq_weights_info", "mq_weights_free",
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
-    "mq_linear_host", "mq_set_option",
+    "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_set_option",
     "mq_last_launch_count",
 ]
 
@@ -78,6 +78,10 @@ def lib() -> C.CDLL:
     L.mq_linear_host_staging_bytes.argtypes = [vp, i64]
     L.mq_linear_host.restype = i32
     L.mq_linear_host.argtypes = [vp, vp, i32, i64, vp, i32, vp, sz, vp, sz, vp]
+    L.mq_quantize_act8.restype = i32
+    L.mq_quantize_act8.argtypes = [vp, i32, i64, i64, i64, vp, vp, vp]
+    L.mq_gemm_a8.restype = i32
+    L.mq_gemm_a8.argtypes = [vp, vp, vp, i64, vp, i32, i64, vp, vp, vp, sz, vp]
     L.mq_set_option.restype = i32
     L.mq_set_option.argtypes = [C.c_char_p, i64]
     L.mq_last_launch_count.restype = i32
@@ -289,3 +293,33 @@ def mq_linear_host(w: Weights, A_host: torch.Tensor, Y_host: torch.Tensor, stagi
                                 _dtype_code(Y_host.dtype), staging.data_ptr(), staging.numel(), workspace.data_ptr(),
                                 workspace.numel(), _stream()), "mq_linear_host")
     return Y_host
+
+
+def mq_quantize_act8(A: torch.Tensor) -> Tuple[torch.Tensor, torch.Tensor]:
+    """W4A8: per-token int8 activations (q_max = 127).  Returns (qA8 int8 [M,K], sA float32 [M])."""
+    M, K = A.shape
+    q8 = torch.empty((M, K), dtype=torch.int8, device=A.device)
+    sA = torch.empty((M,), dtype=torch.float32, device=A.device)
+    lda = A.stride(0) if M > 1 else K
+    _check(lib().mq_quantize_act8(A.data_ptr(), _dtype_code(A.dtype), M, K, lda, q8.data_ptr(), sA.data_ptr(), _stream()),
+           "mq_quantize_act8")
+    return q8, sA
+
+
+def mq_gemm_a8(w: Weights, qA8: torch.Tensor, sA: torch.Tensor, M: int, Y: Optional[torch.Tensor] = None,
+               out_dtype: torch.dtype = torch.bfloat16, dbg: bool = False, workspace: Optional[torch.Tensor] = None):
+    """W4A8 fused base + residual GEMM (int8 activations).  Same contract as mq_gemm."""
+    N = w.info()["N"]
+    if Y is None:
+        Y = torch.empty((M, N), dtype=out_dtype, device=qA8.device)
+    need = mq_gemm_workspace_bytes(w, M)
+    if need and workspace is None:
+        workspace = new_workspace(need, qA8.device)
+    d0 = torch.empty((M, N), dtype=torch.int32, device=qA8.device) if dbg else None
+    d1 = torch.empty((M, N), dtype=torch.int32, device=qA8.device) if dbg else None
+    ldy = Y.stride(0) if M > 1 else N
+    _check(lib().mq_gemm_a8(w.handle, qA8.data_ptr(), sA.data_ptr(), M, Y.data_ptr(), _dtype_code(Y.dtype), ldy,
+                            d0.data_ptr() if dbg else None, d1.data_ptr() if dbg else None,
+                            workspace.data_ptr() if workspace is not None else None,
+                            workspace.numel() if workspace is not None else 0, _stream()), "mq_gemm_a8")
+    return (Y, d0, d1) if dbg else Y

@@ -69,7 +69,9 @@ constexpr int META_LAST = 1 << 29;           // last K-step of the segment: accu
 // of its unpack group in this CTA (mod 256); bits 12-27: sequence number of the cell's first
 // stored quarter among the quarters of its unpack group (mod 65536)
 
-template <int BT, bool FUSED = false>
+// A8: W4A8 variant (the paper's other precision): per-token int8 activations, 1 byte per element in
+// the token area; the unpack groups only re-order them (no expansion), accumulators are 16 x the true value.
+template <int BT, bool FUSED = false, bool A8 = false>
 struct Cfg {
   // Unpack groups (4 warps each).  An item costs a group ~1000 cycles of mostly latency (loads,
   // TMEM/shared stores, proxy fences), so prefill runs four groups side by side.
@@ -78,7 +80,8 @@ struct Cfg {
   static constexpr int SK = BT <= 32 ? 4 : 2;                    // K-steps per P stage
   static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // K-steps per U stage (item)
   static constexpr int IPS = SK / UK;                            // items per P stage
-  static constexpr int PSTAGES = BT <= 32 ? 4 : (BT == 64 ? 6 : 4);
+  static constexpr int PSTAGES = A8 ? (BT == 16 ? 4 : (BT == 32 ? 3 : (BT == 64 ? 4 : 3)))
+                                    : (BT <= 32 ? 4 : (BT == 64 ? 6 : 4));
   static constexpr int USTAGES = G;                                   // one per unpack group
   // Unpacked residual cells (TMEM): every unpack group owns a private ring of RG stages.  A ring
   // shared between the groups would be unsafe: mbarrier parity waits cannot tell "my turn" from
@@ -94,7 +97,10 @@ struct Cfg {
   static constexpr int P_W = SK * TILE_BYTES;
   // token area of a P stage: packed int4 tokens [SK][BT][64 B], or (FUSED) raw 16-bit activations
   // [SK][8 rows][256 B] fetched by a tensor map over A itself
-  static constexpr int TOK_KSTEP = FUSED ? 8 * BK * 2 : BT * (BK / 2);
+  static constexpr int TOK_KSTEP = FUSED ? 8 * BK * 2 : (A8 ? BT * BK : BT * (BK / 2));
+  static constexpr float ACC_INV = A8 ? 0.0625f : 0.00390625f;   // accumulators are x16 (A8) or x256
+  static constexpr int ACC_SHIFT = A8 ? 4 : 8;
+  static_assert(!(FUSED && A8), "the fused quantizer is 4-bit only");
   static constexpr int P_TOK = SK * TOK_KSTEP;
   static constexpr int P_STAGE = P_W + P_TOK;
   static constexpr int U_SUB = BT * BK;                          // one int8 token sub-tile
@@ -303,10 +309,10 @@ __device__ __forceinline__ void store_y(void* Y, size_t o, float y) {
 // all other CTAs (atomic max + grid-wide arrival count, hidden behind the first weight stage's HBM
 // latency), and the unpack groups quantize the fp16/bf16 tokens of their K-steps straight into the int8
 // operand tile -- no packed activations, no second kernel.
-template <int BT, bool FUSED>
-__global__ void __launch_bounds__(Cfg<BT, FUSED>::NUM_THREADS, 1)
+template <int BT, bool FUSED, bool A8>
+__global__ void __launch_bounds__(Cfg<BT, FUSED, A8>::NUM_THREADS, 1)
 mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
-  using C = Cfg<BT, FUSED>;
+  using C = Cfg<BT, FUSED, A8>;
   constexpr int SK = C::SK, UK = C::UK, IPS = C::IPS;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -444,7 +450,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           if constexpr (FUSED)   // raw activations: box {128 elements, 8 rows} of the 16-bit tensor map over A
             tma_load_2d(dst + C::P_W + j * C::TOK_KSTEP, &tmap_a, (cur.ks + j) * BK, 0, fb);
           else
-            tma_load_2d(dst + C::P_W + j * C::TOK_KSTEP, &tmap_a, (cur.ks + j) * (BK / 2), cur.tt * BT, fb);
+            tma_load_2d(dst + C::P_W + j * C::TOK_KSTEP, &tmap_a, (cur.ks + j) * (A8 ? BK : BK / 2), cur.tt * BT, fb);
         }
       }
       // metadata words of the stage (lane j writes K-step j), then the second arrival publishes them.
@@ -720,7 +726,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         // expansion (2 logic ops per 8 elements), the stores and the fences.  The cell's unpacked weights ride in the U stage's own residual columns
         // (R stage = U stage), so FULL_U / EMPTY_U cover them and no separate hand-off is needed.
         static_assert(UK != 1 || (BT * 4) % 128 == 0, "token chunks per thread");
-        constexpr int TCH = BT * 4 / 128;   // 16-byte packed token chunks per thread
+        constexpr int TCH = BT * (A8 ? 8 : 4) / 128;   // 16-byte token chunks per thread and K-step
         const int m = mw[0];
         const bool valid = (m & META_VALID) != 0;
         const int mask = valid ? (m & 0xF) : 0;
@@ -728,7 +734,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (valid) {
 #pragma unroll
           for (int c = 0; c < 4; ++c) v4[c] = lds128(pw + c * (BN * 16) + row * 16);
-          const uint32_t pt1 = sP + ps * C::P_STAGE + C::P_W + sub * (BT * (BK / 2));
+          const uint32_t pt1 = sP + ps * C::P_STAGE + C::P_W + sub * C::TOK_KSTEP;
 #pragma unroll
           for (int i = 0; i < TCH; ++i) t4[i] = lds128(pt1 + (gtid + 128u * i) * 16);
           // the loads must have landed before the P stage is handed back
@@ -783,11 +789,19 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           const uint32_t ut1 = sU + us * C::U_STAGE;
 #pragma unroll
           for (int i = 0; i < TCH; ++i) {
-            const uint32_t idx = gtid + 128u * i, t = idx >> 2, c = idx & 3;
-            uint32_t tw[8];
-            unpack16(t4[i], tw);
-            sts128(ut1 + t * 128 + (((2 * c) ^ (t & 7)) << 4), tw);
-            sts128(ut1 + t * 128 + (((2 * c + 1) ^ (t & 7)) << 4), tw + 4);
+            if constexpr (A8) {
+              // 16 int8 tokens elements: only the even / odd re-ordering the weights' expansion produces
+              const uint32_t idx = gtid + 128u * i, t = idx >> 3, c = idx & 7;
+              const uint32_t tw[4] = {__byte_perm(t4[i].x, t4[i].y, 0x6420), __byte_perm(t4[i].x, t4[i].y, 0x7531),
+                                      __byte_perm(t4[i].z, t4[i].w, 0x6420), __byte_perm(t4[i].z, t4[i].w, 0x7531)};
+              sts128(ut1 + t * 128 + ((c ^ (t & 7)) << 4), tw);
+            } else {
+              const uint32_t idx = gtid + 128u * i, t = idx >> 2, c = idx & 3;
+              uint32_t tw[8];
+              unpack16(t4[i], tw);
+              sts128(ut1 + t * 128 + (((2 * c) ^ (t & 7)) << 4), tw);
+              sts128(ut1 + t * 128 + (((2 * c + 1) ^ (t & 7)) << 4), tw + 4);
+            }
           }
         }
         tmem_st_wait();
@@ -844,6 +858,17 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
             quant8_i8x16(lds128(pt + jj * C::TOK_KSTEP + t * (BK * 2) + c8 * 16), s, inv_s, p.a_bf16 != 0, ev, od);
             const uint32_t dst = ut + jj * C::U_SUB + t * 128 + ((((c8 >> 1)) ^ (t & 7)) << 4) + (c8 & 1) * 8;
             asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(dst), "r"(ev), "r"(od) : "memory");
+          }
+        }
+      } else if constexpr (A8) {
+#pragma unroll
+        for (uint32_t idx = gtid; idx < (uint32_t)(UK * BT * 8); idx += 128) {
+          const uint32_t jj = idx / (BT * 8), rem = idx % (BT * 8), t = rem >> 3, c = rem & 7;
+          if ((int)jj < nk) {
+            const uint4 tv = lds128(pt + idx * 16);
+            const uint32_t tw[4] = {__byte_perm(tv.x, tv.y, 0x6420), __byte_perm(tv.x, tv.y, 0x7531),
+                                    __byte_perm(tv.z, tv.w, 0x6420), __byte_perm(tv.z, tv.w, 0x7531)};
+            sts128(ut + jj * C::U_SUB + t * 128 + ((c ^ (t & 7)) << 4), tw);
           }
         }
       } else {
@@ -1002,7 +1027,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       const int n = nt * BN + n_loc;
       const int t_base = tt * BT;
       const int t_cnt = min(BT, p.M - t_base);
-      const float swn = __ldg(p.sw + n) * 0.00390625f, srn = __ldg(p.sr + n) * 0.00390625f;  // / 256: accumulators are x256
+      const float swn = __ldg(p.sw + n) * C::ACC_INV, srn = __ldg(p.sr + n) * C::ACC_INV;  // accumulators are x256 (x16: A8)
       auto emit = [&](int t, float sat, int32_t a0, int32_t a1) {
         const float y = sat * ((float)a0 * swn + (float)a1 * srn);
         const size_t o = (size_t)(t_base + t) * p.ldy + n;
@@ -1010,8 +1035,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           store_y<true>(p.Y, o, y);
         else
           store_y<false>(p.Y, o, y);
-        if (p.dbg0) p.dbg0[(size_t)(t_base + t) * p.N + n] = a0 >> 8;
-        if (p.dbg1) p.dbg1[(size_t)(t_base + t) * p.N + n] = a1 >> 8;
+        if (p.dbg0) p.dbg0[(size_t)(t_base + t) * p.N + n] = a0 >> C::ACC_SHIFT;
+        if (p.dbg1) p.dbg1[(size_t)(t_base + t) * p.N + n] = a1 >> C::ACC_SHIFT;
       };
 
       mbar_wait(bar(B_TFULL + a0s), aphase);
@@ -1147,7 +1172,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
         const int n = nt * BN + n0;
         const float4 sw4 = *reinterpret_cast<const float4*>(p.sw + n), sr4 = *reinterpret_cast<const float4*>(p.sr + n);
-        const float sat = (FUSED ? sa_s[t] : __ldg(p.sa + t_base + t)) * 0.00390625f;    // / 256: accumulators are x256
+        const float sat = (FUSED ? sa_s[t] : __ldg(p.sa + t_base + t)) * C::ACC_INV;    // accumulators are x256 (x16: A8)
         float y[4];
         y[0] = sat * ((float)s0.x * sw4.x + (float)s1.x * sr4.x);
         y[1] = sat * ((float)s0.y * sw4.y + (float)s1.y * sr4.y);
@@ -1176,8 +1201,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           }
         }
         const size_t od = (size_t)(t_base + t) * p.N + n;
-        if (p.dbg0) *reinterpret_cast<int4*>(p.dbg0 + od) = make_int4(s0.x >> 8, s0.y >> 8, s0.z >> 8, s0.w >> 8);
-        if (p.dbg1) *reinterpret_cast<int4*>(p.dbg1 + od) = make_int4(s1.x >> 8, s1.y >> 8, s1.z >> 8, s1.w >> 8);
+        if (p.dbg0) *reinterpret_cast<int4*>(p.dbg0 + od) = make_int4(s0.x >> C::ACC_SHIFT, s0.y >> C::ACC_SHIFT, s0.z >> C::ACC_SHIFT, s0.w >> C::ACC_SHIFT);
+        if (p.dbg1) *reinterpret_cast<int4*>(p.dbg1 + od) = make_int4(s1.x >> C::ACC_SHIFT, s1.y >> C::ACC_SHIFT, s1.z >> C::ACC_SHIFT, s1.w >> C::ACC_SHIFT);
       }
       // the last contributor to finish returns the tile's counters to zero for the next call
       named_bar_sync(1, 128);
@@ -1311,12 +1336,12 @@ Plan make_plan(const mq_weights* w, int64_t M) {
   return pl;
 }
 
-template <int BT, bool FUSED = false>
+template <int BT, bool FUSED = false, bool A8 = false>
 int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t st) {
-  using C = Cfg<BT, FUSED>;
+  using C = Cfg<BT, FUSED, A8>;
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(mq_gemm_kernel<BT, FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) !=
+    if (cudaFuncSetAttribute(mq_gemm_kernel<BT, FUSED, A8>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) !=
         cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
@@ -1333,7 +1358,7 @@ int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = options().pdl ? 1 : 0;
-  if (cudaLaunchKernelEx(&cfg, mq_gemm_kernel<BT, FUSED>, tmap, gp) != cudaSuccess) {
+  if (cudaLaunchKernelEx(&cfg, mq_gemm_kernel<BT, FUSED, A8>, tmap, gp) != cudaSuccess) {
     cudaGetLastError();
     return MQ_ERR_CUDA;
   }
@@ -1359,8 +1384,9 @@ namespace {
 // and qA / sA are unused.
 int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
               int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes, void* cuda_stream,
-              const void* fused_A, mq_dtype a_dtype, int64_t lda, uint32_t* fz_ctrl) {
+              const void* fused_A, mq_dtype a_dtype, int64_t lda, uint32_t* fz_ctrl, bool a8 = false) {
   const bool fused = fused_A != nullptr;
+  if (a8 && (fused || (w && (long double)127 * 7 * 16 * (long double)w->K >= 2147483648.0L))) return MQ_ERR_ACC_OVERFLOW;
   if (!w) return MQ_ERR_INVALID_ARG;
   if (M < 0 || M > (1 << 30)) return MQ_ERR_UNSUPPORTED_SHAPE;
   if (y_dtype != MQ_F16 && y_dtype != MQ_BF16) return MQ_ERR_INVALID_ARG;
@@ -1388,9 +1414,11 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   CUtensorMap tmap;
   memset(&tmap, 0, sizeof(tmap));
   if (fused && pl.BT != 16) return MQ_ERR_INVALID_ARG;
-  const cuuint64_t gdim[2] = {(cuuint64_t)(w->K / 2), (cuuint64_t)M};
-  const cuuint64_t gstride[1] = {(cuuint64_t)(w->K / 2)};
-  const cuuint32_t box[2] = {(cuuint32_t)(BK / 2), (cuuint32_t)pl.BT};
+  // (W4A8: int8 activations [M rows][K bytes], box {128 B, BT rows})
+  const cuuint64_t row_bytes = a8 ? (cuuint64_t)w->K : (cuuint64_t)(w->K / 2);
+  const cuuint64_t gdim[2] = {row_bytes, (cuuint64_t)M};
+  const cuuint64_t gstride[1] = {row_bytes};
+  const cuuint32_t box[2] = {(cuuint32_t)(a8 ? BK : BK / 2), (cuuint32_t)pl.BT};
   const cuuint32_t estr[2] = {1, 1};
   if (!fused && enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(qA), gdim, gstride, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -1448,10 +1476,13 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
 
   cudaStream_t st = (cudaStream_t)cuda_stream;
   switch (pl.BT) {
-    case 16: rc = fused ? launch<16, true>(tmap, gp, pl.grid, st) : launch<16>(tmap, gp, pl.grid, st); break;
-    case 32: rc = launch<32>(tmap, gp, pl.grid, st); break;
-    case 64: rc = launch<64>(tmap, gp, pl.grid, st); break;
-    case 128: rc = launch<128>(tmap, gp, pl.grid, st); break;
+    case 16:
+      rc = fused ? launch<16, true>(tmap, gp, pl.grid, st)
+                 : (a8 ? launch<16, false, true>(tmap, gp, pl.grid, st) : launch<16>(tmap, gp, pl.grid, st));
+      break;
+    case 32: rc = a8 ? launch<32, false, true>(tmap, gp, pl.grid, st) : launch<32>(tmap, gp, pl.grid, st); break;
+    case 64: rc = a8 ? launch<64, false, true>(tmap, gp, pl.grid, st) : launch<64>(tmap, gp, pl.grid, st); break;
+    case 128: rc = a8 ? launch<128, false, true>(tmap, gp, pl.grid, st) : launch<128>(tmap, gp, pl.grid, st); break;
     default: rc = MQ_ERR_INVALID_ARG;
   }
   if (rc == MQ_OK) mq::set_launch_count(1);
@@ -1465,6 +1496,13 @@ extern "C" int mq_gemm(const mq_weights* w, const void* qA, const float* sA, int
                        void* cuda_stream) {
   return gemm_impl(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, nullptr, MQ_F16, 0,
                    nullptr);
+}
+
+extern "C" int mq_gemm_a8(const mq_weights* w, const int8_t* qA8, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
+                          int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
+                          void* cuda_stream) {
+  return gemm_impl(w, qA8, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, nullptr, MQ_F16, 0,
+                   nullptr, true);
 }
 
 extern "C" size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M) {

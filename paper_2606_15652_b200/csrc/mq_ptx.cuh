@@ -158,14 +158,18 @@ __device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.
 // differ when the product lies within that distance of a half-integer.  Only then (rare; exact ties
 // do occur on fp16 grids) is the division performed.  `inv_s` must be 0 when 1/s is not usable
 // (tiny scales), which forces the division.
-__device__ __forceinline__ int quant1(float x, float s, float inv_s) {
+template <int QMAX>
+__device__ __forceinline__ int quant1q(float x, float s, float inv_s) {
+  // |tp - exact quotient| <= 3 * 2^-24 * (QMAX + 0.5): 1.4e-6 for QMAX = 7, 2.3e-5 for QMAX = 127
+  constexpr float NEAR = QMAX <= 7 ? 4e-6f : 6e-5f;
   const float tp = x * inv_s;
   float r = rintf(tp);
   const float d = fabsf(fabsf(tp - r) - 0.5f);   // distance of tp from the nearest half-integer
-  if (inv_s == 0.f || !(d > 4e-6f)) r = rintf(__fdiv_rn(x, s));
+  if (inv_s == 0.f || !(d > NEAR)) r = rintf(__fdiv_rn(x, s));
   const int q = (int)r;
-  return max(-7, min(7, q));
+  return max(-QMAX, min(QMAX, q));
 }
+__device__ __forceinline__ int quant1(float x, float s, float inv_s) { return quant1q<7>(x, s, inv_s); }
 __device__ __forceinline__ float quant_inv_scale(float s) { return s > 1e-30f ? __frcp_rn(s) : 0.f; }
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {

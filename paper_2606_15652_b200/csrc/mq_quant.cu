@@ -71,6 +71,17 @@ __device__ __forceinline__ void cvt8(const uint4& v, float* f) {
   }
 }
 
+// 8-bit activations (W4A8): 8 elements -> 8 bytes, canonical order
+__device__ __forceinline__ uint2 quant_bytes8(const float* f, float s, float inv_s) {
+  uint32_t w[2] = {0, 0};
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int q = mq::ptx::quant1q<127>(f[i], s, inv_s);
+    w[i >> 2] |= (uint32_t)(q & 0xFF) << (8 * (i & 3));
+  }
+  return make_uint2(w[0], w[1]);
+}
+
 __device__ __forceinline__ uint32_t quant_pack8(const float* f, float s, float inv_s) {
   uint32_t out = 0;
 #pragma unroll
@@ -82,7 +93,8 @@ __device__ __forceinline__ uint32_t quant_pack8(const float* f, float s, float i
 }
 
 // CHUNKS = 16-byte chunks (8 elements) each thread keeps in registers per pass.
-template <bool BF16, int CHUNKS>
+// QMAX = 7: packed int4 output (4 bytes per 8 elements); QMAX = 127: int8 output (8 bytes per 8 elements)
+template <bool BF16, int CHUNKS, int QMAX = 7>
 __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __restrict__ A, int64_t lda, int K,
                                                              uint8_t* __restrict__ qA, float* __restrict__ sA) {
   // PDL: the next kernel (mq_gemm) may start its prologue and weight prefetch now; A may have been
@@ -92,6 +104,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
   const int64_t m = blockIdx.x;
   const uint4* row = reinterpret_cast<const uint4*>(A + m * lda);
   uint32_t* qrow = reinterpret_cast<uint32_t*>(qA + m * (int64_t)(K / 2));
+  uint2* qrow8 = reinterpret_cast<uint2*>(qA + m * (int64_t)K);
   const int nchunk = K / 8;
   __shared__ float red[QT / 32];
 
@@ -123,7 +136,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
 #pragma unroll
   for (int i = 1; i < QT / 32; ++i) amax = fmaxf(amax, red[i]);
 
-  const float s = amax == 0.f ? 1.0f : __fdiv_rn(amax, 7.0f);  // A2 / Eq.1
+  const float s = amax == 0.f ? 1.0f : __fdiv_rn(amax, (float)QMAX);  // A2 / Eq.1
   if (threadIdx.x == 0) sA[m] = s;
   const float inv_s = mq::ptx::quant_inv_scale(s);
 
@@ -133,14 +146,20 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
     if (idx < nchunk) {
       float f[8];
       cvt8<BF16>(cache[c], f);
-      qrow[idx] = quant_pack8(f, s, inv_s);
+      if (QMAX == 7)
+        qrow[idx] = quant_pack8(f, s, inv_s);
+      else
+        qrow8[idx] = quant_bytes8(f, s, inv_s);
     }
   }
   for (int idx = threadIdx.x + CHUNKS * QT; idx < nchunk; idx += QT) {
     uint4 v = __ldg(row + idx);
     float f[8];
     cvt8<BF16>(v, f);
-    qrow[idx] = quant_pack8(f, s, inv_s);
+    if (QMAX == 7)
+      qrow[idx] = quant_pack8(f, s, inv_s);
+    else
+      qrow8[idx] = quant_bytes8(f, s, inv_s);
   }
 }
 
@@ -199,8 +218,11 @@ extern "C" size_t mq_qact_bytes(int64_t M, int64_t K) {
   return (size_t)M * (size_t)K / 2;
 }
 
-extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda, void* qA, float* sA,
-                               void* cuda_stream) {
+namespace {
+
+template <int QMAX>
+int quantize_act_impl(const void* A, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda, void* qA, float* sA,
+                      void* cuda_stream) {
   if (M < 0 || K <= 0 || K % mq::BK != 0 || K > (int64_t)1 << 30) return MQ_ERR_UNSUPPORTED_SHAPE;
   if (a_dtype != MQ_F16 && a_dtype != MQ_BF16) return MQ_ERR_INVALID_ARG;
   mq::set_launch_count(0);
@@ -230,18 +252,18 @@ extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64
   // the whole row stays in registers for K <= 16384 (one pass over global memory, all loads in flight)
   if (a_dtype == MQ_BF16) {
     if (nchunk_per_thread <= 2)
-      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 2>, a, lda, Ki, q8, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 2, QMAX>, a, lda, Ki, q8, sA);
     else if (nchunk_per_thread <= 4)
-      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 4>, a, lda, Ki, q8, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 4, QMAX>, a, lda, Ki, q8, sA);
     else
-      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 8>, a, lda, Ki, q8, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 8, QMAX>, a, lda, Ki, q8, sA);
   } else {
     if (nchunk_per_thread <= 2)
-      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 2>, a, lda, Ki, q8, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 2, QMAX>, a, lda, Ki, q8, sA);
     else if (nchunk_per_thread <= 4)
-      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 4>, a, lda, Ki, q8, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 4, QMAX>, a, lda, Ki, q8, sA);
     else
-      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 8>, a, lda, Ki, q8, sA);
+      le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, 8, QMAX>, a, lda, Ki, q8, sA);
   }
   if (le != cudaSuccess) {
     cudaGetLastError();
@@ -250,6 +272,18 @@ extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64
   mq::set_launch_count(1);
   if (cudaGetLastError() != cudaSuccess) return MQ_ERR_CUDA;
   return MQ_OK;
+}
+
+}  // namespace
+
+extern "C" int mq_quantize_act(const void* A, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda, void* qA, float* sA,
+                               void* cuda_stream) {
+  return quantize_act_impl<7>(A, a_dtype, M, K, lda, qA, sA, cuda_stream);
+}
+
+extern "C" int mq_quantize_act8(const void* A, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda, int8_t* qA8, float* sA,
+                                void* cuda_stream) {
+  return quantize_act_impl<127>(A, a_dtype, M, K, lda, qA8, sA, cuda_stream);
 }
 
 extern "C" int mq_unpack_act(const void* qA, int64_t M, int64_t K, int8_t* q, void* cuda_stream) {

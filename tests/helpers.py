@@ -65,13 +65,13 @@ def make_case(seed: int, M: int, K: int, N: int, bs: int = 64, rho: Optional[flo
     return Case(M, K, N, bs, W, h, A16, a_dtype, L)
 
 
-def oracle_act(case: Case):
-    return oracle.quantize_act(case.A16 if case.a_dtype == "f16" else (case.A16, "bf16"))
+def oracle_act(case: Case, bits: int = 4):
+    return oracle.quantize_act(case.A16 if case.a_dtype == "f16" else (case.A16, "bf16"), bits=bits)
 
 
-def oracle_forward(case: Case, rows: Optional[np.ndarray] = None):
-    """O2 + O8 + O9 (optionally on a subset of token rows)."""
-    qa, sa = oracle_act(case)
+def oracle_forward(case: Case, rows: Optional[np.ndarray] = None, bits: int = 4):
+    """O2 + O8 + O9 (optionally on a subset of token rows); bits = activation width (4: W4A4, 8: W4A8)."""
+    qa, sa = oracle_act(case, bits)
     if rows is not None:
         qa, sa = qa[rows], sa[rows]
     acc0, acc1 = oracle.gemm(qa, case.L.d.qw, case.L.d.qr, case.L.bs, case.L.blk_n, case.L.blk_k)
@@ -94,15 +94,21 @@ def pack_from_oracle(case: Case):
     return mq.mq_pack_prequantized(L.d.qw, L.d.sw, L.bs, L.blk_n, L.blk_k, L.qr_blocks(), L.d.sr)
 
 
-def run_cuda(case: Case, w=None, out_dtype="bf16", workspace=None):
+def run_cuda(case: Case, w=None, out_dtype="bf16", workspace=None, bits: int = 4):
     import torch
     import paper_2606_15652_b200 as mq
     if w is None:
         w = pack_from_oracle(case)
     A = to_device_act(case)
+    odt = torch.bfloat16 if out_dtype == "bf16" else torch.float16
+    if bits == 8:
+        q, sA = mq.mq_quantize_act8(A)
+        Y, d0, d1 = mq.mq_gemm_a8(w, q, sA, case.M, out_dtype=odt, dbg=True, workspace=workspace)
+        torch.cuda.synchronize()
+        return dict(qa=q.cpu().numpy(), sa=sA.cpu().numpy(), acc0=d0.cpu().numpy(), acc1=d1.cpu().numpy(),
+                    Y=Y.float().cpu().numpy().astype(np.float64), w=w, out_dtype=out_dtype)
     qA, sA = mq.mq_quantize_act(A)
-    Y, d0, d1 = mq.mq_gemm(w, qA, sA, case.M, out_dtype=torch.bfloat16 if out_dtype == "bf16" else torch.float16,
-                           dbg=True, workspace=workspace)
+    Y, d0, d1 = mq.mq_gemm(w, qA, sA, case.M, out_dtype=odt, dbg=True, workspace=workspace)
     torch.cuda.synchronize()
     q = mq.mq_unpack_act(qA, case.M, case.K)
     return dict(qa=q.cpu().numpy(), sa=sA.cpu().numpy(), acc0=d0.cpu().numpy(), acc1=d1.cpu().numpy(),

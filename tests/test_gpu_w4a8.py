@@ -1,0 +1,83 @@
+"""W4A8 variant (Table 1 W4A8 rows): per-token int8 activations against the
+same packed int4 base + residual weights.  Same parity bar as W4A4: quantized activations and scales
+bit-exact against the oracle (q_max = 127), acc0 / acc1 bit-exact, Y within tolerance."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+from helpers import assert_parity, make_case, oracle_forward, pack_from_oracle, run_cuda
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mq():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a GPU")
+    import paper_2606_15652_b200 as m
+    m.lib()
+    for k in ("split_k", "token_tile", "max_ctas"):
+        m.mq_set_option(k, 0)
+    return m
+
+
+SHAPES = [
+    (1, 512, 256, 64, 0.10, "f16"), (8, 1024, 384, 64, 0.05, "bf16"), (17, 640, 256, 64, 0.20, "f16"),
+    (33, 1024, 512, 128, 0.25, "f16"), (64, 2048, 256, 64, 0.3, "f16"), (100, 512, 384, 64, 0.10, "bf16"),
+    (130, 512, 256, 128, 0.50, "f16"), (300, 1024, 640, 64, 0.05, "bf16"),
+]
+
+
+@pytest.mark.parametrize("out_dtype", ["bf16", "f16"])
+@pytest.mark.parametrize("M,K,N,bs,rho,dt", SHAPES)
+def test_w4a8_parity_small(mq, M, K, N, bs, rho, dt, out_dtype):
+    case = make_case(700 + M, M, K, N, bs=bs, rho=rho, a_dtype=dt)
+    want = oracle_forward(case, bits=8)
+    assert np.abs(want["qa"].astype(np.int32)).max() == 127
+    got = run_cuda(case, out_dtype=out_dtype, bits=8)
+    assert_parity(got, want, what=f"W4A8 M{M} K{K} N{N} bs{bs} {out_dtype}")
+
+
+@pytest.mark.parametrize("mode,ctas,bt", [(2, 0, 0), (2, 7, 0), (2, 33, 32), (1, 0, 64), (2, 5, 128), (1, 0, 16)])
+def test_w4a8_stream_k_and_token_tiles(mq, mode, ctas, bt):
+    M = 40 if bt in (0, 64) else (12 if bt == 16 else (30 if bt == 32 else 150))
+    case = make_case(800 + bt + ctas, M, 2048, 384, bs=64, rho=0.2)
+    want = oracle_forward(case, bits=8)
+    try:
+        mq.mq_set_option("split_k", mode)
+        mq.mq_set_option("max_ctas", ctas)
+        mq.mq_set_option("token_tile", bt)
+        w = pack_from_oracle(case)
+        ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+        for rep in range(2):
+            got = run_cuda(case, w=w, workspace=ws, bits=8)
+            assert_parity(got, want, what=f"W4A8 split_k {mode} ctas {ctas} bt {bt} rep {rep}")
+    finally:
+        for k in ("split_k", "max_ctas", "token_tile"):
+            mq.mq_set_option(k, 0)
+
+
+def test_w4a8_extreme_values_and_full_size(mq):
+    """all +-127 x +-7: |acc0| = 889 K exactly (int32 head-room of the x16 weight expansion); then a
+    LLaMA3-8B-sized decode and prefill projection on sampled rows."""
+    import torch
+    M, K, N = 8, 4096, 128
+    qw = np.full((N, K), 7, np.int8)
+    qw[1::2] = -7
+    s1 = np.ones(N, np.float32)
+    w = mq.mq_pack_prequantized(qw, s1, 64, np.zeros(0, np.int32), np.zeros(0, np.int32), np.zeros((0, 64, 64), np.int8), s1)
+    A = torch.full((M, K), 3.0, dtype=torch.float16, device="cuda")
+    q8, sA = mq.mq_quantize_act8(A)
+    assert int(q8.min()) == 127
+    Y, d0, d1 = mq.mq_gemm_a8(w, q8, sA, M, dbg=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(np.abs(d0.cpu().numpy()), np.full((M, N), 889 * K)) and not d1.cpu().numpy().any()
+    for (Mf, Kf, Nf) in [(8, 4096, 6144), (512, 4096, 4096)]:
+        case = make_case(880 + Mf, Mf, Kf, Nf, bs=64, rho=0.05, calib_tokens=64)
+        rows = np.arange(Mf) if Mf <= 64 else np.sort(np.random.default_rng(1).choice(Mf, size=64, replace=False))
+        want = oracle_forward(case, rows=rows, bits=8)
+        got = run_cuda(case, bits=8)
+        assert_parity(got, want, rows=rows, what=f"W4A8 full size M{Mf}")
