@@ -50,6 +50,7 @@
 #include <cstring>
 
 #include "mq_internal.h"
+#include <type_traits>
 #include "mq_ptx.cuh"
 
 namespace {
@@ -120,7 +121,8 @@ struct Cfg {
   static constexpr int OFF_BAR = OFF_RP + NQ * QUARTER_BYTES;
   static constexpr int NUM_BARS = 2 * PSTAGES + 2 * USTAGES + 2 * NQ + 2 * RSTAGES + 2 + ACC0_STAGES + ACC1_STAGES + 1;
   static constexpr int OFF_META = OFF_BAR + NUM_BARS * 8;
-  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 12 + 16;   // + token scales (FUSED)
+  static constexpr int SA_TILE = BT >= 64 ? 2 * BT + 4 : 0;   // token scales of the tile being drained (two tiles deep)
+  static constexpr int META_WORDS = PSTAGES * SK + USTAGES * UK + 12 + 16 + SA_TILE;   // + token scales (FUSED)
   static constexpr int OFF_END = OFF_META + META_WORDS * 4;
   static constexpr int SMEM_BYTES = OFF_END + 1024;  // slack for the 1024-byte alignment
   static_assert(SMEM_BYTES <= 232448, "shared memory budget");
@@ -171,10 +173,18 @@ struct GemmParams {
 };
 
 #ifdef MQ_TRACE
-#define MQ_STAMP(slot) do { p.trace[(size_t)blockIdx.x * 64 + (slot)] = clock64(); } while (0)
+#define MQ_STAMP(slot) do { p.trace[(size_t)blockIdx.x * 128 + (slot)] = clock64(); } while (0)
+#define MQ_ACC_DECL(v) long long v = 0
+#define MQ_ACC_BEGIN(v) v -= clock64()
+#define MQ_ACC_END(v) v += clock64()
+#define MQ_ACC_OUT(cond, slot, v) do { if (cond) p.trace[(size_t)blockIdx.x * 128 + (slot)] = (v); } while (0)
 #define MQ_STAMP_IF(cond, slot) do { if (cond) MQ_STAMP(slot); } while (0)
 #else
 #define MQ_STAMP(slot) do { } while (0)
+#define MQ_ACC_DECL(v) do { } while (0)
+#define MQ_ACC_BEGIN(v) do { } while (0)
+#define MQ_ACC_END(v) do { } while (0)
+#define MQ_ACC_OUT(cond, slot, v) do { } while (0)
 #define MQ_STAMP_IF(cond, slot) do { } while (0)
 #endif
 
@@ -334,13 +344,14 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   volatile int32_t* pend = misc + 1;      // [2][4] partial tiles awaiting the fix-up: tile, c_lo, c_hi, lo_slot
   volatile int32_t* acc_flag = misc + 9;
   volatile float* sa_s = reinterpret_cast<volatile float*>(misc + 12);   // [16] FUSED: token scales
+  float* sa_tile = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(const_cast<int32_t*>(misc) + 28) + 15) & ~(uintptr_t)15);   // [2][BT], BT >= 64, 16-byte aligned
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #ifdef MQ_TRACE
   if (threadIdx.x == 0) {
     unsigned long long gt;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-    p.trace[(size_t)blockIdx.x * 64 + 12] = (long long)gt;
+    p.trace[(size_t)blockIdx.x * 128 + 12] = (long long)gt;
     MQ_STAMP(0);
   }
 #endif
@@ -421,6 +432,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       }
     }
     griddep_wait();
+    MQ_ACC_DECL(tp_e);
     bool have = it.next<SK>(cur);
     int ps = 0, si = 0;
     int qseq_g[C::G], rseq_g[C::G];   // residual quarters / cells handed to each unpack group so far
@@ -435,7 +447,10 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     uint32_t pphase = 0;
     while (have) {
       const bool have_n = it.next<SK>(nxt);
+      MQ_ACC_BEGIN(tp_e);
       mbar_wait(bar(B_EMPTY_P + ps), pphase ^ 1);
+      MQ_ACC_END(tp_e);
+      MQ_ACC_OUT(lane == 0, 72, tp_e);
       __syncwarp();
       const uint32_t dst = sP + ps * C::P_STAGE;
       if (elect_one()) {
@@ -537,13 +552,17 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
     constexpr uint32_t IDESC = make_idesc_i8(BN, BT);
     int seg = 0;                 // index of the current segment (selects the accumulator stages)
+    MQ_ACC_DECL(tw_u); MQ_ACC_DECL(tw_a0); MQ_ACC_DECL(tw_tot); MQ_ACC_DECL(tw_meta); MQ_ACC_DECL(tw_mma); MQ_ACC_DECL(tw_commit);
+    MQ_ACC_BEGIN(tw_tot);
     uint32_t acc0_on = 0, acc1_on = 0;
     uint32_t d0 = 0, d1 = 0;
     int a0s = 0, a1s = 0;
     auto seg_first = [&]() {   // first K-step of a segment: claim the accumulator stages
       a0s = seg % C::ACC0_STAGES;
       a1s = seg % C::ACC1_STAGES;
+      MQ_ACC_BEGIN(tw_a0);
       mbar_wait(bar(B_A0E + a0s), (((uint32_t)seg / C::ACC0_STAGES) & 1) ^ 1);
+      MQ_ACC_END(tw_a0);
       tc_fence_after();
       d0 = tmem_base + (uint32_t)(a0s * BT);
       d1 = tmem_base + (uint32_t)(C::ACC1_COL0 + a1s * BT);
@@ -565,7 +584,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       ++seg;
     };
     auto mma_item = [&](const int us, const int item, const uint32_t uphase) {
+      MQ_ACC_BEGIN(tw_u);
       mbar_wait(bar(B_FULL_U + us), uphase);
+      MQ_ACC_END(tw_u);
       tc_fence_after();
       MQ_STAMP_IF(item == 0 && lane == 0, 7);
       MQ_STAMP_IF(item < 16 && lane == 0, 32 + item);
@@ -642,15 +663,19 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       }
 #pragma unroll
       for (int j = 0; j < UK; ++j) {
+        MQ_ACC_BEGIN(tw_meta);
         const int m = lds32(sMetaU + 4u * (uint32_t)(us * UK + j));
         if (!(m & META_VALID)) break;   // the valid K-steps of an item are a prefix
+        MQ_ACC_END(tw_meta);
         if (m & META_FIRST) seg_first();
         const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + (us * UK + j) * A_COLS);
         const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE + j * C::U_SUB);
+        MQ_ACC_BEGIN(tw_mma);
         if (elect_one()) {
 #pragma unroll
           for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? acc0_on : 1u);
         }
+        MQ_ACC_END(tw_mma);
         acc0_on = 1;
         const int mask = m & 0xF;
         if (mask) {
@@ -684,8 +709,10 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
         if (m & META_LAST) seg_last();
       }
+      MQ_ACC_BEGIN(tw_commit);
       __syncwarp();
       if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
+      MQ_ACC_END(tw_commit);
     };
     if constexpr (UK == 1) {
       // Prefill: the U stages are visited in a fixed rotation and the loop is unrolled over them, so
@@ -702,6 +729,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       for (int item = 0; item < n_items; ++item)
         mma_item(item % C::USTAGES, item, ((uint32_t)item / C::USTAGES) & 1);
     }
+    MQ_ACC_END(tw_tot);
+    MQ_ACC_OUT(lane == 0, 64, tw_u); MQ_ACC_OUT(lane == 0, 65, tw_a0); MQ_ACC_OUT(lane == 0, 66, tw_tot); MQ_ACC_OUT(lane == 0, 76, tw_meta); MQ_ACC_OUT(lane == 0, 77, tw_mma); MQ_ACC_OUT(lane == 0, 78, tw_commit);
   } else if (warp >= FIRST_UNPACK_WARP) {
     // ============ unpack groups: int4 -> int8 (x16); weights -> TMEM, tokens -> smem ============
     const int gi = (warp - FIRST_UNPACK_WARP) >> 2;               // group: takes items i = gi (mod 2)
@@ -711,10 +740,14 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     const uint32_t lane_addr = tmem_base + ((uint32_t)(wq * 32) << 16);
     const int rhalf = wq >> 1;                                    // row half of a residual cell
     bool sa_ready = false;                                        // FUSED: token scales observed
+    MQ_ACC_DECL(tu_p); MQ_ACC_DECL(tu_eu); MQ_ACC_DECL(tu_tot); MQ_ACC_DECL(tu_work);
+    MQ_ACC_BEGIN(tu_tot);
     for (int item = gi; item < n_items; item += C::G) {
       const int stage = item / IPS, sub = item - stage * IPS;
       const int ps = stage % C::PSTAGES, us = item % C::USTAGES;
+      MQ_ACC_BEGIN(tu_p);
       mbar_wait(bar(B_FULL_P + ps), ((uint32_t)stage / C::PSTAGES) & 1);
+      MQ_ACC_END(tu_p);
       MQ_STAMP_IF(item == 0 && gtid == 0, 4);
       int mw[UK];
 #pragma unroll
@@ -744,7 +777,10 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(B_EMPTY_P + ps));   // this warp's reads of the P stage are done
+        MQ_ACC_BEGIN(tu_eu);
         mbar_wait(bar(B_EMPTY_U + us), (((uint32_t)item / C::USTAGES) & 1) ^ 1);
+        MQ_ACC_END(tu_eu);
+        MQ_ACC_BEGIN(tu_work);
         tc_fence_after();
         if (valid) {
           {
@@ -815,6 +851,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           if (wq == 0) sts32(sMetaU + 4u * (uint32_t)us, m);
           mbar_arrive(bar(B_FULL_U + us));
         }
+        MQ_ACC_END(tu_work);
         continue;
       }
       // the first K-step's packed weights are fetched before the U stage is known to be free
@@ -945,6 +982,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         }
       }
     }
+    MQ_ACC_END(tu_tot);
+    MQ_ACC_OUT(gtid == 0 && gi == 0, 68, tu_p); MQ_ACC_OUT(gtid == 0 && gi == 0, 69, tu_eu);
+    MQ_ACC_OUT(gtid == 0 && gi == 0, 70, tu_work); MQ_ACC_OUT(gtid == 0 && gi == 0, 71, tu_tot);
   } else {
     // ===================== epilogue warps (2..5) =====================
     griddep_wait();   // s_a, Y, the workspace: ordered after the previous kernel in the stream
@@ -1012,6 +1052,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       named_bar_sync(1, 128);
       if (et == 0) mbar_arrive(bar(B_SA));   // release: the unpack groups may read the token scales
     }
+    MQ_ACC_DECL(te_t); MQ_ACC_DECL(te_d);
     int seg = 0, npend = 0;      // npend: partial tiles published by this CTA (at most 2)
     constexpr bool kBothParts = BT <= 32;
     uint32_t g = u_beg;
@@ -1039,7 +1080,20 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (p.dbg1) p.dbg1[(size_t)(t_base + t) * p.N + n] = a1 >> C::ACC_SHIFT;
       };
 
+      // prefill fast drain (whole tile, all BT tokens, no parity hooks): the tile's token scales go to
+      // shared memory BEFORE the accumulator wait (one scale per epilogue thread), so that no global load
+      // sits between the accumulator's completion and its release
+      const bool whole_k = (k0 == 0 && k1 == p.KS);
+      const bool fast = BT >= 64 && !FUSED && whole_k && t_cnt == BT && !p.dbg0 && !p.dbg1;
+      float* sat = sa_tile + (seg & 1) * BT;
+      if (BT >= 64) {
+        if (fast && et < BT) sat[et] = __ldg(p.sa + t_base + et);
+        named_bar_sync(1, 128);   // every segment: also orders this buffer's readers (two segments ago) before its writers
+      }
+      MQ_ACC_BEGIN(te_t);
       mbar_wait(bar(B_TFULL + a0s), aphase);
+      MQ_ACC_END(te_t);
+      MQ_ACC_BEGIN(te_d);
       tc_fence_after();
       MQ_STAMP_IF(et == 0 && seg == 1, 9);
       const bool has_res = acc_flag[a0s] != 0;  // acc1 is undefined when no residual MMA was issued
@@ -1053,6 +1107,44 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       int32_t* part0 = p.ws_part + ((size_t)blockIdx.x * 2 + slot) * (2 * PART);
       int32_t* part1 = part0 + PART;
 
+      if (BT >= 64 && fast) {
+        // 8-token batches, two in flight: the TMEM loads of batch b+1 run under the arithmetic and the
+        // stores of batch b
+        uint16_t* yp = reinterpret_cast<uint16_t*>(p.Y) + (size_t)t_base * p.ldy + n;
+        auto drain = [&](auto res_c, auto bf_c) {
+          constexpr bool RES = decltype(res_c)::value, BF = decltype(bf_c)::value;
+          uint32_t a[2][8], r[2][8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) r[0][i] = r[1][i] = 0;
+          tmem_ld8(t0addr, a[0]);
+          if (RES) tmem_ld8(t1addr, r[0]);
+#pragma unroll
+          for (int b = 0; b < BT / 8; ++b) {
+            const int cur = b & 1;
+            tmem_ld_wait8(a[cur], r[cur]);
+            if (b + 1 < BT / 8) {
+              tmem_ld8(t0addr + (b + 1) * 8, a[cur ^ 1]);
+              if (RES) tmem_ld8(t1addr + (b + 1) * 8, r[cur ^ 1]);
+            }
+            const float4 s_lo = *reinterpret_cast<const float4*>(sat + b * 8);
+            const float4 s_hi = *reinterpret_cast<const float4*>(sat + b * 8 + 4);
+            const float sv[8] = {s_lo.x, s_lo.y, s_lo.z, s_lo.w, s_hi.x, s_hi.y, s_hi.z, s_hi.w};
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              float y = (float)(int32_t)a[cur][i] * swn;
+              if (RES) y += (float)(int32_t)r[cur][i] * srn;   // same operation order as the general path
+              y *= sv[i];
+              *yp = BF ? __bfloat16_as_ushort(__float2bfloat16_rn(y)) : __half_as_ushort(__float2half_rn(y));
+              yp += p.ldy;
+            }
+          }
+        };
+        if (has_res) {
+          if (p.y_bf16) drain(std::true_type{}, std::true_type{}); else drain(std::true_type{}, std::false_type{});
+        } else {
+          if (p.y_bf16) drain(std::false_type{}, std::true_type{}); else drain(std::false_type{}, std::false_type{});
+        }
+      } else
       for (int c0 = 0; c0 < t_cnt; c0 += 16) {
         uint32_t v0[16], v1[16];
         float sav[16];   // token scales of the chunk, fetched up front (read-only path: one L2 round trip
@@ -1107,6 +1199,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         mbar_arrive(bar(B_A1E + a1s));
         mbar_arrive(bar(B_A0E + a0s));
       }
+      MQ_ACC_END(te_d);
+      MQ_ACC_OUT(et == 0, 74, te_t); MQ_ACC_OUT(et == 0, 75, te_d);
 
       if (!whole) {
         // stream-K fix-up, part 1: publish this partial (release) and count the arrival.  Nothing

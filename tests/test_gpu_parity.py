@@ -459,6 +459,33 @@ def test_gemm_no_hooks_path_matches_hooked_path(mq):
         assert torch.equal(Y.view(torch.int16), Yh.view(torch.int16)), (M, K, N)
 
 
+@pytest.mark.parametrize("bt", [64, 128])
+@pytest.mark.parametrize("rho", [0.0, 0.2])
+@pytest.mark.parametrize("odt", ["bf16", "f16"])
+def test_gemm_prefill_fast_drain_matches_hooked_path(mq, bt, rho, odt):
+    """Whole token tiles without parity hooks take the prefill epilogue's pipelined drain (token scales staged
+    in shared memory, 8-token TMEM batches); its Y must be bit-identical to the hooked path's, with and without
+    a residual accumulator, for both output types, including a ragged last token tile."""
+    import torch
+    dt = torch.bfloat16 if odt == "bf16" else torch.float16
+    try:
+        mq.mq_set_option("token_tile", bt)
+        for M in (bt, 3 * bt, 3 * bt + 5):
+            case = _random_block_case(900 + M + bt, M, 1024, 384, 64, rho)
+            w = pack_from_oracle(case)
+            A = to_device_act(case)
+            qA, sA = mq.mq_quantize_act(A)
+            ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+            Yh, _, _ = mq.mq_gemm(w, qA, sA, M, out_dtype=dt, dbg=True, workspace=ws)
+            Y = torch.full_like(Yh, 7.0)
+            for _ in range(3):
+                mq.mq_gemm(w, qA, sA, M, Y=Y, workspace=ws)
+            torch.cuda.synchronize()
+            assert torch.equal(Y.view(torch.int16), Yh.view(torch.int16)), (M, bt, rho, odt)
+    finally:
+        mq.mq_set_option("token_tile", 0)
+
+
 def test_gemm_seeded_fuzz_against_oracle(mq):
     """40 seeded random combinations of shape, block size, density (uniform-random block pattern) and
     launch options (token tile, split-K mode, CTA cap, PDL on/off): accumulators bit-exact and Y in
