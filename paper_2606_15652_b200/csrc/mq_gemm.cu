@@ -552,7 +552,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
     constexpr uint32_t IDESC = make_idesc_i8(BN, BT);
     int seg = 0;                 // index of the current segment (selects the accumulator stages)
-    MQ_ACC_DECL(tw_u); MQ_ACC_DECL(tw_a0); MQ_ACC_DECL(tw_tot); MQ_ACC_DECL(tw_meta); MQ_ACC_DECL(tw_mma); MQ_ACC_DECL(tw_commit);
+    MQ_ACC_DECL(tw_u); MQ_ACC_DECL(tw_a0); MQ_ACC_DECL(tw_tot);
     MQ_ACC_BEGIN(tw_tot);
     uint32_t acc0_on = 0, acc1_on = 0;
     uint32_t d0 = 0, d1 = 0;
@@ -661,58 +661,47 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
         return;
       }
-#pragma unroll
-      for (int j = 0; j < UK; ++j) {
-        MQ_ACC_BEGIN(tw_meta);
-        const int m = lds32(sMetaU + 4u * (uint32_t)(us * UK + j));
-        if (!(m & META_VALID)) break;   // the valid K-steps of an item are a prefix
-        MQ_ACC_END(tw_meta);
-        if (m & META_FIRST) seg_first();
-        const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + (us * UK + j) * A_COLS);
-        const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE + j * C::U_SUB);
-        MQ_ACC_BEGIN(tw_mma);
+      if constexpr (UK == 1) {
+        // Prefill: ONE elected block per K-step issues the base MMAs, the cell's MMAs and the commit that
+        // hands the U stage back (this warp's dependent instructions per K-step pace the pipeline).
+        const int m = lds32(sMetaU + 4u * (uint32_t)us);
+        const int mask = (m & META_VALID) ? (m & 0xF) : 0;
+        if ((m & META_VALID) && (m & META_FIRST)) seg_first();
+        if (mask && !acc1_on) {
+          // first residual MMA of the segment: the epilogue must have drained this acc1 stage
+          mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
+          tc_fence_after();
+        }
+        const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + us * A_COLS);
+        const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + us * A_COLS);   // the cell rides in its U stage
+        const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE);
+        __syncwarp();
         if (elect_one()) {
+          if (m & META_VALID) {
 #pragma unroll
-          for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? acc0_on : 1u);
-        }
-        MQ_ACC_END(tw_mma);
-        acc0_on = 1;
-        const int mask = m & 0xF;
-        if (mask) {
-          if (!acc1_on) {
-            // first residual MMA of the segment: the epilogue must have drained this acc1 stage
-            mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
-            tc_fence_after();
-          }
-          const int rseq = (m >> 4) & 0xFF;
-          const int rs = UK == 1 ? us : (item & (C::G - 1)) * C::RG + rseq % C::RG;
-          if constexpr (UK != 1) {   // UK == 1: the cell was published together with its U stage
-            mbar_wait(bar(B_FULL_RU + rs), ((uint32_t)rseq / C::RG) & 1);
-            tc_fence_after();
-          }
-          __syncwarp();
-          const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + rs * A_COLS);
-          if (elect_one()) {
-            uint32_t on = acc1_on;
+            for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? acc0_on : 1u);
+            if (mask) {
+              uint32_t on = acc1_on;
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
-              if (mask & (3 << (2 * h))) {
+              for (int h = 0; h < 2; ++h)
+                if (mask & (3 << (2 * h))) {
 #pragma unroll
-                for (int k = 2 * h; k < 2 * h + 2; ++k) {
-                  mma_i8_ts(d1, rt + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
-                  on = 1;
+                  for (int k = 2 * h; k < 2 * h + 2; ++k) {
+                    mma_i8_ts(d1, rt + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
+                    on = 1;
+                  }
                 }
-              }
-            if constexpr (UK != 1) tc_commit(bar(B_EMPTY_RU + rs));
+            }
           }
-          acc1_on = 1;
+          tc_commit(bar(B_EMPTY_U + us));
         }
-        if (m & META_LAST) seg_last();
+        if (m & META_VALID) {
+          acc0_on = 1;
+          if (mask) acc1_on = 1;
+          if (m & META_LAST) seg_last();
+        }
+        return;
       }
-      MQ_ACC_BEGIN(tw_commit);
-      __syncwarp();
-      if (elect_one()) tc_commit(bar(B_EMPTY_U + us));
-      MQ_ACC_END(tw_commit);
     };
     if constexpr (UK == 1) {
       // Prefill: the U stages are visited in a fixed rotation and the loop is unrolled over them, so
@@ -730,7 +719,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         mma_item(item % C::USTAGES, item, ((uint32_t)item / C::USTAGES) & 1);
     }
     MQ_ACC_END(tw_tot);
-    MQ_ACC_OUT(lane == 0, 64, tw_u); MQ_ACC_OUT(lane == 0, 65, tw_a0); MQ_ACC_OUT(lane == 0, 66, tw_tot); MQ_ACC_OUT(lane == 0, 76, tw_meta); MQ_ACC_OUT(lane == 0, 77, tw_mma); MQ_ACC_OUT(lane == 0, 78, tw_commit);
+    MQ_ACC_OUT(lane == 0, 64, tw_u); MQ_ACC_OUT(lane == 0, 65, tw_a0); MQ_ACC_OUT(lane == 0, 66, tw_tot);
   } else if (warp >= FIRST_UNPACK_WARP) {
     // ============ unpack groups: int4 -> int8 (x16); weights -> TMEM, tokens -> smem ============
     const int gi = (warp - FIRST_UNPACK_WARP) >> 2;               // group: takes items i = gi (mod 2)
