@@ -216,7 +216,24 @@ def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_
                 a1.record(stream)
                 stream.synchronize()
                 best0 = min(best0, a0.elapsed_time(a1) / reps)
-            per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3, us_dense=best0 * 1e3,
+            # the W4A8 variant of the same launch: int8 per-token activations, same packed weights
+            q8, s8 = mq.mq_quantize_act8(L.A[m])
+            g8 = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g8, stream=stream):
+                for r in range(reps):
+                    mq.mq_gemm_a8(L.copies[r % N_COPIES], q8, s8, m, Y=L.Y[m], workspace=L.ws[m])
+            for _ in range(3):
+                g8.replay()
+            best8 = 1e30
+            for _ in range(5):
+                graphs[0].replay()
+                a0.record(stream)
+                g8.replay()
+                a1.record(stream)
+                stream.synchronize()
+                best8 = min(best8, a0.elapsed_time(a1) / reps)
+            del g8, q8, s8
+            per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3, us_dense=best0 * 1e3, us_a8=best8 * 1e3,
                                   bytes=algo_bytes(m, L.K, L.N, L.nnz, BS), ops=algo_ops(m, L.K, L.N, L.nnz, BS)))
 
         # ---- W16A16 comparator: cuBLAS bf16 on the same shapes, same rotation
@@ -304,11 +321,14 @@ def roofline_of(r, peaks, traffic):
     int8_peak = 2.0 * peaks["bf16_tflops"]          # kind::i8 runs at twice the bf16 rate (nominal 4.5 vs 2.25 PF)
     t_hbm, t_tensor = by / (peaks["hbm_gbs"] * 1e9), ops / (int8_peak * 1e12)
     per_shape = [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3), us_dense_only=round(s["us_dense"], 3),
+                      us_w4a8=round(s["us_a8"], 3),
                       gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
                       tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in r["per_shape"]]
     kern = f"mq_gemm_kernel ({len(r['per_shape'])} launches of the step, timed alone, cold weights)"
     us0 = sum(s["us_dense"] for s in r["per_shape"])
-    extra = {"residual_overhead": us / us0 - 1.0,
+    us8 = sum(s["us_a8"] for s in r["per_shape"])
+    extra = {"w4a8_time_over_w4a4": us8 / us,
+             "residual_overhead": us / us0 - 1.0,
              "residual_overhead_note": f"time of the {len(r['per_shape'])} launches at rho={RHO} over the same launches on the "
                                        "budget-0 packing of the same weights (floor = rho: the residual adds rho x bytes and ops)"}
     if t_hbm >= t_tensor:
