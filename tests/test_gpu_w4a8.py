@@ -81,3 +81,44 @@ def test_w4a8_extreme_values_and_full_size(mq):
         want = oracle_forward(case, rows=rows, bits=8)
         got = run_cuda(case, bits=8)
         assert_parity(got, want, rows=rows, what=f"W4A8 full size M{Mf}")
+
+
+def test_w4a8_seeded_fuzz_against_oracle(mq):
+    """30 seeded random combinations of shape, block size, density (uniform-random block pattern: cells with
+    every quarter mask) and launch options: int8 codes, scales and accumulators bit-exact, Y in tolerance; the
+    epilogue's hot path (no parity hooks) must reproduce the hooked path's Y bits."""
+    import dataclasses
+    import torch
+    from helpers import to_device_act
+    rng = np.random.default_rng(4242)
+    try:
+        for ci in range(30):
+            bs = int(rng.choice([64, 128]))
+            K = int(rng.choice([128, 256, 640, 1024, 2048]))
+            N = int(rng.choice([128, 256, 384, 512]))
+            M = int(rng.choice([1, 3, 16, 17, 32, 33, 64, 65, 100, 128, 129, 256, 300]))
+            rho = float(rng.choice([0.0, 0.05, 0.1, 0.3, 0.6, 1.0]))
+            opts = dict(split_k=int(rng.choice([0, 0, 1, 2])), max_ctas=int(rng.choice([0, 0, 7, 33])),
+                        pdl=int(rng.choice([1, 1, 0])), token_tile=int(rng.choice([0, 0, 16, 32, 64, 128])))
+            for k, v in opts.items():
+                mq.mq_set_option(k, v)
+            case = make_case(5000 + ci, M, K, N, bs=bs, budget=0)
+            nb = (N // bs) * (K // bs)
+            sel = np.sort(np.random.default_rng(5000 + ci).choice(nb, size=int(rho * nb + 0.5), replace=False))
+            case = dataclasses.replace(case, L=dataclasses.replace(
+                case.L, blk_n=(sel // (K // bs)).astype(np.int32), blk_k=(sel % (K // bs)).astype(np.int32)))
+            want = oracle_forward(case, bits=8)
+            w = pack_from_oracle(case)
+            ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+            got = run_cuda(case, w=w, workspace=ws, bits=8)
+            assert_parity(got, want, what=f"W4A8 fuzz {ci}: M{M} K{K} N{N} bs{bs} rho{rho} {opts}")
+            q8, s8 = mq.mq_quantize_act8(to_device_act(case))
+            Y = torch.empty((M, N), dtype=torch.bfloat16, device="cuda")
+            for _ in range(2):
+                mq.mq_gemm_a8(w, q8, s8, M, Y=Y, workspace=ws)
+            torch.cuda.synchronize()
+            assert np.array_equal(Y.float().cpu().numpy().astype(np.float64), got["Y"]), f"W4A8 fuzz {ci}: hot path differs"
+    finally:
+        for k in ("split_k", "max_ctas", "token_tile"):
+            mq.mq_set_option(k, 0)
+        mq.mq_set_option("pdl", 1)
