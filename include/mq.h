@@ -95,6 +95,16 @@ int mq_unpack_act(const void* qA_dev, int64_t M, int64_t K, int8_t* q_dev, void*
  */
 int mq_pack_weights(const float* W_host, int64_t N, int64_t K, const float* h_host, int block,
                     int64_t budget_blocks, mq_weights** out, void* cuda_stream);
+
+/* Algorithm 1 with DEVICE inputs: W_dev [N,K] fp32 row-major and h_dev [K] (or NULL) are device
+ * pointers (rows 8-byte aligned).  Base quantization, residual, Q(R) and the Delta-Hessian block scores (P:119-125,
+ * P:156) run on the GPU, one CTA per block-row, with mq_pack_weights' arithmetic operation for operation (binary32
+ * division + round-half-even for Eq.1; the score sums in fp64, uncontracted, rows then k ascending), so the selected
+ * set, the integers and the scales are bit-identical to mq_pack_weights'.  The top-K over the N*K/block^2 scores and
+ * the layout run on the host.  Same requirements and errors as mq_pack_weights, plus K <= 51200 (one residual row in
+ * shared memory).  Synchronises `cuda_stream`. */
+int mq_pack_weights_device(const float* W_dev, int64_t N, int64_t K, const float* h_dev, int block,
+                           int64_t budget_blocks, mq_weights** out, void* cuda_stream);
 int mq_pack_prequantized(const int8_t* qW_host, const float* sW_host, int64_t N, int64_t K, int block,
                          int64_t nnz, const int32_t* blk_n_host, const int32_t* blk_k_host,
                          const int8_t* qR_host, const float* sR_host, mq_weights** out,

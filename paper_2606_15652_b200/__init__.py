@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     mq_linear_workspace_bytes,
     mq_pack_prequantized,
     mq_pack_weights,
+    mq_pack_weights_device,
     mq_qact_bytes,
     mq_quantize_act,
     mq_quantize_act8,

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libmq.so")
 MQ_F16, MQ_BF16 = 0, 1
 
 EXPORTS = [
-    "mq_status_string", "mq_qact_bytes", "mq_quantize_act", "mq_unpack_act", "mq_pack_weights",
+    "mq_status_string", "mq_qact_bytes", "mq_quantize_act", "mq_unpack_act", "mq_pack_weights", "mq_pack_weights_device",
     "mq_pack_prequantized", "mq_weights_export", "mq_weights_clone", "mq_weights_info", "mq_weights_free",
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
     "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_set_option",
@@ -56,6 +56,8 @@ def lib() -> C.CDLL:
     L.mq_unpack_act.argtypes = [vp, i64, i64, vp, vp]
     L.mq_pack_weights.restype = i32
     L.mq_pack_weights.argtypes = [vp, i64, i64, vp, i32, i64, C.POINTER(vp), vp]
+    L.mq_pack_weights_device.restype = i32
+    L.mq_pack_weights_device.argtypes = [vp, i64, i64, vp, i32, i64, C.POINTER(vp), vp]
     L.mq_pack_prequantized.restype = i32
     L.mq_pack_prequantized.argtypes = [vp, vp, i64, i64, i32, i64, vp, vp, vp, vp, C.POINTER(vp), vp]
     L.mq_weights_export.restype = i32
@@ -208,6 +210,17 @@ def mq_pack_weights(W: np.ndarray, h: Optional[np.ndarray], block: int, budget_b
     out = C.c_void_p()
     _check(lib().mq_pack_weights(_np_ptr(W), N, K, _np_ptr(h32), block, int(budget_blocks), C.byref(out), _stream()),
            "mq_pack_weights")
+    return Weights(out.value)
+
+
+def mq_pack_weights_device(W: torch.Tensor, h: Optional[torch.Tensor], block: int, budget_blocks: int) -> Weights:
+    """Algorithm 1 with the O(N*K) part on the GPU.  W fp32 [N,K] CUDA tensor (contiguous), h fp32 [K] CUDA tensor or None."""
+    assert W.is_cuda and W.dtype == torch.float32 and W.is_contiguous()
+    N, K = W.shape
+    assert h is None or (h.is_cuda and h.dtype == torch.float32 and h.is_contiguous() and h.numel() == K)
+    out = C.c_void_p()
+    _check(lib().mq_pack_weights_device(W.data_ptr(), N, K, h.data_ptr() if h is not None else None, block,
+                                        int(budget_blocks), C.byref(out), _stream()), "mq_pack_weights_device")
     return Weights(out.value)
 
 

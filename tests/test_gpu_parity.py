@@ -153,6 +153,42 @@ def test_pack_weights_matches_algorithm1(mq, N, K, bs, rho):
     assert np.array_equal(e["qR"], L.qr_blocks()[order])
 
 
+@pytest.mark.parametrize("N,K,bs,rho", [(256, 256, 64, 2 / 16), (384, 1024, 64, 0.05), (256, 512, 128, 0.25),
+                                        (1024, 2048, 64, 0.10), (512, 14336, 64, 0.05)])
+def test_pack_weights_device_matches_algorithm1(mq, N, K, bs, rho):
+    """mq_pack_weights_device (Algorithm 1's O(N*K) part on the GPU) against the oracle's
+    Algorithm 1 and against the host packer: same base ints and scale bits, same selected set (the fp64 score
+    sums keep the host's order, so even near-ties fall the same way), same Q(R) on it."""
+    import torch
+    seed = 0 if N == 256 and K == 256 else 21
+    case = make_case(seed, 16, K, N, bs=bs, rho=rho, n_outlier_ch=2 if seed == 0 else None)
+    budget = synth.budget_from_density(rho, N, K, bs)
+    Wd = torch.from_numpy(np.ascontiguousarray(case.W, np.float32)).cuda()
+    hd = torch.from_numpy(np.ascontiguousarray(case.h, np.float32)).cuda()
+    e = mq.mq_pack_weights_device(Wd, hd, bs, budget).export()
+    L = case.L
+    assert np.array_equal(e["qW"], L.d.qw)
+    assert np.array_equal(e["sW"].view(np.uint32), L.d.sw.view(np.uint32))
+    assert np.array_equal(e["sR"].view(np.uint32), L.d.sr.view(np.uint32))
+    order = np.lexsort((L.blk_k, L.blk_n))
+    assert e["nnz"] == L.nnz and L.nnz > 0
+    assert np.array_equal(e["blk_n"], L.blk_n[order]) and np.array_equal(e["blk_k"], L.blk_k[order])
+    assert np.array_equal(e["qR"], L.qr_blocks()[order])
+    eh = mq.mq_pack_weights(case.W, case.h, bs, budget).export()
+    for k in ("qW", "sW", "sR", "blk_n", "blk_k", "qR"):
+        assert np.array_equal(e[k], eh[k]), k
+    # h = NULL (all ones), budget 0, budget larger than the number of positive scores, an all-zero row
+    W2 = case.W.copy()
+    W2[3] = 0.0
+    W2d = torch.from_numpy(W2).cuda()
+    for (hh, bud) in ((None, 5), (case.h, 0), (case.h, 10 ** 6)):
+        a = mq.mq_pack_weights_device(W2d, None if hh is None else hd, bs, bud).export()
+        b = mq.mq_pack_weights(W2, hh, bs, bud).export()
+        assert a["nnz"] == b["nnz"]
+        for k in ("qW", "sW", "sR", "blk_n", "blk_k", "qR"):
+            assert np.array_equal(a[k], b[k]), (k, bud)
+
+
 def test_pack_weights_zero_h_columns_and_null_h(mq):
     """blocks whose score is zero are never selected (nnz < budget); h = NULL means all ones."""
     N, K, bs = 256, 512, 64
