@@ -154,6 +154,18 @@ int mq_gemm_a8(const mq_weights* w, const int8_t* qA8_dev, const float* sA_dev, 
                mq_dtype y_dtype, int64_t ldy_elems, int32_t* dbg_acc_base_dev, int32_t* dbg_acc_res_dev,
                void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
+/* (3c) The paper's NAIVE pipeline, for the fused-vs-naive ablation (Fig.3), NOT a
+ * fast path: (i) mq_gemm with the residual switched off writes Y0 = s_a s_w acc0 as 16-bit Y, (ii) a separate
+ * sparse-block GEMM re-reads qA_dev and writes the partial output acc1 (int32 [M, N] dense, exact) into scratch_dev,
+ * (iii) a reduce-add kernel forms Y = round(Y0 + s_a s_r acc1).  Three launches; Y is rounded twice, so it agrees with
+ * mq_gemm's only to about one unit in the last place of the larger of |Y0|, |Y|.  scratch_dev: at least
+ * mq_gemm_naive_scratch_bytes(w, M) bytes, 4-byte aligned; it holds acc1 when the call returns (parity hook).
+ * Other arguments, requirements and errors as mq_gemm; M <= 16 * 65535. */
+size_t mq_gemm_naive_scratch_bytes(const mq_weights* w, int64_t M);
+int mq_gemm_naive(const mq_weights* w, const void* qA_dev, const float* sA_dev, int64_t M, void* Y_dev,
+                  mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev, size_t workspace_bytes,
+                  int32_t* scratch_dev, size_t scratch_bytes, void* cuda_stream);
+
 /* One linear layer from raw activations: A_dev fp16/bf16 [M, K] (rows 16-byte aligned, lda_elems % 8 == 0).
  * Default: mq_quantize_act into the workspace followed by mq_gemm on the same stream (two launches
  * chained by programmatic dependent launch).  With option "fused_quant" = 1 and M <= 8 the quantizer runs

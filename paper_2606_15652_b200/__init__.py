@@ -13,6 +13,8 @@ from .binding import (  # noqa: F401
     lib,
     mq_gemm,
     mq_gemm_a8,
+    mq_gemm_naive,
+    mq_gemm_naive_scratch_bytes,
     mq_gemm_workspace_bytes,
     mq_last_launch_count,
     mq_linear,

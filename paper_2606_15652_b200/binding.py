@@ -22,7 +22,7 @@ EXPORTS = [
     "mq_status_string", "mq_qact_bytes", "mq_quantize_act", "mq_unpack_act", "mq_pack_weights", "mq_pack_weights_device",
     "mq_pack_prequantized", "mq_weights_export", "mq_weights_clone", "mq_weights_info", "mq_weights_free",
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
-    "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_set_option",
+    "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_gemm_naive", "mq_gemm_naive_scratch_bytes", "mq_set_option",
     "mq_last_launch_count",
 ]
 
@@ -84,6 +84,10 @@ def lib() -> C.CDLL:
     L.mq_quantize_act8.argtypes = [vp, i32, i64, i64, i64, vp, vp, vp]
     L.mq_gemm_a8.restype = i32
     L.mq_gemm_a8.argtypes = [vp, vp, vp, i64, vp, i32, i64, vp, vp, vp, sz, vp]
+    L.mq_gemm_naive_scratch_bytes.restype = sz
+    L.mq_gemm_naive_scratch_bytes.argtypes = [vp, i64]
+    L.mq_gemm_naive.restype = i32
+    L.mq_gemm_naive.argtypes = [vp, vp, vp, i64, vp, i32, i64, vp, sz, vp, sz, vp]
     L.mq_set_option.restype = i32
     L.mq_set_option.argtypes = [C.c_char_p, i64]
     L.mq_last_launch_count.restype = i32
@@ -336,3 +340,28 @@ def mq_gemm_a8(w: Weights, qA8: torch.Tensor, sA: torch.Tensor, M: int, Y: Optio
                             workspace.data_ptr() if workspace is not None else None,
                             workspace.numel() if workspace is not None else 0, _stream()), "mq_gemm_a8")
     return (Y, d0, d1) if dbg else Y
+
+
+def mq_gemm_naive_scratch_bytes(w: Weights, M: int) -> int:
+    return int(lib().mq_gemm_naive_scratch_bytes(w.handle, M))
+
+
+def mq_gemm_naive(w: Weights, qA: torch.Tensor, sA: torch.Tensor, M: int, Y: Optional[torch.Tensor] = None,
+                  out_dtype: torch.dtype = torch.bfloat16, workspace: Optional[torch.Tensor] = None,
+                  scratch: Optional[torch.Tensor] = None):
+    """The paper's naive 3-kernel pipeline (dense GEMM, sparse-block GEMM, reduce-add): ablation only.
+    Returns (Y, acc1) with acc1 the sparse kernel's int32 partial output [M, N]."""
+    N = w.info()["N"]
+    if Y is None:
+        Y = torch.empty((M, N), dtype=out_dtype, device=qA.device)
+    need = mq_gemm_workspace_bytes(w, M)
+    if need and workspace is None:
+        workspace = new_workspace(need, qA.device)
+    if scratch is None:
+        scratch = torch.empty((M, N), dtype=torch.int32, device=qA.device)
+    ldy = Y.stride(0) if M > 1 else N
+    _check(lib().mq_gemm_naive(w.handle, qA.data_ptr(), sA.data_ptr(), M, Y.data_ptr(), _dtype_code(Y.dtype), ldy,
+                               workspace.data_ptr() if workspace is not None else None,
+                               workspace.numel() if workspace is not None else 0,
+                               scratch.data_ptr(), scratch.numel() * 4, _stream()), "mq_gemm_naive")
+    return Y, scratch

@@ -406,7 +406,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
     auto load_batch = [&](uint32_t ub) {
       const uint32_t u = ub + (uint32_t)lane;
       int2 v = make_int2(0, 0);
-      if (u < u_end) {
+      if (u < u_end && p.unit_meta) {   // unit_meta == NULL: dense-only launch (the naive pipeline's first kernel)
         const uint32_t tile = fdiv(u, p.dKS);
         v = __ldg(p.unit_meta + (size_t)fdiv(tile, p.dTT) * p.KS + (u - tile * (uint32_t)p.KS));
       }
@@ -1467,7 +1467,8 @@ namespace {
 // and qA / sA are unused.
 int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
               int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes, void* cuda_stream,
-              const void* fused_A, mq_dtype a_dtype, int64_t lda, uint32_t* fz_ctrl, bool a8 = false) {
+              const void* fused_A, mq_dtype a_dtype, int64_t lda, uint32_t* fz_ctrl, bool a8 = false,
+              bool ignore_res = false) {
   const bool fused = fused_A != nullptr;
   if (a8 && (fused || (w && (long double)127 * 7 * 16 * (long double)w->K >= 2147483648.0L))) return MQ_ERR_ACC_OVERFLOW;
   if (!w) return MQ_ERR_INVALID_ARG;
@@ -1523,7 +1524,7 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   gp.sw = w->d_sw;
   gp.sr = w->d_sr;
   gp.res = w->d_res;
-  gp.unit_meta = (const int2*)w->d_unit_meta;
+  gp.unit_meta = ignore_res ? nullptr : (const int2*)w->d_unit_meta;
   gp.sa = sA;
   gp.Y = Y;
   gp.dbg0 = dbg0;
@@ -1586,6 +1587,109 @@ extern "C" int mq_gemm_a8(const mq_weights* w, const int8_t* qA8, const float* s
                           void* cuda_stream) {
   return gemm_impl(w, qA8, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, nullptr, MQ_F16, 0,
                    nullptr, true);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// The paper's NAIVE pipeline (Fig.3), for the fused-vs-naive ablation:
+//   (i)   dense W4A4 GEMM: this library's kernel with the residual switched off, 16-bit Y0 = s_a s_w acc0
+//   (ii)  a separate sparse-block GEMM that re-reads the quantized activations from HBM and writes a partial
+//         output (acc1, int32 [M, N]), SIMT dp4a, one CTA per (n-tile, 16 tokens) walking the n-tile's cells
+//   (iii) reduce-add: Y = round16(Y0 + s_a s_r acc1)
+// Three launches and two extra passes over [M, N]; it also rounds twice.
+namespace {
+
+constexpr int NAIVE_TOK = 16;
+
+__device__ __forceinline__ int dp4a_s8(uint32_t a, uint32_t b, int c) {
+  int d;
+  asm("dp4a.s32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
+
+__global__ void __launch_bounds__(128) naive_sparse_kernel(const uint8_t* __restrict__ res, const mq::CellMeta* __restrict__ cells,
+                                                           const int32_t* __restrict__ cell_ptr, const uint8_t* __restrict__ qA,
+                                                           int64_t M, int64_t K, int64_t N, int32_t* __restrict__ acc1) {
+  const int nt = blockIdx.x, row = threadIdx.x, rhalf = row >> 6;
+  const int64_t m0 = (int64_t)blockIdx.y * NAIVE_TOK;
+  const int mt = (int)min((int64_t)NAIVE_TOK, M - m0);
+  int acc[NAIVE_TOK];
+#pragma unroll
+  for (int t = 0; t < NAIVE_TOK; ++t) acc[t] = 0;
+  const uint32_t HI = 0xF0F0F0F0u;
+  for (int c = cell_ptr[nt]; c < cell_ptr[nt + 1]; ++c) {
+    const int km = cells[c].kstep_mask, kstep = km & 0xFFFFFF, mask = (km >> 24) & 0xF;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int q = 2 * h + rhalf;
+      if (!(mask & (1 << q))) continue;
+      const uint8_t* qp = res + ((size_t)cells[c].qoff + (size_t)__popc(mask & ((1 << q) - 1))) * QUARTER_BYTES + (size_t)(row & 63) * 16;
+      const uint4 w0 = *reinterpret_cast<const uint4*>(qp), w1 = *reinterpret_cast<const uint4*>(qp + 1024);
+      const uint32_t ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+      const size_t koff = ((size_t)kstep * BK + (size_t)h * 64) / 2;   // byte offset of the 64 activations in a row of qA
+#pragma unroll
+      for (int t = 0; t < NAIVE_TOK; ++t) {
+        if (t >= mt) break;
+        const uint8_t* ap = qA + (size_t)(m0 + t) * (size_t)(K / 2) + koff;
+        const uint4 a0 = __ldg(reinterpret_cast<const uint4*>(ap)), a1 = __ldg(reinterpret_cast<const uint4*>(ap + 16));
+        const uint32_t aw[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+        int sacc = acc[t];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {   // both operands x16, even / odd nibbles pair up: sum is 256 x the dot product
+          sacc = dp4a_s8((ww[i] << 4) & HI, (aw[i] << 4) & HI, sacc);
+          sacc = dp4a_s8(ww[i] & HI, aw[i] & HI, sacc);
+        }
+        acc[t] = sacc;
+      }
+    }
+  }
+#pragma unroll
+  for (int t = 0; t < NAIVE_TOK; ++t)
+    if (t < mt) acc1[(size_t)(m0 + t) * (size_t)N + (size_t)nt * BN + row] = acc[t] >> 8;
+}
+
+template <bool BF16>
+__global__ void naive_add_kernel(void* __restrict__ Y, int64_t ldy, const int32_t* __restrict__ acc1, const float* __restrict__ sa,
+                                 const float* __restrict__ sr, int64_t M, int64_t N) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= M * N) return;
+  const int64_t m = idx / N, n = idx - m * N;
+  const size_t o = (size_t)m * (size_t)ldy + (size_t)n;
+  float y0;
+  if (BF16)
+    y0 = __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(Y)[o]);
+  else
+    y0 = __half2float(reinterpret_cast<const __half*>(Y)[o]);
+  store_y<BF16>(Y, o, y0 + sa[m] * (sr[n] * (float)acc1[idx]));
+}
+
+}  // namespace
+
+extern "C" size_t mq_gemm_naive_scratch_bytes(const mq_weights* w, int64_t M) {
+  return (!w || M <= 0) ? 0 : (size_t)M * (size_t)w->N * sizeof(int32_t);
+}
+
+extern "C" int mq_gemm_naive(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
+                             int64_t ldy, void* workspace, size_t workspace_bytes, int32_t* scratch, size_t scratch_bytes,
+                             void* cuda_stream) {
+  if (!w) return MQ_ERR_INVALID_ARG;
+  if (M > 0 && (!scratch || ((uintptr_t)scratch & 3))) return MQ_ERR_INVALID_ARG;
+  if (M > 0 && scratch_bytes < mq_gemm_naive_scratch_bytes(w, M)) return MQ_ERR_WORKSPACE;
+  const int rc = gemm_impl(w, qA, sA, M, Y, y_dtype, ldy, nullptr, nullptr, workspace, workspace_bytes, cuda_stream, nullptr,
+                           MQ_F16, 0, nullptr, false, true);
+  if (rc != MQ_OK || M == 0) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const dim3 grid((unsigned)(w->N / BN), (unsigned)((M + NAIVE_TOK - 1) / NAIVE_TOK));
+  if (grid.y > 65535) return MQ_ERR_UNSUPPORTED_SHAPE;
+  naive_sparse_kernel<<<grid, 128, 0, st>>>(w->d_res, w->d_cell_meta, w->d_cell_ptr, (const uint8_t*)qA, M, w->K, w->N, scratch);
+  const int64_t total = M * w->N;
+  const unsigned blocks = (unsigned)((total + 255) / 256);
+  if (y_dtype == MQ_BF16)
+    naive_add_kernel<true><<<blocks, 256, 0, st>>>(Y, ldy, scratch, sA, w->d_sr, M, w->N);
+  else
+    naive_add_kernel<false><<<blocks, 256, 0, st>>>(Y, ldy, scratch, sA, w->d_sr, M, w->N);
+  if (cudaGetLastError() != cudaSuccess) return MQ_ERR_CUDA;
+  mq::set_launch_count(3);
+  return MQ_OK;
 }
 
 extern "C" size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M) {
