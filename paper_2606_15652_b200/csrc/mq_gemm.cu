@@ -1608,7 +1608,7 @@ __device__ __forceinline__ int dp4a_s8(uint32_t a, uint32_t b, int c) {
 
 __global__ void __launch_bounds__(128) naive_sparse_kernel(const uint8_t* __restrict__ res, const mq::CellMeta* __restrict__ cells,
                                                            const int32_t* __restrict__ cell_ptr, const uint8_t* __restrict__ qA,
-                                                           int64_t M, int64_t K, int64_t N, int32_t* __restrict__ acc1) {
+                                                           int64_t M, int64_t K, int64_t N, int32_t* __restrict__ acc1, int cells_per_cta) {
   const int nt = blockIdx.x, row = threadIdx.x, rhalf = row >> 6;
   const int64_t m0 = (int64_t)blockIdx.y * NAIVE_TOK;
   const int mt = (int)min((int64_t)NAIVE_TOK, M - m0);
@@ -1616,7 +1616,11 @@ __global__ void __launch_bounds__(128) naive_sparse_kernel(const uint8_t* __rest
 #pragma unroll
   for (int t = 0; t < NAIVE_TOK; ++t) acc[t] = 0;
   const uint32_t HI = 0xF0F0F0F0u;
-  for (int c = cell_ptr[nt]; c < cell_ptr[nt + 1]; ++c) {
+  // the n-tile's cells are dealt to gridDim.z CTAs (cells_per_cta each); with more than one, the partial sums meet
+  // in acc1 through int32 atomics (exact, so the result does not depend on the order)
+  const int c_lo = cell_ptr[nt] + (int)blockIdx.z * cells_per_cta, c_hi = min(cell_ptr[nt + 1], c_lo + cells_per_cta);
+  if (gridDim.z > 1 && c_lo >= c_hi) return;
+  for (int c = c_lo; c < c_hi; ++c) {
     const int km = cells[c].kstep_mask, kstep = km & 0xFFFFFF, mask = (km >> 24) & 0xF;
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -1644,7 +1648,14 @@ __global__ void __launch_bounds__(128) naive_sparse_kernel(const uint8_t* __rest
   }
 #pragma unroll
   for (int t = 0; t < NAIVE_TOK; ++t)
-    if (t < mt) acc1[(size_t)(m0 + t) * (size_t)N + (size_t)nt * BN + row] = acc[t] >> 8;
+    if (t < mt) {
+      int32_t* dst = acc1 + (size_t)(m0 + t) * (size_t)N + (size_t)nt * BN + row;
+      if (gridDim.z > 1) {
+        if (acc[t]) atomicAdd(dst, acc[t] >> 8);
+      } else {
+        *dst = acc[t] >> 8;
+      }
+    }
 }
 
 template <bool BF16>
@@ -1678,9 +1689,14 @@ extern "C" int mq_gemm_naive(const mq_weights* w, const void* qA, const float* s
                            MQ_F16, 0, nullptr, false, true);
   if (rc != MQ_OK || M == 0) return rc;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const dim3 grid((unsigned)(w->N / BN), (unsigned)((M + NAIVE_TOK - 1) / NAIVE_TOK));
+  // few tokens: split an n-tile's cells over several CTAs so that the kernel is not a handful of long serial loops
+  const int cells_per_cta = M <= 64 ? 2 : (M <= 512 ? 8 : 1 << 20);
+  const unsigned gz = (unsigned)std::max(1, std::min(64, (w->max_cells_per_tile + cells_per_cta - 1) / cells_per_cta));
+  const dim3 grid((unsigned)(w->N / BN), (unsigned)((M + NAIVE_TOK - 1) / NAIVE_TOK), gz);
   if (grid.y > 65535) return MQ_ERR_UNSUPPORTED_SHAPE;
-  naive_sparse_kernel<<<grid, 128, 0, st>>>(w->d_res, w->d_cell_meta, w->d_cell_ptr, (const uint8_t*)qA, M, w->K, w->N, scratch);
+  if (gz > 1 && cudaMemsetAsync(scratch, 0, (size_t)M * (size_t)w->N * sizeof(int32_t), st) != cudaSuccess) return MQ_ERR_CUDA;
+  naive_sparse_kernel<<<grid, 128, 0, st>>>(w->d_res, w->d_cell_meta, w->d_cell_ptr, (const uint8_t*)qA, M, w->K, w->N, scratch,
+                                            gz > 1 ? cells_per_cta : 1 << 20);
   const int64_t total = M * w->N;
   const unsigned blocks = (unsigned)((total + 255) / 256);
   if (y_dtype == MQ_BF16)
