@@ -216,3 +216,62 @@ def round_to_bf16(Y: np.ndarray) -> np.ndarray:
     r = np.rint(scaled)             # RNE
     out[nz] = np.ldexp(r, e - 8)
     return out
+
+
+# ------------------------------------------------------------------------------------------------
+# per-group activation quantization -- the paper's stated activation granularity for
+# the 4-bit setting ("For the 4-bit setting, we adopt per-group and per-channel
+# symmetric quantization for activations and weights, respectively").  The paper gives no group size
+# (reading A5g): `group` is a parameter, consecutive input channels, K % group == 0.
+# Plain numpy on top of O1; no blocking beyond the definition.
+def quantize_act_group(A, group: int, bits: int = 4) -> Tuple[np.ndarray, np.ndarray]:
+    """O2g: Eq.1 applied to every run of `group` consecutive input channels of every token:
+    row (m, g) of the [M*K/group, group] view of A is one quantization unit.  Returns the codes
+    int8 [M, K] and the scales fp32 [M, K/group]."""
+    b16, code = _bits16(A)
+    M, K = b16.shape
+    assert group > 0 and K % group == 0
+    view = b16.reshape(M * (K // group), group)
+    qa, sa = quantize_act(view.view(np.float16) if code == 0 else (view, "bf16"), bits=bits)
+    return qa.reshape(M, K), sa.reshape(M, K // group)
+
+
+def residual_mask(N: int, K: int, bs: int, blk_n: np.ndarray, blk_k: np.ndarray) -> np.ndarray:
+    """The block mask M of Eq.4 as a 0/1 int8 matrix [N, K]."""
+    mask = np.zeros((N, K), np.int8)
+    for bn, bk in zip(np.asarray(blk_n).tolist(), np.asarray(blk_k).tolist()):
+        mask[bn * bs:(bn + 1) * bs, bk * bs:(bk + 1) * bs] = 1
+    return mask
+
+
+def forward_group(A, L: PackedLayer, group: int, cols: Optional[np.ndarray] = None, rows: Optional[np.ndarray] = None):
+    """O2g + O8g + O9g.  With a scale that changes along K the scaled product of Eq.2 holds per group:
+        Y[m, n] = sum_g s_a[m, g] * ( s_w[n] * acc0_g[m, n] + s_r[n] * acc1_g[m, n] )          (binary64)
+        acc0_g[m, n] = sum_{k in group g} q_a[m, k] q_w[n, k]                                   (integers)
+        acc1_g[m, n] = sum_{k in group g} q_a[m, k] (M (.) q_r)[n, k]                           (Eq.4's sparse term)
+    `cols` / `rows` restrict the output channels / tokens (full-size cases).  Returns qa, sa, the per-group
+    integer accumulators [G, M, N], their sums over g (acc0, acc1), Y and the tolerance magnitude
+    mag = sum_g s_a (|s_w acc0_g| + |s_r acc1_g|)."""
+    qa, sa = quantize_act_group(A, group)
+    if rows is not None:
+        qa, sa = qa[rows], sa[rows]
+    qw, qr, sw, sr = L.d.qw, L.d.qr * residual_mask(L.N, L.K, L.bs, L.blk_n, L.blk_k), L.d.sw, L.d.sr
+    if cols is not None:
+        qw, qr, sw, sr = qw[cols], qr[cols], sw[cols], sr[cols]
+    M, K = qa.shape
+    G = K // group
+    N = qw.shape[0]
+    acc0_g = np.empty((G, M, N), np.int64)
+    acc1_g = np.empty((G, M, N), np.int64)
+    Y = np.zeros((M, N), np.float64)
+    mag = np.zeros((M, N), np.float64)
+    sw64, sr64 = sw.astype(np.float64)[None, :], sr.astype(np.float64)[None, :]
+    for g in range(G):
+        ks = slice(g * group, (g + 1) * group)
+        a = qa[:, ks].astype(np.int64)
+        acc0_g[g] = a @ qw[:, ks].astype(np.int64).T
+        acc1_g[g] = a @ qr[:, ks].astype(np.int64).T
+        s = sa[:, g].astype(np.float64)[:, None]
+        Y += s * (sw64 * acc0_g[g] + sr64 * acc1_g[g])
+        mag += s * (np.abs(sw64 * acc0_g[g]) + np.abs(sr64 * acc1_g[g]))
+    return dict(qa=qa, sa=sa, acc0_g=acc0_g, acc1_g=acc1_g, acc0=acc0_g.sum(0), acc1=acc1_g.sum(0), Y=Y, mag=mag)
