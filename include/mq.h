@@ -166,6 +166,30 @@ int mq_gemm_naive(const mq_weights* w, const void* qA_dev, const float* sA_dev, 
                   mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev, size_t workspace_bytes,
                   int32_t* scratch_dev, size_t scratch_bytes, void* cuda_stream);
 
+/* ------------------------------------------------------------------------------------
+ * (3d) Scales that vary along K: per-GROUP activation quantization, the paper's stated activation
+ * granularity for the 4-bit setting ("For the 4-bit setting, we adopt per-group and per-channel symmetric
+ * quantization for activations and weights, respectively"; the group size is not given: reading A5g, `group` in
+ * {32, 64, 128} consecutive input channels, K % group == 0).
+ *
+ * mq_quantize_act_group: Eq.1 on every run of `group` channels of every token.  A_dev fp16/bf16 [M, K]
+ * (16-byte aligned, lda_elems % 8 == 0) -> qA_dev packed int4 [M, K/2] bytes in the canonical nibble order (byte i
+ * of a row = elements 2i | 2i+1 << 4; mq_qact_bytes(M, K) bytes, 16-byte aligned; mq_unpack_act reads it) and
+ * sA_dev float [M, K/group].  One launch, stream-ordered, no allocation.
+ *
+ * mq_gemm_group: Y[m,n] = sum_g s_a[m,g] (s_w[n] acc0_g[m,n] + s_r[n] acc1_g[m,n]) (Eq.2 P:82 and Eq.4 P:106 per
+ * group), acc0_g / acc1_g the exact integer dot products of group g's activation codes with the base / selected
+ * residual codes; the group terms are added in fp32 in ascending g (K-split partial sums in ascending split), then
+ * rounded once to y_dtype.  Parity hooks: dbg_acc_base_g_dev / dbg_acc_res_g_dev int32 [K/group][M][N] or NULL.
+ * workspace_dev: mq_gemm_group_workspace_bytes(w, M) bytes (may be 0), 16-byte aligned, no initial content
+ * required.  A first SIMT (dp4a) path, one or two launches; M <= 16 * 65535.  Errors as mq_gemm. */
+int mq_quantize_act_group(const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda_elems, int group,
+                          void* qA_dev, float* sA_dev, void* cuda_stream);
+size_t mq_gemm_group_workspace_bytes(const mq_weights* w, int64_t M);
+int mq_gemm_group(const mq_weights* w, const void* qA_dev, const float* sA_dev, int group, int64_t M, void* Y_dev,
+                  mq_dtype y_dtype, int64_t ldy_elems, int32_t* dbg_acc_base_g_dev, int32_t* dbg_acc_res_g_dev,
+                  void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
 /* One linear layer from raw activations: A_dev fp16/bf16 [M, K] (rows 16-byte aligned, lda_elems % 8 == 0).
  * Default: mq_quantize_act into the workspace followed by mq_gemm on the same stream (two launches
  * chained by programmatic dependent launch).  With option "fused_quant" = 1 and M <= 8 the quantizer runs

@@ -13,6 +13,8 @@ from .binding import (  # noqa: F401
     lib,
     mq_gemm,
     mq_gemm_a8,
+    mq_gemm_group,
+    mq_gemm_group_workspace_bytes,
     mq_gemm_naive,
     mq_gemm_naive_scratch_bytes,
     mq_gemm_workspace_bytes,
@@ -27,6 +29,7 @@ from .binding import (  # noqa: F401
     mq_qact_bytes,
     mq_quantize_act,
     mq_quantize_act8,
+    mq_quantize_act_group,
     mq_set_option,
     mq_unpack_act,
     new_workspace,

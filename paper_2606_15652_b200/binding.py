@@ -23,7 +23,7 @@ EXPORTS = [
     "mq_pack_prequantized", "mq_weights_export", "mq_weights_clone", "mq_weights_info", "mq_weights_free",
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
     "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_gemm_naive", "mq_gemm_naive_scratch_bytes", "mq_set_option",
-    "mq_last_launch_count",
+    "mq_last_launch_count", "mq_quantize_act_group", "mq_gemm_group_workspace_bytes", "mq_gemm_group",
 ]
 
 _lib = None
@@ -88,6 +88,12 @@ def lib() -> C.CDLL:
     L.mq_gemm_naive_scratch_bytes.argtypes = [vp, i64]
     L.mq_gemm_naive.restype = i32
     L.mq_gemm_naive.argtypes = [vp, vp, vp, i64, vp, i32, i64, vp, sz, vp, sz, vp]
+    L.mq_quantize_act_group.restype = i32
+    L.mq_quantize_act_group.argtypes = [vp, i32, i64, i64, i64, i32, vp, vp, vp]
+    L.mq_gemm_group_workspace_bytes.restype = sz
+    L.mq_gemm_group_workspace_bytes.argtypes = [vp, i64]
+    L.mq_gemm_group.restype = i32
+    L.mq_gemm_group.argtypes = [vp, vp, vp, i32, i64, vp, i32, i64, vp, vp, vp, sz, vp]
     L.mq_set_option.restype = i32
     L.mq_set_option.argtypes = [C.c_char_p, i64]
     L.mq_last_launch_count.restype = i32
@@ -365,3 +371,41 @@ def mq_gemm_naive(w: Weights, qA: torch.Tensor, sA: torch.Tensor, M: int, Y: Opt
                                workspace.numel() if workspace is not None else 0,
                                scratch.data_ptr(), scratch.numel() * 4, _stream()), "mq_gemm_naive")
     return Y, scratch
+
+
+def mq_quantize_act_group(A: torch.Tensor, group: int) -> Tuple[torch.Tensor, torch.Tensor]:
+    """Per-group int4 activations.  Returns (qA uint8 [M,K/2], sA float32 [M,K/group])."""
+    assert A.is_cuda and A.dim() == 2 and A.stride(1) == 1
+    M, K = A.shape
+    qA = torch.empty((M, K // 2), dtype=torch.uint8, device=A.device)
+    sA = torch.empty((M, max(K // max(group, 1), 1)), dtype=torch.float32, device=A.device)
+    lda = A.stride(0) if M > 1 else K
+    _check(lib().mq_quantize_act_group(A.data_ptr(), _dtype_code(A.dtype), M, K, lda, group, qA.data_ptr(), sA.data_ptr(),
+                                       _stream()), "mq_quantize_act_group")
+    return qA, sA
+
+
+def mq_gemm_group_workspace_bytes(w: Weights, M: int) -> int:
+    return int(lib().mq_gemm_group_workspace_bytes(w.handle, M))
+
+
+def mq_gemm_group(w: Weights, qA: torch.Tensor, sA: torch.Tensor, group: int, M: int, Y: Optional[torch.Tensor] = None,
+                  out_dtype: torch.dtype = torch.bfloat16, dbg: bool = False, workspace: Optional[torch.Tensor] = None):
+    """Base + residual GEMM with per-group activation scales.  dbg: also returns the per-group integer
+    accumulators int32 [K/group, M, N] (base, residual)."""
+    inf = w.info()
+    N, K = inf["N"], inf["K"]
+    if Y is None:
+        Y = torch.empty((M, N), dtype=out_dtype, device=qA.device)
+    need = mq_gemm_group_workspace_bytes(w, M)
+    if need and workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=qA.device)
+    G = K // group
+    d0 = torch.empty((G, M, N), dtype=torch.int32, device=qA.device) if dbg else None
+    d1 = torch.empty((G, M, N), dtype=torch.int32, device=qA.device) if dbg else None
+    ldy = Y.stride(0) if M > 1 else N
+    _check(lib().mq_gemm_group(w.handle, qA.data_ptr(), sA.data_ptr(), group, M, Y.data_ptr(), _dtype_code(Y.dtype), ldy,
+                               d0.data_ptr() if dbg else None, d1.data_ptr() if dbg else None,
+                               workspace.data_ptr() if workspace is not None else None,
+                               workspace.numel() if workspace is not None else 0, _stream()), "mq_gemm_group")
+    return (Y, d0, d1) if dbg else Y
