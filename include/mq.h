@@ -220,6 +220,7 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
  *   "token_tile": 0 = automatic, else 16/32/64/128
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
  *   "fused_quant": 0 (default) / 1: see mq_linear
+ *   "group_simt": 0 (default) = mq_gemm_group uses its tensor-core kernel for M > 2; 1 = the dp4a kernel for every M
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
  *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */

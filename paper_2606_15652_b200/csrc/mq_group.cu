@@ -209,6 +209,133 @@ __global__ void __launch_bounds__(BN) gemm_group_kernel(const GParams p) {
   }
 }
 
+
+// ---- tensor-core path (M > 2): legacy warp-level mma.sync m16n8k32 s8 -- a group boundary every 32..128 channels
+// means the int32 sums must leave the accumulator after at most one K-step, which a TMEM-resident tcgen05
+// accumulator makes expensive (a tcgen05.ld drain per group); warp-level fragments are already in registers.
+// 8 warps, warp v = output channels 16 v .. 16 v + 15 of the n-tile, TOKC tokens per CTA in sub-tiles of 8.
+// A fragment = weights, B fragment = tokens.  Both sides expand word j of a 16-byte chunk (8 nibbles) into
+// {even nibbles, odd nibbles} x 16 in int8 and place them in the same K slots, so the K permutation cancels and
+// the accumulator is 256 x the exact dot product.
+constexpr int TOKC = 64;
+constexpr int MMA_THREADS = 256;
+
+__device__ __forceinline__ void mma_s8(int (&d)[4], const uint32_t a0, const uint32_t a1, const uint32_t a2, const uint32_t a3,
+                                       const uint32_t b0, const uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+template <int GROUP, bool BF16>
+__global__ void __launch_bounds__(MMA_THREADS) gemm_group_mma_kernel(const GParams p) {
+  mq::ptx::griddep_launch();
+  mq::ptx::griddep_wait();
+  constexpr uint32_t HI = 0xF0F0F0F0u;
+  constexpr int CPG = GROUP / 32, GPS = 4 / CPG, NST = TOKC / 8;
+  const int nt = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gq = lane >> 2, tq = lane & 3;
+  const int rhalf = warp >> 2;
+  const int r0 = warp * 16 + gq, r1 = r0 + 8;                  // rows of the n-tile this thread's accumulators hold
+  const int64_t n0 = (int64_t)nt * BN + r0, n1 = n0 + 8;
+  const int64_t m0 = (int64_t)blockIdx.y * TOKC;
+  const int nst = (int)min((int64_t)NST, (p.M - m0 + 7) / 8);
+  const int k0 = (int)blockIdx.z * p.ks_per_split, k1 = min(p.KS, k0 + p.ks_per_split);
+  const int G = (int)(p.K / GROUP);
+  const float sw0 = __ldg(p.sw + n0), sw1 = __ldg(p.sw + n1), sr0 = __ldg(p.sr + n0), sr1 = __ldg(p.sr + n1);
+  float y[NST][4];
+#pragma unroll
+  for (int st = 0; st < NST; ++st)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) y[st][i] = 0.f;
+
+  for (int ks = k0; ks < k1; ++ks) {
+    const uint8_t* tile = p.base + ((size_t)nt * p.KS + ks) * TILE_BYTES + (size_t)tq * 4;
+    uint32_t wa[4][4], ra[4][4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const uint32_t x0 = __ldg(reinterpret_cast<const uint32_t*>(tile + c * (BN * 16) + r0 * 16));
+      const uint32_t x1 = __ldg(reinterpret_cast<const uint32_t*>(tile + c * (BN * 16) + r1 * 16));
+      wa[c][0] = (x0 << 4) & HI;
+      wa[c][1] = (x1 << 4) & HI;
+      wa[c][2] = x0 & HI;
+      wa[c][3] = x1 & HI;
+    }
+    bool has[2] = {false, false};   // warp-uniform: a quarter covers 64 rows = 4 whole warps
+    if (p.unit_meta) {
+      const int2 um = __ldg(reinterpret_cast<const int2*>(p.unit_meta) + (size_t)nt * p.KS + ks);
+      const int mask = um.x & 0xF;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int q = 2 * h + rhalf;
+        if (mask & (1 << q)) {
+          has[h] = true;
+          const uint8_t* qp = p.res + ((size_t)um.y + (size_t)__popc(mask & ((1 << q) - 1))) * QUARTER_BYTES + (size_t)tq * 4;
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const uint32_t x0 = __ldg(reinterpret_cast<const uint32_t*>(qp + j * 1024 + (r0 & 63) * 16));
+            const uint32_t x1 = __ldg(reinterpret_cast<const uint32_t*>(qp + j * 1024 + (r1 & 63) * 16));
+            ra[2 * h + j][0] = (x0 << 4) & HI;
+            ra[2 * h + j][1] = (x1 << 4) & HI;
+            ra[2 * h + j][2] = x0 & HI;
+            ra[2 * h + j][3] = x1 & HI;
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int st = 0; st < NST; ++st) {
+      if (st >= nst) break;
+      const int64_t mb = m0 + 8 * st + gq;            // token of this lane's B fragment
+      const int64_t t0 = m0 + 8 * st + 2 * tq, t1 = t0 + 1;   // tokens of this lane's accumulators
+      uint32_t bw[4] = {0, 0, 0, 0};
+      if (mb < p.M) {
+        const uint8_t* ap = p.qA + (size_t)mb * (size_t)(p.K / 2) + (size_t)ks * (BK / 2) + (size_t)tq * 4;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) bw[c] = __ldg(reinterpret_cast<const uint32_t*>(ap + c * 16));
+      }
+#pragma unroll
+      for (int gi = 0; gi < GPS; ++gi) {
+        int d0[4] = {0, 0, 0, 0}, d1[4] = {0, 0, 0, 0};
+#pragma unroll
+        for (int j = 0; j < CPG; ++j) {
+          const int c = gi * CPG + j;
+          const uint32_t b0 = (bw[c] << 4) & HI, b1 = bw[c] & HI;
+          mma_s8(d0, wa[c][0], wa[c][1], wa[c][2], wa[c][3], b0, b1);
+          if (has[c >> 1]) mma_s8(d1, ra[c][0], ra[c][1], ra[c][2], ra[c][3], b0, b1);
+        }
+        const int g = ks * GPS + gi;
+        const float s_t0 = t0 < p.M ? __ldg(p.sa + (size_t)t0 * G + g) : 0.f;
+        const float s_t1 = t1 < p.M ? __ldg(p.sa + (size_t)t1 * G + g) : 0.f;
+        // accumulator i: (row r0, t0), (r0, t1), (r1, t0), (r1, t1); sums are multiples of 256, the shift is exact
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int a0 = d0[i] >> 8, a1 = d1[i] >> 8;
+          const float swv = i < 2 ? sw0 : sw1, srv = i < 2 ? sr0 : sr1, sav = (i & 1) ? s_t1 : s_t0;
+          y[st][i] += sav * (swv * (float)a0 + srv * (float)a1);
+          const int64_t t = (i & 1) ? t1 : t0, n = i < 2 ? n0 : n1;
+          if (t < p.M) {
+            if (p.dbg0) p.dbg0[((size_t)g * p.M + t) * p.N + n] = a0;
+            if (p.dbg1) p.dbg1[((size_t)g * p.M + t) * p.N + n] = a1;
+          }
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int st = 0; st < NST; ++st) {
+    if (st >= nst) break;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int64_t t = m0 + 8 * st + 2 * tq + (i & 1), n = i < 2 ? n0 : n1;
+      if (t >= p.M) continue;
+      if (p.splits == 1)
+        store_y16<BF16>(p.Y, (size_t)t * p.ldy + n, y[st][i]);
+      else
+        p.partial[((size_t)blockIdx.z * p.M + t) * p.N + n] = y[st][i];
+    }
+  }
+}
+
 // the K-splits meet here, in split order (deterministic)
 template <bool BF16>
 __global__ void __launch_bounds__(256) group_reduce_kernel(const float* __restrict__ partial, int splits, int64_t M, int64_t N,
@@ -223,8 +350,11 @@ __global__ void __launch_bounds__(256) group_reduce_kernel(const float* __restri
   store_y16<BF16>(Y, (size_t)m * ldy + n, s);
 }
 
+bool group_use_simt(int64_t M) { return M <= 2 || mq::options().group_simt != 0; }
+
 int group_splits(const mq_weights* w, int64_t M) {
-  const int64_t ctas = (w->N / BN) * ((M + TOK - 1) / TOK);
+  const int tok = group_use_simt(M) ? TOK : TOKC;
+  const int64_t ctas = (w->N / BN) * ((M + tok - 1) / tok);
   const int64_t KS = w->K / BK;
   if (ctas >= TARGET_CTAS) return 1;
   return (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(KS, 32), (TARGET_CTAS + ctas - 1) / ctas));
@@ -287,7 +417,8 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
   if (!qA || !sA || !Y || ldy < w->N) return MQ_ERR_INVALID_ARG;
   if (((uintptr_t)qA & 15) || ((uintptr_t)sA & 3) || ((uintptr_t)Y & 1) || ((uintptr_t)dbg0 & 3) || ((uintptr_t)dbg1 & 3))
     return MQ_ERR_INVALID_ARG;
-  const int64_t mtiles = (M + TOK - 1) / TOK;
+  const bool simt = group_use_simt(M);
+  const int64_t mtiles = simt ? (M + TOK - 1) / TOK : (M + TOKC - 1) / TOKC;
   if (mtiles > 65535) return MQ_ERR_UNSUPPORTED_SHAPE;
   const int rc = mq::check_device();
   if (rc != MQ_OK) return rc;
@@ -317,8 +448,16 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const dim3 grid((unsigned)(w->N / BN), (unsigned)mtiles, (unsigned)splits);
   const bool bf = y_dtype == MQ_BF16;
-#define MQ_LAUNCH_G(GR) \
-  do { if (bf) gemm_group_kernel<GR, true><<<grid, BN, 0, st>>>(p); else gemm_group_kernel<GR, false><<<grid, BN, 0, st>>>(p); } while (0)
+#define MQ_LAUNCH_G(GR)                                                                  \
+  do {                                                                                   \
+    if (simt) {                                                                          \
+      if (bf) gemm_group_kernel<GR, true><<<grid, BN, 0, st>>>(p);                       \
+      else gemm_group_kernel<GR, false><<<grid, BN, 0, st>>>(p);                         \
+    } else {                                                                             \
+      if (bf) gemm_group_mma_kernel<GR, true><<<grid, MMA_THREADS, 0, st>>>(p);          \
+      else gemm_group_mma_kernel<GR, false><<<grid, MMA_THREADS, 0, st>>>(p);            \
+    }                                                                                    \
+  } while (0)
   if (group == 32) MQ_LAUNCH_G(32);
   else if (group == 64) MQ_LAUNCH_G(64);
   else MQ_LAUNCH_G(128);

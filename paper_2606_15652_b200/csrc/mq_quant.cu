@@ -205,6 +205,9 @@ extern "C" int mq_set_option(const char* name, int64_t value) {
   } else if (!strcmp(name, "fused_quant")) {
     if (value > 1) return MQ_ERR_INVALID_ARG;
     o.fused_quant = value;
+  } else if (!strcmp(name, "group_simt")) {
+    if (value > 1) return MQ_ERR_INVALID_ARG;
+    o.group_simt = value;
   } else {
     return MQ_ERR_INVALID_ARG;
   }

@@ -92,6 +92,21 @@ def test_group_parity_small(mq, M, K, N, bs, rho, dt, group):
     check(got, want, group, K, out, f"group {group} M{M} K{K} N{N} bs{bs} {out}")
 
 
+@pytest.mark.parametrize("M,K,N,bs,rho,dt", [SHAPES[0], SHAPES[3], SHAPES[4], SHAPES[8]])
+def test_group_parity_simt_kernel_every_m(mq, M, K, N, bs, rho, dt):
+    """Option group_simt = 1: the dp4a kernel (default for M <= 2 only) on multi-token shapes."""
+    case = make_case(1200 + M, M, K, N, bs=bs, rho=rho, budget=2 if rho is None else None, a_dtype=dt)
+    w = pack_from_oracle(case)
+    try:
+        mq.mq_set_option("group_simt", 1)
+        for group in (32, 128):
+            want = oracle.forward_group(A_of(case), case.L, group)
+            got = run_group(mq, case, group, w)
+            check(got, want, group, K, "bf16", f"simt group {group} M{M} K{K} N{N}")
+    finally:
+        mq.mq_set_option("group_simt", 0)
+
+
 def test_group_budget_zero_and_whole_row_group(mq):
     """Budget 0: acc1_g == 0 and Y is the dense-only product.  Activations constant along K in magnitude per group:
     every group scale equal, so the per-group result must agree with the per-token path (mq_gemm) to rounding."""
