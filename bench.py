@@ -251,7 +251,27 @@ def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_
                 stream.synchronize()
                 bestn = min(bestn, a0.elapsed_time(a1) / reps)
             del gn, scr
+            # per-group activation scales (the paper's W4A4 activation setting), group 128:
+            # mq_gemm_group on the same launch (a first dp4a / mma.sync path, not the tcgen05 kernel)
+            qg, sg = mq.mq_quantize_act_group(L.A[m], 128)
+            wsg = torch.empty(max(mq.mq_gemm_group_workspace_bytes(L.copies[0], m), 16), dtype=torch.uint8, device="cuda")
+            gg = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gg, stream=stream):
+                for r in range(reps):
+                    mq.mq_gemm_group(L.copies[r % N_COPIES], qg, sg, 128, m, Y=L.Y[m], workspace=wsg)
+            for _ in range(3):
+                gg.replay()
+            bestg = 1e30
+            for _ in range(5):
+                graphs[0].replay()
+                a0.record(stream)
+                gg.replay()
+                a1.record(stream)
+                stream.synchronize()
+                bestg = min(bestg, a0.elapsed_time(a1) / reps)
+            del gg, qg, sg, wsg
             per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3, us_dense=best0 * 1e3, us_a8=best8 * 1e3, us_naive=bestn * 1e3,
+                                  us_group=bestg * 1e3,
                                   bytes=algo_bytes(m, L.K, L.N, L.nnz, BS), ops=algo_ops(m, L.K, L.N, L.nnz, BS)))
 
         # ---- W16A16 comparator: cuBLAS bf16 on the same shapes, same rotation
@@ -339,14 +359,18 @@ def roofline_of(r, peaks, traffic):
     int8_peak = 2.0 * peaks["bf16_tflops"]          # kind::i8 runs at twice the bf16 rate (nominal 4.5 vs 2.25 PF)
     t_hbm, t_tensor = by / (peaks["hbm_gbs"] * 1e9), ops / (int8_peak * 1e12)
     per_shape = [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3), us_dense_only=round(s["us_dense"], 3),
-                      us_w4a8=round(s["us_a8"], 3), us_naive3=round(s["us_naive"], 3),
+                      us_w4a8=round(s["us_a8"], 3), us_naive3=round(s["us_naive"], 3), us_group128=round(s["us_group"], 3),
                       gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
                       tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in r["per_shape"]]
     kern = f"mq_gemm_kernel ({len(r['per_shape'])} launches of the step, timed alone, cold weights)"
     us0 = sum(s["us_dense"] for s in r["per_shape"])
     us8 = sum(s["us_a8"] for s in r["per_shape"])
     usn = sum(s["us_naive"] for s in r["per_shape"])
+    usg = sum(s["us_group"] for s in r["per_shape"])
     extra = {"w4a8_time_over_w4a4": us8 / us,
+             "group128_time_over_per_token": usg / us,
+             "group128_note": "mq_gemm_group (per-group activation scales, group 128, P:441; dp4a for M <= 2, mma.sync above) "
+                              "over the per-token fused tcgen05 kernel, same launches",
              "naive3_time_over_fused": usn / us,
              "naive3_note": "the paper's naive pipeline (dense GEMM, separate sparse-block GEMM, reduce-add: mq_gemm_naive) "
                             "over the fused kernel, same launches; paper: 1.9x on RTX 4090 for Qwen3-8B V-proj (Fig.3)",
