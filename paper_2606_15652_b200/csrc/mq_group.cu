@@ -217,8 +217,14 @@ __global__ void __launch_bounds__(BN) gemm_group_kernel(const GParams p) {
 // A fragment = weights, B fragment = tokens.  Both sides expand word j of a 16-byte chunk (8 nibbles) into
 // {even nibbles, odd nibbles} x 16 in int8 and place them in the same K slots, so the K permutation cancels and
 // the accumulator is 256 x the exact dot product.
-constexpr int TOKC = 64;
+constexpr int TOKC = 32;
 constexpr int MMA_THREADS = 256;
+// shared-memory ring (cp.async, 16-byte copies): per stage the K-step's base tile (8 KB, layout as in HBM), its present
+// residual quarters (<= 8 KB, compacted as in HBM) and the CTA's TOKC x 64 B of activation codes (16-byte chunks
+// XOR-swizzled by token pair so that the 8-token fragment loads hit 32 distinct banks)
+constexpr int MMA_STAGES = 4;
+constexpr int ST_BASE = 0, ST_RES = TILE_BYTES, ST_ACT = 2 * TILE_BYTES, STAGE_BYTES = 2 * TILE_BYTES + TOKC * 64;
+constexpr int MMA_SMEM = MMA_STAGES * STAGE_BYTES;
 
 __device__ __forceinline__ void mma_s8(int (&d)[4], const uint32_t a0, const uint32_t a1, const uint32_t a2, const uint32_t a3,
                                        const uint32_t b0, const uint32_t b1) {
@@ -226,72 +232,117 @@ __device__ __forceinline__ void mma_s8(int (&d)[4], const uint32_t a0, const uin
                : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
                : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
 
 template <int GROUP, bool BF16>
-__global__ void __launch_bounds__(MMA_THREADS) gemm_group_mma_kernel(const GParams p) {
+__global__ void __launch_bounds__(MMA_THREADS, 2) gemm_group_mma_kernel(const GParams p) {
+  extern __shared__ __align__(128) uint8_t g_smem[];
+  __shared__ int s_mask[MMA_STAGES];
   mq::ptx::griddep_launch();
   mq::ptx::griddep_wait();
   constexpr uint32_t HI = 0xF0F0F0F0u;
   constexpr int CPG = GROUP / 32, GPS = 4 / CPG, NST = TOKC / 8;
-  const int nt = blockIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31, gq = lane >> 2, tq = lane & 3;
+  const int tid = threadIdx.x;
+  const int nt = blockIdx.x, warp = tid >> 5, lane = tid & 31, gq = lane >> 2, tq = lane & 3;
   const int rhalf = warp >> 2;
   const int r0 = warp * 16 + gq, r1 = r0 + 8;                  // rows of the n-tile this thread's accumulators hold
   const int64_t n0 = (int64_t)nt * BN + r0, n1 = n0 + 8;
   const int64_t m0 = (int64_t)blockIdx.y * TOKC;
   const int nst = (int)min((int64_t)NST, (p.M - m0 + 7) / 8);
   const int k0 = (int)blockIdx.z * p.ks_per_split, k1 = min(p.KS, k0 + p.ks_per_split);
+  const int nk = max(0, k1 - k0);
   const int G = (int)(p.K / GROUP);
   const float sw0 = __ldg(p.sw + n0), sw1 = __ldg(p.sw + n1), sr0 = __ldg(p.sr + n0), sr1 = __ldg(p.sr + n1);
+  const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(g_smem);
+  const int2* umeta = p.unit_meta ? reinterpret_cast<const int2*>(p.unit_meta) + (size_t)nt * p.KS : nullptr;
   float y[NST][4];
 #pragma unroll
   for (int st = 0; st < NST; ++st)
 #pragma unroll
     for (int i = 0; i < 4; ++i) y[st][i] = 0.f;
 
-  for (int ks = k0; ks < k1; ++ks) {
-    const uint8_t* tile = p.base + ((size_t)nt * p.KS + ks) * TILE_BYTES + (size_t)tq * 4;
+  // one K-step into one stage; every thread issues its share and the caller commits the group
+  auto issue = [&](int ks, int stage, int2 um) {
+    const uint32_t sb = smem0 + stage * STAGE_BYTES;
+    const uint8_t* src = p.base + ((size_t)nt * p.KS + ks) * TILE_BYTES;
+#pragma unroll
+    for (int i = 0; i < TILE_BYTES / 16 / MMA_THREADS; ++i) cp_async16(sb + ST_BASE + (tid + i * MMA_THREADS) * 16, src + (size_t)(tid + i * MMA_THREADS) * 16);
+    const int mask = um.x & 0xF;
+    const int nchunk = __popc(mask) * (QUARTER_BYTES / 16);
+    const uint8_t* rsrc = p.res + (size_t)um.y * QUARTER_BYTES;
+    for (int i = tid; i < nchunk; i += MMA_THREADS) cp_async16(sb + ST_RES + i * 16, rsrc + (size_t)i * 16);
+    if (tid < TOKC * 4) {
+      const int t = tid >> 2, c = tid & 3;
+      if (m0 + t < p.M)
+        cp_async16(sb + ST_ACT + t * 64 + ((c ^ (t >> 1)) & 3) * 16,
+                   p.qA + (size_t)(m0 + t) * (size_t)(p.K / 2) + (size_t)ks * (BK / 2) + c * 16);
+    }
+    if (tid == 0) s_mask[stage] = mask;
+  };
+  auto meta = [&](int ks) { return umeta ? __ldg(umeta + ks) : make_int2(0, 0); };
+
+#pragma unroll
+  for (int i = 0; i < MMA_STAGES - 1; ++i) {
+    if (i < nk) issue(k0 + i, i, meta(k0 + i));
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  int2 um_next = (MMA_STAGES - 1 < nk) ? meta(k0 + MMA_STAGES - 1) : make_int2(0, 0);
+
+  for (int it = 0; it < nk; ++it) {
+    const int ks = k0 + it, stage = it % MMA_STAGES;
+    asm volatile("cp.async.wait_group %0;" ::"n"(MMA_STAGES - 2) : "memory");
+    __syncthreads();   // K-step `it` has landed for every thread; the stage read at it - 1 is free
+    {
+      const int nx = it + MMA_STAGES - 1;
+      if (nx < nk) issue(k0 + nx, nx % MMA_STAGES, um_next);
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      if (nx + 1 < nk) um_next = meta(k0 + nx + 1);
+    }
+    const uint32_t sb = smem0 + stage * STAGE_BYTES;
+    const int mask = s_mask[stage];
     uint32_t wa[4][4], ra[4][4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
-      const uint32_t x0 = __ldg(reinterpret_cast<const uint32_t*>(tile + c * (BN * 16) + r0 * 16));
-      const uint32_t x1 = __ldg(reinterpret_cast<const uint32_t*>(tile + c * (BN * 16) + r1 * 16));
+      const uint32_t x0 = lds32(sb + ST_BASE + c * (BN * 16) + r0 * 16 + tq * 4);
+      const uint32_t x1 = lds32(sb + ST_BASE + c * (BN * 16) + r1 * 16 + tq * 4);
       wa[c][0] = (x0 << 4) & HI;
       wa[c][1] = (x1 << 4) & HI;
       wa[c][2] = x0 & HI;
       wa[c][3] = x1 & HI;
     }
-    bool has[2] = {false, false};   // warp-uniform: a quarter covers 64 rows = 4 whole warps
-    if (p.unit_meta) {
-      const int2 um = __ldg(reinterpret_cast<const int2*>(p.unit_meta) + (size_t)nt * p.KS + ks);
-      const int mask = um.x & 0xF;
+    bool has[2];   // warp-uniform: a quarter covers 64 rows = 4 whole warps
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int q = 2 * h + rhalf;
-        if (mask & (1 << q)) {
-          has[h] = true;
-          const uint8_t* qp = p.res + ((size_t)um.y + (size_t)__popc(mask & ((1 << q) - 1))) * QUARTER_BYTES + (size_t)tq * 4;
+    for (int h = 0; h < 2; ++h) {
+      const int q = 2 * h + rhalf;
+      has[h] = (mask >> q) & 1;
+      if (has[h]) {
+        const uint32_t qp = sb + ST_RES + __popc(mask & ((1 << q) - 1)) * QUARTER_BYTES + (r0 & 63) * 16 + tq * 4;
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const uint32_t x0 = __ldg(reinterpret_cast<const uint32_t*>(qp + j * 1024 + (r0 & 63) * 16));
-            const uint32_t x1 = __ldg(reinterpret_cast<const uint32_t*>(qp + j * 1024 + (r1 & 63) * 16));
-            ra[2 * h + j][0] = (x0 << 4) & HI;
-            ra[2 * h + j][1] = (x1 << 4) & HI;
-            ra[2 * h + j][2] = x0 & HI;
-            ra[2 * h + j][3] = x1 & HI;
-          }
+        for (int j = 0; j < 2; ++j) {
+          const uint32_t x0 = lds32(qp + j * 1024), x1 = lds32(qp + j * 1024 + 8 * 16);
+          ra[2 * h + j][0] = (x0 << 4) & HI;
+          ra[2 * h + j][1] = (x1 << 4) & HI;
+          ra[2 * h + j][2] = x0 & HI;
+          ra[2 * h + j][3] = x1 & HI;
         }
       }
     }
 #pragma unroll
     for (int st = 0; st < NST; ++st) {
       if (st >= nst) break;
-      const int64_t mb = m0 + 8 * st + gq;            // token of this lane's B fragment
+      const int tb = 8 * st + gq;                          // token (within the CTA) of this lane's B fragment
       const int64_t t0 = m0 + 8 * st + 2 * tq, t1 = t0 + 1;   // tokens of this lane's accumulators
       uint32_t bw[4] = {0, 0, 0, 0};
-      if (mb < p.M) {
-        const uint8_t* ap = p.qA + (size_t)mb * (size_t)(p.K / 2) + (size_t)ks * (BK / 2) + (size_t)tq * 4;
+      if (m0 + tb < p.M) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) bw[c] = __ldg(reinterpret_cast<const uint32_t*>(ap + c * 16));
+        for (int c = 0; c < 4; ++c) bw[c] = lds32(sb + ST_ACT + tb * 64 + ((c ^ (tb >> 1)) & 3) * 16 + tq * 4);
       }
 #pragma unroll
       for (int gi = 0; gi < GPS; ++gi) {
@@ -321,6 +372,7 @@ __global__ void __launch_bounds__(MMA_THREADS) gemm_group_mma_kernel(const GPara
       }
     }
   }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
   for (int st = 0; st < NST; ++st) {
     if (st >= nst) break;
@@ -348,6 +400,12 @@ __global__ void __launch_bounds__(256) group_reduce_kernel(const float* __restri
   float s = 0.f;
   for (int z = 0; z < splits; ++z) s += partial[(size_t)z * M * N + idx];
   store_y16<BF16>(Y, (size_t)m * ldy + n, s);
+}
+
+template <typename Kern>
+void launch_mma(Kern kern, dim3 grid, cudaStream_t st, const GParams& p) {
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, MMA_SMEM);
+  kern<<<grid, MMA_THREADS, MMA_SMEM, st>>>(p);
 }
 
 bool group_use_simt(int64_t M) { return M <= 2 || mq::options().group_simt != 0; }
@@ -454,8 +512,8 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
       if (bf) gemm_group_kernel<GR, true><<<grid, BN, 0, st>>>(p);                       \
       else gemm_group_kernel<GR, false><<<grid, BN, 0, st>>>(p);                         \
     } else {                                                                             \
-      if (bf) gemm_group_mma_kernel<GR, true><<<grid, MMA_THREADS, 0, st>>>(p);          \
-      else gemm_group_mma_kernel<GR, false><<<grid, MMA_THREADS, 0, st>>>(p);            \
+      if (bf) launch_mma(gemm_group_mma_kernel<GR, true>, grid, st, p);                  \
+      else launch_mma(gemm_group_mma_kernel<GR, false>, grid, st, p);                    \
     }                                                                                    \
   } while (0)
   if (group == 32) MQ_LAUNCH_G(32);
