@@ -241,7 +241,7 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
   return v;
 }
 
-template <int GROUP, bool BF16>
+template <int GROUP, bool BF16, bool DBG>
 __global__ void __launch_bounds__(MMA_THREADS, 2) gemm_group_mma_kernel(const GParams p) {
   extern __shared__ __align__(128) uint8_t g_smem[];
   __shared__ int s_mask[MMA_STAGES];
@@ -259,7 +259,17 @@ __global__ void __launch_bounds__(MMA_THREADS, 2) gemm_group_mma_kernel(const GP
   const int k0 = (int)blockIdx.z * p.ks_per_split, k1 = min(p.KS, k0 + p.ks_per_split);
   const int nk = max(0, k1 - k0);
   const int G = (int)(p.K / GROUP);
-  const float sw0 = __ldg(p.sw + n0), sw1 = __ldg(p.sw + n1), sr0 = __ldg(p.sr + n0), sr1 = __ldg(p.sr + n1);
+  // the accumulators are 256 x the sums: the scales take the 2^-8 (exact), which saves the shifts
+  const float sw0 = __ldg(p.sw + n0) * 0.00390625f, sw1 = __ldg(p.sw + n1) * 0.00390625f;
+  const float sr0 = __ldg(p.sr + n0) * 0.00390625f, sr1 = __ldg(p.sr + n1) * 0.00390625f;
+  const float* sa_cta = p.sa + (size_t)m0 * G;      // token t of the CTA, group g: sa_cta[t * G + g]
+  const int tq2G = 2 * tq * G;
+  uint32_t okmask = 0;                              // bit 2 st + j: token m0 + 8 st + 2 tq + j exists
+#pragma unroll
+  for (int st = 0; st < NST; ++st)
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+      if (m0 + 8 * st + 2 * tq + j < p.M) okmask |= 1u << (2 * st + j);
   const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(g_smem);
   const int2* umeta = p.unit_meta ? reinterpret_cast<const int2*>(p.unit_meta) + (size_t)nt * p.KS : nullptr;
   float y[NST][4];
@@ -355,18 +365,22 @@ __global__ void __launch_bounds__(MMA_THREADS, 2) gemm_group_mma_kernel(const GP
           if (has[c >> 1]) mma_s8(d1, ra[c][0], ra[c][1], ra[c][2], ra[c][3], b0, b1);
         }
         const int g = ks * GPS + gi;
-        const float s_t0 = t0 < p.M ? __ldg(p.sa + (size_t)t0 * G + g) : 0.f;
-        const float s_t1 = t1 < p.M ? __ldg(p.sa + (size_t)t1 * G + g) : 0.f;
-        // accumulator i: (row r0, t0), (r0, t1), (r1, t0), (r1, t1); sums are multiples of 256, the shift is exact
+        const int i0 = st * 8 * G + tq2G + g;
+        const float s_t0 = (okmask >> (2 * st)) & 1 ? __ldg(sa_cta + i0) : 0.f;
+        const float s_t1 = (okmask >> (2 * st + 1)) & 1 ? __ldg(sa_cta + i0 + G) : 0.f;
+        // accumulator i: (row r0, t0), (r0, t1), (r1, t0), (r1, t1); |d| <= 256 * 49 * 128 < 2^24: exact in fp32
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const int a0 = d0[i] >> 8, a1 = d1[i] >> 8;
           const float swv = i < 2 ? sw0 : sw1, srv = i < 2 ? sr0 : sr1, sav = (i & 1) ? s_t1 : s_t0;
-          y[st][i] += sav * (swv * (float)a0 + srv * (float)a1);
-          const int64_t t = (i & 1) ? t1 : t0, n = i < 2 ? n0 : n1;
-          if (t < p.M) {
-            if (p.dbg0) p.dbg0[((size_t)g * p.M + t) * p.N + n] = a0;
-            if (p.dbg1) p.dbg1[((size_t)g * p.M + t) * p.N + n] = a1;
+          float term = swv * (float)d0[i];
+          if (has[(gi * CPG) >> 1] || has[(gi * CPG + CPG - 1) >> 1]) term = fmaf(srv, (float)d1[i], term);
+          y[st][i] = fmaf(sav, term, y[st][i]);
+          if (DBG) {
+            const int64_t t = (i & 1) ? t1 : t0, n = i < 2 ? n0 : n1;
+            if (t < p.M) {
+              if (p.dbg0) p.dbg0[((size_t)g * p.M + t) * p.N + n] = d0[i] >> 8;
+              if (p.dbg1) p.dbg1[((size_t)g * p.M + t) * p.N + n] = d1[i] >> 8;
+            }
           }
         }
       }
@@ -512,8 +526,13 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
       if (bf) gemm_group_kernel<GR, true><<<grid, BN, 0, st>>>(p);                       \
       else gemm_group_kernel<GR, false><<<grid, BN, 0, st>>>(p);                         \
     } else {                                                                             \
-      if (bf) launch_mma(gemm_group_mma_kernel<GR, true>, grid, st, p);                  \
-      else launch_mma(gemm_group_mma_kernel<GR, false>, grid, st, p);                    \
+      if (dbg0 || dbg1) {                                                                \
+        if (bf) launch_mma(gemm_group_mma_kernel<GR, true, true>, grid, st, p);          \
+        else launch_mma(gemm_group_mma_kernel<GR, false, true>, grid, st, p);            \
+      } else {                                                                           \
+        if (bf) launch_mma(gemm_group_mma_kernel<GR, true, false>, grid, st, p);         \
+        else launch_mma(gemm_group_mma_kernel<GR, false, false>, grid, st, p);           \
+      }                                                                                  \
     }                                                                                    \
   } while (0)
   if (group == 32) MQ_LAUNCH_G(32);
