@@ -369,7 +369,7 @@ def roofline_of(r, peaks, traffic):
     usg = sum(s["us_group"] for s in r["per_shape"])
     extra = {"w4a8_time_over_w4a4": us8 / us,
              "group128_time_over_per_token": usg / us,
-             "group128_note": "mq_gemm_group (per-group activation scales, group 128, P:441; dp4a for M <= 2, mma.sync above) "
+             "group128_note": "mq_gemm_group (per-group activation scales, group 128, P:441; mma.sync kernel) "
                               "over the per-token fused tcgen05 kernel, same launches",
              "naive3_time_over_fused": usn / us,
              "naive3_note": "the paper's naive pipeline (dense GEMM, separate sparse-block GEMM, reduce-add: mq_gemm_naive) "

@@ -182,7 +182,7 @@ int mq_gemm_naive(const mq_weights* w, const void* qA_dev, const float* sA_dev, 
  * residual codes; the group terms are added in fp32 in ascending g (K-split partial sums in ascending split), then
  * rounded once to y_dtype.  Parity hooks: dbg_acc_base_g_dev / dbg_acc_res_g_dev int32 [K/group][M][N] or NULL.
  * workspace_dev: mq_gemm_group_workspace_bytes(w, M) bytes (may be 0), 16-byte aligned, no initial content
- * required.  A first SIMT (dp4a) path, one or two launches; M <= 16 * 65535.  Errors as mq_gemm. */
+ * required.  A first path (warp-level mma.sync on a cp.async shared-memory ring, not the tcgen05 kernel), one or two launches; M <= 16 * 65535.  Errors as mq_gemm. */
 int mq_quantize_act_group(const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda_elems, int group,
                           void* qA_dev, float* sA_dev, void* cuda_stream);
 size_t mq_gemm_group_workspace_bytes(const mq_weights* w, int64_t M);
@@ -220,7 +220,7 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
  *   "token_tile": 0 = automatic, else 16/32/64/128
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
  *   "fused_quant": 0 (default) / 1: see mq_linear
- *   "group_simt": 0 (default) = mq_gemm_group uses its tensor-core kernel for M > 2; 1 = the dp4a kernel for every M
+ *   "group_simt": 0 (default) = mq_gemm_group uses its tensor-core (mma.sync) kernel; 1 = its dp4a kernel (ablation)
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
  *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */

@@ -10,7 +10,8 @@
 //   mq_gemm_group         : Eq.2 / Eq.4 per group:
 //                             Y[m,n] = sum_g s_a[m,g] (s_w[n] acc0_g[m,n] + s_r[n] acc1_g[m,n])
 //                           The integer partial sums cannot cross a group boundary, so the fused tcgen05 kernel's
-//                           single int32 accumulator per output does not apply; this FIRST path is SIMT: one
+//                           single int32 accumulator per output does not apply.  Two kernels.  The first one written is SIMT (option
+//                           group_simt; kept as the ablation): one
 //                           thread per output channel, dp4a over the packed nibbles of the same device layout
 //                           (base tiles + residual quarters, mq_internal.h), exact int32 per (group, token,
 //                           channel), rescaled and added in fp32 after every group.  The residual quarters of a
@@ -32,6 +33,8 @@ namespace {
 constexpr int GT = 256;    // threads per CTA of the quantizer
 constexpr int TOK = 16;    // tokens per CTA of the GEMM
 constexpr int TARGET_CTAS = 296;   // 2 x 148 SMs
+constexpr int SIMT_MAX_M = 0;      // largest M served by the dp4a kernel by default (0: option group_simt only; measured:
+                                   // the tensor-core kernel is level at M = 1 and 1.3-4 x faster from M = 2)
 
 template <bool BF16>
 __device__ __forceinline__ void cvt8g(const uint4& v, float* f) {
@@ -210,7 +213,7 @@ __global__ void __launch_bounds__(BN) gemm_group_kernel(const GParams p) {
 }
 
 
-// ---- tensor-core path (M > 2): legacy warp-level mma.sync m16n8k32 s8 -- a group boundary every 32..128 channels
+// ---- tensor-core path (default for every M): legacy warp-level mma.sync m16n8k32 s8 -- a group boundary every 32..128 channels
 // means the int32 sums must leave the accumulator after at most one K-step, which a TMEM-resident tcgen05
 // accumulator makes expensive (a tcgen05.ld drain per group); warp-level fragments are already in registers.
 // 8 warps, warp v = output channels 16 v .. 16 v + 15 of the n-tile, TOKC tokens per CTA in sub-tiles of 8.
@@ -422,14 +425,15 @@ void launch_mma(Kern kern, dim3 grid, cudaStream_t st, const GParams& p) {
   kern<<<grid, MMA_THREADS, MMA_SMEM, st>>>(p);
 }
 
-bool group_use_simt(int64_t M) { return M <= 2 || mq::options().group_simt != 0; }
+bool group_use_simt(int64_t M) { return M <= SIMT_MAX_M || mq::options().group_simt != 0; }
 
 int group_splits(const mq_weights* w, int64_t M) {
   const int tok = group_use_simt(M) ? TOK : TOKC;
   const int64_t ctas = (w->N / BN) * ((M + tok - 1) / tok);
   const int64_t KS = w->K / BK;
   if (ctas >= TARGET_CTAS) return 1;
-  return (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(KS, 32), (TARGET_CTAS + ctas - 1) / ctas));
+  // at least 4 K-steps per split: a CTA's ring must fill before it pays off
+  return (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(std::max<int64_t>(KS / 4, 1), 32), (TARGET_CTAS + ctas - 1) / ctas));
 }
 
 bool group_ok(int group) { return group == 32 || group == 64 || group == 128; }

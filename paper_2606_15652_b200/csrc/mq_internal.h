@@ -74,7 +74,7 @@ struct Options {
   int64_t max_ctas = 0;
   int64_t fused_quant = 0;   // mq_linear with M <= 8: quantize the activations inside the GEMM kernel (slower than
                              // the PDL-chained two-kernel path on B200; off by default)
-  int64_t group_simt = 0;    // mq_gemm_group: 1 = the dp4a kernel for every M (default: M <= 2 only; tensor cores above)
+  int64_t group_simt = 0;    // mq_gemm_group: 1 = the dp4a kernel (ablation); 0 = the mma.sync kernel
   int64_t pdl = 1;   // launch kernels as programmatic dependents of their predecessor in the stream
 };
 Options& options();

@@ -92,9 +92,9 @@ def test_group_parity_small(mq, M, K, N, bs, rho, dt, group):
     check(got, want, group, K, out, f"group {group} M{M} K{K} N{N} bs{bs} {out}")
 
 
-@pytest.mark.parametrize("M,K,N,bs,rho,dt", [SHAPES[0], SHAPES[3], SHAPES[4], SHAPES[8]])
+@pytest.mark.parametrize("M,K,N,bs,rho,dt", [SHAPES[0], SHAPES[1], SHAPES[3], SHAPES[4], SHAPES[8]])
 def test_group_parity_simt_kernel_every_m(mq, M, K, N, bs, rho, dt):
-    """Option group_simt = 1: the dp4a kernel (default for M <= 2 only) on multi-token shapes."""
+    """Option group_simt = 1: the dp4a kernel (not used by default) on single- and multi-token shapes."""
     case = make_case(1200 + M, M, K, N, bs=bs, rho=rho, budget=2 if rho is None else None, a_dtype=dt)
     w = pack_from_oracle(case)
     try:
