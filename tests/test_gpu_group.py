@@ -138,7 +138,7 @@ def test_group_budget_zero_and_whole_row_group(mq):
 
 def test_group_empty_and_errors(mq):
     import torch
-    case = make_case(1400, 4, 512, 256, bs=64, rho=0.1)
+    case = make_case(1400, 4, 2048, 256, bs=64, rho=0.1)    # 16 K-steps, 2 CTAs: the K-split is on
     w = pack_from_oracle(case)
     A = to_device_act(case)
     for bad in (0, 16, 48, 256):
