@@ -3,18 +3,20 @@
     python -m paper_2606_15652_b200.build [--force]
 
 nvcc cross-compiles without a GPU.  The .so lands next to this file and is git-ignored
-(it still travels to the GPU box with the repo snapshot).
+(it still travels to the GPU box with the repo snapshot).  Translation units are compiled
+in parallel and only when they (or a shared header) changed.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libmq.so")
-SOURCES = ["mq_quant.cu", "mq_pack.cu", "mq_gemm.cu", "mq_group.cu"]
+SOURCES = ["mq_quant.cu", "mq_pack.cu", "mq_gemm.cu", "mq_group.cu", "mq_decode.cu", "mq_select.cu"]
 HEADERS = ["mq_internal.h", "mq_ptx.cuh", os.path.join("..", "..", "include", "mq.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
@@ -25,32 +27,35 @@ FLAGS = [
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(OUT):
-        return True
-    t = os.path.getmtime(OUT)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+def _mtime(path: str) -> float:
+    return os.path.getmtime(path) if os.path.exists(path) else 0.0
+
+
+def _compile(src: str, verbose: bool) -> str:
+    o = os.path.join(CSRC, src.replace(".cu", ".o"))
+    cmd = [NVCC, *FLAGS, "-c", os.path.join(CSRC, src), "-o", o]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+    if r.returncode != 0:
+        raise RuntimeError(f"nvcc failed on {src}")
+    return o
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
-        return OUT
-    objs = []
-    for s in SOURCES:
-        o = os.path.join(CSRC, s.replace(".cu", ".o"))
-        cmd = [NVCC, *FLAGS, "-c", os.path.join(CSRC, s), "-o", o]
-        r = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or r.returncode != 0:
-            sys.stderr.write(r.stdout + r.stderr)
+    sources = [s for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
+    common = max([_mtime(os.path.join(CSRC, h)) for h in HEADERS] + [_mtime(os.path.abspath(__file__))])
+    objs = [os.path.join(CSRC, s.replace(".cu", ".o")) for s in sources]
+    stale = [s for s, o in zip(sources, objs)
+             if force or _mtime(o) < max(common, _mtime(os.path.join(CSRC, s)))]
+    if stale:
+        with ThreadPoolExecutor(max_workers=min(len(stale), os.cpu_count() or 4)) as ex:
+            list(ex.map(lambda s: _compile(s, verbose), stale))
+    if stale or _mtime(OUT) < max(_mtime(o) for o in objs):
+        r = subprocess.run([NVCC, "-shared", "-o", OUT, *objs, "-lpthread"], capture_output=True, text=True)
         if r.returncode != 0:
-            raise RuntimeError(f"nvcc failed on {s}")
-        objs.append(o)
-    cmd = [NVCC, "-shared", "-o", OUT, *objs, "-lpthread"]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        sys.stderr.write(r.stdout + r.stderr)
-        raise RuntimeError("link failed")
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError("link failed")
     return OUT
 
 

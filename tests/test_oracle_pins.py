@@ -76,6 +76,112 @@ def test_o1_ties_on_fp16_grid_round_half_even():
     assert q.tolist() == want
 
 
+# ---- O1's per-element quotient, pinned in exact rational arithmetic (Eq.1, reading A3) --------------
+def _rne_int(t: Fraction) -> int:
+    """Round a rational to the nearest integer, halves to even."""
+    f = t.numerator // t.denominator
+    r = t - f
+    if r > Fraction(1, 2) or (r == Fraction(1, 2) and f % 2 == 1):
+        f += 1
+    return f
+
+
+def _round_to_binary32(t: Fraction) -> Fraction:
+    """The IEEE-754 binary32 value nearest to the rational t (ties to even), as an exact rational.
+    Written out by hand: scale to a 24-bit integer significand, round half to even, scale back."""
+    if t == 0:
+        return Fraction(0)
+    sign, a = (-1 if t < 0 else 1), abs(t)
+    e = a.numerator.bit_length() - a.denominator.bit_length()      # 2^(e-1) < a < 2^(e+1)
+    if Fraction(2) ** e > a:
+        e -= 1                                                      # now 2^e <= a < 2^(e+1)
+    e = max(e, -126)                                                # subnormals share the exponent -126
+    ulp = Fraction(2) ** (e - 23)
+    m = _rne_int(a / ulp)                                           # 2^23 <= m <= 2^24 (or < 2^23: subnormal)
+    assert e + 1 <= 127
+    return sign * m * ulp
+
+
+def _expected_code(x: float, s: float, qmax: int) -> int:
+    """Eq.1 as reading A3 fixes it: q = clamp(RNE(fl32(x / s)))."""
+    t32 = _round_to_binary32(Fraction(x) / Fraction(s))
+    return max(-qmax, min(qmax, _rne_int(t32)))
+
+
+def _code_with_reciprocal(x: float, s: float, qmax: int) -> int:
+    """What `x * (1.0f / s)` would give (the mutation this pin must catch): two roundings."""
+    r32 = _round_to_binary32(Fraction(1) / Fraction(s))
+    t32 = _round_to_binary32(Fraction(x) * r32)
+    return max(-qmax, min(qmax, _rne_int(t32)))
+
+
+@pytest.mark.parametrize("bits", [4, 8])
+def test_o1_quotient_is_one_correctly_rounded_binary32_division(bits):
+    """Reading A3 of Eq.1: x / s is ONE IEEE binary32 division, then round half to even.  Rows are
+    built next to the ties (k + 1/2) * s for scales that are not powers of two, where a product with the
+    reciprocal of s lands on the other side of the tie; the expected codes come from exact rationals with
+    the binary32 rounding written out by hand (no floating-point division anywhere on the expected side).
+    The test also counts the elements on which `x * (1.0f / s)` would differ: the pin is only a pin if
+    that count is positive."""
+    qmax = 7 if bits == 4 else 127
+    rng = np.random.default_rng(40 + bits)
+    flips = 0
+    for amax in [5.0, 0.3, 1234.0, 2.2, 6.0e-5, 3.3, 0.0417, 97.0]:
+        amax32 = np.float32(amax)
+        s = float(_round_to_binary32(Fraction(float(amax32)) / qmax))          # the scale, by hand as well
+        ks = rng.integers(-qmax, qmax, size=96)
+        xs = [float(amax32)]
+        for k in ks:
+            centre = np.float32(float(_round_to_binary32((Fraction(int(k)) + Fraction(1, 2)) * Fraction(s))))
+            v = centre
+            for _ in range(3):                                                  # fp32 neighbours on both sides
+                v = np.nextafter(v, np.float32(-np.inf))
+            for _ in range(7):
+                if abs(float(v)) <= float(amax32):
+                    xs.append(float(v))
+                v = np.nextafter(v, np.float32(np.inf))
+        x = np.array(xs, np.float32)
+        q, s_got = oracle.quantize_row(x, bits=bits)
+        assert float(s_got) == s
+        want = [_expected_code(float(v), s, qmax) for v in x]
+        assert q.tolist() == want, f"amax {amax}: codes differ from the exactly rounded quotient"
+        flips += sum(1 for v, w in zip(x, want) if _code_with_reciprocal(float(v), s, qmax) != w)
+    assert flips > 0, "the rows no longer discriminate a division from a reciprocal product"
+
+
+@pytest.mark.parametrize("dt", ["f16", "bf16"])
+def test_o2_near_ties_on_16bit_grids_match_exact_rationals(dt):
+    """The same pin through O2 (per-token activations) on 16-bit inputs: the fp16 / bf16 neighbours
+    of (k + 1/2) * s for non-power-of-two scales, expected codes from exact rationals."""
+    rng = np.random.default_rng(44)
+    K, rows = 256, []
+    for amax in [5.0, 0.3, 1234.0, 2.2, 3.3, 97.0]:
+        if dt == "f16":
+            a16 = float(np.float16(amax))
+        else:
+            a16 = float((np.array([amax], np.float32).view(np.uint32) & 0xFFFF0000).view(np.float32)[0])
+        s = float(_round_to_binary32(Fraction(a16) / 7))
+        x = (rng.integers(-7, 7, size=K).astype(np.float64) + 0.5) * s
+        if dt == "f16":
+            nb = x.astype(np.float16).view(np.int16) + rng.integers(-2, 3, size=K).astype(np.int16)
+            row = nb.view(np.float16).copy()
+            row[0] = np.float16(a16)
+            row = np.where(np.abs(row.astype(np.float32)) <= a16, row, np.float16(0)).view(np.uint16)
+            vals = row.view(np.float16).astype(np.float64)
+        else:
+            b = (x.astype(np.float32).view(np.uint32) >> 16).astype(np.uint16) + rng.integers(0, 3, size=K).astype(np.uint16)
+            b[0] = np.uint16(np.array([a16], np.float32).view(np.uint32)[0] >> 16)
+            f = (b.astype(np.uint32) << 16).view(np.float32)
+            row = np.where(np.abs(f) <= a16, b, np.uint16(0)).astype(np.uint16)
+            vals = (row.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+        rows.append((row, vals, s))
+    bits16 = np.stack([r[0] for r in rows])
+    qa, sa = oracle.quantize_act(bits16.view(np.float16) if dt == "f16" else (bits16, "bf16"))
+    for i, (_, vals, s) in enumerate(rows):
+        assert float(sa[i]) == s
+        assert qa[i].tolist() == [_expected_code(float(v), s, 7) for v in vals]
+
+
 def test_o1_8bit_activations_w4a8():
     """The W4A8 variant (Table 1 W4A8 rows): the same quantizer with q_max = 127.  Hand vector
     (tests/golden/o1_hand_vector_8bit.txt), correctly rounded scale, nearest code, no clipping, symmetry,
@@ -367,3 +473,10 @@ def test_golden_config1_digest(tiny_case):
                acc1=dig(r["acc1"].astype(np.int32)), qw=dig(L.d.qw), qr=dig(L.d.qr),
                blocks=sorted((L.blk_n.astype(int) * 4 + L.blk_k).tolist()))
     assert got == {k: g[k] for k in got}
+
+
+def test_forward_timed_is_the_three_steps_in_sequence(tiny_case):
+    """bench.py times oracle.forward_timed (O2 + O8 + O9 through one C call); it must return exactly what
+    the three separately pinned steps return."""
+    Y = oracle.forward_timed(tiny_case["A"], tiny_case["L"])
+    assert np.array_equal(Y, oracle.forward(tiny_case["A"], tiny_case["L"])["Y"])
