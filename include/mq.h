@@ -128,12 +128,16 @@ void mq_weights_free(mq_weights* w);
  *   Y_dev          : [M,N] fp16/bf16 row-major, `ldy_elems` elements between rows.
  *   dbg_acc_base_dev / dbg_acc_res_dev : optional int32 [M,N] row-major (stride N), 16-byte
  *                    aligned; when non-NULL they receive acc0 / acc1 exactly (parity hooks).
- *   workspace_dev  : at least mq_gemm_workspace_bytes(w, M) bytes, 16-byte aligned; must be
- *                    all-zero before the FIRST call that uses it; afterwards its contents are
- *                    library-private and stay valid from call to call (per-tile counters,
- *                    which every call returns to zero, and int32 partial tiles of the
- *                    stream-K fix-up).  Calls that may run concurrently need distinct
- *                    workspaces.
+ *   workspace_dev  : at least mq_gemm_workspace_bytes(w, M) bytes, 16-byte aligned.  Contract: its first
+ *                    16384 bytes must be ZERO before the first call that uses it (cudaMemset once); they
+ *                    hold the per-tile arrival counters of the split-K fix-up at positions that do not
+ *                    depend on the layer shape, M or the options, and every call returns them to zero.
+ *                    Everything behind those 16 KB (int32 partial tiles, flags) is written before it is
+ *                    read and needs no initial content.  One workspace of the largest size may therefore
+ *                    be shared by calls of different layers, M and options, as long as those calls do not
+ *                    run concurrently (same stream, or otherwise ordered); concurrent calls need distinct
+ *                    workspaces.  An asynchronous fault inside a call leaves the counters undefined:
+ *                    zero the prefix again before re-use.
  * M == 0 is a no-op.
  */
 size_t mq_gemm_workspace_bytes(const mq_weights* w, int64_t M);
@@ -195,9 +199,9 @@ int mq_gemm_group(const mq_weights* w, const void* qA_dev, const float* sA_dev, 
  * chained by programmatic dependent launch).  With option "fused_quant" = 1 and M <= 8 the quantizer runs
  * inside the GEMM kernel (north_star (i) "optionally fused into the GEMM prologue"): one
  * launch, bit-identical Y; the per-token absmax is found with a grid-wide atomic max, the tokens of each
- * K-step are quantized from a TMA-staged raw tile.  Workspace: mq_linear_workspace_bytes(w, M), all-zero
- * before the first call (it carries the GEMM's counters and the fused path's absmax control block, which
- * every call returns to zero). */
+ * K-step are quantized from a TMA-staged raw tile.  Workspace: mq_linear_workspace_bytes(w, M), 256-byte aligned,
+ * same contract as mq_gemm's (first 16384 bytes zero before the first use: the GEMM's counters and the fused
+ * path's absmax control block, which every call returns to zero; the packed activations live behind them). */
 size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M);
 int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t lda_elems,
               void* Y_dev, mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev,
@@ -214,13 +218,22 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
                    mq_dtype y_dtype, void* staging_dev, size_t staging_bytes, void* workspace_dev,
                    size_t workspace_bytes, void* cuda_stream);
 
-/* Tuning / ablation knobs (process-wide, not thread-safe; for benchmarks and tests).
+/* Tuning / ablation knobs.  They are PROCESS-WIDE globals read at call time without locking: set them while no
+ * other thread is inside a library call (benchmarks and tests do; a serving process leaves the defaults).  The
+ * compute calls themselves keep no other mutable state and may be issued from several threads on distinct
+ * streams and workspaces; mq_last_launch_count is a diagnostic of the calling process, not synchronised.
  *   "split_k"   : 0 = automatic, 1 = whole output tiles per CTA, >= 2 = stream-K (the K-steps of
  *                 all tiles cut into equal per-CTA ranges, shared tiles finished by the last arriver)
  *   "token_tile": 0 = automatic, else 16/32/64/128
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
  *   "fused_quant": 0 (default) / 1: see mq_linear
  *   "group_simt": 0 (default) = mq_gemm_group uses its tensor-core (mma.sync) kernel; 1 = its dp4a kernel (ablation)
+ *   "decode_path": 0 (default) = mq_gemm with M <= 32 runs the lean decode kernel (row slabs: a CTA owns 16..128
+ *                 output channels and all of K; TMA ring + mma.sync straight from the packed tiles, no tensor
+ *                 memory, no workspace); 1 = the tcgen05 kernel for every M.  Setting "token_tile", "split_k" >= 2,
+ *                 "max_ctas" or "fused_quant" also selects the tcgen05 kernel.
+ *   "decode_rows": 0 = automatic, else 16 / 32 / 64 / 128 output channels per CTA of the decode kernel
+ *   "decode_big": 0 = automatic, 1 = deep shared-memory ring (one CTA per SM; rows <= 64), 2 = small ring (two per SM)
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
  *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */

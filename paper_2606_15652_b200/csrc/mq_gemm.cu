@@ -38,9 +38,13 @@
 //
 // Work distribution ("stream-K"): the K-steps of all output tiles form one sequence that is
 // cut into gridDim.x equal contiguous ranges, so every SM streams the same number of weight
-// bytes whatever N is.  A tile whose K range is shared by several CTAs is finished by the
-// last of them to arrive: each writes its int32 partial tile to a private workspace slot
-// (plain coalesced stores, integer adds are exact so the result stays bit-identical).
+// bytes whatever N is.  A tile whose K range is shared by S CTAs: each writes its int32 partial
+// tile to a private workspace slot (plain coalesced stores, integer adds are exact so the result
+// stays bit-identical), waits until all S partials are visible and finishes 1/S of the tile.  The
+// wait needs the S contributors co-resident (grid <= SM count, one CTA per SM): an environment that
+// exposes fewer SMs than cudaDevAttrMultiProcessorCount (MPS active-thread percentage, green contexts)
+// must run this kernel with option split_k = 1 (whole tiles, nothing waits).  Decode shapes (M <= 32)
+// do not come here by default: mq_decode.cu serves them with a ticket scheme in which nobody waits.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
@@ -1231,7 +1235,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           if (++spins > (1u << 24)) __trap();
         } while (seen < S);
       }
-      // residual flags of the contributors (bit c - c_lo); S <= 32 in practice, else treat all as set
+      // residual flags of the contributors (bit c - c_lo) for S <= 32; beyond that each flag is read in the loop
+      // (a contributor without residual MMAs never wrote its part1 slot: it must not be added)
       uint32_t fm = 0xffffffffu;
       if (!kBothParts && S <= 32) {
         int f = 0;
@@ -1249,7 +1254,9 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           const int32_t* q0 = p.ws_part + ((size_t)c * 2 + (c == c_lo ? lo_slot : 0)) * (2 * PART) + t * BN + n0;
           const int4 a = __ldcg(reinterpret_cast<const int4*>(q0));
           int4 b = make_int4(0, 0, 0, 0);
-          if (kBothParts || ((fm >> ((c - c_lo) & 31)) & 1u)) b = __ldcg(reinterpret_cast<const int4*>(q0 + PART));
+          const bool has1 = kBothParts || (S <= 32 ? ((fm >> ((c - c_lo) & 31)) & 1u) != 0
+                                                   : __ldcg(p.ws_flag + c * 2 + (c == c_lo ? lo_slot : 0)) != 0);
+          if (has1) b = __ldcg(reinterpret_cast<const int4*>(q0 + PART));
           s0.x += a.x; s0.y += a.y; s0.z += a.z; s0.w += a.w;
           s1.x += b.x; s1.y += b.y; s1.z += b.z; s1.w += b.w;
         }
@@ -1331,6 +1338,12 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 EncodeTiledFn get_encode_fn() {
+  return (EncodeTiledFn)mq::tensor_map_encode_fn();
+}
+
+}  // namespace
+
+void* mq::tensor_map_encode_fn() {
   static EncodeTiledFn fn = nullptr;
   static bool tried = false;
   if (!tried) {
@@ -1343,8 +1356,10 @@ EncodeTiledFn get_encode_fn() {
     else
       cudaGetLastError();
   }
-  return fn;
+  return (void*)fn;
 }
+
+namespace {
 
 size_t align256(size_t x) { return (x + 255) / 256 * 256; }
 
@@ -1402,6 +1417,7 @@ Plan make_plan(const mq_weights* w, int64_t M) {
                                       : tiles * 2 <= G);
   if (o.split_k == 1) stream_k = false;
   if (o.split_k >= 2) stream_k = true;
+  if (tiles > WS_MAX_TILES) stream_k = false;   // one counter per tile in the workspace prefix
   pl.gran = stream_k ? 1 : KS;
   pl.grid = (int)std::min<int64_t>(G, pl.units / pl.gran);
   // Few tiles: cut every tile into the same S parts (grid = tiles * S makes the stream-K ranges
@@ -1411,8 +1427,10 @@ Plan make_plan(const mq_weights* w, int64_t M) {
     pl.grid = (int)(tiles * S);
   }
   if (stream_k) {
-    pl.off_done = align256((size_t)tiles * 4);
-    pl.off_flag = pl.off_done + align256((size_t)tiles * 4);
+    // zero-state words (counters) live in the plan-independent prefix (mq_internal.h); flags and partial
+    // tiles behind it are written before they are read
+    pl.off_done = WS_OFF_DONE;
+    pl.off_flag = WS_PREFIX;
     pl.off_part = pl.off_flag + align256((size_t)pl.grid * 2 * 4);
     pl.ws_bytes = pl.off_part + (size_t)pl.grid * 2 * 2 * bt * BN * 4;
   }
@@ -1422,14 +1440,17 @@ Plan make_plan(const mq_weights* w, int64_t M) {
 template <int BT, bool FUSED = false, bool A8 = false>
 int launch(const CUtensorMap& tmap, const GemmParams& gp, int grid, cudaStream_t st) {
   using C = Cfg<BT, FUSED, A8>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  // the attribute belongs to the (device, function) pair: set it again whenever the current device changes
+  static int attr_dev = -1;
+  int dev = -1;
+  cudaGetDevice(&dev);
+  if (dev != attr_dev) {
     if (cudaFuncSetAttribute(mq_gemm_kernel<BT, FUSED, A8>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) !=
         cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
     }
-    attr_set = true;
+    attr_dev = dev;
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
@@ -1458,7 +1479,10 @@ extern "C" void mq_debug_set_trace(long long* dev_buf) { g_trace = dev_buf; }
 extern "C" size_t mq_gemm_workspace_bytes(const mq_weights* w, int64_t M) {
   if (!w || M <= 0) return 0;
   if (mq::check_device() != MQ_OK) return 0;
-  return make_plan(w, M).ws_bytes;
+  // the larger of the two kernels' needs, so that a workspace sized once serves the call whichever kernel the
+  // options in force at call time select
+  const size_t d = M <= 32 ? mq::decode_workspace_bytes(w, M) : 0;
+  return std::max(d, make_plan(w, M).ws_bytes);
 }
 
 namespace {
@@ -1486,6 +1510,10 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   if (rc != MQ_OK) return rc;
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return MQ_ERR_CUDA;
+
+  // decode shapes: the lean TMEM-free kernel (mq_decode.cu)
+  if (!fused && !a8 && mq::decode_eligible(w, M))
+    return mq::decode_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, ignore_res);
 
   const Plan pl = make_plan(w, M);
   if (pl.units >= (int64_t)1 << 31) return MQ_ERR_UNSUPPORTED_SHAPE;
@@ -1549,7 +1577,7 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   gp.fz_ctrl = fz_ctrl;
   gp.dRowChunks = make_fastdiv((uint32_t)(w->K / 8));
   uint8_t* ws = (uint8_t*)workspace;
-  gp.ws_cnt = (int32_t*)ws;
+  gp.ws_cnt = (int32_t*)(ws + WS_OFF_CNT);
   gp.ws_done = (int32_t*)(ws + pl.off_done);
   gp.ws_flag = (int32_t*)(ws + pl.off_flag);
   gp.ws_part = (int32_t*)(ws + pl.off_part);
@@ -1618,9 +1646,11 @@ __global__ void __launch_bounds__(128) naive_sparse_kernel(const uint8_t* __rest
   const uint32_t HI = 0xF0F0F0F0u;
   // the n-tile's cells are dealt to gridDim.z CTAs (cells_per_cta each); with more than one, the partial sums meet
   // in acc1 through int32 atomics (exact, so the result does not depend on the order)
-  const int c_lo = cell_ptr[nt] + (int)blockIdx.z * cells_per_cta, c_hi = min(cell_ptr[nt + 1], c_lo + cells_per_cta);
-  if (gridDim.z > 1 && c_lo >= c_hi) return;
-  for (int c = c_lo; c < c_hi; ++c) {
+  // (runs of cells_per_cta cells, strided by gridDim.z runs: every cell is visited whatever the cap on gridDim.z)
+  const int c_end = cell_ptr[nt + 1];
+  if (gridDim.z > 1 && cell_ptr[nt] + (int)blockIdx.z * cells_per_cta >= c_end) return;
+  for (int c0 = cell_ptr[nt] + (int)blockIdx.z * cells_per_cta; c0 < c_end; c0 += (int)gridDim.z * cells_per_cta)
+  for (int c = c0; c < min(c_end, c0 + cells_per_cta); ++c) {
     const int km = cells[c].kstep_mask, kstep = km & 0xFFFFFF, mask = (km >> 24) & 0xF;
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -1712,7 +1742,7 @@ extern "C" size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M) {
   if (!w || M <= 0) return 0;
   size_t q = (mq_qact_bytes(M, w->K) + 255) / 256 * 256;
   size_t s = ((size_t)M * 4 + 255) / 256 * 256;
-  return align256(mq_gemm_workspace_bytes(w, M)) + 256 /* fused-quantization control block */ + q + s;
+  return std::max(align256(mq_gemm_workspace_bytes(w, M)), mq::WS_PREFIX) + q + s;
 }
 
 extern "C" int mq_linear(const mq_weights* w, const void* A, mq_dtype a_dtype, int64_t M, int64_t lda, void* Y,
@@ -1728,20 +1758,20 @@ extern "C" int mq_linear(const mq_weights* w, const void* A, mq_dtype a_dtype, i
   // zero-state regions first (the GEMM's counters, the fused path's control block), so that the
   // caller's one-time memset covers them; then the packed activations and their scales
   const size_t g = mq_gemm_workspace_bytes(w, M);
-  const size_t g_al = align256(g);
+  const size_t g_al = std::max(align256(g), mq::WS_PREFIX);   // the prefix also carries the fused path's control block
   uint8_t* base = (uint8_t*)workspace;
-  uint32_t* ctrl = (uint32_t*)(base + g_al);
-  uint8_t* qa = base + g_al + 256;
+  uint32_t* ctrl = (uint32_t*)(base + mq::WS_OFF_FZ);
+  uint8_t* qa = base + g_al;
   float* sa = (float*)(qa + (mq_qact_bytes(M, w->K) + 255) / 256 * 256);
   if ((size_t)((uint8_t*)sa + (size_t)M * 4 - base) > workspace_bytes) return MQ_ERR_WORKSPACE;
   // Decode-sized calls (M <= 8): ONE kernel, the activation quantizer runs inside the GEMM.
   // Larger M: the quantizer as its own kernel (chained by programmatic dependent launch).
   const Options& o = options();
   if (o.fused_quant && M <= 8 && w->K >= 256 && (o.token_tile == 0 || o.token_tile == 16))
-    return gemm_impl(w, nullptr, nullptr, M, Y, y_dtype, ldy, nullptr, nullptr, base, g, cuda_stream, A, a_dtype, lda, ctrl);
+    return gemm_impl(w, nullptr, nullptr, M, Y, y_dtype, ldy, nullptr, nullptr, base, g_al, cuda_stream, A, a_dtype, lda, ctrl);
   int rc = mq_quantize_act(A, a_dtype, M, w->K, lda, qa, sa, cuda_stream);
   if (rc != MQ_OK) return rc;
-  rc = mq_gemm(w, qa, sa, M, Y, y_dtype, ldy, nullptr, nullptr, base, g, cuda_stream);
+  rc = mq_gemm(w, qa, sa, M, Y, y_dtype, ldy, nullptr, nullptr, base, g_al, cuda_stream);
   if (rc == MQ_OK) mq::set_launch_count(2);
   return rc;
 }

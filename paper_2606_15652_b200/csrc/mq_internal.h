@@ -23,6 +23,8 @@
 //            K-steps with one coalesced load (mask 0 = the K-step has no residual cell)
 #pragma once
 
+#include <cuda.h>
+
 #include <cstddef>
 #include <cstdint>
 #include <vector>
@@ -63,6 +65,10 @@ struct mq_weights {
   std::vector<int32_t> h_cell_ptr;
   std::vector<mq::CellMeta> h_cell_meta;
   int max_cells_per_tile = 0;
+  // TMA descriptors over d_base for the decode kernel's row slabs of 16 / 32 / 64 / 128 output channels
+  // (mq_decode.cu; built by mq::build_weight_tmaps when the handle is created or cloned)
+  CUtensorMap tmap_base[4];
+  bool tmap_ok = false;
 };
 
 namespace mq {
@@ -76,6 +82,9 @@ struct Options {
                              // the PDL-chained two-kernel path on B200; off by default)
   int64_t group_simt = 0;    // mq_gemm_group: 1 = the dp4a kernel (ablation); 0 = the mma.sync kernel
   int64_t pdl = 1;   // launch kernels as programmatic dependents of their predecessor in the stream
+  int64_t decode_path = 0;      // 0 = automatic (M <= 32 runs the lean mma.sync decode kernel), 1 = off (tcgen05 kernel)
+  int64_t decode_big = 0;       // decode kernel ring: 0 = automatic, 1 = deep (one CTA per SM), 2 = small (two per SM)
+  int64_t decode_rows = 0;      // 0 = automatic, else 16 / 32 / 64 / 128 output channels per CTA of the decode kernel
 };
 Options& options();
 void set_launch_count(int n);
@@ -83,5 +92,25 @@ void add_launch_count(int n);
 
 int check_device();  // MQ_OK or MQ_ERR_UNSUPPORTED_DEVICE / MQ_ERR_CUDA
 int sm_count();
+
+// Workspace contract shared by the GEMM kernels: the first WS_PREFIX bytes hold every word that must be ZERO
+// between calls (per-tile arrival counters, the fused quantizer's control block) at positions that do not
+// depend on the launch plan; every call returns them to zero.  Everything behind the prefix (partial tiles,
+// flags, packed activations) is written before it is read and needs no initial content.
+constexpr size_t WS_PREFIX = 16384;
+constexpr int WS_MAX_TILES = 1536;                       // counters per array
+constexpr size_t WS_OFF_CNT = 0;                         // int32 [WS_MAX_TILES]
+constexpr size_t WS_OFF_DONE = WS_MAX_TILES * 4;         // int32 [WS_MAX_TILES]
+constexpr size_t WS_OFF_FZ = 2 * WS_MAX_TILES * 4;       // uint32 [32] fused-quantizer control block
+
+// the lean decode kernel (mq_decode.cu): M <= 32, per-token W4A4
+bool decode_eligible(const mq_weights* w, int64_t M);
+size_t decode_workspace_bytes(const mq_weights* w, int64_t M);
+int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
+                int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
+                void* cuda_stream, bool ignore_res);
+int build_weight_tmaps(mq_weights* w);   // MQ_OK or MQ_ERR_CUDA
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency); NULL if absent
+void* tensor_map_encode_fn();
 
 }  // namespace mq

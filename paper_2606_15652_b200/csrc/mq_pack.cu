@@ -221,6 +221,11 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   w->d_cell_ptr = (int32_t*)(p + o_cptr);
   w->d_cell_meta = (CellMeta*)(p + o_cmeta);
   w->d_unit_meta = (int32_t*)(p + o_umeta);
+  if (mq::build_weight_tmaps(w) != MQ_OK) {
+    cudaFree(blob);
+    delete w;
+    return MQ_ERR_CUDA;
+  }
   *out = w;
   return MQ_OK;
 }
@@ -688,6 +693,11 @@ extern "C" int mq_weights_clone(const mq_weights* w, mq_weights** out, void* cud
   c->d_cell_ptr = (int32_t*)((uint8_t*)w->d_cell_ptr + d);
   c->d_cell_meta = (CellMeta*)((uint8_t*)w->d_cell_meta + d);
   c->d_unit_meta = (int32_t*)((uint8_t*)w->d_unit_meta + d);
+  if (mq::build_weight_tmaps(c) != MQ_OK) {
+    cudaFree(blob);
+    delete c;
+    return MQ_ERR_CUDA;
+  }
   *out = c;
   return MQ_OK;
 }
