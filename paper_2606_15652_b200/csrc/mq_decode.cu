@@ -14,9 +14,10 @@
 //
 //   * warp 8 (producer, one thread): per STAGE of UK K-steps ONE tensor-map copy of the slab's packed
 //     weights (the device layout [n-tile][K-step][4 chunks][128 rows][16 B] seen as a 3-D tensor: 16-byte
-//     row pieces x chunks along K x n-tiles; 8-16 KB per copy), one bulk copy per selected residual piece of
-//     the stage (CSR metadata: unit_meta; "prefetch sparse residual blocks") and ONE tensor-map copy
-//     of the stage's packed tokens [UK][MT x 64 B, SWIZZLE_64B].  The weights are static, so the first
+//     row pieces x chunks along K x n-tiles; 8-16 KB per copy) and ONE tensor-map copy of the stage's packed
+//     tokens [UK][MT x 64 B, SWIZZLE_64B]; warp 9 (one thread): one bulk copy per selected residual piece of
+//     the stage (CSR metadata: unit_meta; "prefetch sparse residual blocks") into a FIFO ring, in
+//     parallel with the dense stream so that a residual block never delays it.  The weights are static, so the first
 //     ring-full is requested BEFORE griddepcontrol.wait: it streams while the previous kernel in the stream is
 //     still running (a CTA needs < half an SM, so both kernels are resident together);
 //   * warps 0-7 (consumers): warp = (row tile rt of 16 channels, K group kw): the K-steps of a stage are dealt
@@ -44,7 +45,7 @@ using namespace mq;
 using namespace mq::ptx;
 
 constexpr int DEC_CWARPS = 8;          // consumer warps
-constexpr int DEC_THREADS = 32 * (DEC_CWARPS + 1);
+constexpr int DEC_THREADS = 32 * (DEC_CWARPS + 2);   // + warp 8: weight / token producer, warp 9: residual producer
 constexpr int DEC_QSLOTS = 16;         // residual pieces in flight per CTA (a FIFO ring); >= the pieces of one stage
 constexpr int DEC_MAX_KS = 512;        // K-steps whose metadata fits the shared-memory table (K <= 65536)
 
@@ -178,7 +179,7 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
       prefetch_tmap(&tmap_w);
       prefetch_tmap(&tmap_a);
       for (int s = 0; s < STAGES; ++s) {
-        mbar_init(full_bar(s), 1);               // the producer's arrive; the copies complete the transaction count
+        mbar_init(full_bar(s), 2);               // the two producers' arrivals; the copies complete the transaction count
         mbar_init(empty_bar(s), DEC_CWARPS);     // one arrival per consumer warp
       }
       fence_mbar_init();
@@ -188,7 +189,7 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
         tma_load_3d(sW + s * C::W_BYTES, &tmap_w, row0 * 2, 4 * UK * s, nt, full_bar(s));
       }
     }
-  } else {
+  } else if (warp < DEC_CWARPS) {
     // the n-tile's residual metadata -> shared memory, one thread per stage: the K-steps' {pieces of this slab,
     // first quarter | full mask} and the stage's piece count, so that the single producer thread pays one load
     // per stage on its common path (no residual piece in the stage)
@@ -215,7 +216,29 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
 
   if (warp == DEC_CWARPS) {
     if (lane != 0) return;
-    // ===================== producer (one thread) =====================
+    // ===================== producer of the weight / token stream (one thread) =====================
+    // Every instruction of a single-thread role costs ~7 cycles: this loop is two copy instructions and a wait.
+    DEC_STAMP(true, 2);
+    griddep_wait();   // the packed tokens are the previous kernel's output
+    DEC_STAMP(true, 3);
+    for (int s = 0; s < n_stages; ++s) {
+      const int slot = s % STAGES;
+      const uint32_t fb = full_bar(slot);
+      if (s >= STAGES) mbar_wait(empty_bar(slot), (((uint32_t)s / STAGES) & 1) ^ 1);   // the stage's slot is free
+      if (s >= pre) {
+        mbar_expect_tx(fb, C::W_BYTES);
+        tma_load_3d(sW + slot * C::W_BYTES, &tmap_w, row0 * 2, 4 * UK * s, nt, fb);
+      }
+      mbar_arrive_expect_tx(fb, C::T_BYTES);
+      tma_load_3d(sT + slot * C::T_BYTES, &tmap_a, 0, 0, UK * s, fb);
+      DEC_STAMP(s == 0, 21);
+      DEC_STAMP(s == n_stages - 1, 23);
+    }
+    return;
+  }
+  if (warp == DEC_CWARPS + 1) {
+    if (lane != 0) return;
+    // ===================== producer of the residual pieces (one thread, static data: no dependency wait) =====================
     // FIFO ring of residual pieces: q_issued / q_freed count pieces since the start; qcum[stage slot] = q_issued
     // after that stage, read back when the stage is known to be consumed
     int q_issued = 0, q_freed = 0, consumed = 0;
@@ -233,53 +256,6 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
       for (int i = 1; i < STAGES; ++i) v = i == slot ? qcum[i] : v;
       return v;
     };
-    // number of residual pieces of stage s (for this slab)
-    auto count_pieces = [&](int s) {   // {pieces | K-steps with pieces << 8}
-      uint32_t n;
-      asm volatile("ld.shared.u16 %0, [%1];" : "=r"(n) : "r"(sNP + 2u * (uint32_t)s));
-      return (int)n;
-    };
-    // requests the pieces of stage s into ring slots q_issued.. and publishes {pieces, first slot} of the stage
-    auto issue_pieces = [&](int s, int npk) {
-      const int slot = s % STAGES, np = npk & 0xFF;
-      const uint32_t fb = full_bar(slot);
-      sts_u32(sSMeta + 4u * (uint32_t)slot, (uint32_t)np | ((uint32_t)(q_issued % DEC_QSLOTS) << 8));
-      if (np) {   // (rare path; only the K-steps that own pieces are visited)
-        mbar_expect_tx(fb, (uint32_t)np * C::P_BYTES);
-        int qi = q_issued;
-        for (uint32_t km = (uint32_t)npk >> 8; km; km &= km - 1) {
-          const int ks = s * UK + __ffs((int)km) - 1;
-          const uint2 um = lds_u64(sUM + 8u * (uint32_t)ks);
-          const uint32_t full_mask = um.y >> 28, qoff = um.y & 0x0FFFFFFFu;
-          for (uint32_t mm = um.x & 0xF; mm; mm &= mm - 1) {
-            const int q = __ffs((int)mm) - 1;
-            const uint8_t* src = p.res + ((size_t)qoff + (size_t)__popc(full_mask & ((1u << q) - 1))) * QUARTER_BYTES +
-                                 (size_t)(row0 & 63) * 16;
-            const uint32_t dst = sQ + (uint32_t)(qi % DEC_QSLOTS) * C::P_BYTES;
-            if (C::P_ROWS == 64) {
-              tma_load_1d(dst, src, QUARTER_BYTES, fb);
-            } else {   // the slab's rows of the quarter's two 32-channel chunks
-              tma_load_1d(dst, src, C::P_ROWS * 16, fb);
-              tma_load_1d(dst + C::P_ROWS * 16, src + 1024, C::P_ROWS * 16, fb);
-            }
-            ++qi;
-          }
-        }
-        q_issued = qi;
-      }
-      set_qcum(slot, q_issued);
-    };
-    // ---- before griddepcontrol.wait: the residual pieces of the first ring-full, while they fit the piece ring
-    int pre_q = 0;
-    for (int s = 0; s < pre; ++s) {
-      const int npk = count_pieces(s);
-      if (q_issued + (npk & 0xFF) > DEC_QSLOTS) break;
-      issue_pieces(s, npk);
-      pre_q = s + 1;
-    }
-    DEC_STAMP(true, 2);
-    griddep_wait();   // the packed tokens are the previous kernel's output
-    DEC_STAMP(true, 3);
     auto advance_to = [&](int target) {   // wait (in order) until `target` stages are known to be consumed
       while (consumed < target) {
         mbar_wait(empty_bar(consumed % STAGES), ((uint32_t)consumed / STAGES) & 1);
@@ -290,23 +266,35 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
     for (int s = 0; s < n_stages; ++s) {
       const int slot = s % STAGES;
       const uint32_t fb = full_bar(slot);
-      if (s >= STAGES) advance_to(s - STAGES + 1);   // the stage's slot is free
-      if (s >= pre) {
-        mbar_expect_tx(fb, C::W_BYTES);
-        tma_load_3d(sW + slot * C::W_BYTES, &tmap_w, row0 * 2, 4 * UK * s, nt, fb);
+      if (s >= STAGES) advance_to(s - STAGES + 1);   // the stage's slot (and its metadata word) is free
+      uint32_t npk;   // {pieces | K-steps with pieces << 8}
+      asm volatile("ld.shared.u16 %0, [%1];" : "=r"(npk) : "r"(sNP + 2u * (uint32_t)s));
+      const int np = (int)(npk & 0xFF);
+      while (q_issued + np - q_freed > DEC_QSLOTS) advance_to(consumed + 1);   // room in the piece ring
+      sts_u32(sSMeta + 4u * (uint32_t)slot, (uint32_t)np | ((uint32_t)(q_issued % DEC_QSLOTS) << 8));
+      if (np) {   // only the K-steps that own pieces are visited
+        mbar_expect_tx(fb, (uint32_t)np * C::P_BYTES);
+        for (uint32_t km = npk >> 8; km; km &= km - 1) {
+          const int ks = s * UK + __ffs((int)km) - 1;
+          const uint2 um = lds_u64(sUM + 8u * (uint32_t)ks);
+          const uint32_t full_mask = um.y >> 28, qoff = um.y & 0x0FFFFFFFu;
+          for (uint32_t mm = um.x & 0xF; mm; mm &= mm - 1) {
+            const int q = __ffs((int)mm) - 1;
+            const uint8_t* src = p.res + ((size_t)qoff + (size_t)__popc(full_mask & ((1u << q) - 1))) * QUARTER_BYTES +
+                                 (size_t)(row0 & 63) * 16;
+            const uint32_t dst = sQ + (uint32_t)(q_issued % DEC_QSLOTS) * C::P_BYTES;
+            if (C::P_ROWS == 64) {
+              tma_load_1d(dst, src, QUARTER_BYTES, fb);
+            } else {   // the slab's rows of the quarter's two 32-channel chunks
+              tma_load_1d(dst, src, C::P_ROWS * 16, fb);
+              tma_load_1d(dst + C::P_ROWS * 16, src + 1024, C::P_ROWS * 16, fb);
+            }
+            ++q_issued;
+          }
+        }
       }
-      if (s >= pre_q) {
-        const int npk = count_pieces(s);
-        while (q_issued + (npk & 0xFF) - q_freed > DEC_QSLOTS) advance_to(consumed + 1);   // room in the piece ring
-        issue_pieces(s, npk);
-      }
-      // the arrival releases the metadata words; the phase completes when all bytes have landed
-      // (one copy instruction per stage: every further instruction of this thread costs ~100 cycles of the
-      // stage's budget; a bulk copy per token row was measured 1.5-2 x slower from M = 8)
-      mbar_arrive_expect_tx(fb, C::T_BYTES);
-      tma_load_3d(sT + slot * C::T_BYTES, &tmap_a, 0, 0, UK * s, fb);
-      DEC_STAMP(s == 0, 21);
-      DEC_STAMP(s == n_stages - 1, 23);
+      set_qcum(slot, q_issued);
+      mbar_arrive(fb);   // releases the metadata word; the phase completes when both producers' bytes have landed
     }
     return;
   }
