@@ -31,7 +31,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "fused W4A4+residual GEMM TOPS & frac of INT8/HBM roofline; tokens/s vs W16A16"
 RHO, BS = 0.05, 64
-N_COPIES = 4
+N_COPIES = 4            # weight copies the STEP graphs rotate (458 MB of other layers' weights between two uses)
+L2_BYTES = 126e6        # the per-shape loops rotate enough copies of ONE layer for 3 x L2 (SURVEY 8(d) cold-HBM rule)
 
 
 def load_peaks():
@@ -111,20 +112,24 @@ class ClockSampler:
 class Layer:
     """One projection: host tensors, N_COPIES packed device copies, per-M device buffers."""
 
-    def __init__(self, mq, torch, synth, seed, shape, Ms, n_copies):
+    def __init__(self, mq, torch, synth, seed, shape, Ms, n_copies, rho=RHO, bs=BS, cold_rule=True):
         self.name, self.K, self.N = shape.name, shape.K, shape.N
         t0 = time.time()
         self.W = synth.gen_weight(seed, self.N, self.K)
         X = synth.gen_calib(seed, self.K, 256)
         self.h = (2.0 / X.shape[0] * (X.astype(np.float64) ** 2).sum(0)).astype(np.float32)   # calibration input
-        self.budget = synth.budget_from_density(RHO, self.N, self.K, BS)
-        w0 = mq.mq_pack_weights(self.W, self.h, BS, self.budget)
+        self.budget = synth.budget_from_density(rho, self.N, self.K, bs)
+        w0 = mq.mq_pack_weights(self.W, self.h, bs, self.budget)
+        # cold-HBM rule: copies x packed bytes >= 3 x L2 for the loops that replay ONE layer back to back
+        if cold_rule:
+            n_copies = max(n_copies, int(np.ceil(3 * L2_BYTES / w0.info()["device_bytes"])) + 1)
         self.copies = [w0] + [w0.clone() for _ in range(n_copies - 1)]
         self.nnz = w0.info()["nnz"]
         # the same layer with budget 0 (dense-only W4A4): the zero-residual baseline of the same kernel
-        z0 = mq.mq_pack_weights(self.W, self.h, BS, 0)
-        self.dense = [z0] + [z0.clone() for _ in range(n_copies - 1)]
+        z0 = mq.mq_pack_weights(self.W, self.h, bs, 0) if self.budget else w0
+        self.dense = [z0] + [z0.clone() for _ in range(n_copies - 1)] if self.budget else self.copies
         self.pack_s = time.time() - t0
+        self.W = None                                            # the fp32 weights are not needed any more
         self.A_host, self.A, self.qA, self.sA, self.Y, self.ws = {}, {}, {}, {}, {}, {}
         for m in Ms:
             a = synth.gen_act(seed + m, m, self.K)
@@ -136,7 +141,7 @@ class Layer:
             self.ws[m] = mq.new_workspace(mq.mq_gemm_workspace_bytes(w0, m))
 
 
-def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_e2e=True):
+def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_e2e=True, extras=True):
     """Times one workload (BASELINE.json config): the whole step, the GEMM kernels alone (roofline),
     the cuBLAS bf16 comparator and the end-to-end path through mq_linear with host buffers."""
     cfg, _ = workload_shapes(workload)
@@ -181,98 +186,62 @@ def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_
         ms_step = e0.elapsed_time(e1) / steps
         clocks = sampler.stop()
 
-        # ---- roofline of the dominant kernel (mq_gemm_kernel), timed alone: graphs of GEMM launches only
-        reps = 8
-        per_shape = []
-        for (m, L) in calls:
+        # ---- roofline of the dominant kernel, timed alone: graphs of GEMM launches only.
+        # COLD: one launch per weight copy of the layer, copies x bytes >= 3 x L2, so every launch streams its
+        # weights from HBM; WARM: the same number of launches on ONE copy (L2-resident when it fits), labelled.
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def time_graph(call, n, repeats=5):
+            """us per launch of `call(r)` for r in range(n), replayed from a CUDA graph (best of `repeats`)."""
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=stream):
-                for r in range(reps):
-                    mq.mq_gemm(L.copies[r % N_COPIES], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
-            for _ in range(3):
+                for r in range(n):
+                    call(r)
+            for _ in range(2):
                 g.replay()
-            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             best = 1e30
-            for _ in range(5):
-                # other layers' traffic between repetitions keeps this layer's 4 copies cold in L2
-                graphs[0].replay()
+            for _ in range(repeats):
                 a0.record(stream)
                 g.replay()
                 a1.record(stream)
                 stream.synchronize()
-                best = min(best, a0.elapsed_time(a1) / reps)
+                best = min(best, a0.elapsed_time(a1) / n)
+            del g
+            return best * 1e3
+
+        per_shape = []
+        quant_shapes = {}
+        for (m, L) in calls:
+            nc = len(L.copies)
+            reps = max(nc, 4) if m <= 512 else max(2, min(nc, 4))    # long launches need fewer repetitions
+            gemm = lambda ws_, r: mq.mq_gemm(ws_[r % len(ws_)], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+            us = time_graph(lambda r: gemm(L.copies, r), reps)
+            us_warm = time_graph(lambda r: gemm(L.copies[:1], r), reps)
             # the zero-residual baseline: same kernel, same protocol, the budget-0 packing of the same W
-            gz = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(gz, stream=stream):
-                for r in range(reps):
-                    mq.mq_gemm(L.dense[r % N_COPIES], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
-            for _ in range(3):
-                gz.replay()
-            best0 = 1e30
-            for _ in range(5):
-                graphs[0].replay()
-                a0.record(stream)
-                gz.replay()
-                a1.record(stream)
-                stream.synchronize()
-                best0 = min(best0, a0.elapsed_time(a1) / reps)
-            # the W4A8 variant of the same launch: int8 per-token activations, same packed weights
-            q8, s8 = mq.mq_quantize_act8(L.A[m])
-            g8 = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g8, stream=stream):
-                for r in range(reps):
-                    mq.mq_gemm_a8(L.copies[r % N_COPIES], q8, s8, m, Y=L.Y[m], workspace=L.ws[m])
-            for _ in range(3):
-                g8.replay()
-            best8 = 1e30
-            for _ in range(5):
-                graphs[0].replay()
-                a0.record(stream)
-                g8.replay()
-                a1.record(stream)
-                stream.synchronize()
-                best8 = min(best8, a0.elapsed_time(a1) / reps)
-            del g8, q8, s8
-            # the paper's naive 3-kernel pipeline on the same launch (Fig.3): dense GEMM with the
-            # residual off + sparse-block GEMM + reduce-add
-            scr = torch.empty((m, L.N), dtype=torch.int32, device="cuda")
-            gn = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(gn, stream=stream):
-                for r in range(reps):
-                    mq.mq_gemm_naive(L.copies[r % N_COPIES], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m], scratch=scr)
-            for _ in range(3):
-                gn.replay()
-            bestn = 1e30
-            for _ in range(5):
-                graphs[0].replay()
-                a0.record(stream)
-                gn.replay()
-                a1.record(stream)
-                stream.synchronize()
-                bestn = min(bestn, a0.elapsed_time(a1) / reps)
-            del gn, scr
-            # per-group activation scales (the paper's W4A4 activation setting), group 128:
-            # mq_gemm_group on the same launch (a first dp4a / mma.sync path, not the tcgen05 kernel)
-            qg, sg = mq.mq_quantize_act_group(L.A[m], 128)
-            wsg = torch.empty(max(mq.mq_gemm_group_workspace_bytes(L.copies[0], m), 16), dtype=torch.uint8, device="cuda")
-            gg = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(gg, stream=stream):
-                for r in range(reps):
-                    mq.mq_gemm_group(L.copies[r % N_COPIES], qg, sg, 128, m, Y=L.Y[m], workspace=wsg)
-            for _ in range(3):
-                gg.replay()
-            bestg = 1e30
-            for _ in range(5):
-                graphs[0].replay()
-                a0.record(stream)
-                gg.replay()
-                a1.record(stream)
-                stream.synchronize()
-                bestg = min(bestg, a0.elapsed_time(a1) / reps)
-            del gg, qg, sg, wsg
-            per_shape.append(dict(M=m, layer=L.name, K=L.K, N=L.N, us=best * 1e3, us_dense=best0 * 1e3, us_a8=best8 * 1e3, us_naive=bestn * 1e3,
-                                  us_group=bestg * 1e3,
-                                  bytes=algo_bytes(m, L.K, L.N, L.nnz, BS), ops=algo_ops(m, L.K, L.N, L.nnz, BS)))
+            us0 = time_graph(lambda r: gemm(L.dense, r), reps)
+            row = dict(M=m, layer=L.name, K=L.K, N=L.N, us=us, us_warm=us_warm, us_dense=us0, copies=nc,
+                       bytes=algo_bytes(m, L.K, L.N, L.nnz, BS), ops=algo_ops(m, L.K, L.N, L.nnz, BS))
+            if extras:
+                # the W4A8 variant of the same launch (SURVEY 8(f)-2): int8 per-token activations, same packed weights
+                q8, s8 = mq.mq_quantize_act8(L.A[m])
+                row["us_a8"] = time_graph(lambda r: mq.mq_gemm_a8(L.copies[r % nc], q8, s8, m, Y=L.Y[m], workspace=L.ws[m]), reps, 3)
+                del q8, s8
+                # the paper's naive 3-kernel pipeline on the same launch (Fig.3; SURVEY 8(f)-4a)
+                scr = torch.empty((m, L.N), dtype=torch.int32, device="cuda")
+                row["us_naive"] = time_graph(lambda r: mq.mq_gemm_naive(L.copies[r % nc], L.qA[m], L.sA[m], m, Y=L.Y[m],
+                                                                         workspace=L.ws[m], scratch=scr), reps, 3)
+                del scr
+                # per-group activation scales (SURVEY 8(f)-3; the paper's W4A4 activation setting, P:441), group 128
+                qg, sg = mq.mq_quantize_act_group(L.A[m], 128)
+                wsg = torch.empty(max(mq.mq_gemm_group_workspace_bytes(L.copies[0], m), 16), dtype=torch.uint8, device="cuda")
+                row["us_group"] = time_graph(lambda r: mq.mq_gemm_group(L.copies[r % nc], qg, sg, 128, m, Y=L.Y[m], workspace=wsg), reps, 3)
+                del qg, sg, wsg
+            per_shape.append(row)
+            # the activation quantizer alone (kernel i): HBM, 2 B read + 0.5 B written per element (SURVEY 8(d))
+            if (m, L.K) not in quant_shapes:
+                nq = 8 if m <= 512 else 3
+                quant_shapes[(m, L.K)] = dict(M=m, K=L.K, us=time_graph(lambda r: mq.mq_quantize_act(L.A[m], L.qA[m], L.sA[m]), nq, 3),
+                                              bytes=int(2.5 * m * L.K) + 4 * m)
 
         # ---- W16A16 comparator: cuBLAS bf16 on the same shapes, same rotation
         w16 = {L.name: [torch.randn((L.N, L.K), device="cuda", dtype=torch.bfloat16) * 0.02 for _ in range(2)]
@@ -329,11 +298,59 @@ def measure(workload, steps, warmup, torch, mq, synth, world, dist, local, with_
         ms_step, e2 = max_over_ranks([ms_step, e2e_ms or 0.0], torch, dist, "cuda")
         e2e_ms = e2 if with_e2e else None
     return dict(cfg=cfg, Ms=Ms, layers_cfg=layers_cfg, layers=layers, calls=calls, ms_step=ms_step, clocks=clocks,
-                per_shape=per_shape, ms16=ms16, e2e_ms=e2e_ms,
+                per_shape=per_shape, quant=list(quant_shapes.values()), ms16=ms16, e2e_ms=e2e_ms,
                 ops_step=sum(algo_ops(m, L.K, L.N, L.nnz, BS) for (m, L) in calls),
                 bytes_step=sum(algo_bytes(m, L.K, L.N, L.nnz, BS) for (m, L) in calls),
                 h2d=sum(L.A_host[m].numel() * 2 for (m, L) in calls), d2h=sum(m * L.N * 2 for (m, L) in calls),
                 pack_s=sum(L.pack_s for L in layers))
+
+
+def measure_sweep(workload, torch, mq, synth, layer_names=None):
+    """BASELINE.json configs[3]: the residual density x block size sweep of the Qwen3-8B-shaped layers.  Per (layer,
+    block, rho, M): the GEMM launch alone, cold weights (copies x bytes >= 3 x L2), same protocol as the roofline loop."""
+    cfg, _ = workload_shapes(workload)
+    stream = torch.cuda.Stream()
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    rows = []
+    with torch.cuda.stream(stream):
+        for i, l in enumerate(cfg["layers"]):
+            if layer_names and l.name not in layer_names:
+                continue
+            for bs in cfg.get("block_sweep", [cfg["block"]]):
+                for rho in cfg.get("rho_sweep", [cfg["rho"]]):
+                    L = Layer(mq, torch, synth, cfg["seed"] + i, l, cfg["Ms"], N_COPIES, rho=rho, bs=bs)
+                    for m in cfg["Ms"]:
+                        mq.mq_quantize_act(L.A[m], L.qA[m], L.sA[m])
+                        nc = len(L.copies)
+                        reps = nc if m <= 512 else max(2, min(nc, 4))
+                        g = torch.cuda.CUDAGraph()
+                        mq.mq_gemm(L.copies[0], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+                        stream.synchronize()
+                        with torch.cuda.graph(g, stream=stream):
+                            for r in range(reps):
+                                mq.mq_gemm(L.copies[r % nc], L.qA[m], L.sA[m], m, Y=L.Y[m], workspace=L.ws[m])
+                        g.replay()
+                        best = 1e30
+                        for _ in range(3):
+                            a0.record(stream)
+                            g.replay()
+                            a1.record(stream)
+                            stream.synchronize()
+                            best = min(best, a0.elapsed_time(a1) / reps)
+                        del g
+                        us = best * 1e3
+                        by, ops = algo_bytes(m, l.K, l.N, L.nnz, bs), algo_ops(m, l.K, l.N, L.nnz, bs)
+                        rows.append(dict(layer=l.name, K=l.K, N=l.N, block=bs, rho=rho, nnz=L.nnz, M=m, us=round(us, 3),
+                                         gbs=round(by / (us * 1e-6) / 1e9, 1), tops=round(ops / (us * 1e-6) / 1e12, 2)))
+                    del L
+                    torch.cuda.empty_cache()
+    # overhead of the residual against the rho = 0 run of the same (layer, block, M)
+    base = {(r["layer"], r["block"], r["M"]): r["us"] for r in rows if r["rho"] == 0.0}
+    for r in rows:
+        b = base.get((r["layer"], r["block"], r["M"]))
+        if b:
+            r["over_rho0"] = round(r["us"] / b - 1.0, 4)
+    return rows
 
 
 def max_over_ranks(values, torch, dist, device):
@@ -350,40 +367,59 @@ def aggregate_value(ops_step, ms_step, world):
 
 
 def roofline_of(r, peaks, traffic):
-    """Roofline object of the dominant kernel (mq_gemm_kernel, the launches of one step timed alone).
+    """Roofline object of the dominant kernel (the GEMM launches of one step timed alone, cold weights).
     Decode-shaped workloads are bound by HBM (algorithmic bytes), prefill-shaped ones by
     the INT8 tensor pipe; which one is decided by the slower of the two ideal times."""
     us = sum(s["us"] for s in r["per_shape"])
     by = sum(s["bytes"] for s in r["per_shape"])
     ops = sum(s["ops"] for s in r["per_shape"])
-    int8_peak = 2.0 * peaks["bf16_tflops"]          # kind::i8 runs at twice the bf16 rate (nominal 4.5 vs 2.25 PF)
+    int8_proxy = 2.0 * peaks["bf16_tflops"]          # kind::i8 runs at twice the bf16 rate (nominal 4.5 vs 2.25 PF)
+    int8_peak = peaks.get("int8_probe_tops") or int8_proxy
     t_hbm, t_tensor = by / (peaks["hbm_gbs"] * 1e9), ops / (int8_peak * 1e12)
-    per_shape = [dict(M=s["M"], layer=s["layer"], us=round(s["us"], 3), us_dense_only=round(s["us_dense"], 3),
-                      us_w4a8=round(s["us_a8"], 3), us_naive3=round(s["us_naive"], 3), us_group128=round(s["us_group"], 3),
-                      gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1),
-                      tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2)) for s in r["per_shape"]]
-    kern = f"mq_gemm_kernel ({len(r['per_shape'])} launches of the step, timed alone, cold weights)"
+    has = lambda k: all(k in s for s in r["per_shape"])
+    per_shape = []
+    for s in r["per_shape"]:
+        d = dict(M=s["M"], layer=s["layer"], us_cold=round(s["us"], 3), us_warm=round(s["us_warm"], 3),
+                 us_dense_only=round(s["us_dense"], 3), copies=s["copies"],
+                 gbs=round(s["bytes"] / (s["us"] * 1e-6) / 1e9, 1), tops=round(s["ops"] / (s["us"] * 1e-6) / 1e12, 2))
+        for k, name in (("us_a8", "us_w4a8"), ("us_naive", "us_naive3"), ("us_group", "us_group128")):
+            if k in s:
+                d[name] = round(s[k], 3)
+        per_shape.append(d)
+    kern = ("mq_decode_kernel" if max(s["M"] for s in r["per_shape"]) <= 32 else "mq_gemm_kernel") + \
+           f" ({len(r['per_shape'])} launches of the step, timed alone; cold = one launch per weight copy, copies x bytes >= 3 x L2)"
     us0 = sum(s["us_dense"] for s in r["per_shape"])
-    us8 = sum(s["us_a8"] for s in r["per_shape"])
-    usn = sum(s["us_naive"] for s in r["per_shape"])
-    usg = sum(s["us_group"] for s in r["per_shape"])
-    extra = {"w4a8_time_over_w4a4": us8 / us,
-             "group128_time_over_per_token": usg / us,
-             "group128_note": "mq_gemm_group (per-group activation scales, group 128, P:441; mma.sync kernel) "
-                              "over the per-token fused tcgen05 kernel, same launches",
-             "naive3_time_over_fused": usn / us,
-             "naive3_note": "the paper's naive pipeline (dense GEMM, separate sparse-block GEMM, reduce-add: mq_gemm_naive) "
-                            "over the fused kernel, same launches; paper: 1.9x on RTX 4090 for Qwen3-8B V-proj (Fig.3)",
+    extra = {"us_cold": us, "us_warm": sum(s["us_warm"] for s in r["per_shape"]),
              "residual_overhead": us / us0 - 1.0,
              "residual_overhead_note": f"time of the {len(r['per_shape'])} launches at rho={RHO} over the same launches on the "
                                        "budget-0 packing of the same weights (floor = rho: the residual adds rho x bytes and ops)"}
+    if has("us_a8"):
+        extra["w4a8_time_over_w4a4"] = sum(s["us_a8"] for s in r["per_shape"]) / us
+    if has("us_group"):
+        extra["group128_time_over_per_token"] = sum(s["us_group"] for s in r["per_shape"]) / us
+        extra["group128_note"] = ("mq_gemm_group (per-group activation scales, group 128, P:441; mma.sync kernel) over the "
+                                  "per-token kernel, same launches")
+    if has("us_naive"):
+        extra["naive3_time_over_fused"] = sum(s["us_naive"] for s in r["per_shape"]) / us
+        extra["naive3_note"] = ("the paper's naive pipeline (dense GEMM, separate sparse-block GEMM, reduce-add: mq_gemm_naive) "
+                                "over the fused kernel, same launches; paper: 1.9x on RTX 4090 for Qwen3-8B V-proj (Fig.3)")
+    # kernel (i) alone: HBM, 2.5 B per element (SURVEY 8(d)); launch-bound for decode-sized M
+    qus, qby = sum(q["us"] for q in r["quant"]), sum(q["bytes"] for q in r["quant"])
+    extra["quantize_act"] = {"bound": "hbm", "achieved": qby / (qus * 1e-6) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                             "frac": qby / (qus * 1e-6) / 1e9 / peaks["hbm_gbs"],
+                             "kernel": "mq_quantize_act_kernel, timed alone (graph replay, inputs L2-resident for small M)",
+                             "per_shape": [dict(M=q["M"], K=q["K"], us=round(q["us"], 3),
+                                                gbs=round(q["bytes"] / (q["us"] * 1e-6) / 1e9, 1)) for q in r["quant"]]}
     if t_hbm >= t_tensor:
         a = by / (us * 1e-6) / 1e9
         return {"bound": "hbm", "achieved": a, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": a / peaks["hbm_gbs"],
                 "traffic": traffic, "peak_source": peaks["source"], "kernel": kern, **extra, "per_shape": per_shape}
     a = ops / (us * 1e-6) / 1e12
     return {"bound": "tensor", "achieved": a, "peak": int8_peak, "unit": "TFLOP/s", "frac": a / int8_peak,
-            "traffic": traffic, "peak_source": peaks["source"] + " bf16 burst x 2 (int8 : bf16 nominal ratio)",
+            "frac_of_proxy_2x_bf16_burst": a / int8_proxy, "proxy_peak": int8_proxy,
+            "traffic": traffic,
+            "peak_source": ("measured on this device: mq_probe_int8_peak, a pure tcgen05.mma kind::i8 issue loop (128 x 256 x 32)"
+                            if peaks.get("int8_probe_tops") else peaks["source"] + " bf16 burst x 2 (int8 : bf16 nominal ratio; PROXY)"),
             "kernel": kern, **extra, "per_shape": per_shape}
 
 
@@ -410,6 +446,15 @@ def run_ours(args, rank, world):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = load_peaks()
+    if "rho_sweep" in synth.CONFIGS[args.workload] and args.sweep_only:
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "workload": args.workload, "unit": "us per mq_gemm launch, cold weights",
+                              "sweep": measure_sweep(args.workload, torch, mq, synth)}))
+        return
+    try:
+        peaks["int8_probe_tops"] = max(mq.mq_probe_int8_peak(256, 4000), mq.mq_probe_int8_peak(128, 4000))
+    except Exception:
+        peaks["int8_probe_tops"] = None
     r = measure(args.workload, args.steps, args.warmup, torch, mq, synth, world, dist, local)
     Ms, layers_cfg, calls = r["Ms"], r["layers_cfg"], r["calls"]
     ms_step, e2e_ms = r["ms_step"], r["e2e_ms"]
@@ -422,7 +467,8 @@ def run_ours(args, rank, world):
                                f"{[(l.K, l.N) for l in layers_cfg]}, rho={RHO}, block={BS}, fp16 in, bf16 out",
                    "step": f"mq_quantize_act + mq_gemm for each of the {len(calls)} (M, projection) pairs, CUDA-graph "
                            "replay, kernels chained by programmatic dependent launch",
-                   "l2": f"{N_COPIES} rotating weight copies per layer ({N_COPIES * r['bytes_step'] / len(Ms) / 1e6:.0f} MB > 3x L2)",
+                   "l2": f"step: {N_COPIES} rotating weight copies per layer ({N_COPIES * r['bytes_step'] / len(Ms) / 1e6:.0f} MB of other "
+                         "weights between two uses of a copy > 3x L2); per-shape roofline loops: one launch per copy, copies x bytes >= 3x L2",
                    "parallelism": "replicas (no collective on the path)" if world > 1 else "single GPU"},
         "tokens_per_s": world * sum(Ms) / (ms_step * 1e-3),
         "hbm_gbs_step": r["bytes_step"] / (ms_step * 1e-3) / 1e9,
@@ -433,6 +479,8 @@ def run_ours(args, rank, world):
                 "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"],
                 "api": "mq_linear_host (C ABI, pinned host buffers in and out)"},
         "gpu_launches": args.steps * 2 * len(calls),
+        "int8_peak_tops": {"probe_tcgen05_kind_i8": peaks.get("int8_probe_tops"), "proxy_2x_bf16_burst": 2.0 * peaks["bf16_tflops"],
+                           "nominal": 4500.0},
         "clocks": r["clocks"],
         "pack_seconds": round(r["pack_s"], 2),
     }
@@ -440,7 +488,7 @@ def run_ours(args, rank, world):
     if rank == 0 and world == 1 and args.also and args.also != args.workload:
         # the other regime of the north star (prefill: tensor-bound), same protocol, fewer steps
         torch.cuda.empty_cache()
-        r2 = measure(args.also, max(3, args.steps // 4), 3, torch, mq, synth, world, dist, local, with_e2e=False)
+        r2 = measure(args.also, max(3, args.steps // 4), 3, torch, mq, synth, world, dist, local, with_e2e=False, extras=False)
         rf = roofline_of(r2, peaks, load_traffic(args.also))
         out["also"] = {"workload": args.also, "ms_per_step": r2["ms_step"],
                        "value": r2["ops_step"] / (r2["ms_step"] * 1e-3) / 1e12, "unit": "TOPS",
@@ -448,6 +496,13 @@ def run_ours(args, rank, world):
                        "w16a16_cublas_bf16": {"ms_per_step": r2["ms16"], "speedup_vs_w16a16": r2["ms16"] / r2["ms_step"]},
                        "roofline": rf, "clocks": r2["clocks"]}
         del r2
+    if rank == 0 and world == 1 and args.also2:
+        # BASELINE.json configs[3] (Qwen3-8B-shaped): density x block sweep on one projection (the full sweep over the
+        # four projections is `--workload qwen3_8b`, committed under profiles/)
+        wl, _, ln = args.also2.partition(":")
+        torch.cuda.empty_cache()
+        out["also2"] = {"workload": wl, "layers": ln or "all", "unit": "us per mq_gemm launch, cold weights",
+                        "sweep": measure_sweep(wl, torch, mq, synth, [ln] if ln else None)}
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(args.workload, budget_s=20.0)
@@ -507,6 +562,7 @@ def cpu_baseline(workload, budget_s=20.0, steps=2):
     ops = sum(algo_ops(m, l.K, l.N, L.nnz, BS) for (_, l, L) in layers)
     return {"value": ops / best / 1e12, "unit": "TOPS", "cores": min(oracle.num_threads(), m), "kind": "oracle",
             "threads_available": oracle.num_threads(), "seconds": round(best, 3),
+            "build": "oracle as it stands: g++ -O2 -ffp-contract=off -fopenmp, threads not pinned (not the tuned -O3 -march=native build BASELINE.md section 3 sketched)",
             "sample": f"oracle O2+O8+O9 on M={m} tokens x all {len(layers)} projections of {workload} "
                       f"(best of {passes} passes, {spent:.1f} s of oracle work; the oracle parallelises over tokens only)"}
 
@@ -551,6 +607,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llama3_8b_decode")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep-only", action="store_true",
+                    help="with --workload qwen3_8b: print only the density x block sweep of all four projections")
+    ap.add_argument("--also2", default="qwen3_8b:qkv",
+                    help="density x block sweep reported under \"also2\" (N=1 only): workload[:layer]; empty string = skip")
     ap.add_argument("--also", default="llama3_8b_prefill",
                     help="second workload reported under \"also\" (N=1 only); empty string = skip")
     args = ap.parse_args()

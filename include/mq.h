@@ -241,6 +241,12 @@ int mq_set_option(const char* name, int64_t value);
 /* Number of kernels the last mq_gemm / mq_linear / mq_quantize_act call launched. */
 int mq_last_launch_count(void);
 
+/* Diagnostic: the dense INT8 tensor-pipe throughput of the current device in TOPS, measured with
+ * a pure issue loop of tcgen05.mma.cta_group::1.kind::i8 instructions of shape 128 x n x 32 (n = 128 or 256; operands
+ * resident in shared memory, no loads, no epilogue), `iters` x 32 instructions on every SM.  This is the denominator
+ * the north star's "INT8 tensor-core roofline" refers to on this machine.  Host-synchronous; errors as the other calls. */
+int mq_probe_int8_peak(int n, int iters, double* tops_out, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

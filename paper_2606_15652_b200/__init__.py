@@ -26,6 +26,7 @@ from .binding import (  # noqa: F401
     mq_pack_prequantized,
     mq_pack_weights,
     mq_pack_weights_device,
+    mq_probe_int8_peak,
     mq_qact_bytes,
     mq_quantize_act,
     mq_quantize_act8,

@@ -24,6 +24,7 @@ EXPORTS = [
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
     "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_gemm_naive", "mq_gemm_naive_scratch_bytes", "mq_set_option",
     "mq_last_launch_count", "mq_quantize_act_group", "mq_gemm_group_workspace_bytes", "mq_gemm_group",
+    "mq_probe_int8_peak",
 ]
 
 _lib = None
@@ -98,6 +99,8 @@ def lib() -> C.CDLL:
     L.mq_set_option.argtypes = [C.c_char_p, i64]
     L.mq_last_launch_count.restype = i32
     L.mq_last_launch_count.argtypes = []
+    L.mq_probe_int8_peak.restype = i32
+    L.mq_probe_int8_peak.argtypes = [i32, i32, C.POINTER(C.c_double), vp]
     _lib = L
     return L
 
@@ -133,6 +136,13 @@ def mq_set_option(name: str, value: int) -> None:
 
 def mq_last_launch_count() -> int:
     return int(lib().mq_last_launch_count())
+
+
+def mq_probe_int8_peak(n: int = 256, iters: int = 2000) -> float:
+    """Measured dense INT8 tensor-pipe throughput (TOPS) of the current device: a pure tcgen05.mma kind::i8 issue loop."""
+    out = C.c_double()
+    _check(lib().mq_probe_int8_peak(int(n), int(iters), C.byref(out), _stream()), "mq_probe_int8_peak")
+    return float(out.value)
 
 
 def mq_qact_bytes(M: int, K: int) -> int:

@@ -76,14 +76,17 @@ constexpr int META_LAST = 1 << 29;           // last K-step of the segment: accu
 
 // A8: W4A8 variant (the paper's other precision): per-token int8 activations, 1 byte per element in
 // the token area; the unpack groups only re-order them (no expansion), accumulators are 16 x the true value.
+#ifndef MQ_BT128_UK2
+#define MQ_BT128_UK2 0
+#endif
 template <int BT, bool FUSED = false, bool A8 = false>
 struct Cfg {
   // Unpack groups (4 warps each).  An item costs a group ~1000 cycles of mostly latency (loads,
   // TMEM/shared stores, proxy fences), so prefill runs four groups side by side.
-  static constexpr int G = BT == 128 ? 4 : 2;
+  static constexpr int G = (BT == 128 && !MQ_BT128_UK2) ? 4 : 2;
   static constexpr int NUM_THREADS = 32 * (FIRST_UNPACK_WARP + 4 * G);
   static constexpr int SK = BT <= 32 ? 4 : 2;                    // K-steps per P stage
-  static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : 1);   // K-steps per U stage (item)
+  static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : (MQ_BT128_UK2 ? 2 : 1));   // K-steps per U stage (item)
   static constexpr int IPS = SK / UK;                            // items per P stage
   static constexpr int PSTAGES = A8 ? (BT == 16 ? 4 : (BT == 32 ? 3 : (BT == 64 ? 4 : 3)))
                                     : (BT <= 32 ? 4 : (BT == 64 ? 6 : 4));
@@ -329,7 +332,15 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   using C = Cfg<BT, FUSED, A8>;
   constexpr int SK = C::SK, UK = C::UK, IPS = C::IPS;
   extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  // Known addresses (KA): for the prefill tile the shared-memory window and the tensor-memory allocation are taken as
+  // compile-time constants -- dynamic shared memory starts at 1024 (the first KB is the system's) and a 512-column
+  // allocation can only start at column 0 -- so that every barrier address, descriptor and TMEM operand of the
+  // MMA-issuing warp's loop is an immediate instead of 16 R2UR / UIADD3 per K-step (that warp's dependent
+  // instruction chain paces prefill).  Both assumptions are checked at run time: a mismatch traps.
+  constexpr bool KA = BT == 128 && C::TMEM_COLS == 512;
+  const uint32_t smem_base_rt = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t smem_base = KA ? 1024u : smem_base_rt;
+  if (KA && smem_base_rt != 1024u) __trap();
 
   const uint32_t sU = smem_base + C::OFF_U, sP = smem_base + C::OFF_P, sRP = smem_base + C::OFF_RP,
                  sBar = smem_base + C::OFF_BAR;
@@ -391,7 +402,8 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = (uint32_t)misc[0];
+  const uint32_t tmem_base = KA ? 0u : (uint32_t)misc[0];
+  if (KA && misc[0] != 0) __trap();
   MQ_STAMP_IF(threadIdx.x == 0, 1);
   // PDL: the next kernel in the stream may start its prologue as this grid's CTAs retire
   griddep_launch();
