@@ -275,3 +275,117 @@ def forward_group(A, L: PackedLayer, group: int, cols: Optional[np.ndarray] = No
         Y += s * (sw64 * acc0_g[g] + sr64 * acc1_g[g])
         mag += s * (np.abs(sw64 * acc0_g[g]) + np.abs(sr64 * acc1_g[g]))
     return dict(qa=qa, sa=sa, acc0_g=acc0_g, acc1_g=acc1_g, acc0=acc0_g.sum(0), acc1=acc1_g.sum(0), Y=Y, mag=mag)
+
+
+# ------------------------------------------------------------------------------------------------
+# SURVEY 8(f)-3, second half: PER-BLOCK-LOCAL residual scales (north_star: "residual block list with block
+# coordinates and per-block scales").  DESIGN.md reading A4b: the quantizer of Eq.1 is applied to R inside every
+# block separately: for block B = (bn, bk) and output channel n in bn,
+#     s_rb[n, bk] = max_{k in bk} |R[n, k]| / 7 ,   q_rb[n, k] = round(R[n, k] / s_rb[n, bk])      (O1 on the run)
+# computed for EVERY block before selection, so that the gain of a block does not depend on which other blocks are
+# selected (Theorem 4.1 needs B_B independent of S) -- exactly as in reading A4, with a finer scale.
+# Plain numpy on top of O1; no blocking beyond the definition.
+@dataclass
+class DecompBlockLocal:
+    qw: np.ndarray   # int8 [N,K]
+    sw: np.ndarray   # fp32 [N]
+    R: np.ndarray    # fp32 [N,K]
+    qr: np.ndarray   # int8 [N,K]   block-local codes, whole matrix, before selection
+    srb: np.ndarray  # fp32 [N, K/bs] block-local residual scales
+
+
+def decompose_blocklocal(W: np.ndarray, bs: int) -> DecompBlockLocal:
+    """O3 + O4b: base quantization and R as in O3 (Alg.1 line 1); Q(R) per (channel, k-block) run."""
+    d = decompose(W)
+    N, K = d.R.shape
+    assert K % bs == 0 and N % bs == 0
+    runs = np.ascontiguousarray(d.R.reshape(N * (K // bs), bs))
+    q = np.empty(runs.shape, np.int8)
+    s = np.empty(runs.shape[0], np.float32)
+    lib().orc_quantize_rows(_p(runs), C.c_int64(runs.shape[0]), C.c_int64(bs), _p(q), _p(s))
+    return DecompBlockLocal(d.qw, d.sw, d.R, q.reshape(N, K), s.reshape(N, K // bs))
+
+
+def scores_blocklocal(d: DecompBlockLocal, h: np.ndarray, bs: int) -> Scores:
+    """O6 with the block-local Q(R): A_B = sum_B h_k R^2, B_B = sum_B h_k (R - s_rb q_rb)^2, binary64."""
+    N, K = d.R.shape
+    h64 = np.ascontiguousarray(h, np.float32).astype(np.float64)
+    R = d.R.astype(np.float64)
+    E = R - np.repeat(d.srb.astype(np.float64), bs, axis=1) * d.qr.astype(np.float64)
+    nbn, nbk = N // bs, K // bs
+    A = (h64[None, :] * R * R).reshape(nbn, bs, nbk, bs).sum(axis=(1, 3)).reshape(-1)
+    B = (h64[None, :] * E * E).reshape(nbn, bs, nbk, bs).sum(axis=(1, 3)).reshape(-1)
+    delta = A - B
+    return Scores(A, B, delta, np.maximum(delta, 0.0))
+
+
+@dataclass
+class PackedLayerBlockLocal:
+    N: int
+    K: int
+    bs: int
+    d: DecompBlockLocal
+    sc: Optional[Scores]
+    blk_n: np.ndarray
+    blk_k: np.ndarray
+
+    @property
+    def nnz(self) -> int:
+        return int(self.blk_n.shape[0])
+
+    def qr_blocks(self) -> np.ndarray:
+        out = np.empty((self.nnz, self.bs, self.bs), np.int8)
+        for e in range(self.nnz):
+            n0, k0 = int(self.blk_n[e]) * self.bs, int(self.blk_k[e]) * self.bs
+            out[e] = self.d.qr[n0:n0 + self.bs, k0:k0 + self.bs]
+        return out
+
+    def sr_blocks(self) -> np.ndarray:
+        """fp32 [nnz, bs]: the scale of every row of every selected block."""
+        out = np.empty((self.nnz, self.bs), np.float32)
+        for e in range(self.nnz):
+            n0 = int(self.blk_n[e]) * self.bs
+            out[e] = self.d.srb[n0:n0 + self.bs, int(self.blk_k[e])]
+        return out
+
+
+def algorithm1_blocklocal(W: np.ndarray, h: Optional[np.ndarray], bs: int, budget: int) -> PackedLayerBlockLocal:
+    """Algorithm 1 with block-local residual scales: O3, O4b, O6, O7."""
+    N, K = W.shape
+    d = decompose_blocklocal(W, bs)
+    if h is None:
+        h = np.ones(K, np.float32)
+    sc = scores_blocklocal(d, h, bs)
+    sel = select(sc.S, budget)
+    nbk = K // bs
+    return PackedLayerBlockLocal(N, K, bs, d, sc, (sel // nbk).astype(np.int32), (sel % nbk).astype(np.int32))
+
+
+def forward_blocklocal(A, L: PackedLayerBlockLocal, rows: Optional[np.ndarray] = None):
+    """O2 + O8b + O9b.  With a residual scale that changes from block to block the sparse term of Eq.4 is a sum
+    of per-block scaled integer products:
+        Y[m, n] = s_a[m] * ( s_w[n] * acc0[m, n] + sum_{(bn, bk) in S, n in bn} s_rb[n, bk] * acc1_B[m, n] )     (binary64)
+        acc1_B[m, n] = sum_{k in bk} q_a[m, k] q_rb[n, k]                                                     (integers)
+    Returns qa, sa, acc0, acc1sum (= sum over the selected blocks of acc1_B: an integer checksum of the sparse term,
+    what the CUDA parity hook returns), Y, and the tolerance magnitude mag = |s_a| (|s_w acc0| + sum_B |s_rb acc1_B|)."""
+    qa, sa = quantize_act(A)
+    if rows is not None:
+        qa, sa = qa[rows], sa[rows]
+    M, K = qa.shape
+    N, bs = L.N, L.bs
+    a64 = qa.astype(np.int64)
+    acc0 = a64 @ L.d.qw.astype(np.int64).T
+    acc1sum = np.zeros((M, N), np.int64)
+    sparse = np.zeros((M, N), np.float64)
+    smag = np.zeros((M, N), np.float64)
+    for bn, bk in zip(L.blk_n.tolist(), L.blk_k.tolist()):
+        ns, ks = slice(bn * bs, (bn + 1) * bs), slice(bk * bs, (bk + 1) * bs)
+        accB = a64[:, ks] @ L.d.qr[ns, ks].astype(np.int64).T            # [M, bs]
+        sB = L.d.srb[ns, bk].astype(np.float64)[None, :]
+        acc1sum[:, ns] += accB
+        sparse[:, ns] += sB * accB
+        smag[:, ns] += np.abs(sB * accB)
+    sa64, sw64 = sa.astype(np.float64)[:, None], L.d.sw.astype(np.float64)[None, :]
+    Y = sa64 * (sw64 * acc0 + sparse)
+    mag = np.abs(sa64) * (np.abs(sw64 * acc0) + smag)
+    return dict(qa=qa, sa=sa, acc0=acc0, acc1sum=acc1sum, Y=Y, mag=mag)

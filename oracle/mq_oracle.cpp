@@ -14,6 +14,7 @@
 //   O2 activation        P:439-441       per-token dynamic quantization (A5), 4-bit or 8-bit
 //   O3 base weight + R   Alg.1 line 1    P:124, per output channel (A9)
 //   O4 residual Q(R)     Alg.1 / Eq.4    P:106,124, per output channel over all K (A4)
+//   O4b (oracle/__init__.py) the same operator per (output channel, k-block) run: block-local scales (A4b)
 //   O5 h_j               Alg.1 line 2
 //   O6 Delta-score S_B
 //   O7 TopK              P:124,160,378   (A6, A7)
@@ -115,6 +116,13 @@ int orc_num_threads() {
 void orc_quantize_row(const float* x, int64_t L, int8_t* q, float* s) { quantize_row(x, L, q, s); }
 void orc_quantize_row_bits(const float* x, int64_t L, int bits, int8_t* q, float* s) {
   quantize_row(x, L, q, s, bits == 8 ? 127 : 7);
+}
+
+// O1 on every row of a dense fp32 matrix [rows, L] (used for the block-local residual scales, O4b: the rows are
+// the (channel, k-block) runs of R).
+void orc_quantize_rows(const float* X, int64_t rows, int64_t L, int8_t* q /*[rows,L]*/, float* s /*[rows]*/) {
+#pragma omp parallel for schedule(static)
+  for (int64_t r = 0; r < rows; ++r) quantize_row(X + r * L, L, q + r * L, s + r);
 }
 
 // O2 -- per-token activation quantization ("per-token dynamic activation
