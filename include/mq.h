@@ -109,6 +109,26 @@ int mq_pack_prequantized(const int8_t* qW_host, const float* sW_host, int64_t N,
                          int64_t nnz, const int32_t* blk_n_host, const int32_t* blk_k_host,
                          const int8_t* qR_host, const float* sR_host, mq_weights** out,
                          void* cuda_stream);
+/* Block-local residual scales (second half; north_star "residual block list with block coordinates and
+ * per-block scales"; reading A4b).  Eq.1 is applied to R = W - Q(W) inside every block separately: for
+ * block (bn, bk) and output channel n of bn, s_rb[n, bk] = max_{k in bk} |R[n, k]| / 7, q_rb = round(R / s_rb), computed
+ * for EVERY block before selection (so that a block's gain does not depend on the selected set: Theorem 4.1, P:352,
+ * P:368); scores, top-K and tie rule as mq_pack_weights.  The layer computes
+ *     Y[m,n] = s_a[m] * ( s_w[n] * acc0[m,n] + sum_{selected blocks B containing n} s_rb[n, B] * acc1_B[m,n] )    (Eq.4)
+ * with acc1_B the exact integer dot product over the block's 64 / 128 input channels; the block terms are added in
+ * fp32 in ascending K.  mq_pack_prequantized_blockscale takes sRb_host [nnz][block] (scale of every row of every
+ * selected block) instead of sR.  Handles made by these two calls are served by mq_gemm / mq_linear only (any M; the
+ * decode kernel runs them, 32 tokens per pass beyond M = 32; parity hook dbg_acc_res = the integer sum of the block
+ * accumulators); mq_gemm_a8 / mq_gemm_group / mq_gemm_naive return MQ_ERR_UNSUPPORTED_SHAPE for them, and K <= 65536.
+ * mq_weights_export returns sR = all ones for them; mq_weights_export_blockscale returns sRb [nnz][block] in the same
+ * block order; mq_weights_is_blockscale tells the two kinds of handle apart. */
+int mq_pack_weights_blockscale(const float* W_host, int64_t N, int64_t K, const float* h_host, int block,
+                               int64_t budget_blocks, mq_weights** out, void* cuda_stream);
+int mq_pack_prequantized_blockscale(const int8_t* qW_host, const float* sW_host, int64_t N, int64_t K, int block,
+                                    int64_t nnz, const int32_t* blk_n_host, const int32_t* blk_k_host,
+                                    const int8_t* qR_host, const float* sRb_host, mq_weights** out, void* cuda_stream);
+int mq_weights_export_blockscale(const mq_weights* w, float* sRb_host);
+int mq_weights_is_blockscale(const mq_weights* w);
 /* Reads the device layout back and returns the canonical arrays (any pointer may be
  * NULL = skipped).  Blocks are returned sorted by (blk_n, blk_k).  Host call; syncs. */
 int mq_weights_export(const mq_weights* w, int8_t* qW_host, float* sW_host, int64_t* nnz,

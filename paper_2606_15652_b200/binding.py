@@ -24,7 +24,8 @@ EXPORTS = [
     "mq_gemm_workspace_bytes", "mq_gemm", "mq_linear_workspace_bytes", "mq_linear", "mq_linear_host_staging_bytes",
     "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_gemm_naive", "mq_gemm_naive_scratch_bytes", "mq_set_option",
     "mq_last_launch_count", "mq_quantize_act_group", "mq_gemm_group_workspace_bytes", "mq_gemm_group",
-    "mq_probe_int8_peak",
+    "mq_probe_int8_peak", "mq_pack_weights_blockscale", "mq_pack_prequantized_blockscale", "mq_weights_export_blockscale",
+    "mq_weights_is_blockscale",
 ]
 
 _lib = None
@@ -59,6 +60,14 @@ def lib() -> C.CDLL:
     L.mq_pack_weights.argtypes = [vp, i64, i64, vp, i32, i64, C.POINTER(vp), vp]
     L.mq_pack_weights_device.restype = i32
     L.mq_pack_weights_device.argtypes = [vp, i64, i64, vp, i32, i64, C.POINTER(vp), vp]
+    L.mq_pack_weights_blockscale.restype = i32
+    L.mq_pack_weights_blockscale.argtypes = [vp, i64, i64, vp, i32, i64, C.POINTER(vp), vp]
+    L.mq_pack_prequantized_blockscale.restype = i32
+    L.mq_pack_prequantized_blockscale.argtypes = [vp, vp, i64, i64, i32, i64, vp, vp, vp, vp, C.POINTER(vp), vp]
+    L.mq_weights_export_blockscale.restype = i32
+    L.mq_weights_export_blockscale.argtypes = [vp, vp]
+    L.mq_weights_is_blockscale.restype = i32
+    L.mq_weights_is_blockscale.argtypes = [vp]
     L.mq_pack_prequantized.restype = i32
     L.mq_pack_prequantized.argtypes = [vp, vp, i64, i64, i32, i64, vp, vp, vp, vp, C.POINTER(vp), vp]
     L.mq_weights_export.restype = i32
@@ -205,6 +214,16 @@ class Weights:
                                        _np_ptr(qR), _np_ptr(sR)), "mq_weights_export")
         return dict(qW=qW, sW=sW, sR=sR, blk_n=bn[:nnz], blk_k=bk[:nnz], qR=qR[:nnz], nnz=int(n.value))
 
+    def is_blockscale(self) -> bool:
+        return bool(lib().mq_weights_is_blockscale(self.handle))
+
+    def export_blockscale(self) -> np.ndarray:
+        """Block-local residual scales fp32 [nnz, block], blocks in export()'s order (mq_weights_export_blockscale)."""
+        i = self.info()
+        out = np.empty((max(i["nnz"], 1), i["block"]), np.float32)
+        _check(lib().mq_weights_export_blockscale(self.handle, _np_ptr(out)), "mq_weights_export_blockscale")
+        return out[:i["nnz"]]
+
     def clone(self) -> "Weights":
         out = C.c_void_p()
         _check(lib().mq_weights_clone(self.handle, C.byref(out), _stream()), "mq_weights_clone")
@@ -230,6 +249,35 @@ def mq_pack_weights(W: np.ndarray, h: Optional[np.ndarray], block: int, budget_b
     out = C.c_void_p()
     _check(lib().mq_pack_weights(_np_ptr(W), N, K, _np_ptr(h32), block, int(budget_blocks), C.byref(out), _stream()),
            "mq_pack_weights")
+    return Weights(out.value)
+
+
+def mq_pack_weights_blockscale(W: np.ndarray, h: Optional[np.ndarray], block: int, budget_blocks: int) -> Weights:
+    """Algorithm 1 with block-local residual scales (reading A4b) on the host + device layout."""
+    W = np.ascontiguousarray(W, dtype=np.float32)
+    N, K = W.shape
+    h32 = None if h is None else np.ascontiguousarray(h, dtype=np.float32)
+    out = C.c_void_p()
+    _check(lib().mq_pack_weights_blockscale(_np_ptr(W), N, K, _np_ptr(h32), block, int(budget_blocks), C.byref(out), _stream()),
+           "mq_pack_weights_blockscale")
+    return Weights(out.value)
+
+
+def mq_pack_prequantized_blockscale(qW: np.ndarray, sW: np.ndarray, block: int, blk_n: np.ndarray, blk_k: np.ndarray,
+                                    qR: np.ndarray, sRb: np.ndarray) -> Weights:
+    qW = np.ascontiguousarray(qW, np.int8)
+    N, K = qW.shape
+    sW = np.ascontiguousarray(sW, np.float32)
+    sRb = np.ascontiguousarray(sRb, np.float32)
+    blk_n = np.ascontiguousarray(blk_n, np.int32)
+    blk_k = np.ascontiguousarray(blk_k, np.int32)
+    qR = np.ascontiguousarray(qR, np.int8)
+    nnz = int(blk_n.shape[0])
+    out = C.c_void_p()
+    _check(lib().mq_pack_prequantized_blockscale(_np_ptr(qW), _np_ptr(sW), N, K, block, nnz, _np_ptr(blk_n) if nnz else None,
+                                                 _np_ptr(blk_k) if nnz else None, _np_ptr(qR) if nnz else None,
+                                                 _np_ptr(sRb) if nnz else None, C.byref(out), _stream()),
+           "mq_pack_prequantized_blockscale")
     return Weights(out.value)
 
 

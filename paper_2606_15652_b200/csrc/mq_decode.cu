@@ -51,7 +51,10 @@ constexpr int DEC_MAX_KS = 512;        // K-steps whose metadata fits the shared
 
 // BIG: one CTA per SM with a ring of ~200 KB, for long-K layers with few slabs (K >> N): the bytes in flight, not
 // the CTA count, are then what keeps HBM busy (measured: 14336 x 4096 at 32 rows: 10.8 us with 64 KB per CTA in flight)
-template <int RT, int MT, bool BIG = false>
+// BSC: block-local residual scales (reading A4b): every residual piece carries one scale per row; its integer sum is
+// converted and added in fp32 right after its two MMAs (the scale changes along K, so the sums of different blocks
+// cannot share an integer accumulator).
+template <int RT, int MT, bool BIG = false, bool BSC = false>
 struct DCfg {
   static constexpr int R = 16 * RT;                     // output channels per CTA
   static constexpr int KW = DEC_CWARPS / RT;            // K groups (warps that share a row tile)
@@ -64,13 +67,14 @@ struct DCfg {
   static constexpr int T_BYTES = UK * T_KSTEP;
   static constexpr int P_ROWS = R < 64 ? R : 64;        // rows of a residual piece (one k-half of a quarter)
   static constexpr int P_BYTES = P_ROWS * 32;
-  static constexpr int RING = (BIG ? 217088 : 106496) - DEC_QSLOTS * P_BYTES;
+  static constexpr int PS_BYTES = P_BYTES + (BSC ? P_ROWS * 4 : 0);   // ring slot: codes + (BSC) the rows' scales
+  static constexpr int RING = (BIG ? 217088 : 106496) - DEC_QSLOTS * PS_BYTES;
   static constexpr int MAXST = BIG ? 12 : 6;
   static constexpr int STAGES = RING / (W_BYTES + T_BYTES) > MAXST ? MAXST : RING / (W_BYTES + T_BYTES);
   static constexpr int OFF_W = 0;
   static constexpr int OFF_T = OFF_W + STAGES * W_BYTES;
   static constexpr int OFF_Q = OFF_T + STAGES * T_BYTES;
-  static constexpr int OFF_BAR = OFF_Q + DEC_QSLOTS * P_BYTES;
+  static constexpr int OFF_BAR = OFF_Q + DEC_QSLOTS * PS_BYTES;
   static constexpr int OFF_SMETA = OFF_BAR + 2 * STAGES * 8;     // [STAGES] {residual pieces of the stage in the slot | first ring slot << 8}
   static constexpr int OFF_SA = OFF_SMETA + STAGES * 4;          // [32] token scales
   static constexpr int OFF_NP = OFF_SA + 32 * 4;                 // [DEC_MAX_KS / 2] uint16 per stage {pieces | K-steps with pieces << 8}
@@ -78,7 +82,7 @@ struct DCfg {
                                                                  // of the stage's earlier K-steps << 8, first quarter | full mask << 28}
   static constexpr int SMEM_BYTES = OFF_UM + DEC_MAX_KS * 8 + 1024;   // + slack for the 1024-byte alignment
   // the K groups' partial sums [KW][2 accumulators][MT][R] int32 re-use the ring once all stages are consumed
-  static constexpr int RED_BYTES = KW * 2 * MT * R * 4;
+  static constexpr int RED_BYTES = KW * (BSC ? 3 : 2) * MT * R * 4;
   static_assert(KPW >= 1 && KPW * KW == UK, "the K-steps of a stage are dealt evenly to the K groups");
   static_assert(STAGES >= 2, "ring depth");
   static_assert(T_KSTEP % 512 == 0 && W_BYTES % 1024 == 0, "SWIZZLE_64B boxes need 512-byte aligned destinations");
@@ -88,6 +92,7 @@ struct DCfg {
 
 struct DecParams {
   const uint8_t* res;
+  const float* qscale;     // BSC: [n_quarters][64] block-local residual scale of every row of every stored quarter
   const int2* unit_meta;   // [NT * KS] {quarter mask, first quarter index}; NULL = dense only
   const float* sw;
   const float* sr;
@@ -151,10 +156,10 @@ __device__ __forceinline__ void sts_u64(uint32_t addr, uint32_t a, uint32_t b) {
   asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
 }
 
-template <int RT, int MT, bool BIG>
+template <int RT, int MT, bool BIG, bool BSC>
 __global__ void __launch_bounds__(DEC_THREADS, BIG ? 1 : 2)
 mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_a, const DecParams p) {
-  using C = DCfg<RT, MT, BIG>;
+  using C = DCfg<RT, MT, BIG, BSC>;
   constexpr int R = C::R, KW = C::KW, UK = C::UK, KPW = C::KPW, NST = C::NST, STAGES = C::STAGES;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -273,16 +278,17 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
       while (q_issued + np - q_freed > DEC_QSLOTS) advance_to(consumed + 1);   // room in the piece ring
       sts_u32(sSMeta + 4u * (uint32_t)slot, (uint32_t)np | ((uint32_t)(q_issued % DEC_QSLOTS) << 8));
       if (np) {   // only the K-steps that own pieces are visited
-        mbar_expect_tx(fb, (uint32_t)np * C::P_BYTES);
+        mbar_expect_tx(fb, (uint32_t)np * C::PS_BYTES);
         for (uint32_t km = npk >> 8; km; km &= km - 1) {
           const int ks = s * UK + __ffs((int)km) - 1;
           const uint2 um = lds_u64(sUM + 8u * (uint32_t)ks);
           const uint32_t full_mask = um.y >> 28, qoff = um.y & 0x0FFFFFFFu;
           for (uint32_t mm = um.x & 0xF; mm; mm &= mm - 1) {
             const int q = __ffs((int)mm) - 1;
-            const uint8_t* src = p.res + ((size_t)qoff + (size_t)__popc(full_mask & ((1u << q) - 1))) * QUARTER_BYTES +
-                                 (size_t)(row0 & 63) * 16;
-            const uint32_t dst = sQ + (uint32_t)(q_issued % DEC_QSLOTS) * C::P_BYTES;
+            const size_t qidx = (size_t)qoff + (size_t)__popc(full_mask & ((1u << q) - 1));
+            const uint8_t* src = p.res + qidx * QUARTER_BYTES + (size_t)(row0 & 63) * 16;
+            const uint32_t dst = sQ + (uint32_t)(q_issued % DEC_QSLOTS) * C::PS_BYTES;
+            if (BSC) tma_load_1d(dst + C::P_BYTES, p.qscale + qidx * 64 + (size_t)(row0 & 63), C::P_ROWS * 4, fb);
             if (C::P_ROWS == 64) {
               tma_load_1d(dst, src, QUARTER_BYTES, fb);
             } else {   // the slab's rows of the quarter's two 32-channel chunks
@@ -322,6 +328,11 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
   // NST >= 4 already gives four independent chains per chunk); one residual set
   constexpr int NACC = NST >= 4 ? 1 : 2;
   int d0[NACC][NST][4], d1[NST][4];
+  float f1[BSC ? NST : 1][4];   // BSC: sum over the pieces of s_rb * acc1_piece (fp32, K order inside the warp's K-steps)
+#pragma unroll
+  for (int st = 0; st < (BSC ? NST : 1); ++st)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) f1[st][i] = 0.f;
 #pragma unroll
   for (int st = 0; st < NST; ++st)
 #pragma unroll
@@ -364,13 +375,31 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
           if ((mask >> q) & 1) {   // warp-uniform
             const int ps = (slot0 + __popc(mask & ((1u << q) - 1))) % DEC_QSLOTS;
             uint32_t rx[4];
-            ldmatrix_x4(rx, sQ + ps * C::P_BYTES + r_off);
+            ldmatrix_x4(rx, sQ + ps * C::PS_BYTES + r_off);
+            int dp[BSC ? NST : 1][4];   // BSC: this piece's own integer sums
+            if (BSC) {
+#pragma unroll
+              for (int st = 0; st < NST; ++st)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) dp[st][e] = 0;
+            }
 #pragma unroll
             for (int c2 = 0; c2 < 2; ++c2) {
               const int c = 2 * h + c2;
               const uint32_t a0 = (rx[2 * c2] << 4) & HI, a1 = (rx[2 * c2 + 1] << 4) & HI, a2 = rx[2 * c2] & HI, a3 = rx[2 * c2 + 1] & HI;
 #pragma unroll
-              for (int st = 0; st < NST; ++st) mma_s8(d1[st], a0, a1, a2, a3, (bw[st][c] << 4) & HI, bw[st][c] & HI);
+              for (int st = 0; st < NST; ++st) mma_s8(BSC ? dp[st] : d1[st], a0, a1, a2, a3, (bw[st][c] << 4) & HI, bw[st][c] & HI);
+            }
+            if (BSC) {   // Eq.4 with a block-local scale: s_rb[row] * acc1_piece, added in fp32; d1 keeps the integer checksum
+              const uint32_t sp = sQ + ps * C::PS_BYTES + C::P_BYTES + (uint32_t)(((16 * rt) & (C::P_ROWS - 1)) + g) * 4;
+              const float s_lo = __uint_as_float(lds_u32(sp)) * ACC_INV, s_hi = __uint_as_float(lds_u32(sp + 32)) * ACC_INV;
+#pragma unroll
+              for (int st = 0; st < NST; ++st)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                  f1[st][e] += (float)dp[st][e] * (e < 2 ? s_lo : s_hi);
+                  d1[st][e] += dp[st][e];
+                }
             }
           }
         }
@@ -396,22 +425,27 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const int t = 8 * st + 2 * tq + (e & 1), r = 16 * rt + g + (e >> 1) * 8;
-        red[((kw * 2 + 0) * MT + t) * R + r] = d0[0][st][e];
-        red[((kw * 2 + 1) * MT + t) * R + r] = d1[st][e];
+        constexpr int NA = BSC ? 3 : 2;
+        red[((kw * NA + 0) * MT + t) * R + r] = d0[0][st][e];
+        red[((kw * NA + 1) * MT + t) * R + r] = d1[st][e];
+        if (BSC) red[((kw * NA + 2) * MT + t) * R + r] = __float_as_int(f1[st][e]);
       }
   }
   named_bar_sync(1, 32 * DEC_CWARPS);
   DEC_STAMP(ctid == 0, 16);
   for (int e = ctid; e < p.M * R; e += 32 * DEC_CWARPS) {
     const int t = e / R, r = e - t * R;
+    constexpr int NA = BSC ? 3 : 2;
     int a0 = 0, a1 = 0;
+    float fs = 0.f;
 #pragma unroll
     for (int k = 0; k < KW; ++k) {
-      a0 += red[((k * 2 + 0) * MT + t) * R + r];
-      a1 += red[((k * 2 + 1) * MT + t) * R + r];
+      a0 += red[((k * NA + 0) * MT + t) * R + r];
+      a1 += red[((k * NA + 1) * MT + t) * R + r];
+      if (BSC) fs += __int_as_float(red[((k * NA + 2) * MT + t) * R + r]);   // K groups in ascending order
     }
     const int n = r0 + r;
-    const float y = __uint_as_float(lds_u32(sSA + 4u * (uint32_t)t)) * ((float)a0 * ep_sw + (float)a1 * ep_sr);
+    const float y = __uint_as_float(lds_u32(sSA + 4u * (uint32_t)t)) * (BSC ? (float)a0 * ep_sw + fs : (float)a0 * ep_sw + (float)a1 * ep_sr);
     const size_t o = (size_t)t * p.ldy + n;
     if (p.y_bf16)
       reinterpret_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
@@ -452,15 +486,15 @@ int pick_rows(const mq_weights* w, int64_t M) {
 unsigned long long* g_dec_trace = nullptr;
 #endif
 
-template <int RT, int MT, bool BIG>
+template <int RT, int MT, bool BIG, bool BSC = false>
 int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
-  using C = DCfg<RT, MT, BIG>;
+  using C = DCfg<RT, MT, BIG, BSC>;
   // the attribute belongs to the (device, function) pair: set it whenever the current device changes
   static int attr_dev = -1;
   int dev = -1;
   cudaGetDevice(&dev);
   if (dev != attr_dev) {
-    if (cudaFuncSetAttribute(mq_decode_kernel<RT, MT, BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    if (cudaFuncSetAttribute(mq_decode_kernel<RT, MT, BIG, BSC>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
     }
@@ -476,7 +510,7 @@ int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = options().pdl ? 1 : 0;
-  if (cudaLaunchKernelEx(&cfg, mq_decode_kernel<RT, MT, BIG>, tmw, tma, dp) != cudaSuccess) {
+  if (cudaLaunchKernelEx(&cfg, mq_decode_kernel<RT, MT, BIG, BSC>, tmw, tma, dp) != cudaSuccess) {
     cudaGetLastError();
     return MQ_ERR_CUDA;
   }
@@ -484,7 +518,14 @@ int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& 
 }
 
 template <int RT>
-int dec_launch_mt(int MT, bool big, const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
+int dec_launch_mt(int MT, bool big, bool bsc, const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
+  if (bsc) {   // block-local residual scales (small ring only)
+    switch (MT) {
+      case 8: return dec_launch<RT, 8, false, true>(tmw, tma, dp, grid, st);
+      case 16: return dec_launch<RT, 16, false, true>(tmw, tma, dp, grid, st);
+      default: return dec_launch<RT, 32, false, true>(tmw, tma, dp, grid, st);
+    }
+  }
   if (big) {   // (rows <= 64 only: the deep ring is for layers with few slabs)
     if constexpr (RT <= 4) {
       switch (MT) {
@@ -541,7 +582,10 @@ int build_weight_tmaps(mq_weights* w) {
 
 bool decode_eligible(const mq_weights* w, int64_t M) {
   const Options& o = options();
-  if (!w || M <= 0 || M > 32 || !w->tmap_ok) return false;
+  if (!w || M <= 0 || !w->tmap_ok) return false;
+  // block-local residual scales exist in this kernel only: it serves every M (32 tokens per pass) whatever the knobs say
+  if (w->blockscale) return w->K / BK <= DEC_MAX_KS;
+  if (M > 32) return false;
   // the tcgen05 kernel's own knobs select that kernel (tests and ablations address it through them)
   if (o.decode_path == 1 || o.token_tile != 0 || o.split_k >= 2 || o.max_ctas != 0 || o.fused_quant) return false;
   return w->K / BK <= DEC_MAX_KS;
@@ -549,8 +593,28 @@ bool decode_eligible(const mq_weights* w, int64_t M) {
 
 size_t decode_workspace_bytes(const mq_weights*, int64_t) { return 0; }
 
+static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res);
+
+// M <= 32: one launch.  More tokens (block-local scales only): passes of 32 tokens, each streaming the weights again
+// (from L2 when the layer fits) -- a first path for that reading at prefill sizes, not a fast one.
 int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
                 int32_t* dbg0, int32_t* dbg1, void*, size_t, void* cuda_stream, bool ignore_res) {
+  int launches = 0;
+  for (int64_t m0 = 0; m0 < M; m0 += 32) {
+    const int64_t mc = std::min<int64_t>(32, M - m0);
+    const int rc = decode_gemm_pass(w, (const uint8_t*)qA + (size_t)m0 * (size_t)(w->K / 2), sA + m0, mc,
+                                    (uint8_t*)Y + (size_t)m0 * (size_t)ldy * 2, y_dtype, ldy, dbg0 ? dbg0 + (size_t)m0 * w->N : nullptr,
+                                    dbg1 ? dbg1 + (size_t)m0 * w->N : nullptr, cuda_stream, ignore_res);
+    if (rc != MQ_OK) return rc;
+    ++launches;
+  }
+  set_launch_count(launches);
+  return MQ_OK;
+}
+
+static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res) {
   const int rows = pick_rows(w, M);
   const int MT = M <= 8 ? 8 : (M <= 16 ? 16 : 32);
   // 3-D tensor map over the canonical packed activations [M rows][K/2 bytes]: {64 B of a K-step, M rows, KS K-steps};
@@ -571,6 +635,7 @@ int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M,
 
   DecParams dp;
   dp.res = w->d_res;
+  dp.qscale = w->d_qscale;
   dp.unit_meta = (ignore_res || w->nnz == 0) ? nullptr : (const int2*)w->d_unit_meta;
   dp.sw = w->d_sw;
   dp.sr = w->d_sr;
@@ -595,12 +660,11 @@ int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M,
   const CUtensorMap& tmw = w->tmap_base[rt_index(rows)];
   int rc;
   switch (rows) {
-    case 16: rc = dec_launch_mt<1>(MT, big, tmw, tmap, dp, grid, st); break;
-    case 32: rc = dec_launch_mt<2>(MT, big, tmw, tmap, dp, grid, st); break;
-    case 64: rc = dec_launch_mt<4>(MT, big, tmw, tmap, dp, grid, st); break;
-    default: rc = dec_launch_mt<8>(MT, big, tmw, tmap, dp, grid, st); break;
+    case 16: rc = dec_launch_mt<1>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
+    case 32: rc = dec_launch_mt<2>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
+    case 64: rc = dec_launch_mt<4>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
+    default: rc = dec_launch_mt<8>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
   }
-  if (rc == MQ_OK) set_launch_count(1);
   return rc;
 }
 

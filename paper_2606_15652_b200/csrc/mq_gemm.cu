@@ -1523,6 +1523,8 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return MQ_ERR_CUDA;
 
+  // block-local residual scales (reading A4b) exist in the decode kernel only
+  if (w->blockscale && (fused || a8 || !mq::decode_eligible(w, M))) return MQ_ERR_UNSUPPORTED_SHAPE;
   // decode shapes: the lean TMEM-free kernel (mq_decode.cu)
   if (!fused && !a8 && mq::decode_eligible(w, M))
     return mq::decode_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, ignore_res);
@@ -1725,6 +1727,7 @@ extern "C" int mq_gemm_naive(const mq_weights* w, const void* qA, const float* s
                              int64_t ldy, void* workspace, size_t workspace_bytes, int32_t* scratch, size_t scratch_bytes,
                              void* cuda_stream) {
   if (!w) return MQ_ERR_INVALID_ARG;
+  if (w->blockscale) return MQ_ERR_UNSUPPORTED_SHAPE;   // block-local residual scales: mq_gemm only
   if (M > 0 && (!scratch || ((uintptr_t)scratch & 3))) return MQ_ERR_INVALID_ARG;
   if (M > 0 && scratch_bytes < mq_gemm_naive_scratch_bytes(w, M)) return MQ_ERR_WORKSPACE;
   const int rc = gemm_impl(w, qA, sA, M, Y, y_dtype, ldy, nullptr, nullptr, workspace, workspace_bytes, cuda_stream, nullptr,

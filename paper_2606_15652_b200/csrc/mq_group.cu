@@ -484,6 +484,7 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
                              int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
                              void* cuda_stream) {
   if (!w) return MQ_ERR_INVALID_ARG;
+  if (w->blockscale) return MQ_ERR_UNSUPPORTED_SHAPE;   // block-local residual scales: mq_gemm only
   if (M < 0 || !group_ok(group)) return MQ_ERR_UNSUPPORTED_SHAPE;
   if (y_dtype != MQ_F16 && y_dtype != MQ_BF16) return MQ_ERR_INVALID_ARG;
   if (M == 0) {

@@ -61,6 +61,10 @@ struct mq_weights {
   int32_t* d_cell_ptr = nullptr;       // [N/BN + 1]
   mq::CellMeta* d_cell_meta = nullptr; // [n_cells]
   int32_t* d_unit_meta = nullptr;      // [N/BN][K/BK][2] dense index of the cells: {quarter mask, first quarter}
+  // block-local residual scales (reading A4b; mq_pack_*_blockscale): one scale per row of every stored quarter,
+  // float [n_quarters][64]; d_sr is then unused (all ones)
+  bool blockscale = false;
+  float* d_qscale = nullptr;
   // host copies of the small metadata (used by the launcher and by export)
   std::vector<int32_t> h_cell_ptr;
   std::vector<mq::CellMeta> h_cell_meta;

@@ -63,6 +63,7 @@ inline int quant1(float x, float s) {
 struct SelBlock {
   int32_t bn, bk;
   std::vector<int8_t> q;  // [block][block], row = n, col = k
+  std::vector<float> srow;  // [block] block-local residual scale of every row (blockscale layers only)
 };
 
 struct HostLayer {
@@ -71,6 +72,7 @@ struct HostLayer {
   std::vector<uint8_t> base;  // tiled, see mq_internal.h
   std::vector<float> sw, sr;
   std::vector<SelBlock> blocks;
+  bool blockscale = false;   // reading A4b: the residual scale is per (selected block, row), not per output channel
 };
 
 inline size_t base_offset(int64_t n, int64_t k, int64_t K) {
@@ -143,8 +145,11 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   w->h_cell_ptr.assign((size_t)NT + 1, 0);
 
   std::vector<uint8_t> res((size_t)qs.size() * QUARTER_BYTES, 0);
+  std::vector<float> qscale(L.blockscale ? qs.size() * 64 : 0, 1.0f);
   for (size_t i = 0; i < qs.size(); ++i) {
     const Q& e = qs[i];
+    if (L.blockscale)
+      for (int row = 0; row < 64; ++row) qscale[i * 64 + (size_t)row] = e.b->srow[(size_t)(e.sub_r * 64 + row)];
     if (i == 0 || qs[i - 1].key != e.key) {
       CellMeta m;
       m.kstep_mask = (int32_t)(e.key % KS);
@@ -175,7 +180,8 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   size_t o_cptr = align_up(o_res + std::max<size_t>(res.size(), 16), 256);
   size_t o_cmeta = align_up(o_cptr + ((size_t)NT + 1) * 4, 256);
   size_t o_umeta = align_up(o_cmeta + std::max<size_t>((size_t)w->n_cells, 1) * sizeof(CellMeta), 256);
-  size_t total = align_up(o_umeta + (size_t)NT * KS * 8, 256);
+  size_t o_qscale = align_up(o_umeta + (size_t)NT * KS * 8, 256);
+  size_t total = align_up(o_qscale + std::max<size_t>(qscale.size() * 4, 16), 256);
   // dense per-(n-tile, K-step) lookup of the CSR cells: {quarter mask, first quarter index}
   std::vector<int32_t> umeta((size_t)NT * KS * 2, 0);
   for (int64_t t = 0; t < NT; ++t)
@@ -205,6 +211,8 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
     ok &= cudaMemcpyAsync(p + o_cmeta, w->h_cell_meta.data(), (size_t)w->n_cells * sizeof(CellMeta),
                           cudaMemcpyHostToDevice, stream) == cudaSuccess;
   ok &= cudaMemcpyAsync(p + o_umeta, umeta.data(), umeta.size() * 4, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+  if (!qscale.empty())
+    ok &= cudaMemcpyAsync(p + o_qscale, qscale.data(), qscale.size() * 4, cudaMemcpyHostToDevice, stream) == cudaSuccess;
   ok &= cudaStreamSynchronize(stream) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
@@ -221,6 +229,8 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
   w->d_cell_ptr = (int32_t*)(p + o_cptr);
   w->d_cell_meta = (CellMeta*)(p + o_cmeta);
   w->d_unit_meta = (int32_t*)(p + o_umeta);
+  w->blockscale = L.blockscale;
+  w->d_qscale = (float*)(p + o_qscale);
   if (mq::build_weight_tmaps(w) != MQ_OK) {
     cudaFree(blob);
     delete w;
@@ -232,12 +242,34 @@ int finalize(HostLayer& L, mq_weights** out, cudaStream_t stream) {
 
 }  // namespace
 
+namespace {
+int pack_prequantized_impl(const int8_t* qW, const float* sW, int64_t N, int64_t K, int block, int64_t nnz,
+                           const int32_t* blk_n, const int32_t* blk_k, const int8_t* qR, const float* sR, const float* sRb,
+                           mq_weights** out, void* cuda_stream);
+}
+
 extern "C" int mq_pack_prequantized(const int8_t* qW, const float* sW, int64_t N, int64_t K, int block, int64_t nnz,
                                     const int32_t* blk_n, const int32_t* blk_k, const int8_t* qR, const float* sR,
                                     mq_weights** out, void* cuda_stream) {
+  if (!sR) return MQ_ERR_INVALID_ARG;
+  return pack_prequantized_impl(qW, sW, N, K, block, nnz, blk_n, blk_k, qR, sR, nullptr, out, cuda_stream);
+}
+
+extern "C" int mq_pack_prequantized_blockscale(const int8_t* qW, const float* sW, int64_t N, int64_t K, int block, int64_t nnz,
+                                               const int32_t* blk_n, const int32_t* blk_k, const int8_t* qR, const float* sRb,
+                                               mq_weights** out, void* cuda_stream) {
+  if (nnz > 0 && !sRb) return MQ_ERR_INVALID_ARG;
+  static const float one = 1.0f;
+  return pack_prequantized_impl(qW, sW, N, K, block, nnz, blk_n, blk_k, qR, nullptr, nnz > 0 ? sRb : &one, out, cuda_stream);
+}
+
+namespace {
+int pack_prequantized_impl(const int8_t* qW, const float* sW, int64_t N, int64_t K, int block, int64_t nnz,
+                           const int32_t* blk_n, const int32_t* blk_k, const int8_t* qR, const float* sR, const float* sRb,
+                           mq_weights** out, void* cuda_stream) {
   if (!out) return MQ_ERR_INVALID_ARG;
   *out = nullptr;
-  if (!qW || !sW || !sR || nnz < 0) return MQ_ERR_INVALID_ARG;
+  if (!qW || !sW || nnz < 0) return MQ_ERR_INVALID_ARG;
   if (nnz > 0 && (!blk_n || !blk_k || !qR)) return MQ_ERR_INVALID_ARG;
   int rc = shape_check(N, K, block);
   if (rc != MQ_OK) return rc;
@@ -254,7 +286,11 @@ extern "C" int mq_pack_prequantized(const int8_t* qW, const float* sW, int64_t N
   try {
     L.base.assign((size_t)N * (size_t)K / 2, 0);
     L.sw.assign(sW, sW + N);
-    L.sr.assign(sR, sR + N);
+    if (sR)
+      L.sr.assign(sR, sR + N);
+    else
+      L.sr.assign((size_t)N, 1.0f);
+    L.blockscale = sRb != nullptr;
     L.blocks.resize((size_t)nnz);
   } catch (const std::bad_alloc&) {
     return MQ_ERR_OOM;
@@ -274,16 +310,32 @@ extern "C" int mq_pack_prequantized(const int8_t* qW, const float* sW, int64_t N
     b.bn = blk_n[e];
     b.bk = blk_k[e];
     b.q.assign(qR + (size_t)e * bsz, qR + (size_t)(e + 1) * bsz);
+    if (sRb) b.srow.assign(sRb + (size_t)e * block, sRb + (size_t)(e + 1) * block);
     for (int8_t v : b.q)
       if (v < -7 || v > 7) bad = 1;
   }
   if (bad) return MQ_ERR_INVALID_ARG;
   return finalize(L, out, (cudaStream_t)cuda_stream);
 }
+}  // namespace
 
 // Algorithm 1, in the paper's order.
+namespace {
+int pack_weights_impl(const float* W, int64_t N, int64_t K, const float* h, int block, int64_t budget, bool blockscale,
+                      mq_weights** out, void* cuda_stream);
+}
 extern "C" int mq_pack_weights(const float* W, int64_t N, int64_t K, const float* h, int block, int64_t budget,
                                mq_weights** out, void* cuda_stream) {
+  return pack_weights_impl(W, N, K, h, block, budget, false, out, cuda_stream);
+}
+// Algorithm 1 with block-local residual scales (reading A4b): Q(R) of Eq.1 is applied to every (channel, k-block) run.
+extern "C" int mq_pack_weights_blockscale(const float* W, int64_t N, int64_t K, const float* h, int block, int64_t budget,
+                                          mq_weights** out, void* cuda_stream) {
+  return pack_weights_impl(W, N, K, h, block, budget, true, out, cuda_stream);
+}
+namespace {
+int pack_weights_impl(const float* W, int64_t N, int64_t K, const float* h, int block, int64_t budget, bool blockscale,
+                      mq_weights** out, void* cuda_stream) {
   if (!out) return MQ_ERR_INVALID_ARG;
   *out = nullptr;
   if (!W || budget < 0) return MQ_ERR_INVALID_ARG;
@@ -297,6 +349,7 @@ extern "C" int mq_pack_weights(const float* W, int64_t N, int64_t K, const float
   L.N = N;
   L.K = K;
   L.block = block;
+  L.blockscale = blockscale;
   std::vector<double> score;
   try {
     L.base.assign((size_t)N * (size_t)K / 2, 0);
@@ -322,10 +375,12 @@ extern "C" int mq_pack_weights(const float* W, int64_t N, int64_t K, const float
         put_nibble(&L.base[base_offset(n, k, K)], (int)(k & 1), q);
         R[(size_t)k] = (float)((double)w[k] - (double)s * (double)q);  // Alg.1 line 1
       }
-      const float sr = row_scale(R.data(), K);  // Q(R): per output channel over all K (A4)
-      L.sr[(size_t)n] = sr;
+      const float sr_row = row_scale(R.data(), K);  // Q(R): per output channel over all K (A4)
+      L.sr[(size_t)n] = blockscale ? 1.0f : sr_row;
       // P:156  S_B = [ sum h R^2 - sum h (R - Q(R))^2 ]_+ ; rows ascending, k ascending
       for (int64_t bk = 0; bk < nbk; ++bk) {
+        // A4b: the scale of this row inside this block
+        const float sr = blockscale ? row_scale(R.data() + bk * block, block) : sr_row;
         double a = gain[(size_t)bk], b = loss[(size_t)bk];
         for (int64_t k = bk * block; k < (bk + 1) * block; ++k) {
           double r = (double)R[(size_t)k];
@@ -363,20 +418,25 @@ extern "C" int mq_pack_weights(const float* W, int64_t N, int64_t K, const float
     b.bn = (int32_t)(cand[(size_t)e] / nbk);
     b.bk = (int32_t)(cand[(size_t)e] % nbk);
     b.q.resize((size_t)block * block);
+    if (blockscale) b.srow.resize((size_t)block);
+    std::vector<float> rr((size_t)block);
     for (int i = 0; i < block; ++i) {
       int64_t n = (int64_t)b.bn * block + i;
-      const float s = L.sw[(size_t)n], sr = L.sr[(size_t)n];
+      const float s = L.sw[(size_t)n];
       for (int j = 0; j < block; ++j) {
         int64_t k = (int64_t)b.bk * block + j;
         float wv = W[n * K + k];
         int q = quant1(wv, s);
-        float r = (float)((double)wv - (double)s * (double)q);
-        b.q[(size_t)i * block + j] = (int8_t)quant1(r, sr);
+        rr[(size_t)j] = (float)((double)wv - (double)s * (double)q);
       }
+      const float sr = blockscale ? row_scale(rr.data(), block) : L.sr[(size_t)n];
+      if (blockscale) b.srow[(size_t)i] = sr;
+      for (int j = 0; j < block; ++j) b.q[(size_t)i * block + j] = (int8_t)quant1(rr[(size_t)j], sr);
     }
   });
   return finalize(L, out, (cudaStream_t)cuda_stream);
 }
+}  // namespace
 
 // ------------------------------------------------------------------------------------------------------
 // Algorithm 1 on the device: the O(N*K) part -- base quantization, residual, Q(R) and the
@@ -664,6 +724,46 @@ extern "C" int mq_weights_export(const mq_weights* w, int8_t* qW, float* sW, int
   return MQ_OK;
 }
 
+extern "C" int mq_weights_is_blockscale(const mq_weights* w) { return w && w->blockscale ? 1 : 0; }
+
+// the block-local residual scales of a blockscale layer, [nnz][block], blocks in mq_weights_export's order
+extern "C" int mq_weights_export_blockscale(const mq_weights* w, float* sRb) {
+  if (!w || !sRb) return MQ_ERR_INVALID_ARG;
+  if (!w->blockscale) return MQ_ERR_INVALID_ARG;
+  const int64_t NT = w->N / BN;
+  std::vector<float> qs((size_t)w->n_quarters * 64);
+  if (!qs.empty() && cudaMemcpy(qs.data(), w->d_qscale, qs.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return MQ_ERR_CUDA;
+  struct Out {
+    int32_t bn, bk;
+    int64_t q_r0, q_r1;   // a quarter holding rows 0..63 / 64..127 of the block (block = 64: q_r0 only)
+  };
+  std::vector<Out> outs;
+  for (int64_t t = 0; t < NT; ++t)
+    for (int32_t c = w->h_cell_ptr[(size_t)t]; c < w->h_cell_ptr[(size_t)t + 1]; ++c) {
+      const CellMeta& m = w->h_cell_meta[(size_t)c];
+      const int ks = m.kstep_mask & 0xFFFFFF, mask = (m.kstep_mask >> 24) & 0xF;
+      int64_t qi = m.qoff;
+      if (w->block == 128) {
+        outs.push_back(Out{(int32_t)t, (int32_t)ks, qi, qi + 1});   // quarters q = 2h + r in ascending q: (h0,r0), (h0,r1), ...
+      } else {
+        for (int q = 0; q < 4; ++q)
+          if (mask & (1 << q)) {
+            outs.push_back(Out{(int32_t)(2 * t + (q & 1)), (int32_t)(2 * ks + (q >> 1)), qi, 0});
+            ++qi;
+          }
+      }
+    }
+  std::sort(outs.begin(), outs.end(), [](const Out& a, const Out& b) { return a.bn != b.bn ? a.bn < b.bn : a.bk < b.bk; });
+  if ((int64_t)outs.size() != w->nnz) return MQ_ERR_CUDA;
+  const int bs = w->block;
+  for (size_t e = 0; e < outs.size(); ++e) {
+    for (int row = 0; row < 64; ++row) sRb[e * (size_t)bs + (size_t)row] = qs[(size_t)outs[e].q_r0 * 64 + (size_t)row];
+    if (bs == 128)
+      for (int row = 0; row < 64; ++row) sRb[e * (size_t)bs + 64 + (size_t)row] = qs[(size_t)outs[e].q_r1 * 64 + (size_t)row];
+  }
+  return MQ_OK;
+}
+
 extern "C" int mq_weights_clone(const mq_weights* w, mq_weights** out, void* cuda_stream) {
   if (!w || !out) return MQ_ERR_INVALID_ARG;
   *out = nullptr;
@@ -693,6 +793,7 @@ extern "C" int mq_weights_clone(const mq_weights* w, mq_weights** out, void* cud
   c->d_cell_ptr = (int32_t*)((uint8_t*)w->d_cell_ptr + d);
   c->d_cell_meta = (CellMeta*)((uint8_t*)w->d_cell_meta + d);
   c->d_unit_meta = (int32_t*)((uint8_t*)w->d_unit_meta + d);
+  c->d_qscale = (float*)((uint8_t*)w->d_qscale + d);
   if (mq::build_weight_tmaps(c) != MQ_OK) {
     cudaFree(blob);
     delete c;
