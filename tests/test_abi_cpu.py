@@ -35,7 +35,8 @@ def test_header_symbols_all_exported(mqlib):
 
 def test_binding_has_same_names(mqlib):
     for n in _declared_symbols():
-        if n in ("mq_status_string", "mq_weights_export", "mq_weights_info", "mq_weights_free", "mq_weights_clone"):
+        if n in ("mq_status_string", "mq_weights_export", "mq_weights_info", "mq_weights_free", "mq_weights_clone",
+                 "mq_weights_export_blockscale", "mq_weights_is_blockscale"):
             continue  # exposed as status_string / Weights methods
         assert hasattr(mqlib, n), n
 
