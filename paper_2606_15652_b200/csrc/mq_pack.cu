@@ -438,225 +438,6 @@ int pack_weights_impl(const float* W, int64_t N, int64_t K, const float* h, int 
 }
 }  // namespace
 
-// ------------------------------------------------------------------------------------------------------
-// Algorithm 1 on the device: the O(N*K) part -- base quantization, residual, Q(R) and the
-// Delta-Hessian block scores -- runs in one kernel, one CTA per block-row; the top-K over
-// the N*K/block^2 scores stays on the host (it is tiny), and a second kernel quantizes the selected blocks.
-// The arithmetic is mq_pack_weights', operation for operation: binary32 division and round-half-even for
-// Eq.1, the residual in fp64 rounded once to fp32, and the two score sums in fp64 WITHOUT contraction in the
-// host's order (rows ascending, k ascending, one running sum per block), so that both give the same bits.
-namespace {
-
-__device__ __forceinline__ int dev_quant1(float x, float s) {
-  const int v = (int)rintf(__fdiv_rn(x, s));
-  return v > 7 ? 7 : (v < -7 ? -7 : v);
-}
-__device__ __forceinline__ float dev_block_max(float v, float* red) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
-  __syncthreads();   // red[] may still be read from the previous call
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-  __syncthreads();
-  float m = red[0];
-  for (int i = 1; i < (int)(blockDim.x >> 5); ++i) m = fmaxf(m, red[i]);
-  return m;
-}
-
-constexpr int ALG1_THREADS = 256;
-constexpr int ALG1_MAX_OWN = 8;   // k-blocks per thread: K <= 8 * 256 * block
-
-__global__ void __launch_bounds__(ALG1_THREADS) alg1_score_kernel(const float* __restrict__ W, const float* __restrict__ h,
-                                                                  int64_t K, int block, uint8_t* __restrict__ base,
-                                                                  float* __restrict__ sw, float* __restrict__ sr,
-                                                                  double* __restrict__ score) {
-  extern __shared__ float Rrow[];   // the residual of the current row, [K]
-  __shared__ float red[ALG1_THREADS / 32];
-  const int tid = threadIdx.x;
-  const int64_t bn = blockIdx.x;
-  const int nbk = (int)(K / block);
-  double gain[ALG1_MAX_OWN], loss[ALG1_MAX_OWN];
-#pragma unroll
-  for (int i = 0; i < ALG1_MAX_OWN; ++i) gain[i] = loss[i] = 0.0;
-  for (int r = 0; r < block; ++r) {
-    const int64_t n = bn * block + r;
-    const float* w = W + n * K;
-    float amax = 0.f;
-    for (int64_t k = tid; k < K; k += ALG1_THREADS) amax = fmaxf(amax, fabsf(w[k]));
-    amax = dev_block_max(amax, red);
-    const float s = amax == 0.f ? 1.0f : __fdiv_rn(amax, 7.0f);   // Eq.1, q_max = 7 (A1-A3)
-    float rmax = 0.f;
-    for (int64_t kp = tid; kp < K / 2; kp += ALG1_THREADS) {      // two consecutive k = one packed byte
-      const int64_t k = 2 * kp;
-      const float2 wv = *reinterpret_cast<const float2*>(w + k);
-      const int q0 = dev_quant1(wv.x, s), q1 = dev_quant1(wv.y, s);
-      const float r0 = __double2float_rn(__dsub_rn((double)wv.x, __dmul_rn((double)s, (double)q0)));   // Alg.1 line 1
-      const float r1 = __double2float_rn(__dsub_rn((double)wv.y, __dmul_rn((double)s, (double)q1)));
-      Rrow[k] = r0;
-      Rrow[k + 1] = r1;
-      rmax = fmaxf(rmax, fmaxf(fabsf(r0), fabsf(r1)));
-      const int64_t tile = (n / BN) * (K / BK) + k / BK;
-      const size_t off = (size_t)tile * TILE_BYTES + (size_t)((k % BK) >> 5) * (BN * 16) + (size_t)(n % BN) * 16 + (size_t)((k & 31) >> 1);
-      base[off] = (uint8_t)((q0 & 0xF) | ((q1 & 0xF) << 4));
-    }
-    rmax = dev_block_max(rmax, red);   // (its barriers also publish Rrow)
-    const float srn = rmax == 0.f ? 1.0f : __fdiv_rn(rmax, 7.0f);   // Q(R): per output channel over all K (A4)
-    if (tid == 0) {
-      sw[n] = s;
-      sr[n] = srn;
-    }
-#pragma unroll
-    for (int i = 0; i < ALG1_MAX_OWN; ++i) {
-      const int bk = tid + i * ALG1_THREADS;
-      if (bk < nbk) {
-        double a = gain[i], b = loss[i];
-        for (int k = bk * block; k < (bk + 1) * block; ++k) {
-          const float rf = Rrow[k];
-          const double rr = (double)rf;
-          const double e = __dsub_rn(rr, __dmul_rn((double)srn, (double)dev_quant1(rf, srn)));
-          const double hk = h ? (double)h[k] : 1.0;
-          a = __dadd_rn(a, __dmul_rn(hk, __dmul_rn(rr, rr)));   // P:156, no contraction: the host's bits
-          b = __dadd_rn(b, __dmul_rn(hk, __dmul_rn(e, e)));
-        }
-        gain[i] = a;
-        loss[i] = b;
-      }
-    }
-    __syncthreads();   // Rrow is overwritten by the next row
-  }
-#pragma unroll
-  for (int i = 0; i < ALG1_MAX_OWN; ++i) {
-    const int bk = tid + i * ALG1_THREADS;
-    if (bk < nbk) {
-      const double d = __dsub_rn(gain[i], loss[i]);
-      score[bn * nbk + bk] = d > 0.0 ? d : 0.0;
-    }
-  }
-}
-
-// Q(R) of the selected blocks: q [nnz][block][block] int8 (row = n, col = k)
-__global__ void alg1_resq_kernel(const float* __restrict__ W, int64_t K, int block, const float* __restrict__ sw,
-                                 const float* __restrict__ sr, const int32_t* __restrict__ sel_bn,
-                                 const int32_t* __restrict__ sel_bk, int8_t* __restrict__ q) {
-  const int64_t e = blockIdx.x;
-  const int64_t n0 = (int64_t)sel_bn[e] * block, k0 = (int64_t)sel_bk[e] * block;
-  for (int idx = threadIdx.x; idx < block * block; idx += blockDim.x) {
-    const int i = idx / block, j = idx - i * block;
-    const float s = sw[n0 + i], srn = sr[n0 + i];
-    const float wv = W[(n0 + i) * K + k0 + j];
-    const int qb = dev_quant1(wv, s);
-    const float r = __double2float_rn(__dsub_rn((double)wv, __dmul_rn((double)s, (double)qb)));
-    q[(size_t)e * block * block + idx] = (int8_t)dev_quant1(r, srn);
-  }
-}
-
-}  // namespace
-
-extern "C" int mq_pack_weights_device(const float* W_dev, int64_t N, int64_t K, const float* h_dev, int block, int64_t budget,
-                                      mq_weights** out, void* cuda_stream) {
-  if (!out) return MQ_ERR_INVALID_ARG;
-  *out = nullptr;
-  if (!W_dev || budget < 0) return MQ_ERR_INVALID_ARG;
-  int rc = shape_check(N, K, block);
-  if (rc != MQ_OK) return rc;
-  rc = mq::check_device();
-  if (rc != MQ_OK) return rc;
-  const int64_t nbn = N / block, nbk = K / block, nblocks = nbn * nbk;
-  if (nbk > (int64_t)ALG1_MAX_OWN * ALG1_THREADS || (size_t)K * sizeof(float) > 200 * 1024) return MQ_ERR_UNSUPPORTED_SHAPE;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  HostLayer L;
-  L.N = N;
-  L.K = K;
-  L.block = block;
-  std::vector<double> score;
-  try {
-    L.base.assign((size_t)N * (size_t)K / 2, 0);
-    L.sw.assign((size_t)N, 0.f);
-    L.sr.assign((size_t)N, 0.f);
-    score.assign((size_t)nblocks, 0.0);
-  } catch (const std::bad_alloc&) {
-    return MQ_ERR_OOM;
-  }
-  uint8_t* d_base = nullptr;
-  float *d_sw = nullptr, *d_sr = nullptr;
-  double* d_score = nullptr;
-  int32_t *d_bn = nullptr, *d_bk = nullptr;
-  int8_t* d_q = nullptr;
-  auto cleanup = [&]() {
-    cudaFree(d_base); cudaFree(d_sw); cudaFree(d_sr); cudaFree(d_score); cudaFree(d_bn); cudaFree(d_bk); cudaFree(d_q);
-  };
-  if (cudaMalloc(&d_base, L.base.size()) != cudaSuccess || cudaMalloc(&d_sw, (size_t)N * 4) != cudaSuccess ||
-      cudaMalloc(&d_sr, (size_t)N * 4) != cudaSuccess || cudaMalloc(&d_score, (size_t)nblocks * 8) != cudaSuccess) {
-    cleanup();
-    (void)cudaGetLastError();
-    return MQ_ERR_OOM;
-  }
-  const size_t smem = (size_t)K * sizeof(float);
-  if (cudaFuncSetAttribute(alg1_score_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
-    cleanup();
-    return MQ_ERR_CUDA;
-  }
-  alg1_score_kernel<<<(unsigned)nbn, ALG1_THREADS, smem, st>>>(W_dev, h_dev, K, block, d_base, d_sw, d_sr, d_score);
-  bool ok = cudaMemcpyAsync(L.base.data(), d_base, L.base.size(), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
-            cudaMemcpyAsync(L.sw.data(), d_sw, (size_t)N * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
-            cudaMemcpyAsync(L.sr.data(), d_sr, (size_t)N * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
-            cudaMemcpyAsync(score.data(), d_score, (size_t)nblocks * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
-            cudaStreamSynchronize(st) == cudaSuccess;
-  if (!ok) {
-    cleanup();
-    (void)cudaGetLastError();
-    return MQ_ERR_CUDA;
-  }
-  // TopK: positive scores only, ties -> lower index (A7); as in mq_pack_weights.
-  std::vector<int64_t> cand;
-  for (int64_t b = 0; b < nblocks; ++b)
-    if (score[(size_t)b] > 0.0) cand.push_back(b);
-  const int64_t nnz = std::min<int64_t>(budget, (int64_t)cand.size());
-  auto better = [&](int64_t x, int64_t y) {
-    if (score[(size_t)x] != score[(size_t)y]) return score[(size_t)x] > score[(size_t)y];
-    return x < y;
-  };
-  std::partial_sort(cand.begin(), cand.begin() + nnz, cand.end(), better);
-  cand.resize((size_t)nnz);
-  L.blocks.resize((size_t)nnz);
-  if (nnz > 0) {
-    std::vector<int32_t> hbn((size_t)nnz), hbk((size_t)nnz);
-    for (int64_t e = 0; e < nnz; ++e) {
-      hbn[(size_t)e] = (int32_t)(cand[(size_t)e] / nbk);
-      hbk[(size_t)e] = (int32_t)(cand[(size_t)e] % nbk);
-    }
-    const size_t qbytes = (size_t)nnz * block * block;
-    std::vector<int8_t> hq;
-    try {
-      hq.resize(qbytes);
-    } catch (const std::bad_alloc&) {
-      cleanup();
-      return MQ_ERR_OOM;
-    }
-    ok = cudaMalloc(&d_bn, (size_t)nnz * 4) == cudaSuccess && cudaMalloc(&d_bk, (size_t)nnz * 4) == cudaSuccess &&
-         cudaMalloc(&d_q, qbytes) == cudaSuccess &&
-         cudaMemcpyAsync(d_bn, hbn.data(), (size_t)nnz * 4, cudaMemcpyHostToDevice, st) == cudaSuccess &&
-         cudaMemcpyAsync(d_bk, hbk.data(), (size_t)nnz * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
-    if (ok) {
-      alg1_resq_kernel<<<(unsigned)nnz, 256, 0, st>>>(W_dev, K, block, d_sw, d_sr, d_bn, d_bk, d_q);
-      ok = cudaMemcpyAsync(hq.data(), d_q, qbytes, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
-           cudaStreamSynchronize(st) == cudaSuccess;
-    }
-    if (!ok) {
-      cleanup();
-      (void)cudaGetLastError();
-      return MQ_ERR_CUDA;
-    }
-    for (int64_t e = 0; e < nnz; ++e) {
-      SelBlock& b = L.blocks[(size_t)e];
-      b.bn = hbn[(size_t)e];
-      b.bk = hbk[(size_t)e];
-      b.q.assign(hq.begin() + (size_t)e * block * block, hq.begin() + (size_t)(e + 1) * block * block);
-    }
-  }
-  cleanup();
-  return finalize(L, out, st);
-}
-
 extern "C" int mq_weights_export(const mq_weights* w, int8_t* qW, float* sW, int64_t* nnz, int32_t* blk_n,
                                  int32_t* blk_k, int8_t* qR, float* sR) {
   if (!w) return MQ_ERR_INVALID_ARG;
