@@ -254,6 +254,10 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
  *                 "max_ctas" or "fused_quant" also selects the tcgen05 kernel.
  *   "decode_rows": 0 = automatic, else 16 / 32 / 64 / 128 output channels per CTA of the decode kernel
  *   "decode_big": 0 = automatic, 1 = deep shared-memory ring (one CTA per SM; rows <= 64), 2 = small ring (two per SM)
+ *   "prefill_path": 0 (default) = mq_gemm with M >= 64 runs the whole-tile tcgen05 kernel (128 x 128 output tiles dealt
+ *                 round-robin to persistent CTAs, no workspace) when the last round of tiles is at least 88 % full,
+ *                 else the stream-K tcgen05 kernel; 1 = never; 2 = for every M >= 64.  The stream-K knobs above
+ *                 ("token_tile", "split_k" >= 2, "max_ctas") also select the stream-K kernel.
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
  *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */

@@ -88,6 +88,10 @@ struct Cfg {
   static constexpr int SK = BT <= 32 ? 4 : 2;                    // K-steps per P stage
   static constexpr int UK = BT <= 32 ? 4 : (BT == 64 ? 2 : (MQ_BT128_UK2 ? 2 : 1));   // K-steps per U stage (item)
   static constexpr int IPS = SK / UK;                            // items per P stage
+  // PAIR (prefill tile): the two U stages that hold the two K-steps of one P stage share ONE full / empty barrier pair,
+  // and the MMA warp issues their 8 base MMAs (+ residual MMAs) as one elected block: the MMA queue is shallow, so every
+  // instruction between two K-steps' MMAs is pipe idle time (profiles/r2_probe_int8.md)
+  static constexpr bool PAIR = BT == 128 && UK == 1 && SK == 2;
   static constexpr int PSTAGES = A8 ? (BT == 16 ? 4 : (BT == 32 ? 3 : (BT == 64 ? 4 : 3)))
                                     : (BT <= 32 ? 4 : (BT == 64 ? 6 : 4));
   static constexpr int USTAGES = G;                                   // one per unpack group
@@ -378,7 +382,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
       mbar_init(bar(B_EMPTY_P + i), 4 * IPS);   // one arrival per unpack warp per item
     }
     for (int i = 0; i < C::USTAGES; ++i) {
-      mbar_init(bar(B_FULL_U + i), 4);
+      mbar_init(bar(B_FULL_U + i), C::PAIR ? 8 : 4);   // PAIR: barriers 0, 1 serve stages {0, 1}, {2, 3}
       mbar_init(bar(B_EMPTY_U + i), 1);
     }
     for (int i = 0; i < C::NQ; ++i) {
@@ -719,7 +723,64 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         return;
       }
     };
-    if constexpr (UK == 1) {
+    if constexpr (C::PAIR) {
+      // Prefill tile: one iteration = one P stage = the two K-steps in U stages {2 pr, 2 pr + 1}: one barrier wait,
+      // one elected block with up to 8 base MMAs and the cells' MMAs, one commit.
+      for (int item0 = 0; item0 < n_items; item0 += C::USTAGES) {
+        const uint32_t uphase = ((uint32_t)item0 / C::USTAGES) & 1;
+#pragma unroll
+        for (int pr = 0; pr < 2; ++pr) {
+          if (item0 + 2 * pr >= n_items) break;
+          MQ_ACC_BEGIN(tw_u);
+          mbar_wait(bar(B_FULL_U + pr), uphase);
+          MQ_ACC_END(tw_u);
+          tc_fence_after();
+          const int m0 = lds32(sMetaU + 4u * (uint32_t)(2 * pr)), m1 = lds32(sMetaU + 4u * (uint32_t)(2 * pr + 1));
+          const bool v1 = (m1 & META_VALID) != 0;            // (the first K-step of a P stage always exists)
+          if (m0 & META_FIRST) seg_first();
+          const int mask0 = m0 & 0xF, mask1 = v1 ? (m1 & 0xF) : 0;
+          if ((mask0 | mask1) && !acc1_on) {
+            // first residual MMA of the segment: the epilogue must have drained this acc1 stage
+            mbar_wait(bar(B_A1E + a1s), (((uint32_t)seg / C::ACC1_STAGES) & 1) ^ 1);
+            tc_fence_after();
+          }
+          __syncwarp();
+          if (elect_one()) {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              if (j == 1 && !v1) break;
+              const int us = 2 * pr + j;
+              const uint32_t at = tmem_base + (uint32_t)(C::A_COL0 + us * A_COLS);
+              const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE);
+#pragma unroll
+              for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, (j == 0 && k == 0) ? acc0_on : 1u);
+            }
+            uint32_t on = acc1_on;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              const int mask = j == 0 ? mask0 : mask1;
+              if (!mask) continue;
+              const int us = 2 * pr + j;
+              const uint32_t rt = tmem_base + (uint32_t)(C::R_COL0 + us * A_COLS);   // the cell rides in its U stage
+              const uint64_t dt = make_desc_sw128(sU + us * C::U_STAGE);
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+                if (mask & (3 << (2 * h))) {
+#pragma unroll
+                  for (int k = 2 * h; k < 2 * h + 2; ++k) {
+                    mma_i8_ts(d1, rt + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
+                    on = 1;
+                  }
+                }
+            }
+            tc_commit(bar(B_EMPTY_U + pr));
+          }
+          acc0_on = 1;
+          if (mask0 | mask1) acc1_on = 1;
+          if ((v1 ? m1 : m0) & META_LAST) seg_last();
+        }
+      }
+    } else if constexpr (UK == 1) {
       // Prefill: the U stages are visited in a fixed rotation and the loop is unrolled over them, so
       // that every barrier address, TMEM column and shared-memory descriptor of the hot path is a
       // constant offset (this warp's instruction count per K-step is what paces prefill).
@@ -783,7 +844,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(B_EMPTY_P + ps));   // this warp's reads of the P stage are done
         MQ_ACC_BEGIN(tu_eu);
-        mbar_wait(bar(B_EMPTY_U + us), (((uint32_t)item / C::USTAGES) & 1) ^ 1);
+        mbar_wait(bar(B_EMPTY_U + (C::PAIR ? us >> 1 : us)), (((uint32_t)item / C::USTAGES) & 1) ^ 1);
         MQ_ACC_END(tu_eu);
         MQ_ACC_BEGIN(tu_work);
         tc_fence_after();
@@ -854,7 +915,7 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
           MQ_STAMP_IF(gi == 0 && gtid == 0 && item < 32, 16 + item / 2);
           MQ_STAMP_IF(gi == 0 && gtid == 0, 6);
           if (wq == 0) sts32(sMetaU + 4u * (uint32_t)us, m);
-          mbar_arrive(bar(B_FULL_U + us));
+          mbar_arrive(bar(B_FULL_U + (C::PAIR ? us >> 1 : us)));
         }
         MQ_ACC_END(tu_work);
         continue;
@@ -1528,6 +1589,9 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   // decode shapes: the lean TMEM-free kernel (mq_decode.cu)
   if (!fused && !a8 && mq::decode_eligible(w, M))
     return mq::decode_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, ignore_res);
+  // prefill shapes whose whole tiles fill the machine: the whole-tile kernel (mq_prefill.cu)
+  if (!fused && !a8 && mq::prefill_eligible(w, M))
+    return mq::prefill_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream, ignore_res);
 
   const Plan pl = make_plan(w, M);
   if (pl.units >= (int64_t)1 << 31) return MQ_ERR_UNSUPPORTED_SHAPE;

@@ -89,6 +89,7 @@ struct Options {
   int64_t decode_path = 0;      // 0 = automatic (M <= 32 runs the lean mma.sync decode kernel), 1 = off (tcgen05 kernel)
   int64_t decode_big = 0;       // decode kernel ring: 0 = automatic, 1 = deep (one CTA per SM), 2 = small (two per SM)
   int64_t decode_rows = 0;      // 0 = automatic, else 16 / 32 / 64 / 128 output channels per CTA of the decode kernel
+  int64_t prefill_path = 0;     // 0 = automatic (whole-tile kernel where its last round is mostly full), 1 = off, 2 = always
 };
 Options& options();
 void set_launch_count(int n);
@@ -113,6 +114,10 @@ size_t decode_workspace_bytes(const mq_weights* w, int64_t M);
 int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
                 int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
                 void* cuda_stream, bool ignore_res);
+// the whole-tile prefill kernel (mq_prefill.cu): M >= 64, per-token W4A4, needs no workspace
+bool prefill_eligible(const mq_weights* w, int64_t M);
+int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
+                 int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res);
 int build_weight_tmaps(mq_weights* w);   // MQ_OK or MQ_ERR_CUDA
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency); NULL if absent
 void* tensor_map_encode_fn();
