@@ -215,7 +215,7 @@ extern "C" int mq_set_option(const char* name, int64_t value) {
     if (value != 0 && value != 16 && value != 32 && value != 64 && value != 128) return MQ_ERR_INVALID_ARG;
     o.decode_rows = value;
   } else if (!strcmp(name, "prefill_path")) {
-    if (value > 2) return MQ_ERR_INVALID_ARG;
+    if (value > 3) return MQ_ERR_INVALID_ARG;
     o.prefill_path = value;
   } else if (!strcmp(name, "group_simt")) {
     if (value > 1) return MQ_ERR_INVALID_ARG;
