@@ -713,7 +713,7 @@ bool prefill_eligible(const mq_weights* w, int64_t M) {
   const int64_t tiles = (w->N / BN) * ((M + PF_BT - 1) / PF_BT) / (pairs ? 2 : 1);
   const int64_t slots = pairs ? sm_count() / 2 : sm_count();
   const int64_t rounds = (tiles + slots - 1) / slots;
-  return tiles * 100 >= rounds * slots * 88;
+  return tiles * 100 >= rounds * slots * 50;
 }
 
 int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
