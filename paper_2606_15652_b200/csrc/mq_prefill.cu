@@ -601,8 +601,8 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
       uint16_t* yp0 = reinterpret_cast<uint16_t*>(p.Y) + (size_t)t_base * p.ldy + n;
       // 8-token batches, two in flight: the TMEM loads of batch b+1 run under the arithmetic and the stores of batch b.
       // FULL = whole token tile and no parity hooks: branch-free, one pointer bump per token.
-      auto drain = [&](auto res_c, auto bf_c, auto full_c) {
-        constexpr bool RES = decltype(res_c)::value, BF = decltype(bf_c)::value, FULL = decltype(full_c)::value;
+      auto drain = [&](auto res_c, auto bf_c) {
+        constexpr bool RES = decltype(res_c)::value, BF = decltype(bf_c)::value;
         uint16_t* yp = yp0;
         uint32_t a[2][8], r[2][8];
 #pragma unroll
@@ -616,24 +616,13 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
             float y = (float)(int32_t)av[i] * swn;
             if (RES) y += (float)(int32_t)rv[i] * srn;
             y *= sv[i];
-            const uint16_t h = BF ? __bfloat16_as_ushort(__float2bfloat16_rn(y)) : __half_as_ushort(__float2half_rn(y));
-            if (FULL) {
-              *yp = h;
-            } else if (b * 8 + i < t_cnt) {
-              *yp = h;
-              const size_t di = (size_t)(t_base + b * 8 + i) * p.N + n;
-              if (p.dbg0) p.dbg0[di] = (int32_t)av[i] >> 8;
-#ifndef PF_TRACE
-              if (p.dbg1) p.dbg1[di] = RES ? ((int32_t)rv[i] >> 8) : 0;
-#endif
-            }
+            *yp = BF ? __bfloat16_as_ushort(__float2bfloat16_rn(y)) : __half_as_ushort(__float2half_rn(y));
             yp += p.ldy;
           }
         };
         tmem_ld8(t0addr, a[0]);
         if (RES) tmem_ld8(t1addr, r[0]);
-        // (a rolled loop of two batches: the fully unrolled form of all variants was 700 KB of code, and the
-        // instruction-cache misses it caused showed up in every other warp's chain)
+        // (a rolled loop of two batches: the fully unrolled form of all variants was 700 KB of code)
 #pragma unroll 1
         for (int b = 0; b < PF_BT / 8; b += 2) {
           tmem_ld_wait8(a[0], r[0]);
@@ -648,14 +637,39 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
           emit8(a[1], r[1], b + 1);
         }
       };
-      auto drain2 = [&](auto res_c, auto bf_c) {
-        if (t_cnt == PF_BT && !p.dbg0 && !p.dbg1) drain(res_c, bf_c, std::true_type{});
-        else drain(res_c, bf_c, std::false_type{});
-      };
-      if (has_res) {
-        if (p.y_bf16) drain2(std::true_type{}, std::true_type{}); else drain2(std::true_type{}, std::false_type{});
+      if (t_cnt == PF_BT && !p.dbg0 && !p.dbg1) {
+        if (has_res) {
+          if (p.y_bf16) drain(std::true_type{}, std::true_type{}); else drain(std::true_type{}, std::false_type{});
+        } else {
+          if (p.y_bf16) drain(std::false_type{}, std::true_type{}); else drain(std::false_type{}, std::false_type{});
+        }
       } else {
-        if (p.y_bf16) drain2(std::false_type{}, std::true_type{}); else drain2(std::false_type{}, std::false_type{});
+        // ragged last token tile, or the parity hooks are on: one generic loop, same operation order
+#pragma unroll 1
+        for (int b = 0; b < PF_BT / 8; ++b) {
+          if (b * 8 >= t_cnt) break;
+          uint32_t a[8], r[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) r[i] = 0;
+          tmem_ld8(t0addr + b * 8, a);
+          if (has_res) tmem_ld8(t1addr + b * 8, r);
+          tmem_ld_wait8(a, r);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int t = b * 8 + i;
+            if (t < t_cnt) {
+              float y = (float)(int32_t)a[i] * swn;
+              if (has_res) y += (float)(int32_t)r[i] * srn;
+              y *= sat[t];
+              yp0[(size_t)t * p.ldy] = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y)) : __half_as_ushort(__float2half_rn(y));
+              const size_t di = (size_t)(t_base + t) * p.N + n;
+              if (p.dbg0) p.dbg0[di] = (int32_t)a[i] >> 8;
+#ifndef PF_TRACE
+              if (p.dbg1) p.dbg1[di] = has_res ? ((int32_t)r[i] >> 8) : 0;
+#endif
+            }
+          }
+        }
       }
       // accumulators drained: hand them back to the MMA warp
       tc_fence_before();
