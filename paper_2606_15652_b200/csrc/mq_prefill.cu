@@ -1,30 +1,34 @@
-// mq_prefill.cu -- the fused base + residual int4 GEMM for PREFILL shapes (M > 32 tokens, many whole tiles):
+// mq_prefill.cu -- the fused base + residual int4 GEMM for PREFILL shapes (M >= 64 tokens, many whole tiles):
 // Eq.4, ZipperEngine on the tensor-bound side of the roofline.
 //
 // Same arithmetic and the same building blocks as mq_gemm.cu (weights expanded int4 -> int8 x16 in registers and
 // written to TENSOR MEMORY as the MMA's A operand, tokens expanded into K-major SWIZZLE_128B shared memory as its B
 // operand, tcgen05.mma kind::i8, base and residual accumulators in TMEM, fp32 epilogue), re-cut around what this
-// round's measurements showed (profiles/r2_probe_int8.md):
-//   * the tensor pipe sustains 95 % of peak on 128 x 128 x 32 instructions if it is fed, but its queue is shallow:
-//     every instruction the issuing warp executes between two MMAs is pipe idle time;
-//   * a single-thread role pays ~7 cycles per instruction, so the TMA producer's loop must be a handful of
-//     instructions per stage (in mq_gemm.cu it computes all residual bookkeeping: ~150 instructions per two K-steps,
-//     and the unpack groups wait for it a quarter of the time);
-//   * the base accumulator must be double-buffered (the MMA warp waited 15 % of the time for the epilogue).
+// round's measurements showed (profiles/r2_probe_int8.md, r2_ncu_prefill_gate_up_m8192.md):
+//   * the tensor pipe runs at half speed while other agents write shared and tensor memory, so bytes moved per MAC
+//     are what counts: CTA PAIRS (tcgen05.mma.cta_group::2, M = 256) halve the token expansion and the pipe's
+//     shared-memory operand reads per SM;
+//   * nobody's chain may contain a shared-memory round trip it does not need: the residual metadata lives in lanes
+//     (one coalesced load per 32 K-steps), every role derives the item sequence from it by itself, the MMA warp polls
+//     the next item's barrier before it issues the current item's MMAs;
+//   * the base accumulator is double-buffered: the epilogue of a tile overlaps the K-loop of the next.
 // Tensor memory (512 columns): acc0 2 x 128 | acc1 128 | A operand ring 4 x 32.  There is no room left for a residual
 // operand, so a residual cell is an ITEM OF ITS OWN in the operand ring: right after the base item of its K-step, its
 // expanded weights take the next A stage and its MMAs re-use the token tile of the base item (the paper's re-use of the
 // quantized activation tile), accumulating into acc1 (s_r != s_w).
 //
-// Work: whole output tiles (128 output channels x 128 tokens), tile T = nt * TT + tt, dealt round-robin to the
-// persistent CTAs (concurrent CTAs share n-tiles: the weights stay in L2).  Roles (22 warps, one CTA per SM):
-//   warp 0      producer (one thread): per P stage = two K-steps: one bulk copy of 16 KB packed weights, two tensor
-//               copies of packed tokens [128 x 64 B], the two K-steps' residual metadata (prefetched one stage ahead)
-//   warps 6-21  four unpack groups of four warps; items (base K-step, or residual cell) are dealt to them in rotation.
-//               Base item: packed weights -> int8 x16 -> tcgen05.st; packed tokens -> int8 x16 -> swizzled smem.
-//               Residual item: the cell's packed quarters straight from global memory (rare: ~6 % of the K-steps).
-//   warp 1      MMA issuer: per item one barrier wait, one elected block, one commit
-//   warps 2-5   epilogue: tcgen05.ld, y = s_a (s_w acc0 + s_r acc1), 16-bit stores; overlaps the next tile's K-loop
+// Work: whole output tiles (128 output channels x 128 tokens; PAIR: 256 x 128 per cluster, each CTA its own n-tile and
+// 64 of the tokens), tile T = n * TT + tt, dealt round-robin to the persistent CTAs / clusters (concurrent ones share
+// n-tiles: weights and tokens stay in L2).  Roles (22 warps, one CTA per SM):
+//   warp 0      producer (one thread): per K-step one bulk copy of 8 KB packed weights and one tensor copy of packed
+//               tokens [128 (64) x 64 B] into a ring of 8 (16) stages
+//   warps 6-21  four unpack groups of four warps; item i (base K-step, or residual cell) belongs to group i mod 4 and
+//               to operand stage i mod 4.  Base item: packed weights -> int8 x16 -> tcgen05.st; packed tokens -> int8
+//               x16 -> swizzled shared memory.  Residual item: the cell's packed quarters straight from global memory.
+//   warp 1      MMA issuer (PAIR: the leader CTA's; the peer's only derives the per-tile residual flag)
+//   warps 2-5   epilogue: tcgen05.ld, y = s_a (s_w acc0 + s_r acc1), 16-bit stores
+// PAIR synchronisation: the unpack groups and epilogue warps of both CTAs arrive on the LEADER's barriers (remote
+// mbarrier.arrive through mapa), the leader's tcgen05.commit multicasts to the barrier of the same name in both CTAs.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
@@ -189,6 +193,9 @@ __device__ __forceinline__ void tc_commit2(uint32_t bar) {
 #ifndef PF_EXP_NOS
 #define PF_EXP_NOS 0
 #endif
+#ifndef PF_EXP_NOTMA   // the producer signals its stages without copying anything
+#define PF_EXP_NOTMA 0
+#endif
 #ifdef PF_TRACE   // development: clock stamps of CTA 0 into the dbg1 buffer (8 words per tile)
 #define PF_STAMP(cond, it, slot) do { if (blockIdx.x == 0 && (cond)) reinterpret_cast<long long*>(p.dbg1)[(it) * 8 + (slot)] = clock64(); } while (0)
 #define PF_ADD(cond, it, slot, v) do { if (blockIdx.x == 0 && (cond)) reinterpret_cast<long long*>(p.dbg1)[(it) * 8 + (slot)] += (v); } while (0)
@@ -301,6 +308,10 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
           const uint32_t ps = q % PF_PST;
           mbar_wait(bar(PF_B_EMPTY_P + ps), ((q / PF_PST) & 1) ^ 1);
           const uint32_t fb = bar(PF_B_FULL_P + ps), dst = sP + ps * PF_P_STAGE;
+          if (PF_EXP_NOTMA) {
+            mbar_arrive(fb);
+            continue;
+          }
           mbar_arrive_expect_tx(fb, TILE_BYTES + TOK_BYTES);
           tma_load_1d(dst, wsrc + (size_t)ks * TILE_BYTES, TILE_BYTES, fb);
           tma_load_2d(dst + TILE_BYTES, &tmap_a, ks * (BK / 2), tt * PF_BT + (int)rank * TOKR, fb);
