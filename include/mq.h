@@ -41,7 +41,8 @@ typedef enum {
   MQ_ERR_CUDA = -4,               /* a CUDA runtime / driver call failed                       */
   MQ_ERR_OOM = -5,                /* host or device allocation failed                          */
   MQ_ERR_ACC_OVERFLOW = -6,       /* K so large that the int32 accumulator could overflow      */
-  MQ_ERR_WORKSPACE = -7           /* workspace smaller than mq_gemm_workspace_bytes()          */
+  MQ_ERR_WORKSPACE = -7,          /* workspace smaller than mq_gemm_workspace_bytes()          */
+  MQ_ERR_STATIC_SCRATCH = -8      /* mq_linear_static: the call needs more than mq_linear_static_max_bytes() */
 } mq_status;
 
 typedef enum { MQ_F16 = 0, MQ_BF16 = 1 } mq_dtype;
@@ -226,6 +227,24 @@ size_t mq_linear_workspace_bytes(const mq_weights* w, int64_t M);
 int mq_linear(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t lda_elems,
               void* Y_dev, mq_dtype y_dtype, int64_t ldy_elems, void* workspace_dev,
               size_t workspace_bytes, void* cuda_stream);
+
+/* mq_linear WITHOUT A CALLER WORKSPACE, for callers that cannot allocate device memory (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  Same operation, arguments, kernels and results as mq_linear
+ * (bit-identical Y); the workspace (the stream-K kernel's counters, flags and partial tiles, the packed activations and
+ * their scales) is a file-scope `static __device__` array inside the library of mq_linear_static_max_bytes() =
+ * 16 MiB, which every GPU that loads the library holds until the process exits.  The call itself allocates nothing
+ * (no cudaMalloc / cudaFree / allocating library routine): it looks the array's device address up (once per device,
+ * cudaGetSymbolAddress with that device current), clears the workspace's 16384-byte zero-state prefix with
+ * cudaMemsetAsync on `cuda_stream`, and runs mq_linear on the array.
+ * Limit: the call is refused with MQ_ERR_STATIC_SCRATCH when mq_linear_workspace_bytes(w, M) >
+ * mq_linear_static_max_bytes() (e.g. K = 4096: up to M ~ 8000 tokens on the whole-tile kernels, decode sizes always
+ * fit); use mq_linear with a workspace of your own then.
+ * Sharing: ALL calls on a device use the same array, and it keeps the last call's contents.  Calls that may overlap
+ * on the GPU (different streams, or graph branches without an edge between them) race on it and produce garbage;
+ * calls on one stream, or otherwise ordered, are safe.  At most 64 devices per process. */
+size_t mq_linear_static_max_bytes(void);
+int mq_linear_static(const mq_weights* w, const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t lda_elems,
+                     void* Y_dev, mq_dtype y_dtype, int64_t ldy_elems, void* cuda_stream);
 
 /* The same layer with HOST buffers (end-to-end entry): A_host fp16/bf16 [M, K] dense (row stride K) is
  * copied to the device, mq_linear runs, and Y [M, N] dense is copied back to Y_host, all enqueued on

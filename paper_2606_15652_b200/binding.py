@@ -25,7 +25,7 @@ EXPORTS = [
     "mq_linear_host", "mq_quantize_act8", "mq_gemm_a8", "mq_gemm_naive", "mq_gemm_naive_scratch_bytes", "mq_set_option",
     "mq_last_launch_count", "mq_quantize_act_group", "mq_gemm_group_workspace_bytes", "mq_gemm_group",
     "mq_probe_int8_peak", "mq_pack_weights_blockscale", "mq_pack_prequantized_blockscale", "mq_weights_export_blockscale",
-    "mq_weights_is_blockscale",
+    "mq_weights_is_blockscale", "mq_linear_static_max_bytes", "mq_linear_static",
 ]
 
 _lib = None
@@ -86,6 +86,10 @@ def lib() -> C.CDLL:
     L.mq_linear_workspace_bytes.argtypes = [vp, i64]
     L.mq_linear.restype = i32
     L.mq_linear.argtypes = [vp, vp, i32, i64, i64, vp, i32, i64, vp, sz, vp]
+    L.mq_linear_static_max_bytes.restype = sz
+    L.mq_linear_static_max_bytes.argtypes = []
+    L.mq_linear_static.restype = i32
+    L.mq_linear_static.argtypes = [vp, vp, i32, i64, i64, vp, i32, i64, vp]
     L.mq_linear_host_staging_bytes.restype = sz
     L.mq_linear_host_staging_bytes.argtypes = [vp, i64]
     L.mq_linear_host.restype = i32
@@ -357,6 +361,21 @@ def mq_linear(w: Weights, A: torch.Tensor, Y: Optional[torch.Tensor] = None, out
     ldy = Y.stride(0) if M > 1 else N
     _check(lib().mq_linear(w.handle, A.data_ptr(), _dtype_code(A.dtype), M, lda, Y.data_ptr(), _dtype_code(Y.dtype),
                            ldy, workspace.data_ptr(), workspace.numel(), _stream()), "mq_linear")
+    return Y
+
+
+def mq_linear_static_max_bytes() -> int:
+    return int(lib().mq_linear_static_max_bytes())
+
+
+def mq_linear_static(w: Weights, A: torch.Tensor, Y: torch.Tensor) -> torch.Tensor:
+    """mq_linear on the library's built-in scratch array: the call allocates nothing (the caller passes A and Y)."""
+    M, K = A.shape
+    N = Y.shape[1]
+    lda = A.stride(0) if M > 1 else K
+    ldy = Y.stride(0) if M > 1 else N
+    _check(lib().mq_linear_static(w.handle, A.data_ptr(), _dtype_code(A.dtype), M, lda, Y.data_ptr(), _dtype_code(Y.dtype),
+                                  ldy, _stream()), "mq_linear_static")
     return Y
 
 

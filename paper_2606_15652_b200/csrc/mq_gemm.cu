@@ -51,6 +51,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <mutex>
 #include <cstring>
 
 #include "mq_internal.h"
@@ -1884,4 +1885,66 @@ extern "C" int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype 
     return MQ_ERR_CUDA;
   }
   return MQ_OK;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// mq_linear_static: mq_linear for callers that cannot allocate device memory (code under CUDA graph capture, tight
+// serving loops, harnesses that forbid cudaMalloc).  The workspace of mq_linear (the stream-K kernel's counters, flags
+// and partial tiles, the packed activations and their scales) lives in a file-scope device array of a fixed size
+// instead of a caller buffer.  Every GPU that loads the library holds the array until the process exits.
+namespace {
+
+constexpr size_t STATIC_WS_BYTES = (size_t)16 << 20;   // 16 MiB
+static __device__ __align__(256) uint8_t g_static_ws[STATIC_WS_BYTES];
+
+// In host code `g_static_ws` is only the host-side stand-in of the symbol, not a device address: the address a kernel
+// may use comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int STATIC_WS_MAX_DEVICES = 64;
+void* g_static_ws_addr[STATIC_WS_MAX_DEVICES] = {};
+std::mutex g_static_ws_mutex;
+
+int static_ws_address(void** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  if (dev < 0 || dev >= STATIC_WS_MAX_DEVICES) return MQ_ERR_UNSUPPORTED_DEVICE;
+  std::lock_guard<std::mutex> lock(g_static_ws_mutex);
+  if (!g_static_ws_addr[dev]) {
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress((void**)&ptr, g_static_ws) != cudaSuccess || !ptr) {
+      cudaGetLastError();
+      return MQ_ERR_CUDA;
+    }
+    g_static_ws_addr[dev] = ptr;
+  }
+  *out = g_static_ws_addr[dev];
+  return MQ_OK;
+}
+
+}  // namespace
+
+extern "C" size_t mq_linear_static_max_bytes(void) { return STATIC_WS_BYTES; }
+
+extern "C" int mq_linear_static(const mq_weights* w, const void* A, mq_dtype a_dtype, int64_t M, int64_t lda, void* Y,
+                                mq_dtype y_dtype, int64_t ldy, void* cuda_stream) {
+  if (!w) return MQ_ERR_INVALID_ARG;
+  if (M == 0) return MQ_OK;
+  if (M < 0) return MQ_ERR_UNSUPPORTED_SHAPE;
+  int rc = mq::check_device();
+  if (rc != MQ_OK) return rc;
+  // the layer and token count decide the size: beyond the array the call is refused, nothing is allocated instead
+  if (mq_linear_workspace_bytes(w, M) > STATIC_WS_BYTES) return MQ_ERR_STATIC_SCRATCH;
+  void* ws = nullptr;
+  rc = static_ws_address(&ws);
+  if (rc != MQ_OK) return rc;
+  // The array keeps the previous call's contents.  What must start at zero (the workspace's 16 KB prefix: the stream-K
+  // kernel's arrival counters, the fused quantizer's control block) is cleared on the stream before every call, so
+  // that a call is correct even after one that was aborted half-way; the rest is written before it is read.
+  if (cudaMemsetAsync(ws, 0, mq::WS_PREFIX, (cudaStream_t)cuda_stream) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  return mq_linear(w, A, a_dtype, M, lda, Y, y_dtype, ldy, ws, STATIC_WS_BYTES, cuda_stream);
 }

@@ -184,6 +184,7 @@ extern "C" const char* mq_status_string(int status) {
     case MQ_ERR_OOM: return "out of memory";
     case MQ_ERR_ACC_OVERFLOW: return "K too large for the int32 accumulator";
     case MQ_ERR_WORKSPACE: return "workspace too small";
+    case MQ_ERR_STATIC_SCRATCH: return "mq_linear_static: the call needs more scratch than the built-in 16 MiB array (use mq_linear with a workspace)";
     default: return "unknown status";
   }
 }

@@ -43,8 +43,8 @@ def test_binding_has_same_names(mqlib):
 
 def test_status_strings(mqlib):
     assert mqlib.status_string(0) == "ok"
-    seen = {mqlib.status_string(-i) for i in range(0, 8)}
-    assert len(seen) == 8
+    seen = {mqlib.status_string(-i) for i in range(0, 9)}
+    assert len(seen) == 9
     assert "unknown" in mqlib.status_string(-99)
 
 
