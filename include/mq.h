@@ -257,6 +257,16 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
                    mq_dtype y_dtype, void* staging_dev, size_t staging_bytes, void* workspace_dev,
                    size_t workspace_bytes, void* cuda_stream);
 
+/* Concurrency and co-residency.  The decode kernel (M <= 32) and the whole-tile prefill kernels (M >= 64) contain no
+ * wait of one CTA for another (CTA pairs are clusters, co-scheduled by the hardware), so calls on different streams may
+ * overlap freely.  The stream-K kernel (the remaining shapes, mq_gemm_a8, option-selected paths) splits the K range of
+ * a tile over S CTAs that WAIT for each other's partial tiles: its grid (<= the device's SM count, one CTA per SM) must
+ * be co-resident.  That holds when the call has the GPU to itself; it does not hold under an MPS active-thread
+ * percentage or a green context that exposes fewer SMs than cudaDevAttrMultiProcessorCount, or while another
+ * long-running kernel holds SMs (including a second stream-K call on another stream): the waiting CTAs then run into
+ * the kernel's watchdog (__trap, which poisons the context) instead of hanging.  In such environments set option
+ * "split_k" = 1 (whole tiles per CTA, nothing waits) and leave "fused_quant" at 0. */
+
 /* Tuning / ablation knobs.  They are PROCESS-WIDE globals read at call time without locking: set them while no
  * other thread is inside a library call (benchmarks and tests do; a serving process leaves the defaults).  The
  * compute calls themselves keep no other mutable state and may be issued from several threads on distinct

@@ -43,8 +43,9 @@
 // stays bit-identical), waits until all S partials are visible and finishes 1/S of the tile.  The
 // wait needs the S contributors co-resident (grid <= SM count, one CTA per SM): an environment that
 // exposes fewer SMs than cudaDevAttrMultiProcessorCount (MPS active-thread percentage, green contexts)
-// must run this kernel with option split_k = 1 (whole tiles, nothing waits).  Decode shapes (M <= 32)
-// do not come here by default: mq_decode.cu serves them with a ticket scheme in which nobody waits.
+// must run this kernel with option split_k = 1 (whole tiles, nothing waits).  Decode shapes (M <= 32) and
+// prefill shapes (M >= 64) do not come here by default: mq_decode.cu (row slabs: no CTA ever waits for another)
+// and mq_prefill.cu (whole tiles; CTA pairs are co-scheduled by the hardware as clusters) serve them.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
