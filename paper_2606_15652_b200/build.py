@@ -16,7 +16,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libmq.so")
-SOURCES = ["mq_quant.cu", "mq_pack.cu", "mq_gemm.cu", "mq_group.cu", "mq_decode.cu", "mq_prefill.cu", "mq_pack_device.cu", "mq_probe.cu"]
+SOURCES = ["mq_quant.cu", "mq_pack.cu", "mq_gemm.cu", "mq_group.cu", "mq_group_tc.cu", "mq_decode.cu", "mq_prefill.cu", "mq_pack_device.cu", "mq_probe.cu"]
 HEADERS = ["mq_internal.h", "mq_ptx.cuh", os.path.join("..", "..", "include", "mq.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [

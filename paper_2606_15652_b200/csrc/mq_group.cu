@@ -496,9 +496,14 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
     return MQ_ERR_INVALID_ARG;
   const bool simt = group_use_simt(M);
   const int64_t mtiles = simt ? (M + TOK - 1) / TOK : (M + TOKC - 1) / TOKC;
-  if (mtiles > 65535) return MQ_ERR_UNSUPPORTED_SHAPE;
   const int rc = mq::check_device();
   if (rc != MQ_OK) return rc;
+  // group = 128 (one group per K-step), prefill token counts: the tcgen05 kernel, accumulator drained per K-step
+  if (mq::group_tc_eligible(w, group, M)) {
+    if ((uintptr_t)qA & 15) return MQ_ERR_INVALID_ARG;
+    return mq::group_tc_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream);
+  }
+  if (mtiles > 65535) return MQ_ERR_UNSUPPORTED_SHAPE;
   const int splits = group_splits(w, M);
   const size_t need = mq_gemm_group_workspace_bytes(w, M);
   if (need && (!workspace || ((uintptr_t)workspace & 15))) return MQ_ERR_INVALID_ARG;

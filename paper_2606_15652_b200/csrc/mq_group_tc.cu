@@ -1,0 +1,569 @@
+// mq_group_tc.cu -- per-GROUP activation scales (reading A5g) on the tcgen05 tensor path, group = 128 channels:
+//   Y[m,n] = sum_g s_a[m,g] (s_w[n] acc0_g[m,n] + s_r[n] acc1_g[m,n])          Eq.2, Eq.4 P:106 per group
+// (first half).  A group of 128 channels is exactly one K-step of the packed layout, so the integer sum
+// of a group is what ONE K-step's MMAs leave in the accumulator: the accumulator is drained after every K-step.
+//
+// The kernel is mq_prefill.cu's single-CTA form (whole 128 x 128 tiles dealt to persistent CTAs; weights expanded
+// int4 -> int8 x16 in registers -> tcgen05.st into TENSOR MEMORY as the A operand; tokens expanded into K-major
+// SWIZZLE_128B shared memory as the B operand; tcgen05.mma kind::i8; residual cells as operand-ring items of their own)
+// with a different accumulator discipline:
+//   * the base accumulator is double-buffered PER K-STEP: the MMAs of K-step k+1 run into the other 128 columns while
+//     the epilogue warps read the sums of K-step k (tcgen05.ld), scale them and add them to fp32 running sums held in
+//     registers.  Measured (one-off probe): eight warps drain, convert and FMA a 128 x 128 int32 accumulator in ~313
+//     cycles, less than the ~560 cycles a K-step takes in the per-token kernel, so the drain hides behind the MMAs;
+//   * the residual accumulator is single-buffered and handed over per CELL (cells are rare);
+//   * eight epilogue warps (two per TMEM lane quadrant, 64 tokens each) keep 64 fp32 sums per thread for the whole
+//     tile; the group scales of the tile's tokens for the NEXT K-step are gathered into shared memory while the current
+//     one is being drained.
+// Tensor memory (512 columns): acc0 2 x 128 | acc1 128 | A operand ring 4 x 32.  Roles (16 warps = 512 threads, the
+// largest block that still gets 128 registers per thread: the epilogue needs them; one CTA per SM):
+//   warp 0 producer (TMA) | warp 1 MMA issuer | warps 2-9 epilogue | warps 10-13 weight unpack (one per TMEM lane
+//   quadrant; every item) | warps 14-15 token unpack (shared memory has no quadrant rule; every base item).
+// Arithmetic per output and group, in the order of mq_group.cu's mma.sync kernel: term = s_w * acc0 (s_w carries the
+// 2^-8 of the x16 operands, exact), term = fma(s_r, acc1, term) if the K-step owns a cell, y = fma(s_a, term, y),
+// groups in ascending order; one rounding to the 16-bit output at the end (tolerance T2 of DESIGN.md section 4).
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+
+#include "mq_internal.h"
+#include "mq_ptx.cuh"
+
+namespace {
+
+using namespace mq;
+using namespace mq::ptx;
+
+constexpr int GT_BT = 128;                        // tokens per tile (MMA N)
+constexpr int GT_UST = 4;                         // operand (U) stages
+constexpr int GT_EWARPS = 8;                      // epilogue warps: lane quadrant = warp % 4, token half = (warp - 2) / 4
+constexpr int GT_WWARPS = 4;                      // weight-unpack warps (one per TMEM lane quadrant)
+constexpr int GT_TWARPS = 2;                      // token-unpack warps
+constexpr int GT_WARP_W0 = 2 + GT_EWARPS, GT_WARP_T0 = GT_WARP_W0 + GT_WWARPS;
+constexpr int GT_WARPS = GT_WARP_T0 + GT_TWARPS;
+constexpr int GT_THREADS = 32 * GT_WARPS;         // 512: the largest block that still gets 128 registers per thread
+constexpr int GT_A_COLS = BK / 4;                 // 32 TMEM columns hold 128 int8 per lane (one K-step)
+constexpr int GT_ACC1_COL = 2 * GT_BT;
+constexpr int GT_A_COL0 = 3 * GT_BT;
+constexpr int GT_PST = 8;                         // packed (P) stages of one K-step
+constexpr int GT_U_STAGE = GT_BT * BK;            // int8 token sub-tile of one K-step (16 KB)
+constexpr int GT_TOK_KSTEP = GT_BT * (BK / 2);    // packed tokens of one K-step (8 KB)
+constexpr int GT_P_STAGE = TILE_BYTES + GT_TOK_KSTEP;
+constexpr int GT_OFF_U = 0;
+constexpr int GT_OFF_P = GT_OFF_U + GT_UST * GT_U_STAGE;
+constexpr int GT_OFF_BAR = GT_OFF_P + GT_PST * GT_P_STAGE;
+// barriers: FULL_P[8] EMPTY_P[8] FULL_U[4] EMPTY_U[4] GFULL[2] GEMPTY[2] A1E
+constexpr int GT_B_FULL_P = 0, GT_B_EMPTY_P = GT_PST, GT_B_FULL_U = 2 * GT_PST, GT_B_EMPTY_U = GT_B_FULL_U + GT_UST,
+              GT_B_GFULL = GT_B_EMPTY_U + GT_UST, GT_B_GEMPTY = GT_B_GFULL + 2, GT_B_A1E = GT_B_GEMPTY + 2, GT_NUM_BARS = GT_B_A1E + 1;
+constexpr int GT_OFF_MISC = GT_OFF_BAR + GT_NUM_BARS * 8 + 8;     // [0] tmem base
+constexpr int GT_OFF_SA = (GT_OFF_MISC + 16 + 15) / 16 * 16;      // [2][128] group scales of the tile's tokens (this / next K-step)
+constexpr int GT_SMEM_BYTES = GT_OFF_SA + 2 * GT_BT * 4 + 1024;   // + slack for the 1024-byte alignment
+static_assert(GT_SMEM_BYTES <= 232448, "shared memory budget");
+static_assert(GT_A_COL0 + GT_UST * GT_A_COLS == 512, "tensor memory budget");
+static_assert(GT_OFF_P % 1024 == 0 && GT_P_STAGE % 1024 == 0 && GT_U_STAGE % 1024 == 0, "swizzle atoms need 1024-byte alignment");
+
+struct GtParams {
+  const uint8_t* base;
+  const uint8_t* res;
+  const int2* unit_meta;   // [NT * KS] {quarter mask, first quarter}; NULL = dense only
+  const float* sw;
+  const float* sr;
+  const float* sa;         // [M][KS] group scales
+  void* Y;
+  int32_t* dbg0;           // [KS][M][N] per-group base sums, or NULL
+  int32_t* dbg1;           // [KS][M][N] per-group residual sums, or NULL
+  int64_t ldy;
+  int M, N, KS, NT, TT;
+  int tiles;
+  int y_bf16;
+};
+
+__device__ __forceinline__ void gt_unpack16(const uint4& p, uint32_t* o) {
+  const uint32_t HI = 0xF0F0F0F0u;
+  o[0] = (p.x << 4) & HI;
+  o[1] = p.x & HI;
+  o[2] = (p.y << 4) & HI;
+  o[3] = p.y & HI;
+  o[4] = (p.z << 4) & HI;
+  o[5] = p.z & HI;
+  o[6] = (p.w << 4) & HI;
+  o[7] = p.w & HI;
+}
+__device__ __forceinline__ uint4 gt_lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void gt_sts128(uint32_t addr, const uint32_t* v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
+}
+// wait for the outstanding tcgen05.ld's; the registers of the batches being waited for are tied to the statement so
+// that no use of them can be scheduled above it (see mq_ptx.cuh)
+__device__ __forceinline__ void gt_ld_wait32(uint32_t* a, uint32_t* b) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;"
+               : "+r"(a[0]), "+r"(a[1]), "+r"(a[2]), "+r"(a[3]), "+r"(a[4]), "+r"(a[5]), "+r"(a[6]), "+r"(a[7]), "+r"(a[8]), "+r"(a[9]),
+                 "+r"(a[10]), "+r"(a[11]), "+r"(a[12]), "+r"(a[13]), "+r"(a[14]), "+r"(a[15]), "+r"(b[0]), "+r"(b[1]), "+r"(b[2]),
+                 "+r"(b[3]), "+r"(b[4]), "+r"(b[5]), "+r"(b[6]), "+r"(b[7]), "+r"(b[8]), "+r"(b[9]), "+r"(b[10]), "+r"(b[11]),
+                 "+r"(b[12]), "+r"(b[13]), "+r"(b[14]), "+r"(b[15])
+               :
+               : "memory");
+}
+
+template <bool DBG>
+__global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const GtParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sU = smem_base + GT_OFF_U, sP = smem_base + GT_OFF_P, sBar = smem_base + GT_OFF_BAR, sMisc = smem_base + GT_OFF_MISC,
+                 sSA = smem_base + GT_OFF_SA;
+  auto bar = [&](int i) { return sBar + 8u * (uint32_t)i; };
+  volatile int32_t* misc = reinterpret_cast<volatile int32_t*>(smem_raw + (sMisc - smem_u32(smem_raw)));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int KS = p.KS;
+  const int tile0 = (int)blockIdx.x, tstride = (int)gridDim.x;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tmap(&tmap_a);
+    for (int i = 0; i < GT_PST; ++i) {
+      mbar_init(bar(GT_B_FULL_P + i), 1);            // the producer's arrival; the copies complete the transaction count
+      mbar_init(bar(GT_B_EMPTY_P + i), GT_WWARPS + GT_TWARPS);   // every unpack warp has its part in registers
+    }
+    for (int i = 0; i < GT_UST; ++i) {
+      mbar_init(bar(GT_B_FULL_U + i), GT_WWARPS + GT_TWARPS);
+      mbar_init(bar(GT_B_EMPTY_U + i), 1);
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(bar(GT_B_GFULL + i), 1);             // tcgen05.commit after the K-step's MMAs
+      mbar_init(bar(GT_B_GEMPTY + i), GT_EWARPS);    // every epilogue warp has read its part of the buffer
+    }
+    mbar_init(bar(GT_B_A1E), GT_EWARPS);
+    fence_mbar_init();
+  }
+  if (warp == 1) {
+    tmem_alloc(sMisc, 512);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = (uint32_t)misc[0];
+  griddep_launch();
+
+  // residual metadata: every role that needs it keeps the {quarter mask, first quarter} words of 32 consecutive K-steps
+  // in its lanes (one coalesced load per chunk, requested one chunk ahead) and derives the item sequence from them
+  auto load_chunk = [&](int T, int c0) -> int2 {
+    int2 v = make_int2(0, 0);
+    if (p.unit_meta && T < p.tiles && c0 + lane < KS) v = __ldg(p.unit_meta + (size_t)(T / p.TT) * KS + c0 + lane);
+    return v;
+  };
+  auto next_chunk = [&](int& T, int& c0) {
+    c0 += 32;
+    if (c0 >= KS) {
+      c0 = 0;
+      T += tstride;
+    }
+  };
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // ===================== producer (one thread): one K-step per stage =====================
+      griddep_wait();   // the packed tokens are the previous kernel's output
+      uint32_t q = 0;
+      for (int T = tile0; T < p.tiles; T += tstride) {
+        const int nt = T / p.TT, tt = T - nt * p.TT;
+        const uint8_t* wsrc = p.base + (size_t)nt * KS * TILE_BYTES;
+        for (int ks = 0; ks < KS; ++ks, ++q) {
+          const uint32_t ps = q % GT_PST;
+          mbar_wait(bar(GT_B_EMPTY_P + ps), ((q / GT_PST) & 1) ^ 1);
+          const uint32_t fb = bar(GT_B_FULL_P + ps), dst = sP + ps * GT_P_STAGE;
+          mbar_arrive_expect_tx(fb, TILE_BYTES + GT_TOK_KSTEP);
+          tma_load_1d(dst, wsrc + (size_t)ks * TILE_BYTES, TILE_BYTES, fb);
+          tma_load_2d(dst + TILE_BYTES, &tmap_a, ks * (BK / 2), tt * GT_BT, fb);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
+    constexpr uint32_t IDESC = make_idesc_i8(BN, GT_BT);
+    uint32_t item = 0, kq = 0, cq = 0;   // operand-ring items, K-steps and cells so far
+    bool pre_ok = false;                 // the barrier of the item about to be processed was already seen complete
+    // the operand stage of item i: FULL_U[i & 3], phase (i >> 2) & 1; the next item's barrier is polled once BEFORE this
+    // item's MMAs are issued, so that the round trip hides under the tensor pipe's work
+    auto acquire = [&]() {
+      if (!pre_ok) mbar_wait(bar(GT_B_FULL_U + (int)(item & 3)), (item >> 2) & 1);
+      tc_fence_after();
+      pre_ok = mbar_try_wait(bar(GT_B_FULL_U + (int)((item + 1) & 3)), ((item + 1) >> 2) & 1);
+    };
+    int pT = tile0, pc0 = 0;
+    int2 um_next = load_chunk(pT, pc0);
+    for (int T = tile0; T < p.tiles; T += tstride) {
+      for (int c0 = 0; c0 < KS; c0 += 32) {
+        const int2 um = um_next;
+        next_chunk(pT, pc0);
+        um_next = load_chunk(pT, pc0);
+        const uint32_t bits = __ballot_sync(0xffffffffu, (um.x & 0xF) != 0);
+        const int nk = min(32, KS - c0);
+        for (int j = 0; j < nk; ++j, ++kq) {
+          const bool has = (bits >> j) & 1;
+          const int us = (int)(item & 3), buf = (int)(kq & 1);
+          acquire();
+          mbar_wait(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
+          tc_fence_after();
+          const uint32_t d0 = tmem_base + (uint32_t)(buf * GT_BT);
+          const uint32_t at = tmem_base + (uint32_t)(GT_A_COL0 + us * GT_A_COLS);
+          const uint64_t dt = make_desc_sw128(sU + us * GT_U_STAGE);
+          if (elect_one()) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? 0u : 1u);   // a fresh sum per group
+            if (!has) {
+              tc_commit(bar(GT_B_EMPTY_U + us));
+              tc_commit(bar(GT_B_GFULL + buf));
+            }
+          }
+          __syncwarp();
+          ++item;
+          if (has) {
+            // residual cell of this K-step: its weights in the next stage's A columns, the tokens of this K-step's
+            // stage (the paper's re-use of the activation tile), second accumulator, also a fresh sum
+            const uint32_t mask = (uint32_t)__shfl_sync(0xffffffffu, um.x, j) & 0xF;
+            const int us2 = (int)(item & 3);
+            acquire();
+            mbar_wait(bar(GT_B_A1E), (cq & 1) ^ 1);   // the epilogue has read the previous cell's sums
+            tc_fence_after();
+            const uint32_t d1 = tmem_base + (uint32_t)GT_ACC1_COL;
+            const uint32_t at2 = tmem_base + (uint32_t)(GT_A_COL0 + us2 * GT_A_COLS);
+            if (elect_one()) {
+              uint32_t on = 0;
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+                if (mask & (3u << (2 * h))) {
+#pragma unroll
+                  for (int k = 2 * h; k < 2 * h + 2; ++k) {
+                    mma_i8_ts(d1, at2 + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
+                    on = 1;
+                  }
+                }
+              tc_commit(bar(GT_B_EMPTY_U + us2));
+              tc_commit(bar(GT_B_EMPTY_U + us));
+              tc_commit(bar(GT_B_GFULL + buf));   // both accumulators of the K-step are complete
+            }
+            __syncwarp();
+            ++item;
+            ++cq;
+          }
+        }
+      }
+    }
+  }
+  else if (warp >= GT_WARP_W0) {
+    // ============ unpack warps: int4 -> int8 (x16); weights -> TMEM (warps 10-13), tokens -> swizzled shared memory (14-15) ============
+    // Both kinds walk all items in order; item i uses operand stage i % 4.  A stage is complete when all six warps have
+    // arrived (for a residual item the token warps have nothing to do, but arrive in order all the same).
+    const bool wrole = warp < GT_WARP_T0;
+    const int wq = warp & 3;                            // TMEM lane quadrant of a weight warp
+    const uint32_t row = (uint32_t)(wq * 32 + lane);    // output channel inside the tile
+    const uint32_t ttid = (uint32_t)((warp - GT_WARP_T0) * 32 + lane);   // 0..63 among the token warps
+    const uint32_t lane_base = tmem_base + ((uint32_t)(wq * 32) << 16) + (uint32_t)GT_A_COL0;
+    const int rhalf = (int)(row >> 6);
+    uint32_t item = 0, q = 0;   // items / K-steps so far (the K-step counter names the P stage)
+    auto wait_stage = [&](uint32_t idx) {   // operand stage idx % 4 has been consumed by the MMAs of item idx - 4
+      mbar_wait(bar(GT_B_EMPTY_U + (int)(idx & 3)), ((idx >> 2) & 1) ^ 1);
+      tc_fence_after();
+    };
+    auto publish = [&](uint32_t idx) {   // this warp's part of the item is in place: tell the MMA warp
+      if (wrole) tmem_st_wait();
+      tc_fence_before();
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(GT_B_FULL_U + (int)(idx & 3)));
+    };
+    int pT = tile0, pc0 = 0;
+    int2 um_next = load_chunk(pT, pc0);
+    for (int T = tile0; T < p.tiles; T += tstride) {
+      for (int c0 = 0; c0 < KS; c0 += 32) {
+        const int2 um = um_next;
+        next_chunk(pT, pc0);
+        um_next = load_chunk(pT, pc0);
+        const uint32_t bits = __ballot_sync(0xffffffffu, (um.x & 0xF) != 0);
+        const int nk = min(32, KS - c0);
+        for (int j = 0; j < nk; ++j) {
+          const uint32_t idx = item + (uint32_t)j + (uint32_t)__popc(bits & ((1u << j) - 1));   // item number of K-step j's base item
+          const bool has = (bits >> j) & 1;
+          const uint32_t ps = (q + (uint32_t)j) % GT_PST;
+          mbar_wait(bar(GT_B_FULL_P + ps), ((q + (uint32_t)j) / GT_PST) & 1);
+          const uint32_t pw = sP + ps * GT_P_STAGE, pt = pw + TILE_BYTES;
+          if (wrole) {
+            // ---- base item, weights: one thread per output channel ----
+            uint4 v4[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) v4[c] = gt_lds128(pw + c * (BN * 16) + row * 16);
+            asm volatile("" ::"r"(v4[0].x), "r"(v4[1].x), "r"(v4[2].x), "r"(v4[3].x));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps));   // the packed stage is in registers: back to the producer
+            wait_stage(idx);
+            uint32_t o[32];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) gt_unpack16(v4[c], o + 8 * c);
+            tmem_st32(lane_base + (uint32_t)((idx & 3) * GT_A_COLS), o);
+            publish(idx);
+            if (has) {
+              // ---- residual item: the cell's packed rows straight from global memory ----
+              const uint32_t rmask = (uint32_t)__shfl_sync(0xffffffffu, um.x, j) & 0xF;
+              const uint32_t qoff = (uint32_t)__shfl_sync(0xffffffffu, um.y, j);
+              uint4 r4[2][2];
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                const int qq = 2 * h + rhalf;
+                r4[h][0] = make_uint4(0, 0, 0, 0);
+                r4[h][1] = make_uint4(0, 0, 0, 0);
+                if (rmask & (1u << qq)) {
+                  const uint8_t* src = p.res + ((size_t)qoff + (size_t)__popc(rmask & ((1u << qq) - 1))) * QUARTER_BYTES + (size_t)(row & 63) * 16;
+                  r4[h][0] = __ldg(reinterpret_cast<const uint4*>(src));
+                  r4[h][1] = __ldg(reinterpret_cast<const uint4*>(src + 1024));
+                }
+              }
+              wait_stage(idx + 1);
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                if (!(rmask & (3u << (2 * h)))) continue;   // k-half without any block: never read by the MMA
+                uint32_t ro[16];
+                gt_unpack16(r4[h][0], ro);
+                gt_unpack16(r4[h][1], ro + 8);
+                tmem_st16(lane_base + (uint32_t)(((idx + 1) & 3) * GT_A_COLS + 16 * h), ro);
+              }
+              publish(idx + 1);
+            }
+          } else {
+            // ---- base item, tokens: 512 chunks of 16 bytes (8 nibbles x 4 ... ) dealt to 64 threads ----
+            uint4 t4[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) t4[i] = gt_lds128(pt + (ttid + 64u * i) * 16);
+            asm volatile("" ::"r"(t4[0].x), "r"(t4[1].x), "r"(t4[2].x), "r"(t4[3].x), "r"(t4[4].x), "r"(t4[5].x), "r"(t4[6].x), "r"(t4[7].x));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps));
+            wait_stage(idx);
+            const uint32_t su = sU + (idx & 3) * GT_U_STAGE;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const uint32_t ti = ttid + 64u * i, t = ti >> 2, c = ti & 3;
+              uint32_t tw[8];
+              gt_unpack16(t4[i], tw);
+              gt_sts128(su + t * 128 + (((2 * c) ^ (t & 7)) << 4), tw);
+              gt_sts128(su + t * 128 + (((2 * c + 1) ^ (t & 7)) << 4), tw + 4);
+            }
+            publish(idx);
+            if (has) {   // nothing to expand for a residual item: keep the stage's arrival count in step
+              wait_stage(idx + 1);
+              publish(idx + 1);
+            }
+          }
+        }
+        item += (uint32_t)nk + (uint32_t)__popc(nk == 32 ? bits : (bits & ((1u << nk) - 1)));
+        q += (uint32_t)nk;
+      }
+    }
+  }
+  else {
+    // ===================== epilogue warps (2..9): drain every K-step's sums into fp32 running sums =====================
+    // Register budget (128 per thread): 64 running sums + three batches of 16 + a dozen scalars; whether a K-step owns a
+    // cell is therefore fetched from global memory one K-step ahead instead of kept in lanes.
+    griddep_wait();   // the group scales and Y are ordered after the previous kernel in the stream
+    const int half = (warp - 2) >> 2;             // which 64 tokens of the tile; TMEM lane quadrant = warp % 4
+    const int et = (warp - 2) * 32 + lane;        // 0..255 within the epilogue group
+    const uint32_t acc0_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(half * 64);
+    float y[64];
+#pragma unroll
+    for (int i = 0; i < 64; ++i) y[i] = 0.f;
+    // group scales s_a[t, g] of the tile's 128 tokens: gathered by threads 0..127 two K-steps ahead (a register), written
+    // to the double-buffered shared array one K-step ahead, read by everybody in the K-step itself
+    int fT = tile0, fks = 0;   // the K-step the next gather is for
+    auto gather = [&]() -> float {
+      float v = 0.f;
+      if (et < GT_BT && fT < p.tiles) {
+        const int t = (fT % p.TT) * GT_BT + et;
+        if (t < p.M) v = __ldg(p.sa + (size_t)t * KS + fks);
+      }
+      if (++fks == KS) {
+        fks = 0;
+        fT += tstride;
+      }
+      return v;
+    };
+    {
+      const float v0 = gather();
+      if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + 4u * (uint32_t)et), "f"(v0) : "memory");
+    }
+    float v_held = gather();   // for K-step 1
+    auto cell_of = [&](int T, int ks) -> int {   // quarter mask of K-step ks of tile T (0 = no cell)
+      return (p.unit_meta && T < p.tiles) ? (__ldg(&p.unit_meta[(size_t)(T / p.TT) * KS + ks].x) & 0xF) : 0;
+    };
+    uint32_t kq = 0;
+    int has_next = cell_of(tile0, 0);
+    for (int T = tile0; T < p.tiles; T += tstride) {
+      for (int ks = 0; ks < KS; ++ks, ++kq) {
+        const bool has = has_next != 0;
+        has_next = ks + 1 < KS ? cell_of(T, ks + 1) : cell_of(T + tstride, 0);
+        const int buf = (int)(kq & 1);
+        // publish the scales of K-step kq + 1, request those of K-step kq + 2
+        named_bar_sync(1, 32 * GT_EWARPS);   // the readers of K-step kq - 1 are done; K-step kq's scales are visible
+        if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + (uint32_t)((buf ^ 1) * GT_BT * 4) + 4u * (uint32_t)et), "f"(v_held) : "memory");
+        v_held = gather();
+        mbar_wait(bar(GT_B_GFULL + buf), (kq >> 1) & 1);
+        tc_fence_after();
+        const uint32_t sa_cur = sSA + (uint32_t)(buf * GT_BT * 4) + (uint32_t)(half * 64 * 4);
+        const float swn = __ldg(p.sw + (T / p.TT) * BN + (warp & 3) * 32 + lane) * 0.00390625f;   // accumulators are x256
+        const float srn = __ldg(p.sr + (T / p.TT) * BN + (warp & 3) * 32 + lane) * 0.00390625f;
+        // four batches of 16 tokens; the base sums are double-buffered in registers (batch b + 1 is in flight while batch
+        // b is scaled and added), the residual sums (K-steps with a cell only) single-buffered
+        uint32_t a[2][16], r[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) r[i] = 0;
+        tmem_ld16(acc0_addr + (uint32_t)(buf * GT_BT), a[0]);
+        if (has) tmem_ld16(acc0_addr + (uint32_t)GT_ACC1_COL, r);
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+          const int cur = b & 1;
+          gt_ld_wait32(a[cur], r);
+          if (b < 3) tmem_ld16(acc0_addr + (uint32_t)(buf * GT_BT + (b + 1) * 16), a[cur ^ 1]);
+          if (b == 3) {   // this warp's part of both accumulators is in registers: hand them back to the MMA warp
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              mbar_arrive(bar(GT_B_GEMPTY + buf));
+              if (has) mbar_arrive(bar(GT_B_A1E));
+            }
+          }
+#pragma unroll
+          for (int i4 = 0; i4 < 4; ++i4) {
+            const uint4 s4 = gt_lds128(sa_cur + (uint32_t)((b * 16 + i4 * 4) * 4));
+            const float sav[4] = {__uint_as_float(s4.x), __uint_as_float(s4.y), __uint_as_float(s4.z), __uint_as_float(s4.w)};
+#pragma unroll
+            for (int ii = 0; ii < 4; ++ii) {
+              const int i = 4 * i4 + ii;
+              float term = swn * (float)(int32_t)a[cur][i];
+              if (has) term = fmaf(srn, (float)(int32_t)r[i], term);
+              y[b * 16 + i] = fmaf(sav[ii], term, y[b * 16 + i]);
+            }
+          }
+          if (DBG) {   // parity hooks: the per-group integer sums
+            const int n = (T / p.TT) * BN + (warp & 3) * 32 + lane, t0 = (T % p.TT) * GT_BT + half * 64 + b * 16;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+              if (t0 + i < p.M) {
+                const size_t di = ((size_t)ks * p.M + (size_t)(t0 + i)) * p.N + n;
+                if (p.dbg0) p.dbg0[di] = (int32_t)a[cur][i] >> 8;
+                if (p.dbg1) p.dbg1[di] = (int32_t)r[i] >> 8;
+              }
+            }
+          }
+          if (has && b < 3) tmem_ld16(acc0_addr + (uint32_t)(GT_ACC1_COL + (b + 1) * 16), r);   // r is free again
+        }
+      }
+      // the tile's sums are complete: one rounding to the 16-bit output
+      const int t_first = (T % p.TT) * GT_BT + half * 64;
+      uint16_t* yp = reinterpret_cast<uint16_t*>(p.Y) + (size_t)t_first * p.ldy + (T / p.TT) * BN + (warp & 3) * 32 + lane;
+#pragma unroll
+      for (int i = 0; i < 64; ++i) {
+        if (t_first + i < p.M)
+          yp[(size_t)i * p.ldy] = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y[i])) : __half_as_ushort(__float2half_rn(y[i]));
+        y[i] = 0.f;
+      }
+    }
+  }
+
+
+  // teardown (single-lane regions re-converge first: bar.sync must be reached warp-convergent)
+  __syncwarp();
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+}  // namespace
+
+namespace mq {
+
+// group = 128 only (one group per K-step); small token counts stay on the mma.sync kernel (mq_group.cu)
+bool group_tc_eligible(const mq_weights* w, int group, int64_t M) {
+  const Options& o = options();
+  return w && !w->blockscale && group == 128 && M >= 64 && o.group_tc != 0 && o.group_simt == 0;
+}
+
+int group_tc_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                  int32_t* dbg0, int32_t* dbg1, void* cuda_stream) {
+  typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  EncodeTiledFn enc = (EncodeTiledFn)tensor_map_encode_fn();
+  if (!enc) return MQ_ERR_CUDA;
+  // 2-D tensor map over the canonical packed activations [M rows][K/2 bytes]: box = one K-step of one token tile;
+  // rows past M read as zero
+  CUtensorMap tmap;
+  memset(&tmap, 0, sizeof(tmap));
+  const cuuint64_t row_bytes = (cuuint64_t)(w->K / 2);
+  const cuuint64_t gdim[2] = {row_bytes, (cuuint64_t)M};
+  const cuuint64_t gstride[1] = {row_bytes};
+  const cuuint32_t box[2] = {(cuuint32_t)(BK / 2), (cuuint32_t)GT_BT};
+  const cuuint32_t estr[2] = {1, 1};
+  if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(qA), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return MQ_ERR_CUDA;
+
+  GtParams gp;
+  gp.base = w->d_base;
+  gp.res = w->d_res;
+  gp.unit_meta = w->nnz > 0 ? (const int2*)w->d_unit_meta : nullptr;
+  gp.sw = w->d_sw;
+  gp.sr = w->d_sr;
+  gp.sa = sA;
+  gp.Y = Y;
+  gp.dbg0 = dbg0;
+  gp.dbg1 = dbg1;
+  gp.ldy = ldy;
+  gp.M = (int)M;
+  gp.N = (int)w->N;
+  gp.KS = (int)(w->K / BK);
+  gp.NT = (int)(w->N / BN);
+  gp.TT = (int)((M + GT_BT - 1) / GT_BT);
+  const int64_t tiles = (int64_t)gp.NT * gp.TT;
+  if (tiles >= ((int64_t)1 << 31) || M >= ((int64_t)1 << 31)) return MQ_ERR_UNSUPPORTED_SHAPE;
+  gp.tiles = (int)tiles;
+  gp.y_bf16 = y_dtype == MQ_BF16;
+
+  const bool dbg = dbg0 || dbg1;   // the parity hooks are a separate instantiation
+  auto kern = dbg ? mq_group_tc_kernel<true> : mq_group_tc_kernel<false>;
+  static int attr_dev[2] = {-1, -1};   // the attribute belongs to the (device, function) pair
+  int dev = -1;
+  cudaGetDevice(&dev);
+  if (dev != attr_dev[dbg]) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, GT_SMEM_BYTES) != cudaSuccess) {
+      cudaGetLastError();
+      return MQ_ERR_CUDA;
+    }
+    attr_dev[dbg] = dev;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)std::min<int64_t>(tiles, sm_count()));
+  cfg.blockDim = dim3(GT_THREADS);
+  cfg.dynamicSmemBytes = GT_SMEM_BYTES;
+  cfg.stream = (cudaStream_t)cuda_stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = options().pdl ? 1 : 0;
+  if (cudaLaunchKernelEx(&cfg, kern, tmap, gp) != cudaSuccess) {
+    cudaGetLastError();
+    return MQ_ERR_CUDA;
+  }
+  set_launch_count(1);
+  return MQ_OK;
+}
+
+}  // namespace mq

@@ -84,6 +84,7 @@ struct Options {
   int64_t max_ctas = 0;
   int64_t fused_quant = 0;   // mq_linear with M <= 8: quantize the activations inside the GEMM kernel (slower than
                              // the PDL-chained two-kernel path on B200; off by default)
+  int64_t group_tc = 1;      // mq_gemm_group, group = 128, M >= 64: 1 = the tcgen05 kernel (mq_group_tc.cu); 0 = the mma.sync kernel
   int64_t group_simt = 0;    // mq_gemm_group: 1 = the dp4a kernel (ablation); 0 = the mma.sync kernel
   int64_t pdl = 1;   // launch kernels as programmatic dependents of their predecessor in the stream
   int64_t decode_path = 0;      // 0 = automatic (M <= 32 runs the lean mma.sync decode kernel), 1 = off (tcgen05 kernel)
@@ -118,6 +119,10 @@ int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M,
 bool prefill_eligible(const mq_weights* w, int64_t M);
 int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
                  int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res);
+// per-group activation scales, group = 128, on the tcgen05 path (mq_group_tc.cu): M >= 64, no workspace
+bool group_tc_eligible(const mq_weights* w, int group, int64_t M);
+int group_tc_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                  int32_t* dbg0, int32_t* dbg1, void* cuda_stream);
 int build_weight_tmaps(mq_weights* w);   // MQ_OK or MQ_ERR_CUDA
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency); NULL if absent
 void* tensor_map_encode_fn();

@@ -218,6 +218,9 @@ extern "C" int mq_set_option(const char* name, int64_t value) {
   } else if (!strcmp(name, "prefill_path")) {
     if (value > 3) return MQ_ERR_INVALID_ARG;
     o.prefill_path = value;
+  } else if (!strcmp(name, "group_tc")) {
+    if (value > 1) return MQ_ERR_INVALID_ARG;
+    o.group_tc = value;
   } else if (!strcmp(name, "group_simt")) {
     if (value > 1) return MQ_ERR_INVALID_ARG;
     o.group_simt = value;
