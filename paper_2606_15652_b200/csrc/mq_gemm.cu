@@ -832,19 +832,21 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
         const bool valid = (m & META_VALID) != 0;
         const int mask = valid ? (m & 0xF) : 0;
         uint4 v4[4], t4[TCH];   // packed operands stay packed (32 registers) across the wait
+        uint32_t landed = 0;
         if (valid) {
 #pragma unroll
           for (int c = 0; c < 4; ++c) v4[c] = lds128(pw + c * (BN * 16) + row * 16);
           const uint32_t pt1 = sP + ps * C::P_STAGE + C::P_W + sub * C::TOK_KSTEP;
 #pragma unroll
           for (int i = 0; i < TCH; ++i) t4[i] = lds128(pt1 + (gtid + 128u * i) * 16);
-          // the loads must have landed before the P stage is handed back
-          asm volatile("" ::"r"(v4[0].x), "r"(v4[1].x), "r"(v4[2].x), "r"(v4[3].x));
+          // the loads must have landed before the P stage is handed back: the arrival depends on every loaded word
+          landed = fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]);
 #pragma unroll
-          for (int i = 0; i < TCH; ++i) asm volatile("" ::"r"(t4[i].x));
+          for (int i = 0; i < TCH; ++i) landed ^= fold4(t4[i]);
+          landed = zero_after(landed);
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(B_EMPTY_P + ps));   // this warp's reads of the P stage are done
+        if (lane == 0) mbar_arrive(bar(B_EMPTY_P + ps) + landed);   // this warp's reads of the P stage are done
         MQ_ACC_BEGIN(tu_eu);
         mbar_wait(bar(B_EMPTY_U + (C::PAIR ? us >> 1 : us)), (((uint32_t)item / C::USTAGES) & 1) ^ 1);
         MQ_ACC_END(tu_eu);

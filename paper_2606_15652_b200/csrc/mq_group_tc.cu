@@ -61,7 +61,8 @@ constexpr int GT_B_FULL_P = 0, GT_B_EMPTY_P = GT_PST, GT_B_FULL_U = 2 * GT_PST, 
               GT_B_GFULL = GT_B_EMPTY_U + GT_UST, GT_B_GEMPTY = GT_B_GFULL + 2, GT_B_A1E = GT_B_GEMPTY + 2, GT_NUM_BARS = GT_B_A1E + 1;
 constexpr int GT_OFF_MISC = GT_OFF_BAR + GT_NUM_BARS * 8 + 8;     // [0] tmem base
 constexpr int GT_OFF_SA = (GT_OFF_MISC + 16 + 15) / 16 * 16;      // [2][128] group scales of the tile's tokens (this / next K-step)
-constexpr int GT_SMEM_BYTES = GT_OFF_SA + 2 * GT_BT * 4 + 1024;   // + slack for the 1024-byte alignment
+constexpr int GT_OFF_YST = (GT_OFF_SA + 2 * GT_BT * 4 + 127) / 128 * 128;   // [128 tokens][128 channels] 16-bit: the finished tile, staged
+constexpr int GT_SMEM_BYTES = GT_OFF_YST + GT_BT * BN * 2 + 1024;  // + slack for the 1024-byte alignment
 static_assert(GT_SMEM_BYTES <= 232448, "shared memory budget");
 static_assert(GT_A_COL0 + GT_UST * GT_A_COLS == 512, "tensor memory budget");
 static_assert(GT_OFF_P % 1024 == 0 && GT_P_STAGE % 1024 == 0 && GT_U_STAGE % 1024 == 0, "swizzle atoms need 1024-byte alignment");
@@ -80,6 +81,9 @@ struct GtParams {
   int M, N, KS, NT, TT;
   int tiles;
   int y_bf16;
+#ifdef GT_TRACE
+  long long* trace;
+#endif
 };
 
 __device__ __forceinline__ void gt_unpack16(const uint4& p, uint32_t* o) {
@@ -112,6 +116,14 @@ __device__ __forceinline__ void gt_ld_wait32(uint32_t* a, uint32_t* b) {
                :
                : "memory");
 }
+
+#ifdef GT_TRACE   // development: per-role wait-time sums of CTA 0 into p.trace (long long [64])
+#define GT_T0() const long long gt_c0 = clock64()
+#define GT_ACC(slot) do { gt_acc[(slot) & 1] += clock64() - gt_c0; } while (0)   // two register accumulators per role
+#else
+#define GT_T0() do { } while (0)
+#define GT_ACC(slot) do { } while (0)
+#endif
 
 template <bool DBG>
 __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const GtParams p) {
@@ -151,6 +163,10 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)misc[0];
   griddep_launch();
+#ifdef GT_TRACE
+  const long long gt_start = clock64();
+  long long gt_acc[2] = {0, 0}, gt_drain = 0, gt_tile = 0;
+#endif
 
   // residual metadata: every role that needs it keeps the {quarter mask, first quarter} words of 32 consecutive K-steps
   // in its lanes (one coalesced load per chunk, requested one chunk ahead) and derives the item sequence from them
@@ -193,7 +209,11 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     // the operand stage of item i: FULL_U[i & 3], phase (i >> 2) & 1; the next item's barrier is polled once BEFORE this
     // item's MMAs are issued, so that the round trip hides under the tensor pipe's work
     auto acquire = [&]() {
-      if (!pre_ok) mbar_wait(bar(GT_B_FULL_U + (int)(item & 3)), (item >> 2) & 1);
+      if (!pre_ok) {
+        GT_T0();
+        mbar_wait(bar(GT_B_FULL_U + (int)(item & 3)), (item >> 2) & 1);
+        GT_ACC(0);
+      }
       tc_fence_after();
       pre_ok = mbar_try_wait(bar(GT_B_FULL_U + (int)((item + 1) & 3)), ((item + 1) >> 2) & 1);
     };
@@ -210,7 +230,11 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           const bool has = (bits >> j) & 1;
           const int us = (int)(item & 3), buf = (int)(kq & 1);
           acquire();
-          mbar_wait(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
+          {
+            GT_T0();
+            mbar_wait(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
+            GT_ACC(1);
+          }
           tc_fence_after();
           const uint32_t d0 = tmem_base + (uint32_t)(buf * GT_BT);
           const uint32_t at = tmem_base + (uint32_t)(GT_A_COL0 + us * GT_A_COLS);
@@ -270,7 +294,9 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     const int rhalf = (int)(row >> 6);
     uint32_t item = 0, q = 0;   // items / K-steps so far (the K-step counter names the P stage)
     auto wait_stage = [&](uint32_t idx) {   // operand stage idx % 4 has been consumed by the MMAs of item idx - 4
+      GT_T0();
       mbar_wait(bar(GT_B_EMPTY_U + (int)(idx & 3)), ((idx >> 2) & 1) ^ 1);
+      GT_ACC(7);
       tc_fence_after();
     };
     auto publish = [&](uint32_t idx) {   // this warp's part of the item is in place: tell the MMA warp
@@ -293,16 +319,21 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           const uint32_t idx = item + (uint32_t)j + (uint32_t)__popc(bits & ((1u << j) - 1));   // item number of K-step j's base item
           const bool has = (bits >> j) & 1;
           const uint32_t ps = (q + (uint32_t)j) % GT_PST;
-          mbar_wait(bar(GT_B_FULL_P + ps), ((q + (uint32_t)j) / GT_PST) & 1);
+          {
+            GT_T0();
+            mbar_wait(bar(GT_B_FULL_P + ps), ((q + (uint32_t)j) / GT_PST) & 1);
+            GT_ACC(6);
+          }
           const uint32_t pw = sP + ps * GT_P_STAGE, pt = pw + TILE_BYTES;
           if (wrole) {
             // ---- base item, weights: one thread per output channel ----
             uint4 v4[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) v4[c] = gt_lds128(pw + c * (BN * 16) + row * 16);
-            asm volatile("" ::"r"(v4[0].x), "r"(v4[1].x), "r"(v4[2].x), "r"(v4[3].x));
+            // the packed stage is in registers: back to the producer (the arrival depends on every loaded word, see zero_after)
+            const uint32_t landed = zero_after(fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]));
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps));   // the packed stage is in registers: back to the producer
+            if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps) + landed);
             wait_stage(idx);
             uint32_t o[32];
 #pragma unroll
@@ -341,9 +372,12 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             uint4 t4[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) t4[i] = gt_lds128(pt + (ttid + 64u * i) * 16);
-            asm volatile("" ::"r"(t4[0].x), "r"(t4[1].x), "r"(t4[2].x), "r"(t4[3].x), "r"(t4[4].x), "r"(t4[5].x), "r"(t4[6].x), "r"(t4[7].x));
+            uint32_t chk = 0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) chk ^= fold4(t4[i]);
+            const uint32_t landed = zero_after(chk);
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps));
+            if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps) + landed);
             wait_stage(idx);
             const uint32_t su = sU + (idx & 3) * GT_U_STAGE;
 #pragma unroll
@@ -384,7 +418,9 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       float v = 0.f;
       if (et < GT_BT && fT < p.tiles) {
         const int t = (fT % p.TT) * GT_BT + et;
-        if (t < p.M) v = __ldg(p.sa + (size_t)t * KS + fks);
+        // (asm volatile: the request must be ISSUED here, a K-step ahead of its use; as a plain __ldg the compiler
+        // sinks it to the use and the epilogue eats an L2 round trip, ~1000 cycles, in every K-step)
+        if (t < p.M) asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p.sa + (size_t)t * KS + fks));
       }
       if (++fks == KS) {
         fks = 0;
@@ -398,7 +434,9 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     }
     float v_held = gather();   // for K-step 1
     auto cell_of = [&](int T, int ks) -> int {   // quarter mask of K-step ks of tile T (0 = no cell)
-      return (p.unit_meta && T < p.tiles) ? (__ldg(&p.unit_meta[(size_t)(T / p.TT) * KS + ks].x) & 0xF) : 0;
+      int v = 0;
+      if (p.unit_meta && T < p.tiles) asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(&p.unit_meta[(size_t)(T / p.TT) * KS + ks].x));
+      return v & 0xF;
     };
     uint32_t kq = 0;
     int has_next = cell_of(tile0, 0);
@@ -408,11 +446,22 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         has_next = ks + 1 < KS ? cell_of(T, ks + 1) : cell_of(T + tstride, 0);
         const int buf = (int)(kq & 1);
         // publish the scales of K-step kq + 1, request those of K-step kq + 2
-        named_bar_sync(1, 32 * GT_EWARPS);   // the readers of K-step kq - 1 are done; K-step kq's scales are visible
+        {
+          GT_T0();
+          named_bar_sync(1, 32 * GT_EWARPS);   // the readers of K-step kq - 1 are done; K-step kq's scales are visible
+          GT_ACC(2);
+        }
         if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + (uint32_t)((buf ^ 1) * GT_BT * 4) + 4u * (uint32_t)et), "f"(v_held) : "memory");
         v_held = gather();
-        mbar_wait(bar(GT_B_GFULL + buf), (kq >> 1) & 1);
+        {
+          GT_T0();
+          mbar_wait(bar(GT_B_GFULL + buf), (kq >> 1) & 1);
+          GT_ACC(3);
+        }
         tc_fence_after();
+#ifdef GT_TRACE
+        const long long gt_d0 = clock64();
+#endif
         const uint32_t sa_cur = sSA + (uint32_t)(buf * GT_BT * 4) + (uint32_t)(half * 64 * 4);
         const float swn = __ldg(p.sw + (T / p.TT) * BN + (warp & 3) * 32 + lane) * 0.00390625f;   // accumulators are x256
         const float srn = __ldg(p.sr + (T / p.TT) * BN + (warp & 3) * 32 + lane) * 0.00390625f;
@@ -461,20 +510,78 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           }
           if (has && b < 3) tmem_ld16(acc0_addr + (uint32_t)(GT_ACC1_COL + (b + 1) * 16), r);   // r is free again
         }
+#ifdef GT_TRACE
+        gt_drain += clock64() - gt_d0;
+#endif
       }
-      // the tile's sums are complete: one rounding to the 16-bit output
-      const int t_first = (T % p.TT) * GT_BT + half * 64;
-      uint16_t* yp = reinterpret_cast<uint16_t*>(p.Y) + (size_t)t_first * p.ldy + (T / p.TT) * BN + (warp & 3) * 32 + lane;
+      // the tile's sums are complete: one rounding to the 16-bit output.  A thread owns one channel of 64 tokens; the
+      // tile is transposed through shared memory so that global memory sees 16-byte stores of whole 256-byte rows
+      // (64 two-byte stores per thread to 64 different rows kept the epilogue warps ~30 000 cycles per tile)
+#ifdef GT_NO_STAGE
+      {
+        const int t_first = (T % p.TT) * GT_BT + half * 64;
+        uint16_t* yp = reinterpret_cast<uint16_t*>(p.Y) + (size_t)t_first * p.ldy + (T / p.TT) * BN + (warp & 3) * 32 + lane;
 #pragma unroll
-      for (int i = 0; i < 64; ++i) {
-        if (t_first + i < p.M)
-          yp[(size_t)i * p.ldy] = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y[i])) : __half_as_ushort(__float2half_rn(y[i]));
-        y[i] = 0.f;
+        for (int i = 0; i < 64; ++i) {
+          if (t_first + i < p.M)
+            yp[(size_t)i * p.ldy] = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y[i])) : __half_as_ushort(__float2half_rn(y[i]));
+          y[i] = 0.f;
+        }
       }
+#else
+      {
+#ifdef GT_TRACE
+        const long long gt_t0 = clock64();
+#endif
+        const uint32_t yst = smem_base + GT_OFF_YST;
+        const int n_loc = (warp & 3) * 32 + lane;
+#pragma unroll
+        for (int i = 0; i < 64; ++i) {
+          const uint16_t h = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y[i])) : __half_as_ushort(__float2half_rn(y[i]));
+          asm volatile("st.shared.u16 [%0], %1;" ::"r"(yst + (uint32_t)(((half * 64 + i) * BN + n_loc) * 2)), "h"(h) : "memory");
+          y[i] = 0.f;
+        }
+        named_bar_sync(2, 32 * GT_EWARPS);
+        const int t_base = (T % p.TT) * GT_BT, n0 = (T / p.TT) * BN;
+        uint8_t* yg = reinterpret_cast<uint8_t*>(p.Y) + ((size_t)t_base * p.ldy + n0) * 2;
+        const bool vec = ((p.ldy & 7) == 0) && ((reinterpret_cast<uintptr_t>(p.Y) & 15) == 0);   // rows 16-byte aligned
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const int c = et + 256 * i, t = c >> 4, part = c & 15;   // 16 chunks of 16 bytes per token row
+          if (t_base + t < p.M) {
+            const uint4 v = gt_lds128(yst + (uint32_t)(t * (BN * 2) + part * 16));
+            uint8_t* dst = yg + (size_t)t * p.ldy * 2 + part * 16;
+            if (vec) {
+              *reinterpret_cast<uint4*>(dst) = v;
+            } else {
+              const uint32_t w4[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                reinterpret_cast<uint16_t*>(dst)[2 * k] = (uint16_t)(w4[k] & 0xFFFF);
+                reinterpret_cast<uint16_t*>(dst)[2 * k + 1] = (uint16_t)(w4[k] >> 16);
+              }
+            }
+          }
+        }
+        named_bar_sync(2, 32 * GT_EWARPS);   // the staging tile is free for the next tile
+#ifdef GT_TRACE
+        gt_tile += clock64() - gt_t0;
+#endif
+      }
+#endif
     }
   }
 
 
+#ifdef GT_TRACE
+  if (blockIdx.x == 0 && lane == 0 && (warp == 1 || warp == 2 || warp == GT_WARP_W0 || warp == GT_WARP_T0)) {
+    p.trace[32 + warp] = clock64() - gt_start;
+    const int base = warp == 1 ? 0 : (warp == 2 ? 2 : (warp == GT_WARP_W0 ? 6 : 8));
+    p.trace[base] = gt_acc[0];
+    p.trace[base + 1] = gt_acc[1];
+    if (warp == 2) { p.trace[4] = gt_drain; p.trace[5] = gt_tile; }
+  }
+#endif
   // teardown (single-lane regions re-converge first: bar.sync must be reached warp-convergent)
   __syncwarp();
   tc_fence_before();
@@ -535,6 +642,11 @@ int group_tc_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t 
   if (tiles >= ((int64_t)1 << 31) || M >= ((int64_t)1 << 31)) return MQ_ERR_UNSUPPORTED_SHAPE;
   gp.tiles = (int)tiles;
   gp.y_bf16 = y_dtype == MQ_BF16;
+#ifdef GT_TRACE
+  gp.trace = (long long*)dbg1;
+  gp.dbg1 = nullptr;
+  dbg1 = nullptr;
+#endif
 
   const bool dbg = dbg0 || dbg1;   // the parity hooks are a separate instantiation
   auto kern = dbg ? mq_group_tc_kernel<true> : mq_group_tc_kernel<false>;

@@ -187,6 +187,19 @@ __device__ __forceinline__ int quant1q(float x, float s, float inv_s) {
 __device__ __forceinline__ int quant1(float x, float s, float inv_s) { return quant1q<7>(x, s, inv_s); }
 __device__ __forceinline__ float quant_inv_scale(float s) { return s > 1e-30f ? __frcp_rn(s) : 0.f; }
 
+// Always 0, but computed from x in a way neither compiler stage folds (the square of an integer is 0 or 1 modulo 4,
+// so bit 1 of it is clear).  Added to an address, it makes that instruction DEPEND on x: it cannot issue before the
+// loads that produced x have landed.  Used where a buffer is handed back to a producer right after loading from it
+// into registers: an empty asm statement naming the registers constrains the compiler, not the hardware, and the
+// hand-off could be issued while the loads were still in flight (seen as stale operand data once in a few thousand
+// tiles, depending on timing).
+__device__ __forceinline__ uint32_t zero_after(uint32_t x) {
+  uint32_t y;
+  asm volatile("mul.lo.u32 %0, %1, %1;" : "=r"(y) : "r"(x));
+  return y & 2u;
+}
+__device__ __forceinline__ uint32_t fold4(const uint4& v) { return v.x ^ v.y ^ v.z ^ v.w; }
+
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
