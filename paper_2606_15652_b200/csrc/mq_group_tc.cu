@@ -125,6 +125,12 @@ __device__ __forceinline__ void gt_ld_wait32(uint32_t* a, uint32_t* b) {
 #define GT_ACC(slot) do { } while (0)
 #endif
 
+__device__ __forceinline__ void gt_tie16(uint32_t* a) {
+  asm volatile(""
+               : "+r"(a[0]), "+r"(a[1]), "+r"(a[2]), "+r"(a[3]), "+r"(a[4]), "+r"(a[5]), "+r"(a[6]), "+r"(a[7]), "+r"(a[8]), "+r"(a[9]),
+                 "+r"(a[10]), "+r"(a[11]), "+r"(a[12]), "+r"(a[13]), "+r"(a[14]), "+r"(a[15]));
+}
+
 template <bool DBG>
 __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid_constant__ CUtensorMap tmap_a, const GtParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -165,7 +171,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
   griddep_launch();
 #ifdef GT_TRACE
   const long long gt_start = clock64();
-  long long gt_acc[2] = {0, 0}, gt_drain = 0, gt_tile = 0;
+  long long gt_acc[2] = {0, 0}, gt_drain = 0, gt_tile = 0, gt_m1 = 0, gt_m2 = 0, gt_m3 = 0;
 #endif
 
   // residual metadata: every role that needs it keeps the {quarter mask, first quarter} words of 32 consecutive K-steps
@@ -413,18 +419,25 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     for (int i = 0; i < 64; ++i) y[i] = 0.f;
     // group scales s_a[t, g] of the tile's 128 tokens: gathered by threads 0..127 two K-steps ahead (a register), written
     // to the double-buffered shared array one K-step ahead, read by everybody in the K-step itself
+    // (pointers advanced by one per K-step and recomputed once per tile: no integer division in the K-step loop)
     int fT = tile0, fks = 0;   // the K-step the next gather is for
-    auto gather = [&]() -> float {
-      float v = 0.f;
+    const float* fp = nullptr;   // &s_a[token of this thread in tile fT][fks], or NULL (no such token / not a gathering thread)
+    auto gather_tile = [&]() {
+      fp = nullptr;
       if (et < GT_BT && fT < p.tiles) {
         const int t = (fT % p.TT) * GT_BT + et;
-        // (asm volatile: the request must be ISSUED here, a K-step ahead of its use; as a plain __ldg the compiler
-        // sinks it to the use and the epilogue eats an L2 round trip, ~1000 cycles, in every K-step)
-        if (t < p.M) asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p.sa + (size_t)t * KS + fks));
+        if (t < p.M) fp = p.sa + (size_t)t * KS;
       }
+    };
+    gather_tile();
+    auto gather = [&]() -> float {
+      float v = 0.f;
+      // (asm volatile: the request must be ISSUED here, a K-step ahead of its use; a plain __ldg may be sunk to the use)
+      if (fp) asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(fp + fks));
       if (++fks == KS) {
         fks = 0;
         fT += tstride;
+        gather_tile();
       }
       return v;
     };
@@ -433,17 +446,34 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + 4u * (uint32_t)et), "f"(v0) : "memory");
     }
     float v_held = gather();   // for K-step 1
-    auto cell_of = [&](int T, int ks) -> int {   // quarter mask of K-step ks of tile T (0 = no cell)
+    // whether the NEXT K-step owns a cell: one load per K-step from a pointer that walks the tile's metadata row
+    const int2* mp = p.unit_meta ? p.unit_meta + (size_t)(tile0 / p.TT) * KS : nullptr;   // (tile0 < tiles: the grid is <= tiles)
+    auto cell_at = [&](const int2* q) -> int {
       int v = 0;
-      if (p.unit_meta && T < p.tiles) asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(&p.unit_meta[(size_t)(T / p.TT) * KS + ks].x));
+      if (q) asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(&q->x));
       return v & 0xF;
     };
     uint32_t kq = 0;
-    int has_next = cell_of(tile0, 0);
+    int has_next = cell_at(mp);
     for (int T = tile0; T < p.tiles; T += tstride) {
+      const int n = (T / p.TT) * BN + (warp & 3) * 32 + lane;   // this thread's output channel
+      const float swn = __ldg(p.sw + n) * 0.00390625f, srn = __ldg(p.sr + n) * 0.00390625f;   // accumulators are x256
       for (int ks = 0; ks < KS; ++ks, ++kq) {
+#ifdef GT_TRACE
+        const long long gt_a = clock64();
+#endif
         const bool has = has_next != 0;
-        has_next = ks + 1 < KS ? cell_of(T, ks + 1) : cell_of(T + tstride, 0);
+        if (mp) {
+          if (ks + 1 < KS) {
+            ++mp;
+          } else {
+            mp = T + tstride < p.tiles ? p.unit_meta + (size_t)((T + tstride) / p.TT) * KS : nullptr;
+          }
+        }
+        has_next = cell_at(mp);
+#ifdef GT_TRACE
+        gt_m1 += clock64() - gt_a;
+#endif
         const int buf = (int)(kq & 1);
         // publish the scales of K-step kq + 1, request those of K-step kq + 2
         {
@@ -451,8 +481,18 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           named_bar_sync(1, 32 * GT_EWARPS);   // the readers of K-step kq - 1 are done; K-step kq's scales are visible
           GT_ACC(2);
         }
+#ifdef GT_TRACE
+        const long long gt_b = clock64();
+#endif
         if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + (uint32_t)((buf ^ 1) * GT_BT * 4) + 4u * (uint32_t)et), "f"(v_held) : "memory");
+#ifdef GT_TRACE
+        const long long gt_c = clock64();
+        gt_m2 += gt_c - gt_b;
+#endif
         v_held = gather();
+#ifdef GT_TRACE
+        gt_m3 += clock64() - gt_c;
+#endif
         {
           GT_T0();
           mbar_wait(bar(GT_B_GFULL + buf), (kq >> 1) & 1);
@@ -463,8 +503,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         const long long gt_d0 = clock64();
 #endif
         const uint32_t sa_cur = sSA + (uint32_t)(buf * GT_BT * 4) + (uint32_t)(half * 64 * 4);
-        const float swn = __ldg(p.sw + (T / p.TT) * BN + (warp & 3) * 32 + lane) * 0.00390625f;   // accumulators are x256
-        const float srn = __ldg(p.sr + (T / p.TT) * BN + (warp & 3) * 32 + lane) * 0.00390625f;
         // four batches of 16 tokens; the base sums are double-buffered in registers (batch b + 1 is in flight while batch
         // b is scaled and added), the residual sums (K-steps with a cell only) single-buffered
         uint32_t a[2][16], r[16];
@@ -476,7 +514,13 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         for (int b = 0; b < 4; ++b) {
           const int cur = b & 1;
           gt_ld_wait32(a[cur], r);
-          if (b < 3) tmem_ld16(acc0_addr + (uint32_t)(buf * GT_BT + (b + 1) * 16), a[cur ^ 1]);
+          if (b < 3) {
+            tmem_ld16(acc0_addr + (uint32_t)(buf * GT_BT + (b + 1) * 16), a[cur ^ 1]);
+            // (an empty statement that "modifies" the current batch: the arithmetic on it cannot be scheduled above
+            // it, hence not above the load just issued; otherwise the compiler sinks the load below the arithmetic
+            // and every batch pays the full tensor-memory latency)
+            gt_tie16(a[cur]);
+          }
           if (b == 3) {   // this warp's part of both accumulators is in registers: hand them back to the MMA warp
             tc_fence_before();
             __syncwarp();
@@ -498,7 +542,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             }
           }
           if (DBG) {   // parity hooks: the per-group integer sums
-            const int n = (T / p.TT) * BN + (warp & 3) * 32 + lane, t0 = (T % p.TT) * GT_BT + half * 64 + b * 16;
+            const int t0 = (T % p.TT) * GT_BT + half * 64 + b * 16;
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
               if (t0 + i < p.M) {
@@ -579,7 +623,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     const int base = warp == 1 ? 0 : (warp == 2 ? 2 : (warp == GT_WARP_W0 ? 6 : 8));
     p.trace[base] = gt_acc[0];
     p.trace[base + 1] = gt_acc[1];
-    if (warp == 2) { p.trace[4] = gt_drain; p.trace[5] = gt_tile; }
+    if (warp == 2) { p.trace[4] = gt_drain; p.trace[5] = gt_tile; p.trace[20] = gt_m1; p.trace[21] = gt_m2; p.trace[22] = gt_m3; }
   }
 #endif
   // teardown (single-lane regions re-converge first: bar.sync must be reached warp-convergent)
