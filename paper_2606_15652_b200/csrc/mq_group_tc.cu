@@ -503,56 +503,57 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         const long long gt_d0 = clock64();
 #endif
         const uint32_t sa_cur = sSA + (uint32_t)(buf * GT_BT * 4) + (uint32_t)(half * 64 * 4);
-        // four batches of 16 tokens; the base sums are double-buffered in registers (batch b + 1 is in flight while batch
-        // b is scaled and added), the residual sums (K-steps with a cell only) single-buffered
-        uint32_t a[2][16], r[16];
+        // four batches of 16 tokens, double-buffered in registers (batch b + 1 is in flight while batch b is scaled and
+        // added).  The residual sums of a K-step that owns a cell (one in twenty) take a second pass of the same shape:
+        // inside the first pass the compiler if-converts the cell test and EVERY element pays for it.
+        auto pass = [&](uint32_t col0, float scale, int32_t* dbg, bool last) {
+          uint32_t a[2][16];
+          tmem_ld16(acc0_addr + col0, a[0]);
 #pragma unroll
-        for (int i = 0; i < 16; ++i) r[i] = 0;
-        tmem_ld16(acc0_addr + (uint32_t)(buf * GT_BT), a[0]);
-        if (has) tmem_ld16(acc0_addr + (uint32_t)GT_ACC1_COL, r);
-#pragma unroll
-        for (int b = 0; b < 4; ++b) {
-          const int cur = b & 1;
-          gt_ld_wait32(a[cur], r);
-          if (b < 3) {
-            tmem_ld16(acc0_addr + (uint32_t)(buf * GT_BT + (b + 1) * 16), a[cur ^ 1]);
-            // (an empty statement that "modifies" the current batch: the arithmetic on it cannot be scheduled above
-            // it, hence not above the load just issued; otherwise the compiler sinks the load below the arithmetic
-            // and every batch pays the full tensor-memory latency)
-            gt_tie16(a[cur]);
-          }
-          if (b == 3) {   // this warp's part of both accumulators is in registers: hand them back to the MMA warp
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-              mbar_arrive(bar(GT_B_GEMPTY + buf));
-              if (has) mbar_arrive(bar(GT_B_A1E));
-            }
-          }
-#pragma unroll
-          for (int i4 = 0; i4 < 4; ++i4) {
-            const uint4 s4 = gt_lds128(sa_cur + (uint32_t)((b * 16 + i4 * 4) * 4));
-            const float sav[4] = {__uint_as_float(s4.x), __uint_as_float(s4.y), __uint_as_float(s4.z), __uint_as_float(s4.w)};
-#pragma unroll
-            for (int ii = 0; ii < 4; ++ii) {
-              const int i = 4 * i4 + ii;
-              float term = swn * (float)(int32_t)a[cur][i];
-              if (has) term = fmaf(srn, (float)(int32_t)r[i], term);
-              y[b * 16 + i] = fmaf(sav[ii], term, y[b * 16 + i]);
-            }
-          }
-          if (DBG) {   // parity hooks: the per-group integer sums
-            const int t0 = (T % p.TT) * GT_BT + half * 64 + b * 16;
-#pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              if (t0 + i < p.M) {
-                const size_t di = ((size_t)ks * p.M + (size_t)(t0 + i)) * p.N + n;
-                if (p.dbg0) p.dbg0[di] = (int32_t)a[cur][i] >> 8;
-                if (p.dbg1) p.dbg1[di] = (int32_t)r[i] >> 8;
+          for (int b = 0; b < 4; ++b) {
+            const int cur = b & 1;
+            gt_ld_wait32(a[cur], a[cur ^ 1]);
+            if (b < 3) {
+              tmem_ld16(acc0_addr + col0 + (uint32_t)((b + 1) * 16), a[cur ^ 1]);
+              // (an empty statement that "modifies" the current batch: the arithmetic on it cannot be scheduled above
+              // it, hence not above the load just issued; otherwise the compiler sinks the load below the arithmetic
+              // and every batch pays the full tensor-memory latency)
+              gt_tie16(a[cur]);
+            } else if (last) {   // this warp's part of the accumulators is in registers: hand them back to the MMA warp
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) {
+                mbar_arrive(bar(GT_B_GEMPTY + buf));
+                if (has) mbar_arrive(bar(GT_B_A1E));
               }
             }
+#pragma unroll
+            for (int i4 = 0; i4 < 4; ++i4) {
+              const uint4 s4 = gt_lds128(sa_cur + (uint32_t)((b * 16 + i4 * 4) * 4));
+              const float sav[4] = {__uint_as_float(s4.x), __uint_as_float(s4.y), __uint_as_float(s4.z), __uint_as_float(s4.w)};
+#pragma unroll
+              for (int ii = 0; ii < 4; ++ii) {
+                const int i = 4 * i4 + ii;
+                y[b * 16 + i] = fmaf(sav[ii], scale * (float)(int32_t)a[cur][i], y[b * 16 + i]);
+              }
+            }
+            if (DBG && dbg) {   // parity hooks: the per-group integer sums
+              const int t0 = (T % p.TT) * GT_BT + half * 64 + b * 16;
+#pragma unroll
+              for (int i = 0; i < 16; ++i)
+                if (t0 + i < p.M) dbg[((size_t)ks * p.M + (size_t)(t0 + i)) * p.N + n] = (int32_t)a[cur][i] >> 8;
+            }
           }
-          if (has && b < 3) tmem_ld16(acc0_addr + (uint32_t)(GT_ACC1_COL + (b + 1) * 16), r);   // r is free again
+        };
+        pass((uint32_t)(buf * GT_BT), swn, p.dbg0, !has);
+        if (has) {
+          pass((uint32_t)GT_ACC1_COL, srn, p.dbg1, true);
+        } else if (DBG && p.dbg1) {
+#pragma unroll 1
+          for (int i = 0; i < 64; ++i) {
+            const int t = (T % p.TT) * GT_BT + half * 64 + i;
+            if (t < p.M) p.dbg1[((size_t)ks * p.M + (size_t)t) * p.N + n] = 0;
+          }
         }
 #ifdef GT_TRACE
         gt_drain += clock64() - gt_d0;
