@@ -562,18 +562,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       // the tile's sums are complete: one rounding to the 16-bit output.  A thread owns one channel of 64 tokens; the
       // tile is transposed through shared memory so that global memory sees 16-byte stores of whole 256-byte rows
       // (64 two-byte stores per thread to 64 different rows kept the epilogue warps ~30 000 cycles per tile)
-#ifdef GT_NO_STAGE
-      {
-        const int t_first = (T % p.TT) * GT_BT + half * 64;
-        uint16_t* yp = reinterpret_cast<uint16_t*>(p.Y) + (size_t)t_first * p.ldy + (T / p.TT) * BN + (warp & 3) * 32 + lane;
-#pragma unroll
-        for (int i = 0; i < 64; ++i) {
-          if (t_first + i < p.M)
-            yp[(size_t)i * p.ldy] = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y[i])) : __half_as_ushort(__float2half_rn(y[i]));
-          y[i] = 0.f;
-        }
-      }
-#else
       {
 #ifdef GT_TRACE
         const long long gt_t0 = clock64();
@@ -613,7 +601,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         gt_tile += clock64() - gt_t0;
 #endif
       }
-#endif
     }
   }
 
