@@ -879,15 +879,17 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
                 const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
                 const int slot = gi * C::QG + qs % C::QG;
                 mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::QG) & 1);
+                uint32_t landed = 0;   // (the slot's hand-back depends on the loaded words: zero_after, mq_ptx.cuh)
                 if (r == rhalf) {
                   const uint32_t rp = sRP + slot * QUARTER_BYTES;
                   const uint4 r0 = lds128(rp + (row & 63) * 16);
                   const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
                   unpack16(r0, ro);
                   unpack16(r1, ro + 8);
+                  landed = zero_after(fold4(r0) ^ fold4(r1));
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot));
+                if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot) + landed);
               }
               tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + us * A_COLS + 16 * h), ro);
             }
@@ -1033,15 +1035,17 @@ mq_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const GemmParams p) {
               const int qs = (qseq0 + __popc(mask & ((1 << q) - 1))) & 0xFFFF;
               const int slot = gi * C::QG + qs % C::QG;
               mbar_wait(bar(B_FULL_Q + slot), ((uint32_t)qs / C::QG) & 1);
+              uint32_t landed = 0;
               if (r == rhalf) {
                 const uint32_t rp = sRP + slot * QUARTER_BYTES;
                 const uint4 r0 = lds128(rp + (row & 63) * 16);
                 const uint4 r1 = lds128(rp + 1024 + (row & 63) * 16);
                 unpack16(r0, ro);
                 unpack16(r1, ro + 8);
+                landed = zero_after(fold4(r0) ^ fold4(r1));
               }
               __syncwarp();
-              if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot));
+              if (lane == 0) mbar_arrive(bar(B_EMPTY_Q + slot) + landed);
             }
             tmem_st16(lane_addr + (uint32_t)(C::R_COL0 + rs * A_COLS + 16 * h), ro);
           }
