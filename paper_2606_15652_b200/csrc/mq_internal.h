@@ -116,9 +116,9 @@ int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M,
                 int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* workspace, size_t workspace_bytes,
                 void* cuda_stream, bool ignore_res);
 // the whole-tile prefill kernel (mq_prefill.cu): M >= 64, per-token W4A4, needs no workspace
-bool prefill_eligible(const mq_weights* w, int64_t M);
+bool prefill_eligible(const mq_weights* w, int64_t M, bool a8 = false);
 int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
-                 int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res);
+                 int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool a8 = false);
 // per-group activation scales, group = 128, on the tcgen05 path (mq_group_tc.cu): M >= 64, no workspace
 bool group_tc_eligible(const mq_weights* w, int group, int64_t M);
 int group_tc_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,

@@ -103,6 +103,18 @@ __device__ __forceinline__ void pf_unpack16(const uint4& p, uint32_t* o) {
   o[6] = (p.w << 4) & HI;
   o[7] = p.w & HI;
 }
+// W4A8: the int8 tokens come straight from global memory in canonical element order, so the weights are expanded in
+// canonical order too: word 2i = elements (0,1,2,3), word 2i + 1 = elements (4,5,6,7) of the i-th group of eight
+__device__ __forceinline__ void pf_unpack16c(const uint4& p, uint32_t* o) {
+  const uint32_t HI = 0xF0F0F0F0u;
+  const uint32_t w[4] = {p.x, p.y, p.z, p.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const uint32_t ev = (w[i] << 4) & HI, od = w[i] & HI;   // elements 0,2,4,6 | 1,3,5,7
+    o[2 * i] = __byte_perm(ev, od, 0x5140);
+    o[2 * i + 1] = __byte_perm(ev, od, 0x7362);
+  }
+}
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
@@ -210,8 +222,12 @@ __device__ __forceinline__ void tc_commit2(uint32_t bar) {
 // its own n-tile into its own tensor memory and HALF of the token tile (64 tokens) into its own shared memory; the
 // leader (rank 0) issues tcgen05.mma.cta_group::2 (M = 256) for both.  Per SM that halves the token expansion and the
 // tensor pipe's shared-memory operand reads.
-template <bool PAIR>
+// A8 (W4A8, single-CTA form only): the tokens are int8 [M][K]; a tensor copy puts the tile's 128 x 128 B of a K-step
+// straight into the operand stage in the MMA's SWIZZLE_128B layout (issued by the unpack group that owns the item, as
+// soon as the stage is free): no token pass through the CUDA cores at all.  Accumulators are x16 (weights only).
+template <bool PAIR, bool A8 = false>
 __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_constant__ CUtensorMap tmap_a, const PfParams p) {
+  static_assert(!(PAIR && A8), "W4A8 runs in the single-CTA form");
   using L = PfL<PAIR>;
   constexpr int PF_PST = L::PST, PF_U_STAGE = L::U_STAGE, PF_P_STAGE = L::P_STAGE, PF_OFF_U = L::OFF_U, PF_OFF_P = L::OFF_P,
                 PF_OFF_BAR = L::OFF_BAR, PF_OFF_MISC = L::OFF_MISC, PF_OFF_SA = L::OFF_SA, PF_B_FULL_P = L::B_FULL_P,
@@ -299,7 +315,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
   if (warp == 0) {
     if (lane == 0) {
       // ===================== producer (one thread): one K-step per stage =====================
-      griddep_wait();   // the packed tokens are the previous kernel's output
+      if (!A8) griddep_wait();   // the packed tokens are the previous kernel's output (A8: only static weights here)
       uint32_t q = 0;
       for (int T = tile0; T < p.tiles; T += tstride) {
         const int nt = nt_of(T), tt = T % p.TT;
@@ -312,9 +328,9 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
             mbar_arrive(fb);
             continue;
           }
-          mbar_arrive_expect_tx(fb, TILE_BYTES + TOK_BYTES);
+          mbar_arrive_expect_tx(fb, TILE_BYTES + (A8 ? 0u : TOK_BYTES));
           tma_load_1d(dst, wsrc + (size_t)ks * TILE_BYTES, TILE_BYTES, fb);
-          tma_load_2d(dst + TILE_BYTES, &tmap_a, ks * (BK / 2), tt * PF_BT + (int)rank * TOKR, fb);
+          if (!A8) tma_load_2d(dst + TILE_BYTES, &tmap_a, ks * (BK / 2), tt * PF_BT + (int)rank * TOKR, fb);
         }
       }
     }
@@ -499,6 +515,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
       PF_FINE(7);
       ++n_mine;
     };
+    if (A8) griddep_wait();   // the int8 tokens this group requests are the previous kernel's output
     int pT = tile0, pc0 = 0;
     int3 um_next = load_chunk(pT, pc0);
     for (int T = tile0; T < p.tiles; T += tstride) {
@@ -526,19 +543,27 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
 #pragma unroll
             for (int c = 0; c < 4; ++c) v4[c] = PF_EXP_NOW ? make_uint4(row, c, ps, g) : pf_lds128(pw + c * (BN * 16) + row * 16);
 #pragma unroll
-            for (int i = 0; i < TL; ++i) t4[i] = PF_EXP_NOT ? make_uint4(row, i, ps, g) : pf_lds128(pt + (gtid + 128u * i) * 16);
+            for (int i = 0; i < TL; ++i)
+              t4[i] = (A8 || PF_EXP_NOT) ? make_uint4(row, i, ps, g) : pf_lds128(pt + (gtid + 128u * i) * 16);
             PF_FINE(2);
             mbar_wait(bar(PF_B_EMPTY_U + g), (n_mine & 1) ^ 1);   // the poll runs under the loads' latency
             tc_fence_after();
             PF_FINE(3);
+            if (A8 && gtid == 0) {   // the stage is free: request the K-step's int8 token tile straight into it
+              mbar_expect_tx(bar(PF_B_FULL_U + g), (uint32_t)PF_U_STAGE);
+              tma_load_2d(su, &tmap_a, (c0 + j) * BK, (T % p.TT) * PF_BT, bar(PF_B_FULL_U + g));
+            }
             {
               uint32_t o[32];
 #pragma unroll
-              for (int c = 0; c < 4; ++c) pf_unpack16(v4[c], o + 8 * c);
+              for (int c = 0; c < 4; ++c) {
+                if (A8) pf_unpack16c(v4[c], o + 8 * c);
+                else pf_unpack16(v4[c], o + 8 * c);
+              }
               tmem_st32(lane_addr, o);
             }
 #pragma unroll
-            for (int i = 0; i < TL; ++i) {
+            for (int i = 0; i < (A8 ? 0 : TL); ++i) {
               const uint32_t ti = gtid + 128u * i, t = ti >> 2, c = ti & 3;
               uint32_t tw[8];
               pf_unpack16(t4[i], tw);
@@ -577,8 +602,13 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
             for (int h = 0; h < 2; ++h) {
               if (!(umask & (3u << (2 * h)))) continue;   // k-half without any block: never read by the MMA
               uint32_t ro[16];
-              pf_unpack16(r4[h][0], ro);
-              pf_unpack16(r4[h][1], ro + 8);
+              if (A8) {
+                pf_unpack16c(r4[h][0], ro);
+                pf_unpack16c(r4[h][1], ro + 8);
+              } else {
+                pf_unpack16(r4[h][0], ro);
+                pf_unpack16(r4[h][1], ro + 8);
+              }
               tmem_st16(lane_addr + (uint32_t)(16 * h), ro);
             }
             publish();
@@ -601,7 +631,9 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
       const int nt = nt_of(T), tt = T % p.TT, buf = it & 1;
       const int n = nt * BN + n_loc, t_base = tt * PF_BT;
       const int t_cnt = min(PF_BT, p.M - t_base);
-      const float swn = __ldg(p.sw + n) * 0.00390625f, srn = __ldg(p.sr + n) * 0.00390625f;   // accumulators are x256
+      constexpr float ACC_INV = A8 ? 0.0625f : 0.00390625f;   // accumulators are x256 (both operands x16), A8: x16
+      constexpr int ACC_SHIFT = A8 ? 4 : 8;
+      const float swn = __ldg(p.sw + n) * ACC_INV, srn = __ldg(p.sr + n) * ACC_INV;
       float* sat = sa_tile + buf * PF_BT;
       sat[et] = et < t_cnt ? __ldg(p.sa + t_base + et) : 0.f;
       named_bar_sync(1, 128);   // also orders this buffer's readers (two tiles ago) before its writers
@@ -674,9 +706,9 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
               y *= sat[t];
               yp0[(size_t)t * p.ldy] = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y)) : __half_as_ushort(__float2half_rn(y));
               const size_t di = (size_t)(t_base + t) * p.N + n;
-              if (p.dbg0) p.dbg0[di] = (int32_t)a[i] >> 8;
+              if (p.dbg0) p.dbg0[di] = (int32_t)a[i] >> ACC_SHIFT;
 #ifndef PF_TRACE
-              if (p.dbg1) p.dbg1[di] = has_res ? ((int32_t)r[i] >> 8) : 0;
+              if (p.dbg1) p.dbg1[di] = has_res ? ((int32_t)r[i] >> ACC_SHIFT) : 0;
 #endif
             }
           }
@@ -728,21 +760,24 @@ static bool prefill_use_pairs(const mq_weights* w) {
   return pp != 2 && (w->N / BN) % 2 == 0 && sm_count() >= 2;
 }
 
-bool prefill_eligible(const mq_weights* w, int64_t M) {
+bool prefill_eligible(const mq_weights* w, int64_t M, bool a8) {
   const Options& o = options();
   if (!w || w->blockscale || o.prefill_path == 1) return false;
   if (o.token_tile || o.split_k >= 2 || o.max_ctas || o.fused_quant) return false;   // knobs of the stream-K kernel
   if (M < 64) return false;
   if (o.prefill_path >= 2) return true;
-  const bool pairs = prefill_use_pairs(w);
+  const bool pairs = !a8 && prefill_use_pairs(w);
   const int64_t tiles = (w->N / BN) * ((M + PF_BT - 1) / PF_BT) / (pairs ? 2 : 1);
   const int64_t slots = pairs ? sm_count() / 2 : sm_count();
   const int64_t rounds = (tiles + slots - 1) / slots;
+  // (W4A8: the token tile of an item is requested only when its operand stage is free, so a CTA needs a few tiles to
+  // amortise that latency: measured crossover against the stream-K kernel between one and five rounds)
+  if (a8 && tiles < 3 * slots) return false;
   return tiles * 100 >= rounds * slots * 50;
 }
 
 int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
-                 int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res) {
+                 int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool a8) {
   typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -752,14 +787,16 @@ int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M
   // rows past M read as zero
   CUtensorMap tmap;
   memset(&tmap, 0, sizeof(tmap));
-  const cuuint64_t row_bytes = (cuuint64_t)(w->K / 2);
+  // (W4A8: int8 activations [M rows][K bytes]; box = 128 B x 128 rows, written in the MMA's SWIZZLE_128B layout)
+  const cuuint64_t row_bytes = a8 ? (cuuint64_t)w->K : (cuuint64_t)(w->K / 2);
   const cuuint64_t gdim[2] = {row_bytes, (cuuint64_t)M};
   const cuuint64_t gstride[1] = {row_bytes};
-  const bool pairs = prefill_use_pairs(w);
-  const cuuint32_t box[2] = {(cuuint32_t)(BK / 2), (cuuint32_t)(pairs ? PF_BT / 2 : PF_BT)};
+  const bool pairs = !a8 && prefill_use_pairs(w);
+  const cuuint32_t box[2] = {(cuuint32_t)(a8 ? BK : BK / 2), (cuuint32_t)(pairs ? PF_BT / 2 : PF_BT)};
   const cuuint32_t estr[2] = {1, 1};
   if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(qA), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+          a8 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
     return MQ_ERR_CUDA;
 
   PfParams pp;
@@ -783,17 +820,18 @@ int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M
   pp.tiles = (int)tiles;
   pp.y_bf16 = y_dtype == MQ_BF16;
 
-  auto kern = pairs ? mq_prefill_kernel<true> : mq_prefill_kernel<false>;
+  auto kern = a8 ? mq_prefill_kernel<false, true> : (pairs ? mq_prefill_kernel<true> : mq_prefill_kernel<false>);
   const int smem_bytes = pairs ? PfL<true>::SMEM_BYTES : PfL<false>::SMEM_BYTES;
-  static int attr_dev[2] = {-1, -1};   // the attribute belongs to the (device, function) pair
+  static int attr_dev[3] = {-1, -1, -1};   // the attribute belongs to the (device, function) pair
+  const int kidx = a8 ? 2 : (pairs ? 1 : 0);
   int dev = -1;
   cudaGetDevice(&dev);
-  if (dev != attr_dev[pairs]) {
+  if (dev != attr_dev[kidx]) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes) != cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
     }
-    attr_dev[pairs] = dev;
+    attr_dev[kidx] = dev;
   }
   cudaLaunchConfig_t cfg = {};
   const int64_t slots = pairs ? sm_count() / 2 : sm_count();

@@ -122,3 +122,74 @@ def test_w4a8_seeded_fuzz_against_oracle(mq):
         for k in ("split_k", "max_ctas", "token_tile"):
             mq.mq_set_option(k, 0)
         mq.mq_set_option("pdl", 1)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# W4A8 on the whole-tile kernel (csrc/mq_prefill.cu, template A8: the int8 token tile of a K-step goes by TMA straight
+# into the MMA's operand stage, the weights are expanded in canonical element order).  mq_gemm_a8 picks it by itself for
+# large M (the full-size cases of test_gpu_fullsize.py); option "prefill_path" = 2 forces it on small shapes.
+def with_prefill(mq, fn, path=2):
+    try:
+        mq.mq_set_option("prefill_path", path)
+        return fn()
+    finally:
+        mq.mq_set_option("prefill_path", 0)
+
+
+@pytest.mark.parametrize("out_dtype", ["bf16", "f16"])
+@pytest.mark.parametrize("M", [64, 65, 128, 129, 200, 333])
+def test_w4a8_whole_tile_token_counts(mq, M, out_dtype):
+    case = make_case(1500 + M, M, 640, 512, bs=64, rho=0.10, a_dtype="f16" if M % 2 else "bf16")
+    want = oracle_forward(case, bits=8)
+    got = with_prefill(mq, lambda: run_cuda(case, out_dtype=out_dtype, bits=8))
+    assert mq.mq_last_launch_count() == 1
+    assert_parity(got, want, what=f"W4A8 whole-tile M{M} {out_dtype}")
+    assert np.abs(want["acc1"]).sum() > 0
+
+
+@pytest.mark.parametrize("K", [128, 384, 1152, 4224, 4480])
+def test_w4a8_whole_tile_k_steps(mq, K):
+    case = make_case(1530 + K // 128, 192, K, 256, bs=64, rho=0.12)
+    want = oracle_forward(case, bits=8)
+    w = pack_from_oracle(case)
+
+    def run():
+        for rep in range(3):
+            assert_parity(run_cuda(case, w=w, bits=8), want, what=f"W4A8 whole-tile K{K} rep {rep}")
+    with_prefill(mq, run)
+
+
+@pytest.mark.parametrize("bs,budget_frac", [(64, 1.0), (128, 1.0), (64, 0.5), (64, 0.0)])
+def test_w4a8_whole_tile_residual_density(mq, bs, budget_frac):
+    case = make_case(1560 + bs, 160, 1024, 512, bs=bs, rho=budget_frac)
+    want = oracle_forward(case, bits=8)
+    got = with_prefill(mq, lambda: run_cuda(case, bits=8))
+    assert_parity(got, want, what=f"W4A8 whole-tile bs {bs} budget {budget_frac}")
+
+
+def test_w4a8_whole_tile_many_tiles_and_path_3(mq):
+    """N = 2048, M = 1100: 16 x 9 = 144 tiles; option 3 (CTA pairs) falls back to the single-CTA form for W4A8."""
+    case = make_case(1570, 1100, 512, 2048, bs=64, rho=0.06)
+    rows = np.unique(np.concatenate([np.arange(0, 1100, 37), np.arange(1020, 1100)]))
+    want = oracle_forward(case, rows=rows, bits=8)
+    for path in (2, 3):
+        got = with_prefill(mq, lambda: run_cuda(case, rows=rows, bits=8), path)
+        assert_parity(got, want, rows=rows, what=f"W4A8 whole-tile 144 tiles, path {path}")
+
+
+def test_w4a8_whole_tile_extremes(mq):
+    """+-127 tokens against +-7 weights: |acc0| = 127 * 7 * K exactly through the x16 accumulators."""
+    import torch
+    M, K, N = 130, 4096, 256
+    qw = np.full((N, K), 7, np.int8)
+    qw[1::2] = -7
+    s1 = np.ones(N, np.float32)
+    w = mq.mq_pack_prequantized(qw, s1, 64, np.array([0, 1], np.int32), np.array([0, K // 64 - 1], np.int32),
+                                np.full((2, 64, 64), -7, np.int8), s1)
+    A = torch.full((M, K), 127.0, dtype=torch.float16, device="cuda")
+    q8, sA = mq.mq_quantize_act8(A)
+    Y, d0, d1 = with_prefill(mq, lambda: mq.mq_gemm_a8(w, q8, sA, M, dbg=True))
+    torch.cuda.synchronize()
+    d0, d1 = d0.cpu().numpy(), d1.cpu().numpy()
+    assert (d0[:, 0::2] == 127 * 7 * K).all() and (d0[:, 1::2] == -127 * 7 * K).all()
+    assert (d1[:, :128] == -127 * 7 * 64).all() and not d1[:, 128:].any()
