@@ -94,8 +94,11 @@ __device__ __forceinline__ uint32_t quant_pack8(const float* f, float s, float i
 
 // CHUNKS = 16-byte chunks (8 elements) each thread keeps in registers per pass.
 // QMAX = 7: packed int4 output (4 bytes per 8 elements); QMAX = 127: int8 output (8 bytes per 8 elements)
-template <bool BF16, int CHUNKS, int QMAX = 7>
-__global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __restrict__ A, int64_t lda, int K,
+// QTT = threads per row: 256 for few rows (one row's latency chain is what counts), 128 for many rows (twice as many rows
+// resident per SM: the kernel is bound by the load -> reduce -> store chain of a row, not by bandwidth, until enough
+// rows are in flight)
+template <bool BF16, int CHUNKS, int QMAX = 7, int QTT = QT>
+__global__ void __launch_bounds__(QTT) mq_quantize_act_kernel(const uint16_t* __restrict__ A, int64_t lda, int K,
                                                              uint8_t* __restrict__ qA, float* __restrict__ sA) {
   // PDL: the next kernel (mq_gemm) may start its prologue and weight prefetch now; A may have been
   // written by the previous kernel, so wait for it before the first load.
@@ -106,13 +109,13 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
   uint32_t* qrow = reinterpret_cast<uint32_t*>(qA + m * (int64_t)(K / 2));
   uint2* qrow8 = reinterpret_cast<uint2*>(qA + m * (int64_t)K);
   const int nchunk = K / 8;
-  __shared__ float red[QT / 32];
+  __shared__ float red[QTT / 32];
 
   uint4 cache[CHUNKS];
   float amax = 0.f;
 #pragma unroll
   for (int c = 0; c < CHUNKS; ++c) {
-    int idx = threadIdx.x + c * QT;
+    int idx = threadIdx.x + c * QTT;
     if (idx < nchunk) {
       cache[c] = __ldg(row + idx);
       float f[8];
@@ -121,7 +124,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
       for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(f[i]));
     }
   }
-  for (int idx = threadIdx.x + CHUNKS * QT; idx < nchunk; idx += QT) {  // rows longer than the register cache
+  for (int idx = threadIdx.x + CHUNKS * QTT; idx < nchunk; idx += QTT) {  // rows longer than the register cache
     uint4 v = __ldg(row + idx);
     float f[8];
     cvt8<BF16>(v, f);
@@ -134,7 +137,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
   __syncthreads();
   amax = red[0];
 #pragma unroll
-  for (int i = 1; i < QT / 32; ++i) amax = fmaxf(amax, red[i]);
+  for (int i = 1; i < QTT / 32; ++i) amax = fmaxf(amax, red[i]);
 
   const float s = amax == 0.f ? 1.0f : __fdiv_rn(amax, (float)QMAX);  // A2 / Eq.1
   if (threadIdx.x == 0) sA[m] = s;
@@ -142,7 +145,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
 
 #pragma unroll
   for (int c = 0; c < CHUNKS; ++c) {
-    int idx = threadIdx.x + c * QT;
+    int idx = threadIdx.x + c * QTT;
     if (idx < nchunk) {
       float f[8];
       cvt8<BF16>(cache[c], f);
@@ -152,7 +155,7 @@ __global__ void __launch_bounds__(QT) mq_quantize_act_kernel(const uint16_t* __r
         qrow8[idx] = quant_bytes8(f, s, inv_s);
     }
   }
-  for (int idx = threadIdx.x + CHUNKS * QT; idx < nchunk; idx += QT) {
+  for (int idx = threadIdx.x + CHUNKS * QTT; idx < nchunk; idx += QTT) {
     uint4 v = __ldg(row + idx);
     float f[8];
     cvt8<BF16>(v, f);
@@ -269,7 +272,17 @@ int quantize_act_impl(const void* A, mq_dtype a_dtype, int64_t M, int64_t K, int
   uint8_t* q8 = (uint8_t*)qA;
   cudaError_t le;
   // the whole row stays in registers for K <= 16384 (one pass over global memory, all loads in flight)
-  if (a_dtype == MQ_BF16) {
+  const bool bf = a_dtype == MQ_BF16;
+  if (M >= 2048 && K / 8 <= 4 * 128) {   // many short rows: 128 threads per row (measured: +12 % at M = 8192, K = 4096;
+                                          // longer rows lose occupancy to the register cache, fewer rows gain nothing)
+    cfg.blockDim = dim3(128);
+    const int cpt = (int)((K / 8 + 127) / 128);
+#define MQ_Q128(CH)                                                                                                    \
+  (bf ? cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, CH, QMAX, 128>, a, lda, Ki, q8, sA)                       \
+      : cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<false, CH, QMAX, 128>, a, lda, Ki, q8, sA))
+    le = cpt <= 4 ? MQ_Q128(4) : (cpt <= 8 ? MQ_Q128(8) : MQ_Q128(16));
+#undef MQ_Q128
+  } else if (bf) {
     if (nchunk_per_thread <= 2)
       le = cudaLaunchKernelEx(&cfg, mq_quantize_act_kernel<true, 2, QMAX>, a, lda, Ki, q8, sA);
     else if (nchunk_per_thread <= 4)
