@@ -262,7 +262,7 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
 
 /* Concurrency and co-residency.  The decode kernel (M <= 32) and the whole-tile prefill kernels (M >= 64) contain no
  * wait of one CTA for another (CTA pairs are clusters, co-scheduled by the hardware), so calls on different streams may
- * overlap freely.  The stream-K kernel (the remaining shapes, mq_gemm_a8, option-selected paths) splits the K range of
+ * overlap freely.  The stream-K kernel (the remaining shapes, small-M mq_gemm_a8, option-selected paths) splits the K range of
  * a tile over S CTAs that WAIT for each other's partial tiles: its grid (<= the device's SM count, one CTA per SM) must
  * be co-resident.  That holds when the call has the GPU to itself; it does not hold under an MPS active-thread
  * percentage or a green context that exposes fewer SMs than cudaDevAttrMultiProcessorCount, or while another
@@ -288,9 +288,12 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
  *   "decode_rows": 0 = automatic, else 16 / 32 / 64 / 128 output channels per CTA of the decode kernel
  *   "decode_big": 0 = automatic, 1 = deep shared-memory ring (one CTA per SM; rows <= 64), 2 = small ring (two per SM)
  *   "prefill_path": 0 (default) = mq_gemm with M >= 64 runs the whole-tile tcgen05 kernel (128 x 128 output tiles dealt
- *                 round-robin to persistent CTAs, no workspace) when the last round of tiles is at least 88 % full,
- *                 else the stream-K tcgen05 kernel; 1 = never; 2 = for every M >= 64.  The stream-K knobs above
- *                 ("token_tile", "split_k" >= 2, "max_ctas") also select the stream-K kernel.
+ *                 round-robin to persistent CTAs, no workspace; CTA pairs with tcgen05.mma.cta_group::2 when the layer
+ *                 has an even number of 128-channel tiles) when the last round of tiles is at least half full, else
+ *                 the stream-K tcgen05 kernel; mq_gemm_a8 runs the whole-tile kernel's W4A8 form (single CTAs, int8
+ *                 token tiles by TMA straight into the MMA operand stage) from three rounds of tiles per CTA upwards;
+ *                 1 = never; 2 = for every M >= 64, one CTA per tile; 3 = for every M >= 64, CTA pairs where possible.
+ *                 The stream-K knobs above ("token_tile", "split_k" >= 2, "max_ctas") also select the stream-K kernel.
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor
  *                 in the stream (prologue and weight prefetch overlap its tail); 0 = plain launches
  * Returns MQ_ERR_INVALID_ARG for an unknown name or value. */
