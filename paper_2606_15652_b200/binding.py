@@ -384,14 +384,17 @@ def mq_linear_host_staging_bytes(w: Weights, M: int) -> int:
 
 
 def mq_linear_host(w: Weights, A_host: torch.Tensor, Y_host: torch.Tensor, staging: torch.Tensor,
-                   workspace: torch.Tensor) -> torch.Tensor:
+                   workspace: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
     """End-to-end entry with HOST tensors (pinned for asynchronous copies): enqueues H2D copy, mq_linear and
-    D2H copy on the current stream; the caller synchronises before reading Y_host."""
+    D2H copy on `stream` (default: the current stream); the caller synchronises that stream before reading Y_host.
+    Independent calls given different streams (and their own staging and workspace) overlap one call's copies with
+    another's kernels."""
     M, K = A_host.shape
     assert A_host.is_contiguous() and Y_host.is_contiguous() and not A_host.is_cuda and not Y_host.is_cuda
+    st = _stream() if stream is None else stream.cuda_stream
     _check(lib().mq_linear_host(w.handle, A_host.data_ptr(), _dtype_code(A_host.dtype), M, Y_host.data_ptr(),
                                 _dtype_code(Y_host.dtype), staging.data_ptr(), staging.numel(), workspace.data_ptr(),
-                                workspace.numel(), _stream()), "mq_linear_host")
+                                workspace.numel(), st), "mq_linear_host")
     return Y_host
 
 

@@ -431,6 +431,30 @@ def test_linear_host_buffers_end_to_end(mq):
             assert np.array_equal(Y_host.float().numpy().astype(np.float64), got["Y"])
 
 
+def test_linear_host_calls_on_their_own_streams(mq):
+    """Independent mq_linear_host calls, each on its own stream with its own staging and workspace (how bench.py's
+    end-to-end leg overlaps one call's copies with another's kernels): every result equals the device path."""
+    import torch
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    jobs = []
+    for j, (M, K, N) in enumerate([(40, 1024, 384), (3, 512, 256), (70, 768, 640), (8, 1024, 384), (1, 2048, 128)]):
+        case = make_case(171 + j, M, K, N, bs=64, rho=0.1)
+        w = pack_from_oracle(case)
+        got = run_cuda(case, w=w)
+        jobs.append((w, torch.from_numpy(case.A16).pin_memory(), torch.empty((M, N), dtype=torch.bfloat16).pin_memory(),
+                     torch.empty(mq.mq_linear_host_staging_bytes(w, M), dtype=torch.uint8, device="cuda"),
+                     mq.new_workspace(mq.mq_linear_workspace_bytes(w, M)), got["Y"]))
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for j, (w, A_host, Y_host, stg, ws, _) in enumerate(jobs):
+            Y_host.zero_()
+            mq.mq_linear_host(w, A_host, Y_host, stg, ws, streams[j % 3])
+        for s in streams:
+            s.synchronize()
+        for j, (_, _, Y_host, _, _, want) in enumerate(jobs):
+            assert np.array_equal(Y_host.float().numpy().astype(np.float64), want), f"job {j}, round {rep}"
+
+
 def test_m_zero_is_noop(mq):
     import torch
     case = make_case(51, 1, 256, 128, rho=0.0)
