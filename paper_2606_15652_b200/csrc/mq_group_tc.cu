@@ -3,31 +3,38 @@
 // (first half).  A group of 128 channels is exactly one K-step of the packed layout, so the integer sum
 // of a group is what ONE K-step's MMAs leave in the accumulator: the accumulator is drained after every K-step.
 //
-// The kernel is mq_prefill.cu's single-CTA form (whole 128 x 128 tiles dealt to persistent CTAs; weights expanded
-// int4 -> int8 x16 in registers -> tcgen05.st into TENSOR MEMORY as the A operand; tokens expanded into K-major
-// SWIZZLE_128B shared memory as the B operand; tcgen05.mma kind::i8; residual cells as operand-ring items of their own)
-// with a different accumulator discipline:
+// Whole 128 x 128 tiles are dealt to persistent CTAs as in mq_prefill.cu, but the operands are the other way round: the
+// TOKENS are the A operand (expanded int4 -> int8 x16 in registers -> tcgen05.st into TENSOR MEMORY, TMEM lane = token),
+// the WEIGHTS are the B operand (expanded into K-major SWIZZLE_128B shared memory); tcgen05.mma kind::i8; residual
+// cells are operand-ring items of their own (their weights in a B buffer, the K-step's tokens re-used from tensor
+// memory).  So an accumulator lane is a token and a column a channel, and an epilogue thread owns ONE token:
+// the group scale s_a[t, g], the factor that changes every K-step, is a register (one 4-byte load per thread and
+// K-step), and the channel scales, which do not change, are applied once per tile.  (The first version had channels
+// in the lanes: every thread then needed the 64 group scales of its tokens from shared memory in every K-step, 64 KB
+// per K-step through the shared-memory pipe, plus a block-wide barrier per K-step to publish them.)
 //   * the base accumulator is double-buffered PER K-STEP: the MMAs of K-step k+1 run into the other 128 columns while
-//     the epilogue warps read the sums of K-step k (tcgen05.ld), scale them and add them to fp32 running sums held in
-//     registers.  Measured (one-off probe): eight warps drain, convert and FMA a 128 x 128 int32 accumulator in ~313
-//     cycles, less than the ~560 cycles a K-step takes in the per-token kernel, so the drain hides behind the MMAs;
-//   * the residual accumulator is single-buffered and handed over per CELL (cells are rare);
-//   * eight epilogue warps (two per TMEM lane quadrant, 64 tokens each) keep 64 fp32 sums per thread for the whole
-//     tile; the group scales of the tile's tokens for the NEXT K-step are gathered into shared memory while the current
-//     one is being drained.
-// Tensor memory (512 columns): acc0 2 x 128 | acc1 128 | A operand ring 4 x 32.  Roles (16 warps = 512 threads, the
-// largest block that still gets 128 registers per thread: the epilogue needs them; one CTA per SM):
-//   warp 0 producer (TMA) | warp 1 MMA issuer | warps 2-9 epilogue | warps 10-13 weight unpack (one per TMEM lane
-//   quadrant; every item) | warps 14-15 token unpack (shared memory has no quadrant rule; every base item).
-// Arithmetic per output and group, in the order of mq_group.cu's mma.sync kernel: term = s_w * acc0 (s_w carries the
-// 2^-8 of the x16 operands, exact), term = fma(s_r, acc1, term) if the K-step owns a cell, y = fma(s_a, term, y),
-// groups in ascending order; one rounding to the 16-bit output at the end (tolerance T2 of DESIGN.md section 4).
+//     the epilogue warps read the sums of K-step k (tcgen05.ld), convert them and add them to fp32 running sums held in
+//     registers; the residual accumulator is single-buffered and handed over per CELL (cells are rare);
+//   * the running sums are kept in units of s_w: y = sum_g s_a acc0_g + (s_a rho) acc1_g, rho = s_r / s_w, and
+//     Y = (s_w / 256) y at the end of the tile (the operands are x16): two instructions per base sum (I2F, FFMA).  A tile
+//     with a channel whose s_w is 0 (or whose ratio is not finite) keeps units of 1 instead (a third instruction);
+//   * eight epilogue warps (two per TMEM lane quadrant, 64 channels each) keep 64 fp32 sums per thread for the whole
+//     tile and store them as 128 contiguous bytes of the token's Y row.
+// Tensor memory (512 columns): acc0 2 x 128 | acc1 128 | A operand ring 4 x 32.  Roles (16 warps = 512 threads in four
+// warp groups; the block starts with 128 registers per thread and setmaxnreg moves 32 per thread from the other groups
+// to the epilogue: 160 there (64 sums + two batches of 32 columns in flight), 96 elsewhere; one CTA per SM):
+//   warp 0 producer (TMA) | warp 1 MMA issuer | warps 2-3 weight unpack (rows 0..63 -> shared memory) |
+//   warps 4-11 epilogue | warps 12-15 token unpack (one per TMEM lane quadrant: a token row each -> tensor memory, plus
+//   the weight rows 64..127 and the residual cells -> shared memory, so that all six unpack warps carry about the same).
+// Arithmetic per output: fp32, groups in ascending order, one rounding to the 16-bit output at the end (tolerance T2 of
+// DESIGN.md section 4).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <type_traits>
 #include <cstring>
 
 #include "mq_internal.h"
@@ -38,19 +45,22 @@ namespace {
 using namespace mq;
 using namespace mq::ptx;
 
-constexpr int GT_BT = 128;                        // tokens per tile (MMA N)
+constexpr int GT_BT = 128;                        // tokens per tile (MMA M: the tokens are the A operand, TMEM lane = token)
 constexpr int GT_UST = 4;                         // operand (U) stages
-constexpr int GT_EWARPS = 8;                      // epilogue warps: lane quadrant = warp % 4, token half = (warp - 2) / 4
-constexpr int GT_WWARPS = 4;                      // weight-unpack warps (one per TMEM lane quadrant)
-constexpr int GT_TWARPS = 2;                      // token-unpack warps
-constexpr int GT_WARP_W0 = 2 + GT_EWARPS, GT_WARP_T0 = GT_WARP_W0 + GT_WWARPS;
+constexpr int GT_EWARPS = 8;                      // epilogue warps: lane quadrant = warp % 4, channel half = (warp - GT_WARP_E0) / 4
+constexpr int GT_WWARPS = 2;                      // weight-unpack warps (weight rows 0..63 -> shared memory)
+constexpr int GT_TWARPS = 4;                      // token-unpack warps (one per TMEM lane quadrant; also weight rows 64..127 and the cells)
+// warp groups of four (setmaxnreg acts on whole warp groups): {producer, MMA, weight unpack x 2} | epilogue | epilogue | token unpack
+constexpr int GT_WARP_W0 = 2, GT_WARP_E0 = GT_WARP_W0 + GT_WWARPS, GT_WARP_T0 = GT_WARP_E0 + GT_EWARPS;
 constexpr int GT_WARPS = GT_WARP_T0 + GT_TWARPS;
+constexpr int GT_REGS_EPI = 160, GT_REGS_REST = 96;   // registers per thread after the split: 256 x 160 + 256 x 96 = 64 K
+static_assert(GT_WARP_E0 == 4 && GT_WARP_T0 == 12 && GT_WARPS == 16, "roles fill whole warp groups");
 constexpr int GT_THREADS = 32 * GT_WARPS;         // 512: the largest block that still gets 128 registers per thread
 constexpr int GT_A_COLS = BK / 4;                 // 32 TMEM columns hold 128 int8 per lane (one K-step)
 constexpr int GT_ACC1_COL = 2 * GT_BT;
 constexpr int GT_A_COL0 = 3 * GT_BT;
 constexpr int GT_PST = 8;                         // packed (P) stages of one K-step
-constexpr int GT_U_STAGE = GT_BT * BK;            // int8 token sub-tile of one K-step (16 KB)
+constexpr int GT_U_STAGE = BN * BK;               // int8 weight sub-tile of one K-step (16 KB), the B operand
 constexpr int GT_TOK_KSTEP = GT_BT * (BK / 2);    // packed tokens of one K-step (8 KB)
 constexpr int GT_P_STAGE = TILE_BYTES + GT_TOK_KSTEP;
 constexpr int GT_OFF_U = 0;
@@ -60,9 +70,10 @@ constexpr int GT_OFF_BAR = GT_OFF_P + GT_PST * GT_P_STAGE;
 constexpr int GT_B_FULL_P = 0, GT_B_EMPTY_P = GT_PST, GT_B_FULL_U = 2 * GT_PST, GT_B_EMPTY_U = GT_B_FULL_U + GT_UST,
               GT_B_GFULL = GT_B_EMPTY_U + GT_UST, GT_B_GEMPTY = GT_B_GFULL + 2, GT_B_A1E = GT_B_GEMPTY + 2, GT_NUM_BARS = GT_B_A1E + 1;
 constexpr int GT_OFF_MISC = GT_OFF_BAR + GT_NUM_BARS * 8 + 8;     // [0] tmem base
-constexpr int GT_OFF_SA = (GT_OFF_MISC + 16 + 15) / 16 * 16;      // [2][128] group scales of the tile's tokens (this / next K-step)
-constexpr int GT_OFF_YST = (GT_OFF_SA + 2 * GT_BT * 4 + 127) / 128 * 128;   // [128 tokens][128 channels] 16-bit: the finished tile, staged
-constexpr int GT_SMEM_BYTES = GT_OFF_YST + GT_BT * BN * 2 + 1024;  // + slack for the 1024-byte alignment
+// per-tile channel constants, double-buffered by tile parity: [2]{[{fin, rho, bscale, s_r}][128] floats, flag word}
+constexpr int GT_OFF_TC = (GT_OFF_MISC + 16 + 15) / 16 * 16;
+constexpr int GT_TC_BYTES = 4 * BN * 4 + 16;
+constexpr int GT_SMEM_BYTES = GT_OFF_TC + 2 * GT_TC_BYTES + 1024;  // + slack for the 1024-byte alignment
 static_assert(GT_SMEM_BYTES <= 232448, "shared memory budget");
 static_assert(GT_A_COL0 + GT_UST * GT_A_COLS == 512, "tensor memory budget");
 static_assert(GT_OFF_P % 1024 == 0 && GT_P_STAGE % 1024 == 0 && GT_U_STAGE % 1024 == 0, "swizzle atoms need 1024-byte alignment");
@@ -136,7 +147,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sU = smem_base + GT_OFF_U, sP = smem_base + GT_OFF_P, sBar = smem_base + GT_OFF_BAR, sMisc = smem_base + GT_OFF_MISC,
-                 sSA = smem_base + GT_OFF_SA;
+                 sTC = smem_base + GT_OFF_TC;
   auto bar = [&](int i) { return sBar + 8u * (uint32_t)i; };
   volatile int32_t* misc = reinterpret_cast<volatile int32_t*>(smem_raw + (sMisc - smem_u32(smem_raw)));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -159,6 +170,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     }
     mbar_init(bar(GT_B_A1E), GT_EWARPS);
     fence_mbar_init();
+    for (int i = 0; i < 2; ++i) asm volatile("st.shared.u32 [%0], %1;" ::"r"(sTC + (uint32_t)(i * GT_TC_BYTES + 4 * BN * 4)), "r"(0u) : "memory");
   }
   if (warp == 1) {
     tmem_alloc(sMisc, 512);
@@ -169,6 +181,11 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
   tc_fence_after();
   const uint32_t tmem_base = (uint32_t)misc[0];
   griddep_launch();
+  // The block is launched with 128 registers per thread (512 threads: the whole register file).  The epilogue warp groups
+  // take 160 (64 running sums + two batches of 32 accumulator columns in flight), the other two give theirs up: the
+  // first statement of every role (inside the role's branch, so that the compiler knows which budget holds where).
+#define GT_REGS_DEC() asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(GT_REGS_REST))
+#define GT_REGS_INC() asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(GT_REGS_EPI))
 #ifdef GT_TRACE
   const long long gt_start = clock64();
   long long gt_acc[2] = {0, 0}, gt_drain = 0, gt_tile = 0, gt_m1 = 0, gt_m2 = 0, gt_m3 = 0;
@@ -189,128 +206,43 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     }
   };
 
-  if (warp == 0) {
-    if (lane == 0) {
-      // ===================== producer (one thread): one K-step per stage =====================
-      griddep_wait();   // the packed tokens are the previous kernel's output
-      uint32_t q = 0;
-      for (int T = tile0; T < p.tiles; T += tstride) {
-        const int nt = T / p.TT, tt = T - nt * p.TT;
-        const uint8_t* wsrc = p.base + (size_t)nt * KS * TILE_BYTES;
-        for (int ks = 0; ks < KS; ++ks, ++q) {
-          const uint32_t ps = q % GT_PST;
-          mbar_wait(bar(GT_B_EMPTY_P + ps), ((q / GT_PST) & 1) ^ 1);
-          const uint32_t fb = bar(GT_B_FULL_P + ps), dst = sP + ps * GT_P_STAGE;
-          mbar_arrive_expect_tx(fb, TILE_BYTES + GT_TOK_KSTEP);
-          tma_load_1d(dst, wsrc + (size_t)ks * TILE_BYTES, TILE_BYTES, fb);
-          tma_load_2d(dst + TILE_BYTES, &tmap_a, ks * (BK / 2), tt * GT_BT, fb);
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
-    constexpr uint32_t IDESC = make_idesc_i8(BN, GT_BT);
-    uint32_t item = 0, kq = 0, cq = 0;   // operand-ring items, K-steps and cells so far
-    bool pre_ok = false;                 // the barrier of the item about to be processed was already seen complete
-    // the operand stage of item i: FULL_U[i & 3], phase (i >> 2) & 1; the next item's barrier is polled once BEFORE this
-    // item's MMAs are issued, so that the round trip hides under the tensor pipe's work
-    auto acquire = [&]() {
-      if (!pre_ok) {
-        GT_T0();
-        mbar_wait(bar(GT_B_FULL_U + (int)(item & 3)), (item >> 2) & 1);
-        GT_ACC(0);
-      }
-      tc_fence_after();
-      pre_ok = mbar_try_wait(bar(GT_B_FULL_U + (int)((item + 1) & 3)), ((item + 1) >> 2) & 1);
-    };
-    int pT = tile0, pc0 = 0;
-    int2 um_next = load_chunk(pT, pc0);
-    for (int T = tile0; T < p.tiles; T += tstride) {
-      for (int c0 = 0; c0 < KS; c0 += 32) {
-        const int2 um = um_next;
-        next_chunk(pT, pc0);
-        um_next = load_chunk(pT, pc0);
-        const uint32_t bits = __ballot_sync(0xffffffffu, (um.x & 0xF) != 0);
-        const int nk = min(32, KS - c0);
-        for (int j = 0; j < nk; ++j, ++kq) {
-          const bool has = (bits >> j) & 1;
-          const int us = (int)(item & 3), buf = (int)(kq & 1);
-          acquire();
-          {
-            GT_T0();
-            mbar_wait(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
-            GT_ACC(1);
-          }
-          tc_fence_after();
-          const uint32_t d0 = tmem_base + (uint32_t)(buf * GT_BT);
-          const uint32_t at = tmem_base + (uint32_t)(GT_A_COL0 + us * GT_A_COLS);
-          const uint64_t dt = make_desc_sw128(sU + us * GT_U_STAGE);
-          if (elect_one()) {
-#pragma unroll
-            for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? 0u : 1u);   // a fresh sum per group
-            if (!has) {
-              tc_commit(bar(GT_B_EMPTY_U + us));
-              tc_commit(bar(GT_B_GFULL + buf));
-            }
-          }
-          __syncwarp();
-          ++item;
-          if (has) {
-            // residual cell of this K-step: its weights in the next stage's A columns, the tokens of this K-step's
-            // stage (the paper's re-use of the activation tile), second accumulator, also a fresh sum
-            const uint32_t mask = (uint32_t)__shfl_sync(0xffffffffu, um.x, j) & 0xF;
-            const int us2 = (int)(item & 3);
-            acquire();
-            mbar_wait(bar(GT_B_A1E), (cq & 1) ^ 1);   // the epilogue has read the previous cell's sums
-            tc_fence_after();
-            const uint32_t d1 = tmem_base + (uint32_t)GT_ACC1_COL;
-            const uint32_t at2 = tmem_base + (uint32_t)(GT_A_COL0 + us2 * GT_A_COLS);
-            if (elect_one()) {
-              uint32_t on = 0;
-#pragma unroll
-              for (int h = 0; h < 2; ++h)
-                if (mask & (3u << (2 * h))) {
-#pragma unroll
-                  for (int k = 2 * h; k < 2 * h + 2; ++k) {
-                    mma_i8_ts(d1, at2 + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, on);
-                    on = 1;
-                  }
-                }
-              tc_commit(bar(GT_B_EMPTY_U + us2));
-              tc_commit(bar(GT_B_EMPTY_U + us));
-              tc_commit(bar(GT_B_GFULL + buf));   // both accumulators of the K-step are complete
-            }
-            __syncwarp();
-            ++item;
-            ++cq;
-          }
-        }
-      }
-    }
-  }
-  else if (warp >= GT_WARP_W0) {
-    // ============ unpack warps: int4 -> int8 (x16); weights -> TMEM (warps 10-13), tokens -> swizzled shared memory (14-15) ============
-    // Both kinds walk all items in order; item i uses operand stage i % 4.  A stage is complete when all six warps have
-    // arrived (for a residual item the token warps have nothing to do, but arrive in order all the same).
-    const bool wrole = warp < GT_WARP_T0;
-    const int wq = warp & 3;                            // TMEM lane quadrant of a weight warp
-    const uint32_t row = (uint32_t)(wq * 32 + lane);    // output channel inside the tile
-    const uint32_t ttid = (uint32_t)((warp - GT_WARP_T0) * 32 + lane);   // 0..63 among the token warps
+  // the unpack role, instantiated for the token warps (warp group 3) and the weight warps (in warp group 0)
+  auto unpack_role = [&](auto trole_c) {
+    constexpr bool trole = decltype(trole_c)::value;
+    // ============ unpack warps: int4 -> int8 (x16).  Token warps (12-15, one per TMEM lane quadrant): token row -> TENSOR
+    // MEMORY (the A operand), plus their share of the weight rows (64..127) and the residual cells -> swizzled shared
+    // memory (the B operand).  Weight warps (2-3): weight rows 0..63 -> swizzled shared memory. ============
+    // All six walk all items in order; item i uses operand stage i % 4 (A columns and B buffer alike).  A stage is
+    // complete when all six warps have arrived (for a residual item the weight warps have nothing to do, but arrive in
+    // order all the same).
+    const int wq = warp & 3;                            // TMEM lane quadrant of a token warp
+    const uint32_t row = (uint32_t)(wq * 32 + lane);    // token warps: token inside the tile = TMEM lane; also the channel whose cell rows it expands
+    const uint32_t wrow = trole ? 64u + (row & 63u) : (uint32_t)((warp - GT_WARP_W0) * 32 + lane);   // weight row this thread expands
+    const uint32_t wc0 = trole ? 2u * (row >> 6) : 0u;  // ... and its first 16-byte chunk (token warps: two chunks, weight warps: all four)
+    const uint32_t tsw = (row >> 1) & 3u;               // the token tile arrives with SWIZZLE_64B: chunk c of row r at ((c ^ (r >> 1 & 3)) << 4)
     const uint32_t lane_base = tmem_base + ((uint32_t)(wq * 32) << 16) + (uint32_t)GT_A_COL0;
     const int rhalf = (int)(row >> 6);
     uint32_t item = 0, q = 0;   // items / K-steps so far (the K-step counter names the P stage)
     auto wait_stage = [&](uint32_t idx) {   // operand stage idx % 4 has been consumed by the MMAs of item idx - 4
       GT_T0();
-      mbar_wait(bar(GT_B_EMPTY_U + (int)(idx & 3)), ((idx >> 2) & 1) ^ 1);
+      mbar_wait_parked(bar(GT_B_EMPTY_U + (int)(idx & 3)), ((idx >> 2) & 1) ^ 1);
       GT_ACC(7);
       tc_fence_after();
     };
     auto publish = [&](uint32_t idx) {   // this warp's part of the item is in place: tell the MMA warp
-      if (wrole) tmem_st_wait();
+      if (trole) tmem_st_wait();
       tc_fence_before();
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(GT_B_FULL_U + (int)(idx & 3)));
+    };
+    // 16 packed bytes (chunk c of weight row r) -> 32 int8 at the row's 16-byte columns 2c, 2c + 1 of the K-major
+    // SWIZZLE_128B operand buffer
+    auto expand_to_smem = [&](uint32_t su, uint32_t r, uint32_t c, const uint4& v) {
+      uint32_t tw[8];
+      gt_unpack16(v, tw);
+      gt_sts128(su + r * 128 + (((2 * c) ^ (r & 7)) << 4), tw);
+      gt_sts128(su + r * 128 + (((2 * c + 1) ^ (r & 7)) << 4), tw + 4);
     };
     int pT = tile0, pc0 = 0;
     int2 um_next = load_chunk(pT, pc0);
@@ -327,17 +259,20 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           const uint32_t ps = (q + (uint32_t)j) % GT_PST;
           {
             GT_T0();
-            mbar_wait(bar(GT_B_FULL_P + ps), ((q + (uint32_t)j) / GT_PST) & 1);
+            mbar_wait_parked(bar(GT_B_FULL_P + ps), ((q + (uint32_t)j) / GT_PST) & 1);
             GT_ACC(6);
           }
           const uint32_t pw = sP + ps * GT_P_STAGE, pt = pw + TILE_BYTES;
-          if (wrole) {
-            // ---- base item, weights: one thread per output channel ----
-            uint4 v4[4];
+          const uint32_t su = sU + (idx & 3) * GT_U_STAGE;
+          if (trole) {
+            // ---- base item: one token row -> TMEM, two chunks of a weight row -> shared memory ----
+            uint4 v4[4], w2[2];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) v4[c] = gt_lds128(pw + c * (BN * 16) + row * 16);
+            for (int c = 0; c < 4; ++c) v4[c] = gt_lds128(pt + row * 64 + (((uint32_t)c ^ tsw) << 4));
+#pragma unroll
+            for (int c = 0; c < 2; ++c) w2[c] = gt_lds128(pw + (wc0 + (uint32_t)c) * (BN * 16) + wrow * 16);
             // the packed stage is in registers: back to the producer (the arrival depends on every loaded word, see zero_after)
-            const uint32_t landed = zero_after(fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]));
+            const uint32_t landed = zero_after(fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]) ^ fold4(w2[0]) ^ fold4(w2[1]));
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps) + landed);
             wait_stage(idx);
@@ -345,9 +280,13 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
 #pragma unroll
             for (int c = 0; c < 4; ++c) gt_unpack16(v4[c], o + 8 * c);
             tmem_st32(lane_base + (uint32_t)((idx & 3) * GT_A_COLS), o);
+#pragma unroll
+            for (int c = 0; c < 2; ++c) expand_to_smem(su, wrow, wc0 + (uint32_t)c, w2[c]);
             publish(idx);
             if (has) {
-              // ---- residual item: the cell's packed rows straight from global memory ----
+              // ---- residual item: the cell's packed rows straight from global memory -> the next stage's B buffer; this
+              //      thread = channel `row`; a k-half that holds a block is written for all 128 channels (zeros where the
+              //      other row half has no block), a k-half without any block is never read by the MMA ----
               const uint32_t rmask = (uint32_t)__shfl_sync(0xffffffffu, um.x, j) & 0xF;
               const uint32_t qoff = (uint32_t)__shfl_sync(0xffffffffu, um.y, j);
               uint4 r4[2][2];
@@ -363,37 +302,26 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
                 }
               }
               wait_stage(idx + 1);
+              const uint32_t su2 = sU + ((idx + 1) & 3) * GT_U_STAGE;
 #pragma unroll
               for (int h = 0; h < 2; ++h) {
-                if (!(rmask & (3u << (2 * h)))) continue;   // k-half without any block: never read by the MMA
-                uint32_t ro[16];
-                gt_unpack16(r4[h][0], ro);
-                gt_unpack16(r4[h][1], ro + 8);
-                tmem_st16(lane_base + (uint32_t)(((idx + 1) & 3) * GT_A_COLS + 16 * h), ro);
+                if (!(rmask & (3u << (2 * h)))) continue;
+                expand_to_smem(su2, row, (uint32_t)(2 * h), r4[h][0]);
+                expand_to_smem(su2, row, (uint32_t)(2 * h + 1), r4[h][1]);
               }
               publish(idx + 1);
             }
           } else {
-            // ---- base item, tokens: 512 chunks of 16 bytes (8 nibbles x 4 ... ) dealt to 64 threads ----
-            uint4 t4[8];
+            // ---- base item: one weight row (0..63), four chunks -> shared memory ----
+            uint4 v4[4];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) t4[i] = gt_lds128(pt + (ttid + 64u * i) * 16);
-            uint32_t chk = 0;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) chk ^= fold4(t4[i]);
-            const uint32_t landed = zero_after(chk);
+            for (int c = 0; c < 4; ++c) v4[c] = gt_lds128(pw + c * (BN * 16) + wrow * 16);
+            const uint32_t landed = zero_after(fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]));
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps) + landed);
             wait_stage(idx);
-            const uint32_t su = sU + (idx & 3) * GT_U_STAGE;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              const uint32_t ti = ttid + 64u * i, t = ti >> 2, c = ti & 3;
-              uint32_t tw[8];
-              gt_unpack16(t4[i], tw);
-              gt_sts128(su + t * 128 + (((2 * c) ^ (t & 7)) << 4), tw);
-              gt_sts128(su + t * 128 + (((2 * c + 1) ^ (t & 7)) << 4), tw + 4);
-            }
+            for (int c = 0; c < 4; ++c) expand_to_smem(su, wrow, (uint32_t)c, v4[c]);
             publish(idx);
             if (has) {   // nothing to expand for a residual item: keep the stage's arrival count in step
               wait_stage(idx + 1);
@@ -405,34 +333,150 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         q += (uint32_t)nk;
       }
     }
+  };
+
+  if (warp < GT_WARP_E0) {
+    GT_REGS_DEC();   // one instruction for the whole warp group
+    if (warp == 0) {
+      if (lane == 0) {
+        // ===================== producer (one thread): one K-step per stage =====================
+        griddep_wait();   // the packed tokens are the previous kernel's output
+        uint32_t q = 0;
+        for (int T = tile0; T < p.tiles; T += tstride) {
+          const int nt = T / p.TT, tt = T - nt * p.TT;
+          const uint8_t* wsrc = p.base + (size_t)nt * KS * TILE_BYTES;
+          for (int ks = 0; ks < KS; ++ks, ++q) {
+            const uint32_t ps = q % GT_PST;
+            mbar_wait_parked(bar(GT_B_EMPTY_P + ps), ((q / GT_PST) & 1) ^ 1);
+            const uint32_t fb = bar(GT_B_FULL_P + ps), dst = sP + ps * GT_P_STAGE;
+            mbar_arrive_expect_tx(fb, TILE_BYTES + GT_TOK_KSTEP);
+            tma_load_1d(dst, wsrc + (size_t)ks * TILE_BYTES, TILE_BYTES, fb);
+            tma_load_2d(dst + TILE_BYTES, &tmap_a, ks * (BK / 2), tt * GT_BT, fb);
+          }
+        }
+      }
+    } else if (warp == 1) {
+      // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
+      constexpr uint32_t IDESC = make_idesc_i8(GT_BT, BN);   // M = 128 tokens (A, tensor memory), N = 128 channels (B, shared memory)
+      uint32_t item = 0, kq = 0, cq = 0;   // operand-ring items, K-steps and cells so far
+      bool pre_ok = false;                 // the barrier of the item about to be processed was already seen complete
+      // the operand stage of item i: FULL_U[i & 3], phase (i >> 2) & 1; the next item's barrier is polled once BEFORE this
+      // item's MMAs are issued, so that the round trip hides under the tensor pipe's work
+      auto acquire = [&]() {
+        if (!pre_ok) {
+          GT_T0();
+          mbar_wait_parked(bar(GT_B_FULL_U + (int)(item & 3)), (item >> 2) & 1);
+          GT_ACC(0);
+        }
+        tc_fence_after();
+        pre_ok = mbar_try_wait(bar(GT_B_FULL_U + (int)((item + 1) & 3)), ((item + 1) >> 2) & 1);
+      };
+      int pT = tile0, pc0 = 0;
+      int2 um_next = load_chunk(pT, pc0);
+      for (int T = tile0; T < p.tiles; T += tstride) {
+        for (int c0 = 0; c0 < KS; c0 += 32) {
+          const int2 um = um_next;
+          next_chunk(pT, pc0);
+          um_next = load_chunk(pT, pc0);
+          const uint32_t bits = __ballot_sync(0xffffffffu, (um.x & 0xF) != 0);
+          const int nk = min(32, KS - c0);
+          for (int j = 0; j < nk; ++j, ++kq) {
+            const bool has = (bits >> j) & 1;
+            const int us = (int)(item & 3), buf = (int)(kq & 1);
+            acquire();
+            {
+              GT_T0();
+              mbar_wait_parked(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
+              GT_ACC(1);
+            }
+            tc_fence_after();
+            const uint32_t d0 = tmem_base + (uint32_t)(buf * GT_BT);
+            const uint32_t at = tmem_base + (uint32_t)(GT_A_COL0 + us * GT_A_COLS);
+            const uint64_t dt = make_desc_sw128(sU + us * GT_U_STAGE);
+            if (elect_one()) {
+  #pragma unroll
+              for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? 0u : 1u);   // a fresh sum per group
+              if (!has) {
+                tc_commit(bar(GT_B_EMPTY_U + us));
+                tc_commit(bar(GT_B_GFULL + buf));
+              }
+            }
+            __syncwarp();
+            ++item;
+            if (has) {
+              // residual cell of this K-step: its weights in the next stage's B buffer, the tokens of this K-step's
+              // stage (the paper's re-use of the activation tile), second accumulator, also a fresh sum
+              const uint32_t mask = (uint32_t)__shfl_sync(0xffffffffu, um.x, j) & 0xF;
+              const int us2 = (int)(item & 3);
+              acquire();
+              mbar_wait_parked(bar(GT_B_A1E), (cq & 1) ^ 1);   // the epilogue has read the previous cell's sums
+              tc_fence_after();
+              const uint32_t d1 = tmem_base + (uint32_t)GT_ACC1_COL;
+              const uint64_t dt2 = make_desc_sw128(sU + us2 * GT_U_STAGE);
+              if (elect_one()) {
+                uint32_t on = 0;
+  #pragma unroll
+                for (int h = 0; h < 2; ++h)
+                  if (mask & (3u << (2 * h))) {
+  #pragma unroll
+                    for (int k = 2 * h; k < 2 * h + 2; ++k) {
+                      mma_i8_ts(d1, at + (uint32_t)(k * 8), dt2 + (uint64_t)(k * 2), IDESC, on);
+                      on = 1;
+                    }
+                  }
+                tc_commit(bar(GT_B_EMPTY_U + us2));
+                tc_commit(bar(GT_B_EMPTY_U + us));
+                tc_commit(bar(GT_B_GFULL + buf));   // both accumulators of the K-step are complete
+              }
+              __syncwarp();
+              ++item;
+              ++cq;
+            }
+          }
+        }
+      }
+    } else {
+      unpack_role(std::false_type{});   // weight warps
+    }
+  } else if (warp >= GT_WARP_T0) {
+    GT_REGS_DEC();
+    unpack_role(std::true_type{});      // token warps
   }
   else {
-    // ===================== epilogue warps (2..9): drain every K-step's sums into fp32 running sums =====================
-    // Register budget (128 per thread): 64 running sums + three batches of 16 + a dozen scalars; whether a K-step owns a
-    // cell is therefore fetched from global memory one K-step ahead instead of kept in lanes.
+    // ===================== epilogue warps (4..11): drain every K-step's sums into fp32 running sums =====================
+    // A thread owns ONE token (its TMEM lane) and 64 channels (columns): the group scale s_a[t, g] is a register, the
+    // channel scales are applied once per tile.  Register budget (160 per thread after the split): 64 running sums + two
+    // batches of 32 + two dozen scalars; whether a K-step owns a cell is fetched from global memory one K-step ahead.
+    GT_REGS_INC();
     griddep_wait();   // the group scales and Y are ordered after the previous kernel in the stream
-    const int half = (warp - 2) >> 2;             // which 64 tokens of the tile; TMEM lane quadrant = warp % 4
-    const int et = (warp - 2) * 32 + lane;        // 0..255 within the epilogue group
-    const uint32_t acc0_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(half * 64);
+    const int half = (warp - GT_WARP_E0) >> 2;        // which 64 channels of the tile; TMEM lane quadrant = warp % 4
+    const int et = (warp - GT_WARP_E0) * 32 + lane;   // 0..255 within the epilogue group
+    const int trow = (warp & 3) * 32 + lane;          // this thread's token inside the tile
+    // Values the K-step loop uses again and again are made opaque to the compiler (an empty asm that "modifies" them):
+    // otherwise it re-derives them from %tid and the shared-memory window at every use (special-register reads, shifts,
+    // uniform-register moves: a third of the loop's time went there) instead of keeping six registers.
+    uint32_t acc0_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(half * 64);
+    uint32_t b_gfull = bar(GT_B_GFULL), b_gempty = bar(GT_B_GEMPTY), b_a1e = bar(GT_B_A1E);
+    uint32_t lane0 = lane == 0 ? 1u : 0u;
+    asm volatile("" : "+r"(acc0_addr), "+r"(b_gfull), "+r"(b_gempty), "+r"(b_a1e), "+r"(lane0));
     float y[64];
 #pragma unroll
     for (int i = 0; i < 64; ++i) y[i] = 0.f;
-    // group scales s_a[t, g] of the tile's 128 tokens: gathered by threads 0..127 two K-steps ahead (a register), written
-    // to the double-buffered shared array one K-step ahead, read by everybody in the K-step itself
-    // (pointers advanced by one per K-step and recomputed once per tile: no integer division in the K-step loop)
-    int fT = tile0, fks = 0;   // the K-step the next gather is for
-    const float* fp = nullptr;   // &s_a[token of this thread in tile fT][fks], or NULL (no such token / not a gathering thread)
+    // group scales s_a[t, g] of this thread's token: one scalar per K-step, requested two K-steps ahead
+    // (a pointer advanced by one per K-step and recomputed once per tile: no integer division in the K-step loop)
+    int fT = tile0, fks = 0;     // the K-step the next request is for
+    const float* fp = nullptr;   // &s_a[token of this thread in tile fT][0], or NULL (no such token)
     auto gather_tile = [&]() {
       fp = nullptr;
-      if (et < GT_BT && fT < p.tiles) {
-        const int t = (fT % p.TT) * GT_BT + et;
+      if (fT < p.tiles) {
+        const int t = (fT % p.TT) * GT_BT + trow;
         if (t < p.M) fp = p.sa + (size_t)t * KS;
       }
     };
     gather_tile();
     auto gather = [&]() -> float {
       float v = 0.f;
-      // (asm volatile: the request must be ISSUED here, a K-step ahead of its use; a plain __ldg may be sunk to the use)
+      // (asm volatile: the request must be ISSUED here, ahead of its use; a plain __ldg may be sunk to the use)
       if (fp) asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(fp + fks));
       if (++fks == KS) {
         fks = 0;
@@ -441,11 +485,8 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       }
       return v;
     };
-    {
-      const float v0 = gather();
-      if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + 4u * (uint32_t)et), "f"(v0) : "memory");
-    }
-    float v_held = gather();   // for K-step 1
+    float sa_cur = gather();   // K-step 0
+    float sa_nxt = gather();   // K-step 1
     // whether the NEXT K-step owns a cell: one load per K-step from a pointer that walks the tile's metadata row
     const int2* mp = p.unit_meta ? p.unit_meta + (size_t)(tile0 / p.TT) * KS : nullptr;   // (tile0 < tiles: the grid is <= tiles)
     auto cell_at = [&](const int2* q) -> int {
@@ -453,15 +494,59 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       if (q) asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(&q->x));
       return v & 0xF;
     };
-    uint32_t kq = 0;
+    uint32_t kq = 0, tile_no = 0;
     int has_next = cell_at(mp);
-    for (int T = tile0; T < p.tiles; T += tstride) {
-      const int n = (T / p.TT) * BN + (warp & 3) * 32 + lane;   // this thread's output channel
-      const float swn = __ldg(p.sw + n) * 0.00390625f, srn = __ldg(p.sr + n) * 0.00390625f;   // accumulators are x256
+    // The sums leave tensor memory in batches of 32 channels (two tcgen05.ld of 16 columns), two register buffers: while
+    // one batch is scaled and added the next one is in flight -- across passes and K-steps too: the first batch of the
+    // NEXT pass (the residual sums of this K-step, or the base sums of the tile's next K-step, whose MMAs finished long
+    // ago) is requested before the arithmetic of this pass's last batch.  tcgen05.wait::ld waits for every outstanding
+    // load of the thread, so there is exactly one batch outstanding at every wait.
+    uint32_t a[2][32];
+    auto issue = [&](uint32_t col, uint32_t* dst) {
+      tmem_ld16(acc0_addr + col, dst);
+      tmem_ld16(acc0_addr + col + 16u, dst + 16);
+    };
+    auto landed = [&](uint32_t* v) { gt_ld_wait32(v, v + 16); };
+    // (an empty statement that "modifies" a batch: the arithmetic on it cannot be scheduled above it, hence not above the
+    // loads just issued; otherwise the compiler sinks the loads below the arithmetic and every batch pays the full
+    // tensor-memory latency)
+    auto tie = [&](uint32_t* v) {
+      gt_tie16(v);
+      gt_tie16(v + 16);
+    };
+    auto request_base = [&](uint32_t k) {   // first batch of K-step k's base sums -> a[0]
+      GT_T0();
+      mbar_wait_parked(b_gfull + 8u * (k & 1u), (k >> 1) & 1);
+      GT_ACC(3);
+      tc_fence_after();
+      issue((k & 1) * (uint32_t)BN, a[0]);
+    };
+    for (int T = tile0; T < p.tiles; T += tstride, ++tile_no) {
+      const int n0 = (T / p.TT) * BN;
+      // Per-tile channel constants in shared memory (double-buffered by tile parity, one barrier per tile).  The running
+      // sums are kept in units of s_w: y = sum_g s_a acc0_g + (s_a rho) acc1_g with rho = s_r / s_w, times fin = s_w / 256
+      // at the end: two instructions per base sum (I2F, FFMA).  A tile that holds a channel with s_w = 0 (or a ratio that
+      // is not finite) keeps its sums in units of 1 and pays a third instruction (bscale = s_w, rho = s_r, fin = 1/256).
+      const uint32_t tc = sTC + (tile_no & 1u) * (uint32_t)GT_TC_BYTES;
+      if (et < BN) {
+        const float sw_raw = __ldg(p.sw + n0 + et), sr_raw = __ldg(p.sr + n0 + et);
+        const float ratio = __fdiv_rn(sr_raw, sw_raw);
+        const bool odd = sw_raw == 0.f || !(fabsf(ratio) <= 3.0e38f);
+        asm volatile("st.shared.f32 [%0], %1;" ::"r"(tc + 4u * (uint32_t)et), "f"(sw_raw * 0.00390625f) : "memory");          // fin (regular tile)
+        asm volatile("st.shared.f32 [%0], %1;" ::"r"(tc + 4u * (uint32_t)(BN + et)), "f"(odd ? 0.f : ratio) : "memory");      // rho (regular tile)
+        asm volatile("st.shared.f32 [%0], %1;" ::"r"(tc + 4u * (uint32_t)(2 * BN + et)), "f"(sw_raw) : "memory");             // bscale (irregular tile)
+        asm volatile("st.shared.f32 [%0], %1;" ::"r"(tc + 4u * (uint32_t)(3 * BN + et)), "f"(sr_raw) : "memory");             // rho (irregular tile)
+        // [4 * BN]: the number (+ 1) of the last irregular tile that used this buffer, written by any thread that sees an
+        // odd channel (zero at kernel start; never cleared: a stale number does not match)
+        if (odd) asm volatile("st.shared.u32 [%0], %1;" ::"r"(tc + 4u * (uint32_t)(4 * BN)), "r"(tile_no + 1u) : "memory");
+      }
+      named_bar_sync(1, 32 * GT_EWARPS);   // the constants of this tile are visible; everybody has left tile T - 2 * stride
+      uint32_t flag;
+      asm volatile("ld.shared.u32 %0, [%1];" : "=r"(flag) : "r"(tc + 4u * (uint32_t)(4 * BN)));
+      const bool slow = flag == tile_no + 1u;
+      const uint32_t tc_half = tc + (uint32_t)(half * 64 * 4);
+      request_base(kq);   // (no load is left in flight across the tile's output stage)
       for (int ks = 0; ks < KS; ++ks, ++kq) {
-#ifdef GT_TRACE
-        const long long gt_a = clock64();
-#endif
         const bool has = has_next != 0;
         if (mp) {
           if (ks + 1 < KS) {
@@ -471,132 +556,127 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           }
         }
         has_next = cell_at(mp);
-#ifdef GT_TRACE
-        gt_m1 += clock64() - gt_a;
-#endif
         const int buf = (int)(kq & 1);
-        // publish the scales of K-step kq + 1, request those of K-step kq + 2
-        {
-          GT_T0();
-          named_bar_sync(1, 32 * GT_EWARPS);   // the readers of K-step kq - 1 are done; K-step kq's scales are visible
-          GT_ACC(2);
-        }
-#ifdef GT_TRACE
-        const long long gt_b = clock64();
-#endif
-        if (et < GT_BT) asm volatile("st.shared.f32 [%0], %1;" ::"r"(sSA + (uint32_t)((buf ^ 1) * GT_BT * 4) + 4u * (uint32_t)et), "f"(v_held) : "memory");
-#ifdef GT_TRACE
-        const long long gt_c = clock64();
-        gt_m2 += gt_c - gt_b;
-#endif
-        v_held = gather();
-#ifdef GT_TRACE
-        gt_m3 += clock64() - gt_c;
-#endif
-        {
-          GT_T0();
-          mbar_wait(bar(GT_B_GFULL + buf), (kq >> 1) & 1);
-          GT_ACC(3);
-        }
-        tc_fence_after();
+        const float sa = sa_cur;   // s_a[this token, this K-step's group]
+        sa_cur = sa_nxt;
+        sa_nxt = gather();         // K-step kq + 2
 #ifdef GT_TRACE
         const long long gt_d0 = clock64();
 #endif
-        const uint32_t sa_cur = sSA + (uint32_t)(buf * GT_BT * 4) + (uint32_t)(half * 64 * 4);
-        // four batches of 16 tokens, double-buffered in registers (batch b + 1 is in flight while batch b is scaled and
-        // added).  The residual sums of a K-step that owns a cell (one in twenty) take a second pass of the same shape:
-        // inside the first pass the compiler if-converts the cell test and EVERY element pays for it.
-        auto pass = [&](uint32_t col0, float scale, int32_t* dbg, bool last) {
-          uint32_t a[2][16];
-          tmem_ld16(acc0_addr + col0, a[0]);
+        // y += s_a * sum (base, regular tile) | s_a * (bscale * sum) (base, irregular tile) | (s_a * rho) * sum (residual)
+        auto add32 = [&](const uint32_t* v, int b, auto mode_c, int32_t* dbg) {
+          constexpr int MODE = decltype(mode_c)::value;
 #pragma unroll
-          for (int b = 0; b < 4; ++b) {
-            const int cur = b & 1;
-            gt_ld_wait32(a[cur], a[cur ^ 1]);
-            if (b < 3) {
-              tmem_ld16(acc0_addr + col0 + (uint32_t)((b + 1) * 16), a[cur ^ 1]);
-              // (an empty statement that "modifies" the current batch: the arithmetic on it cannot be scheduled above
-              // it, hence not above the load just issued; otherwise the compiler sinks the load below the arithmetic
-              // and every batch pays the full tensor-memory latency)
-              gt_tie16(a[cur]);
-            } else if (last) {   // this warp's part of the accumulators is in registers: hand them back to the MMA warp
-              tc_fence_before();
-              __syncwarp();
-              if (lane == 0) {
-                mbar_arrive(bar(GT_B_GEMPTY + buf));
-                if (has) mbar_arrive(bar(GT_B_A1E));
-              }
+          for (int i4 = 0; i4 < 8; ++i4) {
+            float cs[4] = {0.f, 0.f, 0.f, 0.f};
+            if (MODE != 0) {
+              const uint4 c4 = gt_lds128(tc_half + (uint32_t)(((MODE == 1 ? 2 : (slow ? 3 : 1)) * BN) * 4) + (uint32_t)((b * 32 + i4 * 4) * 4));
+              cs[0] = __uint_as_float(c4.x);
+              cs[1] = __uint_as_float(c4.y);
+              cs[2] = __uint_as_float(c4.z);
+              cs[3] = __uint_as_float(c4.w);
             }
 #pragma unroll
-            for (int i4 = 0; i4 < 4; ++i4) {
-              const uint4 s4 = gt_lds128(sa_cur + (uint32_t)((b * 16 + i4 * 4) * 4));
-              const float sav[4] = {__uint_as_float(s4.x), __uint_as_float(s4.y), __uint_as_float(s4.z), __uint_as_float(s4.w)};
-#pragma unroll
-              for (int ii = 0; ii < 4; ++ii) {
-                const int i = 4 * i4 + ii;
-                y[b * 16 + i] = fmaf(sav[ii], scale * (float)(int32_t)a[cur][i], y[b * 16 + i]);
-              }
+            for (int ii = 0; ii < 4; ++ii) {
+              const int i = 4 * i4 + ii;
+              const float f = (float)(int32_t)v[i];
+              if (MODE == 0) y[b * 32 + i] = fmaf(sa, f, y[b * 32 + i]);
+              if (MODE == 1) y[b * 32 + i] = fmaf(sa, cs[ii] * f, y[b * 32 + i]);
+              if (MODE == 2) y[b * 32 + i] = fmaf(sa * cs[ii], f, y[b * 32 + i]);
             }
-            if (DBG && dbg) {   // parity hooks: the per-group integer sums
-              const int t0 = (T % p.TT) * GT_BT + half * 64 + b * 16;
+          }
+          if (DBG && dbg) {   // parity hooks: the per-group integer sums
+            const int t = (T % p.TT) * GT_BT + trow;
+            if (t < p.M) {
 #pragma unroll
-              for (int i = 0; i < 16; ++i)
-                if (t0 + i < p.M) dbg[((size_t)ks * p.M + (size_t)(t0 + i)) * p.N + n] = (int32_t)a[cur][i] >> 8;
+              for (int i = 0; i < 32; ++i) dbg[((size_t)ks * p.M + (size_t)t) * p.N + n0 + half * 64 + b * 32 + i] = (int32_t)v[i] >> 8;
             }
           }
         };
-        pass((uint32_t)(buf * GT_BT), swn, p.dbg0, !has);
+        auto hand_back = [&]() {   // this warp's part of the K-step's accumulators is in registers: back to the MMA warp
+          tc_fence_before();
+          __syncwarp();
+          if (lane0) {
+            mbar_arrive(b_gempty + 8u * (uint32_t)buf);
+            if (has) mbar_arrive(b_a1e);
+          }
+        };
+        // ---- base sums (a[0] was requested during the previous pass) ----
+        landed(a[0]);
+        issue((uint32_t)(buf * BN) + 32u, a[1]);
+        tie(a[0]);
+        if (!slow) add32(a[0], 0, std::integral_constant<int, 0>{}, p.dbg0); else add32(a[0], 0, std::integral_constant<int, 1>{}, p.dbg0);
+        landed(a[1]);
+        if (!has) {
+          hand_back();
+          if (ks + 1 < KS) request_base(kq + 1);
+        } else {
+          issue((uint32_t)GT_ACC1_COL, a[0]);
+        }
+        tie(a[1]);
+        if (!slow) add32(a[1], 1, std::integral_constant<int, 0>{}, p.dbg0); else add32(a[1], 1, std::integral_constant<int, 1>{}, p.dbg0);
+        // ---- residual sums of a K-step that owns a cell (a pass of its own: inside the base pass the compiler if-converts
+        //      the cell test and EVERY element pays for it) ----
         if (has) {
-          pass((uint32_t)GT_ACC1_COL, srn, p.dbg1, true);
+          landed(a[0]);
+          issue((uint32_t)GT_ACC1_COL + 32u, a[1]);
+          tie(a[0]);
+          add32(a[0], 0, std::integral_constant<int, 2>{}, p.dbg1);
+          landed(a[1]);
+          hand_back();
+          if (ks + 1 < KS) request_base(kq + 1);
+          tie(a[1]);
+          add32(a[1], 1, std::integral_constant<int, 2>{}, p.dbg1);
         } else if (DBG && p.dbg1) {
+          const int t = (T % p.TT) * GT_BT + trow;
+          if (t < p.M) {
 #pragma unroll 1
-          for (int i = 0; i < 64; ++i) {
-            const int t = (T % p.TT) * GT_BT + half * 64 + i;
-            if (t < p.M) p.dbg1[((size_t)ks * p.M + (size_t)t) * p.N + n] = 0;
+            for (int i = 0; i < 64; ++i) p.dbg1[((size_t)ks * p.M + (size_t)t) * p.N + n0 + half * 64 + i] = 0;
           }
         }
 #ifdef GT_TRACE
         gt_drain += clock64() - gt_d0;
 #endif
       }
-      // the tile's sums are complete: one rounding to the 16-bit output.  A thread owns one channel of 64 tokens; the
-      // tile is transposed through shared memory so that global memory sees 16-byte stores of whole 256-byte rows
-      // (64 two-byte stores per thread to 64 different rows kept the epilogue warps ~30 000 cycles per tile)
+      // the tile's sums are complete: times the channel constant, one rounding to the 16-bit output.  A thread owns 64
+      // consecutive channels of one token: 128 contiguous bytes of Y, stored as eight 16-byte pieces
       {
 #ifdef GT_TRACE
         const long long gt_t0 = clock64();
 #endif
-        const uint32_t yst = smem_base + GT_OFF_YST;
-        const int n_loc = (warp & 3) * 32 + lane;
-#pragma unroll
-        for (int i = 0; i < 64; ++i) {
-          const uint16_t h = p.y_bf16 ? __bfloat16_as_ushort(__float2bfloat16_rn(y[i])) : __half_as_ushort(__float2half_rn(y[i]));
-          asm volatile("st.shared.u16 [%0], %1;" ::"r"(yst + (uint32_t)(((half * 64 + i) * BN + n_loc) * 2)), "h"(h) : "memory");
-          y[i] = 0.f;
-        }
-        named_bar_sync(2, 32 * GT_EWARPS);
-        const int t_base = (T % p.TT) * GT_BT, n0 = (T / p.TT) * BN;
-        uint8_t* yg = reinterpret_cast<uint8_t*>(p.Y) + ((size_t)t_base * p.ldy + n0) * 2;
+        const int t = (T % p.TT) * GT_BT + trow;
+        uint8_t* yrow = reinterpret_cast<uint8_t*>(p.Y) + ((size_t)t * p.ldy + n0 + half * 64) * 2;
         const bool vec = ((p.ldy & 7) == 0) && ((reinterpret_cast<uintptr_t>(p.Y) & 15) == 0);   // rows 16-byte aligned
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const int c = et + 256 * i, t = c >> 4, part = c & 15;   // 16 chunks of 16 bytes per token row
-          if (t_base + t < p.M) {
-            const uint4 v = gt_lds128(yst + (uint32_t)(t * (BN * 2) + part * 16));
-            uint8_t* dst = yg + (size_t)t * p.ldy * 2 + part * 16;
+        for (int i8 = 0; i8 < 8; ++i8) {
+          uint32_t w4[4];
+#pragma unroll
+          for (int h4 = 0; h4 < 2; ++h4) {
+            const uint4 c4 = gt_lds128(tc_half + (uint32_t)((i8 * 8 + h4 * 4) * 4));   // fin of four channels
+            const float fin[4] = {__uint_as_float(c4.x), __uint_as_float(c4.y), __uint_as_float(c4.z), __uint_as_float(c4.w)};
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int i = i8 * 8 + h4 * 4 + 2 * e;
+              const float v0 = y[i] * (slow ? 0.00390625f : fin[2 * e]), v1 = y[i + 1] * (slow ? 0.00390625f : fin[2 * e + 1]);
+              const uint32_t lo = p.y_bf16 ? (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v0)) : (uint32_t)__half_as_ushort(__float2half_rn(v0));
+              const uint32_t hi = p.y_bf16 ? (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v1)) : (uint32_t)__half_as_ushort(__float2half_rn(v1));
+              w4[h4 * 2 + e] = lo | (hi << 16);
+              y[i] = 0.f;
+              y[i + 1] = 0.f;
+            }
+          }
+          if (t < p.M) {
             if (vec) {
-              *reinterpret_cast<uint4*>(dst) = v;
+              *reinterpret_cast<uint4*>(yrow + i8 * 16) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
             } else {
-              const uint32_t w4[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                reinterpret_cast<uint16_t*>(dst)[2 * k] = (uint16_t)(w4[k] & 0xFFFF);
-                reinterpret_cast<uint16_t*>(dst)[2 * k + 1] = (uint16_t)(w4[k] >> 16);
+                reinterpret_cast<uint16_t*>(yrow + i8 * 16)[2 * k] = (uint16_t)(w4[k] & 0xFFFF);
+                reinterpret_cast<uint16_t*>(yrow + i8 * 16)[2 * k + 1] = (uint16_t)(w4[k] >> 16);
               }
             }
           }
         }
-        named_bar_sync(2, 32 * GT_EWARPS);   // the staging tile is free for the next tile
 #ifdef GT_TRACE
         gt_tile += clock64() - gt_t0;
 #endif
@@ -606,12 +686,12 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
 
 
 #ifdef GT_TRACE
-  if (blockIdx.x == 0 && lane == 0 && (warp == 1 || warp == 2 || warp == GT_WARP_W0 || warp == GT_WARP_T0)) {
+  if (blockIdx.x == 0 && lane == 0 && (warp == 1 || warp == GT_WARP_E0 || warp == GT_WARP_W0 || warp == GT_WARP_T0)) {
     p.trace[32 + warp] = clock64() - gt_start;
-    const int base = warp == 1 ? 0 : (warp == 2 ? 2 : (warp == GT_WARP_W0 ? 6 : 8));
+    const int base = warp == 1 ? 0 : (warp == GT_WARP_E0 ? 2 : (warp == GT_WARP_W0 ? 6 : 8));
     p.trace[base] = gt_acc[0];
     p.trace[base + 1] = gt_acc[1];
-    if (warp == 2) { p.trace[4] = gt_drain; p.trace[5] = gt_tile; p.trace[20] = gt_m1; p.trace[21] = gt_m2; p.trace[22] = gt_m3; }
+    if (warp == GT_WARP_E0) { p.trace[4] = gt_drain; p.trace[5] = gt_tile; p.trace[20] = gt_m1; p.trace[21] = gt_m2; p.trace[22] = gt_m3; }
   }
 #endif
   // teardown (single-lane regions re-converge first: bar.sync must be reached warp-convergent)
@@ -641,8 +721,9 @@ int group_tc_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t 
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
   EncodeTiledFn enc = (EncodeTiledFn)tensor_map_encode_fn();
   if (!enc) return MQ_ERR_CUDA;
-  // 2-D tensor map over the canonical packed activations [M rows][K/2 bytes]: box = one K-step of one token tile;
-  // rows past M read as zero
+  // 2-D tensor map over the canonical packed activations [M rows][K/2 bytes]: box = one K-step of one token tile
+  // (128 rows of 64 bytes, 16-byte chunks XOR-swizzled by (row >> 1) & 3 so that a thread per row reads without bank
+  // conflicts); rows past M read as zero
   CUtensorMap tmap;
   memset(&tmap, 0, sizeof(tmap));
   const cuuint64_t row_bytes = (cuuint64_t)(w->K / 2);
@@ -651,7 +732,7 @@ int group_tc_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t 
   const cuuint32_t box[2] = {(cuuint32_t)(BK / 2), (cuuint32_t)GT_BT};
   const cuuint32_t estr[2] = {1, 1};
   if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(qA), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+          CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
     return MQ_ERR_CUDA;
 
   GtParams gp;

@@ -53,6 +53,26 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   }
 }
 
+// The same wait with a suspend-time hint: the thread is parked by the hardware until the phase completes (or the hint, in
+// nanoseconds, runs out) instead of coming back every few dozen cycles.  A spinning warp costs issue slots and ALU-pipe
+// cycles (try_wait, counter, compare, branch per round) that the warps doing the arithmetic on the same scheduler need;
+// for roles that wait most of the time this is the wait to use.
+__device__ __forceinline__ bool mbar_try_wait_parked(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity), "r"(20000u)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_parked(uint32_t bar, uint32_t parity) {
+  uint32_t spins = 0;
+  while (!mbar_try_wait_parked(bar, parity)) {
+    if (++spins > (1u << 20)) __trap();
+  }
+}
+
 // ---- proxies / fences -------------------------------------------------------------------
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }

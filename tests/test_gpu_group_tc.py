@@ -5,7 +5,8 @@ int32 accumulators [K/128, M, N] bit-exact (parity hooks = the kernel's second i
 
 The cases aim at what is specific to this kernel: an accumulator that is drained after EVERY K-step (two buffers, handed
 back and forth between the MMA warp and eight epilogue warps), a residual accumulator handed over per cell, group scales
-gathered two K-steps ahead across tile boundaries, ragged last token tiles, K-step counts around the ring depths and the
+requested two K-steps ahead across tile boundaries, channel scales applied once per tile (and the tiles where that is
+not possible), ragged last token tiles, K-step counts around the ring depths and the
 32-K-step metadata chunk, tiles with a cell in every K-step and in none, more tiles than CTAs, both output types, the
 transposed (vector) and the unaligned (scalar) output store, and repeated calls on a long-K layer that must give the
 same bits every time (the packed-stage hand-off hazard this kernel exposed).
@@ -89,6 +90,38 @@ def test_group_tc_irregular_block_pattern(mq):
         w = pack_from_oracle(case)
         got = run_group(mq, case, 128, w, dbg=(trial != 1))
         check(got, want_of(case), 128, K, "bf16", f"group tc irregular blocks, density {dens}")
+
+
+def test_group_tc_channels_with_a_zero_scale(mq):
+    """The kernel keeps its running sums in units of s_w (channel scale applied once per tile) and falls back to units
+    of 1 for a tile that holds a channel with s_w = 0.  (a) all-zero weight rows (the oracle gives them scale 1 and
+    codes 0: output exactly 0), (b) a channel whose base scale is forced to 0 while its residual blocks and s_r stay
+    (only the residual term is left) and one with both scales forced to 0 (output 0), next to regular tiles in the same
+    launch."""
+    rng = np.random.default_rng(1477)
+    N, K, bs, M = 384, 1024, 64, 150
+    W = synth.gen_weight(1477, N, K)
+    W[5, :] = 0.0
+    W[130:134, :] = 0.0
+    d = oracle.decompose(W)
+    assert not d.qw[5].any() and not d.qr[5].any()
+    nb = (N // bs) * (K // bs)
+    sel = np.sort(rng.choice(nb, size=nb // 4, replace=False))
+    L = oracle.PackedLayer(N, K, bs, d, None, (sel // (K // bs)).astype(np.int32), (sel % (K // bs)).astype(np.int32))
+    case = Case(M, K, N, bs, W, None, synth.gen_act(1477, M, K), "f16", L)
+    for variant in ("zero rows", "base scale forced to 0"):
+        if variant != "zero rows":
+            d.sw[200] = 0.0          # tile 1 of 3; its blocks and s_r stay
+            d.sw[201] = 0.0
+            d.sr[201] = 0.0
+            assert d.sr[200] != 0.0
+        w = pack_from_oracle(case)
+        want = want_of(case)
+        for dbg in (True, False):
+            got = run_group(mq, case, 128, w, dbg=dbg)
+            check(got, want, 128, K, "bf16", f"group tc, {variant}, dbg {dbg}")
+        assert not got["Y"][:, 5].any() and not got["Y"][:, 130:134].any()
+    assert np.abs(want["Y"][:, 200]).sum() > 0 and not got["Y"][:, 201].any()
 
 
 def test_group_tc_more_tiles_than_ctas(mq):
