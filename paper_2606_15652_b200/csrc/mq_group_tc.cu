@@ -386,7 +386,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             acquire();
             {
               GT_T0();
-              mbar_wait_parked(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
+              mbar_wait(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
               GT_ACC(1);
             }
             tc_fence_after();
@@ -462,40 +462,35 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     float y[64];
 #pragma unroll
     for (int i = 0; i < 64; ++i) y[i] = 0.f;
-    // group scales s_a[t, g] of this thread's token: one scalar per K-step, requested two K-steps ahead
+    // group scales s_a[t, g] of this thread's token: one scalar per K-step, requested one K-step ahead
     // (a pointer advanced by one per K-step and recomputed once per tile: no integer division in the K-step loop)
     int fT = tile0, fks = 0;     // the K-step the next request is for
-    const float* fp = nullptr;   // &s_a[token of this thread in tile fT][0], or NULL (no such token)
+    // &s_a[token of this thread in tile fT][0].  Always a valid row: a token past M (ragged last tile; its accumulator
+    // rows are zero and it is never stored) reads the last row, requests past the last tile re-read the last one
+    const float* fp = p.sa;
     auto gather_tile = [&]() {
-      fp = nullptr;
-      if (fT < p.tiles) {
-        const int t = (fT % p.TT) * GT_BT + trow;
-        if (t < p.M) fp = p.sa + (size_t)t * KS;
-      }
+      if (fT < p.tiles) fp = p.sa + (size_t)min((fT % p.TT) * GT_BT + trow, p.M - 1) * KS;
     };
     gather_tile();
-    auto gather = [&]() -> float {
-      float v = 0.f;
+    auto gather_into = [&](float& v) {
       // (asm volatile: the request must be ISSUED here, ahead of its use; a plain __ldg may be sunk to the use)
-      if (fp) asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(fp + fks));
+      asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(fp + fks));
       if (++fks == KS) {
         fks = 0;
         fT += tstride;
         gather_tile();
       }
+    };
+    auto gather = [&]() -> float {
+      float v;
+      gather_into(v);
       return v;
     };
-    float sa_cur = gather();   // K-step 0
-    float sa_nxt = gather();   // K-step 1
-    // whether the NEXT K-step owns a cell: one load per K-step from a pointer that walks the tile's metadata row
-    const int2* mp = p.unit_meta ? p.unit_meta + (size_t)(tile0 / p.TT) * KS : nullptr;   // (tile0 < tiles: the grid is <= tiles)
-    auto cell_at = [&](const int2* q) -> int {
-      int v = 0;
-      if (q) asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(&q->x));
-      return v & 0xF;
-    };
+    float sa_nxt = gather();   // K-step 0
+    // which K-steps own a cell: the metadata words of 32 consecutive K-steps in the lanes, as in the other roles
+    int pT = tile0, pc0 = 0;
+    int2 um_next = load_chunk(pT, pc0);
     uint32_t kq = 0, tile_no = 0;
-    int has_next = cell_at(mp);
     // The sums leave tensor memory in batches of 32 channels (two tcgen05.ld of 16 columns), two register buffers: while
     // one batch is scaled and added the next one is in flight -- across passes and K-steps too: the first batch of the
     // NEXT pass (the residual sums of this K-step, or the base sums of the tile's next K-step, whose MMAs finished long
@@ -516,7 +511,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     };
     auto request_base = [&](uint32_t k) {   // first batch of K-step k's base sums -> a[0]
       GT_T0();
-      mbar_wait_parked(b_gfull + 8u * (k & 1u), (k >> 1) & 1);
+      mbar_wait(b_gfull + 8u * (k & 1u), (k >> 1) & 1);
       GT_ACC(3);
       tc_fence_after();
       issue((k & 1) * (uint32_t)BN, a[0]);
@@ -546,20 +541,20 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       const bool slow = flag == tile_no + 1u;
       const uint32_t tc_half = tc + (uint32_t)(half * 64 * 4);
       request_base(kq);   // (no load is left in flight across the tile's output stage)
-      for (int ks = 0; ks < KS; ++ks, ++kq) {
-        const bool has = has_next != 0;
-        if (mp) {
-          if (ks + 1 < KS) {
-            ++mp;
-          } else {
-            mp = T + tstride < p.tiles ? p.unit_meta + (size_t)((T + tstride) / p.TT) * KS : nullptr;
-          }
-        }
-        has_next = cell_at(mp);
+      for (int c0 = 0; c0 < KS; c0 += 32) {
+        const int2 um = um_next;
+        next_chunk(pT, pc0);
+        um_next = load_chunk(pT, pc0);
+        const uint32_t bits = __ballot_sync(0xffffffffu, (um.x & 0xF) != 0);
+        const int nk = min(32, KS - c0);
+      for (int j = 0; j < nk; ++j, ++kq) {
+        const int ks = c0 + j;
+        const bool has = (bits >> j) & 1;
         const int buf = (int)(kq & 1);
-        const float sa = sa_cur;   // s_a[this token, this K-step's group]
-        sa_cur = sa_nxt;
-        sa_nxt = gather();         // K-step kq + 2
+        // s_a[this token, this K-step's group], requested one K-step ago; the next one is requested now, into the same
+        // register (nothing may touch that register before the next K-step: a copy right behind the load would wait for it)
+        const float sa = sa_nxt;
+        gather_into(sa_nxt);
 #ifdef GT_TRACE
         const long long gt_d0 = clock64();
 #endif
@@ -637,6 +632,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
 #ifdef GT_TRACE
         gt_drain += clock64() - gt_d0;
 #endif
+      }
       }
       // the tile's sums are complete: times the channel constant, one rounding to the 16-bit output.  A thread owns 64
       // consecutive channels of one token: 128 contiguous bytes of Y, stored as eight 16-byte pieces
