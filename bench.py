@@ -408,8 +408,8 @@ def roofline_of(r, peaks, traffic):
     if has("us_group"):
         extra["group128_time_over_per_token"] = sum(s["us_group"] for s in r["per_shape"]) / us
         extra["group128_note"] = ("mq_gemm_group (per-group activation scales, group 128, P:441; tcgen05 kernel with a "
-                                  "per-K-step accumulator drain for M >= 64, mma.sync kernel below) over the per-token "
-                                  "kernel, same launches")
+                                  "per-K-step accumulator drain for M >= 64, the decode kernel with a per-K-step "
+                                  "conversion for M <= 32) over the per-token kernel, same launches")
     if has("us_naive"):
         extra["naive3_time_over_fused"] = sum(s["us_naive"] for s in r["per_shape"]) / us
         extra["naive3_note"] = ("the paper's naive pipeline (dense GEMM, separate sparse-block GEMM, reduce-add: mq_gemm_naive) "

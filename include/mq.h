@@ -209,8 +209,10 @@ int mq_gemm_naive(const mq_weights* w, const void* qA_dev, const float* sA_dev, 
  * workspace_dev: mq_gemm_group_workspace_bytes(w, M) bytes (may be 0), 16-byte aligned, no initial content
  * required.  Kernels: group = 128 and M >= 64 run on the tcgen05 tensor path (mq_group_tc.cu: whole 128 x 128 tiles, the
  * TMEM accumulator double-buffered and drained after every K-step = group into fp32 running sums; one launch, no
- * workspace; option "group_tc" = 0 switches it off); every other case runs the warp-level mma.sync kernel on a cp.async
- * shared-memory ring (one or two launches; M <= 16 * 65535).  Errors as mq_gemm. */
+ * workspace); group = 128 and M <= 32 run in the row-slab decode kernel (mq_decode.cu, the sums of a K-step converted
+ * and added right after its MMAs; one launch, no workspace); option "group_tc" = 0 switches both off; every other
+ * case runs the warp-level mma.sync kernel on a cp.async shared-memory ring (one or two launches; M <= 16 * 65535).
+ * Errors as mq_gemm. */
 int mq_quantize_act_group(const void* A_dev, mq_dtype a_dtype, int64_t M, int64_t K, int64_t lda_elems, int group,
                           void* qA_dev, float* sA_dev, void* cuda_stream);
 size_t mq_gemm_group_workspace_bytes(const mq_weights* w, int64_t M);
@@ -280,7 +282,8 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
  *   "max_ctas"  : 0 = all SMs, else cap on the persistent grid
  *   "fused_quant": 0 (default) / 1: see mq_linear
  *   "group_simt": 0 (default) = mq_gemm_group uses its tensor-core (mma.sync) kernel; 1 = its dp4a kernel (ablation)
- *   "group_tc"  : 1 (default) = mq_gemm_group with group = 128 and M >= 64 runs the tcgen05 kernel; 0 = the mma.sync kernel
+ *   "group_tc"  : 1 (default) = mq_gemm_group with group = 128 runs the tcgen05 kernel for M >= 64 and the decode kernel
+ *                 for M <= 32; 0 = the mma.sync kernel for every M
  *   "decode_path": 0 (default) = mq_gemm with M <= 32 runs the lean decode kernel (row slabs: a CTA owns 16..128
  *                 output channels and all of K; TMA ring + mma.sync straight from the packed tiles, no tensor
  *                 memory, no workspace); 1 = the tcgen05 kernel for every M.  Setting "token_tile", "split_k" >= 2,

@@ -28,6 +28,10 @@
 //     the quantized activation tile; separate because s_r != s_w);
 //   * the K groups meet in shared memory (int32, exact), then the epilogue (Eq.2, Eq.4):
 //     y = s_a (s_w acc0 + s_r acc1) in fp32, one rounding to bf16 / fp16, coalesced along the channels.
+// Two more forms of the same kernel: BSC (block-local residual scales, reading A4b: a piece's integer sum is scaled
+// and added in fp32 right after its MMAs) and GRP (per-group activation scales, group = 128 = one K-step, P:441:
+// the K-step's sums are scaled by s_a[t, g] and added in fp32 right after its MMAs, 16 tokens at a time; serves
+// mq_gemm_group for M <= 32).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
@@ -54,7 +58,11 @@ constexpr int DEC_MAX_KS = 512;        // K-steps whose metadata fits the shared
 // BSC: block-local residual scales (reading A4b): every residual piece carries one scale per row; its integer sum is
 // converted and added in fp32 right after its two MMAs (the scale changes along K, so the sums of different blocks
 // cannot share an integer accumulator).
-template <int RT, int MT, bool BIG = false, bool BSC = false>
+// GRP: per-group activation scales, group = 128 = one K-step (reading A5g; mq_gemm_group for M <= 32): the integer
+// sums of a K-step are converted and added to fp32 running sums right after its MMAs,
+//   y += s_a[t, g] * (s_w * acc0_g)  (+ s_a[t, g] * (s_r * acc1_g) for a K-step that owns residual pieces),
+// in mq_group.cu's order; the K groups' fp32 partial sums meet in shared memory in ascending order (tolerance T2).
+template <int RT, int MT, bool BIG = false, bool BSC = false, bool GRP = false>
 struct DCfg {
   static constexpr int R = 16 * RT;                     // output channels per CTA
   static constexpr int KW = DEC_CWARPS / RT;            // K groups (warps that share a row tile)
@@ -82,7 +90,7 @@ struct DCfg {
                                                                  // of the stage's earlier K-steps << 8, first quarter | full mask << 28}
   static constexpr int SMEM_BYTES = OFF_UM + DEC_MAX_KS * 8 + 1024;   // + slack for the 1024-byte alignment
   // the K groups' partial sums [KW][2 accumulators][MT][R] int32 re-use the ring once all stages are consumed
-  static constexpr int RED_BYTES = KW * (BSC ? 3 : 2) * MT * R * 4;
+  static constexpr int RED_BYTES = KW * (BSC ? 3 : (GRP ? 1 : 2)) * MT * R * 4;
   static_assert(KPW >= 1 && KPW * KW == UK, "the K-steps of a stage are dealt evenly to the K groups");
   static_assert(STAGES >= 2, "ring depth");
   static_assert(T_KSTEP % 512 == 0 && W_BYTES % 1024 == 0, "SWIZZLE_64B boxes need 512-byte aligned destinations");
@@ -96,9 +104,9 @@ struct DecParams {
   const int2* unit_meta;   // [NT * KS] {quarter mask, first quarter index}; NULL = dense only
   const float* sw;
   const float* sr;
-  const float* sa;
+  const float* sa;         // [M] token scales; GRP: [M][KS] group scales
   void* Y;
-  int32_t* dbg0;
+  int32_t* dbg0;           // [M][N] sums, or NULL; GRP: [KS][M][N] per-group sums
   int32_t* dbg1;
   int64_t ldy;
   int M, N, KS;
@@ -156,10 +164,11 @@ __device__ __forceinline__ void sts_u64(uint32_t addr, uint32_t a, uint32_t b) {
   asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
 }
 
-template <int RT, int MT, bool BIG, bool BSC>
+template <int RT, int MT, bool BIG, bool BSC, bool GRP = false>
 __global__ void __launch_bounds__(DEC_THREADS, BIG ? 1 : 2)
 mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_a, const DecParams p) {
-  using C = DCfg<RT, MT, BIG, BSC>;
+  using C = DCfg<RT, MT, BIG, BSC, GRP>;
+  static_assert(!(BSC && GRP), "block-local residual scales and per-group activation scales are not combined");
   constexpr int R = C::R, KW = C::KW, UK = C::UK, KPW = C::KPW, NST = C::NST, STAGES = C::STAGES;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -307,7 +316,7 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
 
   // ===================== consumers: warp = (row tile rt, K group kw) =====================
   griddep_wait();   // s_a and Y are ordered after the previous kernel in the stream
-  if (threadIdx.x < 32) sts_u32(sSA + 4u * threadIdx.x, __float_as_uint((int)threadIdx.x < p.M ? __ldg(p.sa + threadIdx.x) : 0.f));
+  if (!GRP && threadIdx.x < 32) sts_u32(sSA + 4u * threadIdx.x, __float_as_uint((int)threadIdx.x < p.M ? __ldg(p.sa + threadIdx.x) : 0.f));
   constexpr uint32_t HI = 0xF0F0F0F0u;
   constexpr float ACC_INV = 0.00390625f;   // the accumulators are 256 x the sums (both operands x16)
   const int rt = warp % RT, kw = warp / RT;
@@ -327,19 +336,29 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
   // base accumulator sets: with few token groups the K-steps alternate between two sets (independent MMA chains;
   // NST >= 4 already gives four independent chains per chunk); one residual set
   constexpr int NACC = NST >= 4 ? 1 : 2;
-  int d0[NACC][NST][4], d1[NST][4];
-  float f1[BSC ? NST : 1][4];   // BSC: sum over the pieces of s_rb * acc1_piece (fp32, K order inside the warp's K-steps)
+  int d0[GRP ? 1 : NACC][GRP ? 1 : NST][4], d1[GRP ? 1 : NST][4];   // (GRP: the sums of a K-step live inside its block below)
+  // BSC: sum over the pieces of s_rb * acc1_piece; GRP: the running sums y (fp32, K order inside the warp's K-steps)
+  float f1[(BSC || GRP) ? NST : 1][4];
 #pragma unroll
-  for (int st = 0; st < (BSC ? NST : 1); ++st)
+  for (int st = 0; st < ((BSC || GRP) ? NST : 1); ++st)
 #pragma unroll
     for (int i = 0; i < 4; ++i) f1[st][i] = 0.f;
+  // GRP: channel scales of this thread's fragment rows (g, g + 8), with the 2^-8 of the x16 operands
+  float g_sw[2] = {0.f, 0.f}, g_sr[2] = {0.f, 0.f};
+  if (GRP) {
 #pragma unroll
-  for (int st = 0; st < NST; ++st)
+    for (int h = 0; h < 2; ++h) {
+      g_sw[h] = __ldg(p.sw + r0 + 16 * rt + g + 8 * h) * ACC_INV;
+      g_sr[h] = __ldg(p.sr + r0 + 16 * rt + g + 8 * h) * ACC_INV;
+    }
+  }
+#pragma unroll
+  for (int st = 0; st < (GRP ? 1 : NST); ++st)
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       d1[st][i] = 0;
 #pragma unroll
-      for (int a = 0; a < NACC; ++a) d0[a][st][i] = 0;
+      for (int a = 0; a < (GRP ? 1 : NACC); ++a) d0[a][st][i] = 0;
     }
 
   for (int s = 0; s < n_stages; ++s) {
@@ -351,6 +370,82 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
 #pragma unroll
     for (int jj = 0; jj < KPW; ++jj) {
       const int j = kw + KW * jj;   // this warp's K-step of the stage
+      if (GRP) {
+        // ---- per-group scales: the K-step's sums are converted and added at once.  Two token column groups (16 tokens) at
+        //      a time, so that the sums, the token fragments and the group scales of a pass fit the registers ----
+        constexpr int SH = NST < 2 ? NST : 2;
+        const int ks = s * UK + j;
+        const int ksg = min(ks, KS - 1);   // (K-steps past K in the last stage hold zeros: sums 0, any valid scale will do)
+        uint32_t wx[8];
+        const uint32_t wj = sW + slot * C::W_BYTES + j * 4 * C::CH_BYTES + w_off;
+        ldmatrix_x4(wx, wj);
+        ldmatrix_x4(wx + 4, wj + 2 * C::CH_BYTES);
+        uint32_t meta = 0;
+        if (smeta & 0xFF) meta = lds_u32(sUM + 8u * (uint32_t)ksg);
+        const uint32_t mask = ks < KS ? (meta & 0xF) : 0;
+        const int slot0 = (int)((smeta >> 8) + ((meta >> 8) & 0xFF));
+#pragma unroll
+        for (int sh = 0; sh < NST; sh += SH) {
+          float sav[SH][2];   // s_a[t, g] of this thread's tokens 8 st + 2 tq, + 1 (tokens past M: zero operands, any valid row)
+#pragma unroll
+          for (int st = 0; st < SH; ++st)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) sav[st][h] = __ldg(p.sa + (size_t)min(8 * (sh + st) + 2 * tq + h, p.M - 1) * (size_t)KS + ksg);
+          uint32_t bw[SH][4];
+#pragma unroll
+          for (int st = 0; st < SH; ++st) ldmatrix_x4(bw[st], sT + slot * C::T_BYTES + j * C::T_KSTEP + (sh + st) * 512 + t_off);
+          int dg[SH][4];
+#pragma unroll
+          for (int st = 0; st < SH; ++st)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) dg[st][e] = 0;
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const uint32_t a0 = (wx[2 * c] << 4) & HI, a1 = (wx[2 * c + 1] << 4) & HI, a2 = wx[2 * c] & HI, a3 = wx[2 * c + 1] & HI;
+#pragma unroll
+            for (int st = 0; st < SH; ++st) mma_s8(dg[st], a0, a1, a2, a3, (bw[st][c] << 4) & HI, bw[st][c] & HI);
+          }
+#pragma unroll
+          for (int st = 0; st < SH; ++st)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {   // y += s_a[t, g] * (s_w * acc0_g)
+              f1[sh + st][e] = fmaf(sav[st][e & 1], g_sw[e >> 1] * (float)dg[st][e], f1[sh + st][e]);
+              const int t = 8 * (sh + st) + 2 * tq + (e & 1);
+              if (p.dbg0 && ks < KS && t < p.M) p.dbg0[((size_t)ks * p.M + t) * p.N + r0 + 16 * rt + g + (e >> 1) * 8] = dg[st][e] >> 8;
+            }
+          if (mask || p.dbg1) {
+#pragma unroll
+            for (int st = 0; st < SH; ++st)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) dg[st][e] = 0;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              const int q = 2 * h + rhalf;
+              if ((mask >> q) & 1) {   // warp-uniform
+                const int ps = (slot0 + __popc(mask & ((1u << q) - 1))) % DEC_QSLOTS;
+                uint32_t rx[4];
+                ldmatrix_x4(rx, sQ + ps * C::PS_BYTES + r_off);
+#pragma unroll
+                for (int c2 = 0; c2 < 2; ++c2) {
+                  const int c = 2 * h + c2;
+                  const uint32_t a0 = (rx[2 * c2] << 4) & HI, a1 = (rx[2 * c2 + 1] << 4) & HI, a2 = rx[2 * c2] & HI, a3 = rx[2 * c2 + 1] & HI;
+#pragma unroll
+                  for (int st = 0; st < SH; ++st) mma_s8(dg[st], a0, a1, a2, a3, (bw[st][c] << 4) & HI, bw[st][c] & HI);
+                }
+              }
+            }
+#pragma unroll
+            for (int st = 0; st < SH; ++st)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {   // y += s_a[t, g] * (s_r * acc1_g)
+                if (mask) f1[sh + st][e] = fmaf(sav[st][e & 1], g_sr[e >> 1] * (float)dg[st][e], f1[sh + st][e]);
+                const int t = 8 * (sh + st) + 2 * tq + (e & 1);
+                if (p.dbg1 && ks < KS && t < p.M) p.dbg1[((size_t)ks * p.M + t) * p.N + r0 + 16 * rt + g + (e >> 1) * 8] = dg[st][e] >> 8;
+              }
+          }
+        }
+        continue;
+      }
       uint32_t bw[NST][4];
 #pragma unroll
       for (int st = 0; st < NST; ++st) ldmatrix_x4(bw[st], sT + slot * C::T_BYTES + j * C::T_KSTEP + st * 512 + t_off);
@@ -413,7 +508,7 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
   for (int st = 0; st < NST; ++st)
 #pragma unroll
     for (int i = 0; i < 4; ++i)
-      if (NACC > 1) d0[0][st][i] += d0[NACC - 1][st][i];
+      if (!GRP && NACC > 1) d0[0][GRP ? 0 : st][i] += d0[GRP ? 0 : NACC - 1][GRP ? 0 : st][i];
 
   // ---------------- the K groups meet in shared memory, then the epilogue ----------------
   // red[kw][acc][t][r]: the ring is free once every warp has passed its last stage
@@ -425,34 +520,43 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
         const int t = 8 * st + 2 * tq + (e & 1), r = 16 * rt + g + (e >> 1) * 8;
-        constexpr int NA = BSC ? 3 : 2;
-        red[((kw * NA + 0) * MT + t) * R + r] = d0[0][st][e];
-        red[((kw * NA + 1) * MT + t) * R + r] = d1[st][e];
-        if (BSC) red[((kw * NA + 2) * MT + t) * R + r] = __float_as_int(f1[st][e]);
+        constexpr int NA = BSC ? 3 : (GRP ? 1 : 2);
+        if (GRP) {
+          red[(kw * MT + t) * R + r] = __float_as_int(f1[st][e]);
+        } else {
+          red[((kw * NA + 0) * MT + t) * R + r] = d0[0][GRP ? 0 : st][e];
+          red[((kw * NA + 1) * MT + t) * R + r] = d1[GRP ? 0 : st][e];
+          if (BSC) red[((kw * NA + 2) * MT + t) * R + r] = __float_as_int(f1[st][e]);
+        }
       }
   }
   named_bar_sync(1, 32 * DEC_CWARPS);
   DEC_STAMP(ctid == 0, 16);
   for (int e = ctid; e < p.M * R; e += 32 * DEC_CWARPS) {
     const int t = e / R, r = e - t * R;
-    constexpr int NA = BSC ? 3 : 2;
+    constexpr int NA = BSC ? 3 : (GRP ? 1 : 2);
     int a0 = 0, a1 = 0;
     float fs = 0.f;
 #pragma unroll
     for (int k = 0; k < KW; ++k) {
-      a0 += red[((k * NA + 0) * MT + t) * R + r];
-      a1 += red[((k * NA + 1) * MT + t) * R + r];
-      if (BSC) fs += __int_as_float(red[((k * NA + 2) * MT + t) * R + r]);   // K groups in ascending order
+      if (GRP) {
+        fs += __int_as_float(red[(k * MT + t) * R + r]);   // K groups in ascending order
+      } else {
+        a0 += red[((k * NA + 0) * MT + t) * R + r];
+        a1 += red[((k * NA + 1) * MT + t) * R + r];
+        if (BSC) fs += __int_as_float(red[((k * NA + 2) * MT + t) * R + r]);   // K groups in ascending order
+      }
     }
     const int n = r0 + r;
-    const float y = __uint_as_float(lds_u32(sSA + 4u * (uint32_t)t)) * (BSC ? (float)a0 * ep_sw + fs : (float)a0 * ep_sw + (float)a1 * ep_sr);
+    const float y = GRP ? fs
+                        : __uint_as_float(lds_u32(sSA + 4u * (uint32_t)t)) * (BSC ? (float)a0 * ep_sw + fs : (float)a0 * ep_sw + (float)a1 * ep_sr);
     const size_t o = (size_t)t * p.ldy + n;
     if (p.y_bf16)
       reinterpret_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
     else
       reinterpret_cast<__half*>(p.Y)[o] = __float2half_rn(y);
-    if (p.dbg0) p.dbg0[(size_t)t * p.N + n] = a0 >> 8;
-    if (p.dbg1) p.dbg1[(size_t)t * p.N + n] = a1 >> 8;
+    if (!GRP && p.dbg0) p.dbg0[(size_t)t * p.N + n] = a0 >> 8;
+    if (!GRP && p.dbg1) p.dbg1[(size_t)t * p.N + n] = a1 >> 8;
   }
   DEC_STAMP(ctid == 0, 6);
 }
@@ -486,15 +590,15 @@ int pick_rows(const mq_weights* w, int64_t M) {
 unsigned long long* g_dec_trace = nullptr;
 #endif
 
-template <int RT, int MT, bool BIG, bool BSC = false>
+template <int RT, int MT, bool BIG, bool BSC = false, bool GRP = false>
 int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
-  using C = DCfg<RT, MT, BIG, BSC>;
+  using C = DCfg<RT, MT, BIG, BSC, GRP>;
   // the attribute belongs to the (device, function) pair: set it whenever the current device changes
   static int attr_dev = -1;
   int dev = -1;
   cudaGetDevice(&dev);
   if (dev != attr_dev) {
-    if (cudaFuncSetAttribute(mq_decode_kernel<RT, MT, BIG, BSC>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    if (cudaFuncSetAttribute(mq_decode_kernel<RT, MT, BIG, BSC, GRP>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
     }
@@ -510,7 +614,7 @@ int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = options().pdl ? 1 : 0;
-  if (cudaLaunchKernelEx(&cfg, mq_decode_kernel<RT, MT, BIG, BSC>, tmw, tma, dp) != cudaSuccess) {
+  if (cudaLaunchKernelEx(&cfg, mq_decode_kernel<RT, MT, BIG, BSC, GRP>, tmw, tma, dp) != cudaSuccess) {
     cudaGetLastError();
     return MQ_ERR_CUDA;
   }
@@ -518,7 +622,14 @@ int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& 
 }
 
 template <int RT>
-int dec_launch_mt(int MT, bool big, bool bsc, const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
+int dec_launch_mt(int MT, bool big, bool bsc, bool grp, const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
+  if (grp) {   // per-group activation scales (small ring only)
+    switch (MT) {
+      case 8: return dec_launch<RT, 8, false, false, true>(tmw, tma, dp, grid, st);
+      case 16: return dec_launch<RT, 16, false, false, true>(tmw, tma, dp, grid, st);
+      default: return dec_launch<RT, 32, false, false, true>(tmw, tma, dp, grid, st);
+    }
+  }
   if (bsc) {   // block-local residual scales (small ring only)
     switch (MT) {
       case 8: return dec_launch<RT, 8, false, true>(tmw, tma, dp, grid, st);
@@ -594,7 +705,22 @@ bool decode_eligible(const mq_weights* w, int64_t M) {
 size_t decode_workspace_bytes(const mq_weights*, int64_t) { return 0; }
 
 static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
-                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res);
+                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool grp = false);
+
+// per-group activation scales (group = 128) at decode sizes: the same kernel, sums converted per K-step
+bool decode_group_eligible(const mq_weights* w, int group, int64_t M) {
+  const Options& o = options();
+  if (!w || !w->tmap_ok || w->blockscale || group != 128 || M <= 0 || M > 32) return false;
+  if (o.group_tc == 0 || o.group_simt != 0 || o.decode_path == 1) return false;
+  return w->K / BK <= DEC_MAX_KS;
+}
+
+int decode_gemm_group(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                      int32_t* dbg0, int32_t* dbg1, void* cuda_stream) {
+  const int rc = decode_gemm_pass(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream, false, true);
+  if (rc == MQ_OK) set_launch_count(1);
+  return rc;
+}
 
 // M <= 32: one launch.  More tokens (block-local scales only): passes of 32 tokens, each streaming the weights again
 // (from L2 when the layer fits) -- a first path for that reading at prefill sizes, not a fast one.
@@ -614,7 +740,7 @@ int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M,
 }
 
 static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
-                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res) {
+                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool grp) {
   const int rows = pick_rows(w, M);
   const int MT = M <= 8 ? 8 : (M <= 16 ? 16 : 32);
   // 3-D tensor map over the canonical packed activations [M rows][K/2 bytes]: {64 B of a K-step, M rows, KS K-steps};
@@ -656,14 +782,14 @@ static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA
   // deep ring (one CTA per SM): the slabs fit one CTA per SM and each has more stages than the small ring holds
   const Options& o = options();
   const int sms = sm_count() > 0 ? sm_count() : 148;
-  const bool big = o.decode_big == 1 || (o.decode_big == 0 && rows <= 64 && grid <= sms && (w->K / BK) / uk_of_rows(rows) > 8);
+  const bool big = !grp && (o.decode_big == 1 || (o.decode_big == 0 && rows <= 64 && grid <= sms && (w->K / BK) / uk_of_rows(rows) > 8));
   const CUtensorMap& tmw = w->tmap_base[rt_index(rows)];
   int rc;
   switch (rows) {
-    case 16: rc = dec_launch_mt<1>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
-    case 32: rc = dec_launch_mt<2>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
-    case 64: rc = dec_launch_mt<4>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
-    default: rc = dec_launch_mt<8>(MT, big, w->blockscale, tmw, tmap, dp, grid, st); break;
+    case 16: rc = dec_launch_mt<1>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
+    case 32: rc = dec_launch_mt<2>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
+    case 64: rc = dec_launch_mt<4>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
+    default: rc = dec_launch_mt<8>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
   }
   return rc;
 }

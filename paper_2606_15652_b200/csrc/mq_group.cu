@@ -498,6 +498,8 @@ extern "C" int mq_gemm_group(const mq_weights* w, const void* qA, const float* s
   const int64_t mtiles = simt ? (M + TOK - 1) / TOK : (M + TOKC - 1) / TOKC;
   const int rc = mq::check_device();
   if (rc != MQ_OK) return rc;
+  // group = 128, decode token counts: the row-slab decode kernel, sums converted per K-step
+  if (mq::decode_group_eligible(w, group, M)) return mq::decode_gemm_group(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream);
   // group = 128 (one group per K-step), prefill token counts: the tcgen05 kernel, accumulator drained per K-step
   if (mq::group_tc_eligible(w, group, M)) {
     if ((uintptr_t)qA & 15) return MQ_ERR_INVALID_ARG;

@@ -108,6 +108,46 @@ def test_group_parity_simt_kernel_every_m(mq, M, K, N, bs, rho, dt):
         mq.mq_set_option("group_simt", 0)
 
 
+@pytest.mark.parametrize("rows", [16, 32, 64, 128])
+@pytest.mark.parametrize("M", [1, 7, 8, 9, 16, 17, 31, 32])
+def test_group128_decode_kernel_variants(mq, rows, M):
+    """Group 128 at M <= 32 runs in the row-slab decode kernel (csrc/mq_decode.cu, GRP form: the sums of a K-step are
+    converted and added right after its MMAs).  Every slab height (option decode_rows) x every token-count class (8 / 16
+    / 32 token columns, ragged), K-step counts that do not fill the last stage (5, 9, 19 K-steps), a cell in most
+    K-steps, hooks on and off, both output types; one launch."""
+    K = {16: 640, 32: 1152, 64: 2432, 128: 640}[rows]
+    case = make_case(1500 + 40 * rows + M, M, K, 256, bs=64, rho=0.35, a_dtype="bf16" if M % 2 else "f16")
+    w = pack_from_oracle(case)
+    want = oracle.forward_group(A_of(case), case.L, 128)
+    assert np.abs(want["acc1_g"]).sum() > 0
+    try:
+        mq.mq_set_option("decode_rows", rows)
+        for dbg in (True, False):
+            out = "bf16" if (M + rows // 16 + dbg) % 2 else "f16"
+            got = run_group(mq, case, 128, w, out_dtype=out, dbg=dbg)
+            assert mq.mq_last_launch_count() == 1
+            check(got, want, 128, K, out, f"group 128 decode kernel rows {rows} M{M} dbg {dbg}")
+    finally:
+        mq.mq_set_option("decode_rows", 0)
+
+
+def test_group128_decode_kernel_and_mma_sync_kernel_agree(mq):
+    """The same launch through both kernels (option group_tc = 0 selects the mma.sync kernel for every M): the same
+    integer sums, both outputs within T2 of the oracle (their fp32 additions are ordered differently), K = 4096."""
+    case = make_case(1590, 32, 4096, 512, bs=64, rho=0.10)
+    w = pack_from_oracle(case)
+    want = oracle.forward_group(A_of(case), case.L, 128)
+    got1 = run_group(mq, case, 128, w, out_dtype="f16")
+    try:
+        mq.mq_set_option("group_tc", 0)
+        got2 = run_group(mq, case, 128, w, out_dtype="f16")
+    finally:
+        mq.mq_set_option("group_tc", 1)
+    assert np.array_equal(got1["acc0_g"], got2["acc0_g"]) and np.array_equal(got1["acc1_g"], got2["acc1_g"])
+    check(got1, want, 128, 4096, "f16", "group 128, M 32, decode kernel")
+    check(got2, want, 128, 4096, "f16", "group 128, M 32, mma.sync kernel")
+
+
 def test_group_budget_zero_and_whole_row_group(mq):
     """Budget 0: acc1_g == 0 and Y is the dense-only product.  Activations constant along K in magnitude per group:
     every group scale equal, so the per-group result must agree with the per-token path (mq_gemm) to rounding."""
