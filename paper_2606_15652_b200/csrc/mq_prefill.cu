@@ -46,6 +46,17 @@ namespace {
 using namespace mq;
 using namespace mq::ptx;
 
+// Waits of the roles that wait most of the time (producer, unpack groups, epilogue): parked by the hardware (try_wait with
+// a suspend-time hint) instead of spinning.  A spinning warp issues a try_wait, a counter update, a compare and a
+// branch every few dozen cycles, on the same schedulers and the same ALU pipe the unpack warps need: with the waits
+// parked the kernel runs 10-15 % faster (M = 8192: o 1779 -> 1959, gate_up 2092 -> 2346, down 2107 -> 2428 TOPS).
+// PF_EXP_SPIN (development) brings the spinning waits back; PF_EXP_PARK_MMA parks the MMA warp's waits as well.
+#ifdef PF_EXP_SPIN
+#define PF_WAIT_SLACK(b, p) mbar_wait((b), (p))
+#else
+#define PF_WAIT_SLACK(b, p) mbar_wait_parked((b), (p))
+#endif
+
 constexpr int PF_BT = 128;                       // tokens per tile (MMA N)
 constexpr int PF_UST = 4;                        // operand (U) stages = unpack groups
 constexpr int PF_WARPS = 6 + 4 * PF_UST;
@@ -322,7 +333,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
         const uint8_t* wsrc = p.base + (size_t)nt * KS * TILE_BYTES;
         for (int ks = 0; ks < KS; ++ks, ++q) {
           const uint32_t ps = q % PF_PST;
-          mbar_wait(bar(PF_B_EMPTY_P + ps), ((q / PF_PST) & 1) ^ 1);
+          PF_WAIT_SLACK(bar(PF_B_EMPTY_P + ps), ((q / PF_PST) & 1) ^ 1);
           const uint32_t fb = bar(PF_B_FULL_P + ps), dst = sP + ps * PF_P_STAGE;
           if (PF_EXP_NOTMA) {
             mbar_arrive(fb);
@@ -370,7 +381,11 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
 #endif
     auto wait_b = [&](uint32_t b, uint32_t par) {
       if (PAIR && PF_CL_WAIT) mbar_wait_cl(b, par);
+#ifdef PF_EXP_PARK_MMA
+      else mbar_wait_parked(b, par);
+#else
       else mbar_wait(b, par);
+#endif
     };
     auto acquire = [&]() {
 #ifdef PF_TRACE
@@ -535,7 +550,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
             // ---- base item ----
             const uint32_t ps = (q + (uint32_t)j) % PF_PST;
             PF_FINE(0);
-            mbar_wait(bar(PF_B_FULL_P + ps), ((q + (uint32_t)j) / PF_PST) & 1);
+            PF_WAIT_SLACK(bar(PF_B_FULL_P + ps), ((q + (uint32_t)j) / PF_PST) & 1);
             PF_FINE(1);
             constexpr int TL = PAIR ? 2 : 4;   // 16-byte token chunks per thread
             uint4 v4[4], t4[TL];
@@ -546,7 +561,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
             for (int i = 0; i < TL; ++i)
               t4[i] = (A8 || PF_EXP_NOT) ? make_uint4(row, i, ps, g) : pf_lds128(pt + (gtid + 128u * i) * 16);
             PF_FINE(2);
-            mbar_wait(bar(PF_B_EMPTY_U + g), (n_mine & 1) ^ 1);   // the poll runs under the loads' latency
+            PF_WAIT_SLACK(bar(PF_B_EMPTY_U + g), (n_mine & 1) ^ 1);   // the poll runs under the loads' latency
             tc_fence_after();
             PF_FINE(3);
             if (A8 && gtid == 0) {   // the stage is free: request the K-step's int8 token tile straight into it
@@ -596,7 +611,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
                 r4[h][1] = __ldg(reinterpret_cast<const uint4*>(src + 1024));
               }
             }
-            mbar_wait(bar(PF_B_EMPTY_U + g), (n_mine & 1) ^ 1);
+            PF_WAIT_SLACK(bar(PF_B_EMPTY_U + g), (n_mine & 1) ^ 1);
             tc_fence_after();
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -637,7 +652,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) mq_prefill_kernel(const __grid_
       float* sat = sa_tile + buf * PF_BT;
       sat[et] = et < t_cnt ? __ldg(p.sa + t_base + et) : 0.f;
       named_bar_sync(1, 128);   // also orders this buffer's readers (two tiles ago) before its writers
-      mbar_wait(bar(PF_B_TFULL + buf), ((uint32_t)it >> 1) & 1);
+      PF_WAIT_SLACK(bar(PF_B_TFULL + buf), ((uint32_t)it >> 1) & 1);
       tc_fence_after();
       const bool has_res = misc[1 + buf] != 0;   // acc1 is undefined when no residual MMA was issued
       const uint32_t t0addr = tmem_base + lane_off + (uint32_t)(buf * PF_BT), t1addr = tmem_base + lane_off + (uint32_t)PF_ACC1_COL;
