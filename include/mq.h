@@ -287,14 +287,17 @@ int mq_linear_host(const mq_weights* w, const void* A_host, mq_dtype a_dtype, in
  *   "decode_path": 0 (default) = mq_gemm with M <= 32 runs the lean decode kernel (row slabs: a CTA owns 16..128
  *                 output channels and all of K; TMA ring + mma.sync straight from the packed tiles, no tensor
  *                 memory, no workspace); 1 = the tcgen05 kernel for every M.  Setting "token_tile", "split_k" >= 2,
- *                 "max_ctas" or "fused_quant" also selects the tcgen05 kernel.
+ *                 "max_ctas" or "fused_quant" also selects the tcgen05 kernel.  mq_gemm_a8 with M <= 16 (M <= 32 on
+ *                 layers whose slabs are 64 channels or taller) and mq_gemm_group with group = 128 and M <= 32 run
+ *                 forms of the same kernel.
  *   "decode_rows": 0 = automatic, else 16 / 32 / 64 / 128 output channels per CTA of the decode kernel
  *   "decode_big": 0 = automatic, 1 = deep shared-memory ring (one CTA per SM; rows <= 64), 2 = small ring (two per SM)
  *   "prefill_path": 0 (default) = mq_gemm with M >= 64 runs the whole-tile tcgen05 kernel (128 x 128 output tiles dealt
  *                 round-robin to persistent CTAs, no workspace; CTA pairs with tcgen05.mma.cta_group::2 when the layer
  *                 has an even number of 128-channel tiles) when the last round of tiles is at least half full, else
  *                 the stream-K tcgen05 kernel; mq_gemm_a8 runs the whole-tile kernel's W4A8 form (single CTAs, int8
- *                 token tiles by TMA straight into the MMA operand stage) from three rounds of tiles per CTA upwards;
+ *                 token tiles by TMA straight into the MMA operand stage) from three rounds of tiles per CTA upwards
+ *                 (and, for M <= 32, the decode kernel's W4A8 form: see "decode_path");
  *                 1 = never; 2 = for every M >= 64, one CTA per tile; 3 = for every M >= 64, CTA pairs where possible.
  *                 The stream-K knobs above ("token_tile", "split_k" >= 2, "max_ctas") also select the stream-K kernel.
  *   "pdl"       : 1 (default) = kernels are launched as programmatic dependents of their predecessor

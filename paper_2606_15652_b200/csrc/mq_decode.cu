@@ -31,7 +31,8 @@
 // Two more forms of the same kernel: BSC (block-local residual scales, reading A4b: a piece's integer sum is scaled
 // and added in fp32 right after its MMAs) and GRP (per-group activation scales, group = 128 = one K-step, P:441:
 // the K-step's sums are scaled by s_a[t, g] and added in fp32 right after its MMAs, 16 tokens at a time; serves
-// mq_gemm_group for M <= 32).
+// mq_gemm_group for M <= 32), and A8 (W4A8: int8 tokens go into the MMA as they are, the weight nibbles are
+// expanded in canonical order; serves mq_gemm_a8 at decode sizes).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
@@ -62,7 +63,10 @@ constexpr int DEC_MAX_KS = 512;        // K-steps whose metadata fits the shared
 // sums of a K-step are converted and added to fp32 running sums right after its MMAs,
 //   y += s_a[t, g] * (s_w * acc0_g)  (+ s_a[t, g] * (s_r * acc1_g) for a K-step that owns residual pieces),
 // in mq_group.cu's order; the K groups' fp32 partial sums meet in shared memory in ascending order (tolerance T2).
-template <int RT, int MT, bool BIG = false, bool BSC = false, bool GRP = false>
+// A8 (W4A8): the tokens are int8 [M][K] in canonical order and go into the MMA as they are (128 bytes per token
+// and K-step, SWIZZLE_128B); the weight nibbles are expanded into canonical order too (two byte permutes more per word);
+// the accumulators are 16 x the sums.
+template <int RT, int MT, bool BIG = false, bool BSC = false, bool GRP = false, bool A8 = false>
 struct DCfg {
   static constexpr int R = 16 * RT;                     // output channels per CTA
   static constexpr int KW = DEC_CWARPS / RT;            // K groups (warps that share a row tile)
@@ -71,7 +75,7 @@ struct DCfg {
   static constexpr int NST = MT / 8;                    // 8-token MMA column groups
   static constexpr int CH_BYTES = R * 16;               // one 32-channel chunk of the slab
   static constexpr int W_BYTES = 4 * UK * CH_BYTES;     // packed weights of a stage (8 or 16 KB)
-  static constexpr int T_KSTEP = MT * (BK / 2);         // packed tokens of one K-step
+  static constexpr int T_KSTEP = MT * (A8 ? BK : BK / 2);   // tokens of one K-step (packed int4, A8: int8)
   static constexpr int T_BYTES = UK * T_KSTEP;
   static constexpr int P_ROWS = R < 64 ? R : 64;        // rows of a residual piece (one k-half of a quarter)
   static constexpr int P_BYTES = P_ROWS * 32;
@@ -93,7 +97,8 @@ struct DCfg {
   static constexpr int RED_BYTES = KW * (BSC ? 3 : (GRP ? 1 : 2)) * MT * R * 4;
   static_assert(KPW >= 1 && KPW * KW == UK, "the K-steps of a stage are dealt evenly to the K groups");
   static_assert(STAGES >= 2, "ring depth");
-  static_assert(T_KSTEP % 512 == 0 && W_BYTES % 1024 == 0, "SWIZZLE_64B boxes need 512-byte aligned destinations");
+  static_assert(T_KSTEP % 1024 == 0 || (!A8 && T_KSTEP % 512 == 0), "SWIZZLE_64B / _128B boxes need 512- / 1024-byte aligned destinations");
+  static_assert(W_BYTES % 1024 == 0 && (STAGES * W_BYTES) % 1024 == 0, "token stages start 1024-byte aligned");
   static_assert(RED_BYTES <= OFF_Q, "the reduction buffer fits the ring");
   static_assert((BIG ? 1 : 2) * (SMEM_BYTES + 1024) <= 232448, "two CTAs per SM (one: BIG)");
 };
@@ -164,11 +169,11 @@ __device__ __forceinline__ void sts_u64(uint32_t addr, uint32_t a, uint32_t b) {
   asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(addr), "r"(a), "r"(b) : "memory");
 }
 
-template <int RT, int MT, bool BIG, bool BSC, bool GRP = false>
+template <int RT, int MT, bool BIG, bool BSC, bool GRP = false, bool A8 = false>
 __global__ void __launch_bounds__(DEC_THREADS, BIG ? 1 : 2)
 mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_constant__ CUtensorMap tmap_a, const DecParams p) {
-  using C = DCfg<RT, MT, BIG, BSC, GRP>;
-  static_assert(!(BSC && GRP), "block-local residual scales and per-group activation scales are not combined");
+  using C = DCfg<RT, MT, BIG, BSC, GRP, A8>;
+  static_assert(!(BSC && GRP) && !(A8 && (BSC || GRP)), "the variants are not combined");
   constexpr int R = C::R, KW = C::KW, UK = C::UK, KPW = C::KPW, NST = C::NST, STAGES = C::STAGES;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sb = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -318,7 +323,8 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
   griddep_wait();   // s_a and Y are ordered after the previous kernel in the stream
   if (!GRP && threadIdx.x < 32) sts_u32(sSA + 4u * threadIdx.x, __float_as_uint((int)threadIdx.x < p.M ? __ldg(p.sa + threadIdx.x) : 0.f));
   constexpr uint32_t HI = 0xF0F0F0F0u;
-  constexpr float ACC_INV = 0.00390625f;   // the accumulators are 256 x the sums (both operands x16)
+  constexpr float ACC_INV = A8 ? 0.0625f : 0.00390625f;   // the accumulators are 256 x the sums (both operands x16); A8: 16 x
+  constexpr int ACC_SHIFT = A8 ? 4 : 8;
   const int rt = warp % RT, kw = warp / RT;
   const int g = lane >> 2, tq = lane & 3;
   const int lrow = lane & 7, lmat = lane >> 3;   // ldmatrix: this lane supplies row lrow of matrix lmat
@@ -446,6 +452,62 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
         }
         continue;
       }
+      if (A8) {
+        // ---- W4A8: int8 tokens as they are.  MMA k-slots 4 tq .. 4 tq + 3 carry the chunk's elements 8 tq .. 8 tq + 3, slots
+        //      16 + 4 tq .. carry 8 tq + 4 .. 8 tq + 7: the thread's packed weight word (8 nibbles) in canonical order is its
+        //      A fragment pair, 8 consecutive token bytes are its B fragment pair (one 8-byte load) ----
+        auto canon = [&](uint32_t w, uint32_t& lo, uint32_t& hi) {
+          const uint32_t ev = (w << 4) & HI, od = w & HI;   // elements 0,2,4,6 | 1,3,5,7 of the word, x16
+          lo = __byte_perm(ev, od, 0x5140);
+          hi = __byte_perm(ev, od, 0x7362);
+        };
+        // token row 8 st + g of the K-step [MT rows][128 B], 16-byte chunks XOR-swizzled with row & 7 (SWIZZLE_128B)
+        const uint32_t tk = sT + slot * C::T_BYTES + j * C::T_KSTEP + (uint32_t)(g * 128 + (tq & 1) * 8);
+        auto tok8 = [&](int st, int c) { return lds_u64(tk + (uint32_t)(st * 1024) + ((uint32_t)((2 * c + (tq >> 1)) ^ g) << 4)); };
+        uint32_t wx[8];
+        const uint32_t wj = sW + slot * C::W_BYTES + j * 4 * C::CH_BYTES + w_off;
+        ldmatrix_x4(wx, wj);
+        ldmatrix_x4(wx + 4, wj + 2 * C::CH_BYTES);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t a0, a1, a2, a3;
+          canon(wx[2 * c], a0, a2);
+          canon(wx[2 * c + 1], a1, a3);
+#pragma unroll
+          for (int st = 0; st < NST; ++st) {
+            const uint2 tb = tok8(st, c);
+            mma_s8(d0[jj % NACC][st], a0, a1, a2, a3, tb.x, tb.y);
+          }
+        }
+        uint32_t meta = 0;
+        if (smeta & 0xFF) meta = lds_u32(sUM + 8u * (uint32_t)min(s * UK + j, KS - 1));
+        const uint32_t mask = s * UK + j < KS ? (meta & 0xF) : 0;
+        if (mask) {
+          const int slot0 = (int)((smeta >> 8) + ((meta >> 8) & 0xFF));
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const int q = 2 * h + rhalf;
+            if ((mask >> q) & 1) {   // warp-uniform
+              const int ps = (slot0 + __popc(mask & ((1u << q) - 1))) % DEC_QSLOTS;
+              uint32_t rx[4];
+              ldmatrix_x4(rx, sQ + ps * C::PS_BYTES + r_off);
+#pragma unroll
+              for (int c2 = 0; c2 < 2; ++c2) {
+                const int c = 2 * h + c2;
+                uint32_t a0, a1, a2, a3;
+                canon(rx[2 * c2], a0, a2);
+                canon(rx[2 * c2 + 1], a1, a3);
+#pragma unroll
+                for (int st = 0; st < NST; ++st) {
+                  const uint2 tb = tok8(st, c);
+                  mma_s8(d1[st], a0, a1, a2, a3, tb.x, tb.y);
+                }
+              }
+            }
+          }
+        }
+        continue;
+      }
       uint32_t bw[NST][4];
 #pragma unroll
       for (int st = 0; st < NST; ++st) ldmatrix_x4(bw[st], sT + slot * C::T_BYTES + j * C::T_KSTEP + st * 512 + t_off);
@@ -555,8 +617,8 @@ mq_decode_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
       reinterpret_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
     else
       reinterpret_cast<__half*>(p.Y)[o] = __float2half_rn(y);
-    if (!GRP && p.dbg0) p.dbg0[(size_t)t * p.N + n] = a0 >> 8;
-    if (!GRP && p.dbg1) p.dbg1[(size_t)t * p.N + n] = a1 >> 8;
+    if (!GRP && p.dbg0) p.dbg0[(size_t)t * p.N + n] = a0 >> ACC_SHIFT;
+    if (!GRP && p.dbg1) p.dbg1[(size_t)t * p.N + n] = a1 >> ACC_SHIFT;
   }
   DEC_STAMP(ctid == 0, 6);
 }
@@ -590,15 +652,15 @@ int pick_rows(const mq_weights* w, int64_t M) {
 unsigned long long* g_dec_trace = nullptr;
 #endif
 
-template <int RT, int MT, bool BIG, bool BSC = false, bool GRP = false>
+template <int RT, int MT, bool BIG, bool BSC = false, bool GRP = false, bool A8 = false>
 int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
-  using C = DCfg<RT, MT, BIG, BSC, GRP>;
+  using C = DCfg<RT, MT, BIG, BSC, GRP, A8>;
   // the attribute belongs to the (device, function) pair: set it whenever the current device changes
   static int attr_dev = -1;
   int dev = -1;
   cudaGetDevice(&dev);
   if (dev != attr_dev) {
-    if (cudaFuncSetAttribute(mq_decode_kernel<RT, MT, BIG, BSC, GRP>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    if (cudaFuncSetAttribute(mq_decode_kernel<RT, MT, BIG, BSC, GRP, A8>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
       cudaGetLastError();
       return MQ_ERR_CUDA;
     }
@@ -614,7 +676,7 @@ int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = options().pdl ? 1 : 0;
-  if (cudaLaunchKernelEx(&cfg, mq_decode_kernel<RT, MT, BIG, BSC, GRP>, tmw, tma, dp) != cudaSuccess) {
+  if (cudaLaunchKernelEx(&cfg, mq_decode_kernel<RT, MT, BIG, BSC, GRP, A8>, tmw, tma, dp) != cudaSuccess) {
     cudaGetLastError();
     return MQ_ERR_CUDA;
   }
@@ -622,7 +684,17 @@ int dec_launch(const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& 
 }
 
 template <int RT>
-int dec_launch_mt(int MT, bool big, bool bsc, bool grp, const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
+int dec_launch_mt(int MT, bool big, bool bsc, bool grp, bool a8, const CUtensorMap& tmw, const CUtensorMap& tma, const DecParams& dp, int grid, cudaStream_t st) {
+  if (a8) {    // W4A8 (small ring only; 32 token columns of int8 fit the ring for slabs of 64 channels and more, see
+               // decode_a8_eligible)
+    switch (MT) {
+      case 8: return dec_launch<RT, 8, false, false, false, true>(tmw, tma, dp, grid, st);
+      case 16: return dec_launch<RT, 16, false, false, false, true>(tmw, tma, dp, grid, st);
+      default:
+        if constexpr (RT >= 4) return dec_launch<RT, 32, false, false, false, true>(tmw, tma, dp, grid, st);
+        else return MQ_ERR_UNSUPPORTED_SHAPE;
+    }
+  }
   if (grp) {   // per-group activation scales (small ring only)
     switch (MT) {
       case 8: return dec_launch<RT, 8, false, false, true>(tmw, tma, dp, grid, st);
@@ -705,7 +777,26 @@ bool decode_eligible(const mq_weights* w, int64_t M) {
 size_t decode_workspace_bytes(const mq_weights*, int64_t) { return 0; }
 
 static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
-                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool grp = false);
+                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool grp = false, bool a8 = false);
+
+// W4A8 at decode sizes: the same kernel with int8 tokens (A8 form)
+bool decode_a8_eligible(const mq_weights* w, int64_t M) {
+  const Options& o = options();
+  if (!w || !w->tmap_ok || w->blockscale || M <= 0 || M > 32) return false;
+  if (o.decode_path == 1 || o.token_tile != 0 || o.split_k >= 2 || o.max_ctas != 0) return false;
+  // 32 token columns: a stage of 8 K-steps x 32 tokens x 128 B leaves no ring depth; slabs of 64 channels and more have
+  // stages of 2-4 K-steps.  (Forcing 64-channel slabs on the layers that get shorter ones leaves too few CTAs: measured
+  // slower than the stream-K kernel.)
+  if (M > 16 && pick_rows(w, M) < 64) return false;
+  return w->K / BK <= DEC_MAX_KS;
+}
+
+int decode_gemm_a8(const mq_weights* w, const void* qA8, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                   int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res) {
+  const int rc = decode_gemm_pass(w, qA8, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream, ignore_res, false, true);
+  if (rc == MQ_OK) set_launch_count(1);
+  return rc;
+}
 
 // per-group activation scales (group = 128) at decode sizes: the same kernel, sums converted per K-step
 bool decode_group_eligible(const mq_weights* w, int group, int64_t M) {
@@ -740,7 +831,7 @@ int decode_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M,
 }
 
 static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
-                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool grp) {
+                            int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool grp, bool a8) {
   const int rows = pick_rows(w, M);
   const int MT = M <= 8 ? 8 : (M <= 16 ? 16 : 32);
   // 3-D tensor map over the canonical packed activations [M rows][K/2 bytes]: {64 B of a K-step, M rows, KS K-steps};
@@ -750,12 +841,14 @@ static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA
   if (!enc) return MQ_ERR_CUDA;
   CUtensorMap tmap;
   memset(&tmap, 0, sizeof(tmap));
-  const cuuint64_t gdim[3] = {(cuuint64_t)(BK / 2), (cuuint64_t)M, (cuuint64_t)(w->K / BK)};
-  const cuuint64_t gstride[2] = {(cuuint64_t)(w->K / 2), (cuuint64_t)(BK / 2)};
-  const cuuint32_t box[3] = {(cuuint32_t)(BK / 2), (cuuint32_t)MT, (cuuint32_t)uk_of_rows(rows)};
+  // (A8: int8 tokens [M rows][K bytes], 128 B per K-step, SWIZZLE_128B)
+  const cuuint64_t kb = a8 ? (cuuint64_t)BK : (cuuint64_t)(BK / 2);   // token bytes per K-step
+  const cuuint64_t gdim[3] = {kb, (cuuint64_t)M, (cuuint64_t)(w->K / BK)};
+  const cuuint64_t gstride[2] = {(cuuint64_t)(w->K / BK) * kb, kb};
+  const cuuint32_t box[3] = {(cuuint32_t)kb, (cuuint32_t)MT, (cuuint32_t)uk_of_rows(rows)};
   const cuuint32_t estr[3] = {1, 1, 1};
   if (enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(qA), gdim, gstride, box, estr,
-          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+          CU_TENSOR_MAP_INTERLEAVE_NONE, a8 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
     return MQ_ERR_CUDA;
 
@@ -782,14 +875,14 @@ static int decode_gemm_pass(const mq_weights* w, const void* qA, const float* sA
   // deep ring (one CTA per SM): the slabs fit one CTA per SM and each has more stages than the small ring holds
   const Options& o = options();
   const int sms = sm_count() > 0 ? sm_count() : 148;
-  const bool big = !grp && (o.decode_big == 1 || (o.decode_big == 0 && rows <= 64 && grid <= sms && (w->K / BK) / uk_of_rows(rows) > 8));
+  const bool big = !grp && !a8 && (o.decode_big == 1 || (o.decode_big == 0 && rows <= 64 && grid <= sms && (w->K / BK) / uk_of_rows(rows) > 8));
   const CUtensorMap& tmw = w->tmap_base[rt_index(rows)];
   int rc;
   switch (rows) {
-    case 16: rc = dec_launch_mt<1>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
-    case 32: rc = dec_launch_mt<2>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
-    case 64: rc = dec_launch_mt<4>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
-    default: rc = dec_launch_mt<8>(MT, big, w->blockscale, grp, tmw, tmap, dp, grid, st); break;
+    case 16: rc = dec_launch_mt<1>(MT, big, w->blockscale, grp, a8, tmw, tmap, dp, grid, st); break;
+    case 32: rc = dec_launch_mt<2>(MT, big, w->blockscale, grp, a8, tmw, tmap, dp, grid, st); break;
+    case 64: rc = dec_launch_mt<4>(MT, big, w->blockscale, grp, a8, tmw, tmap, dp, grid, st); break;
+    default: rc = dec_launch_mt<8>(MT, big, w->blockscale, grp, a8, tmw, tmap, dp, grid, st); break;
   }
   return rc;
 }

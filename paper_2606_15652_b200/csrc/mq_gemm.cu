@@ -1598,6 +1598,8 @@ int gemm_impl(const mq_weights* w, const void* qA, const float* sA, int64_t M, v
   if (!fused && !a8 && mq::decode_eligible(w, M))
     return mq::decode_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, workspace, workspace_bytes, cuda_stream, ignore_res);
   // prefill shapes whose whole tiles fill the machine: the whole-tile kernel (mq_prefill.cu)
+  if (!fused && a8 && mq::decode_a8_eligible(w, M))
+    return mq::decode_gemm_a8(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream, ignore_res);
   if (!fused && mq::prefill_eligible(w, M, a8))
     return mq::prefill_gemm(w, qA, sA, M, Y, y_dtype, ldy, dbg0, dbg1, cuda_stream, ignore_res, a8);
 

@@ -120,6 +120,10 @@ bool prefill_eligible(const mq_weights* w, int64_t M, bool a8 = false);
 int prefill_gemm(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype,
                  int64_t ldy, int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res, bool a8 = false);
 // per-group activation scales, group = 128, on the tcgen05 path (mq_group_tc.cu): M >= 64, no workspace
+// W4A8 at decode sizes (M <= 32): the decode kernel's A8 form (mq_decode.cu)
+bool decode_a8_eligible(const mq_weights* w, int64_t M);
+int decode_gemm_a8(const mq_weights* w, const void* qA8, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,
+                   int32_t* dbg0, int32_t* dbg1, void* cuda_stream, bool ignore_res);
 // per-group activation scales at decode sizes (group = 128, M <= 32): the decode kernel's GRP form (mq_decode.cu)
 bool decode_group_eligible(const mq_weights* w, int group, int64_t M);
 int decode_gemm_group(const mq_weights* w, const void* qA, const float* sA, int64_t M, void* Y, mq_dtype y_dtype, int64_t ldy,

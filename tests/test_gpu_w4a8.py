@@ -41,6 +41,30 @@ def test_w4a8_parity_small(mq, M, K, N, bs, rho, dt, out_dtype):
     assert_parity(got, want, what=f"W4A8 M{M} K{K} N{N} bs{bs} {out_dtype}")
 
 
+@pytest.mark.parametrize("rows", [16, 32, 64, 128])
+@pytest.mark.parametrize("M", [1, 7, 8, 9, 16, 17, 32])
+def test_w4a8_decode_kernel_variants(mq, rows, M):
+    """W4A8 at M <= 32 runs in the row-slab decode kernel's A8 form (csrc/mq_decode.cu: int8 tokens as they are, weight
+    nibbles expanded in canonical order): every slab height (option decode_rows) x every token-count class, K-step counts
+    that do not fill the last stage, a residual piece in most K-steps; one launch where the form is eligible (32 token
+    columns need slabs of 64 channels or more; the stream-K kernel takes the rest), two calls on one handle."""
+    K = {16: 640, 32: 1152, 64: 2432, 128: 640}[rows]
+    case = make_case(1700 + 40 * rows + M, M, K, 256, bs=64, rho=0.35, a_dtype="bf16" if M % 2 else "f16")
+    want = oracle_forward(case, bits=8)
+    assert np.abs(want["acc1"]).sum() > 0
+    w = pack_from_oracle(case)
+    ws = mq.new_workspace(mq.mq_gemm_workspace_bytes(w, M))
+    try:
+        mq.mq_set_option("decode_rows", rows)
+        for rep in range(2):
+            got = run_cuda(case, w=w, workspace=ws, out_dtype="bf16" if rep else "f16", bits=8)
+            if M <= 16 or rows >= 64:
+                assert mq.mq_last_launch_count() == 1
+            assert_parity(got, want, what=f"W4A8 decode kernel rows {rows} M{M} rep {rep}")
+    finally:
+        mq.mq_set_option("decode_rows", 0)
+
+
 @pytest.mark.parametrize("mode,ctas,bt", [(2, 0, 0), (2, 7, 0), (2, 33, 32), (1, 0, 64), (2, 5, 128), (1, 0, 16)])
 def test_w4a8_stream_k_and_token_tiles(mq, mode, ctas, bt):
     M = 40 if bt in (0, 64) else (12 if bt == 16 else (30 if bt == 32 else 150))
