@@ -244,17 +244,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       gt_sts128(su + r * 128 + (((2 * c) ^ (r & 7)) << 4), tw);
       gt_sts128(su + r * 128 + (((2 * c + 1) ^ (r & 7)) << 4), tw + 4);
     };
-    // An item is published (wait for the tensor-memory stores, fences, arrival) one step LATE: after the packed operands
-    // of the next item have been requested from shared memory, so that the stores' and the fence's latency runs under
-    // those loads instead of sitting in every item's chain (all six unpack warps work on every item: their chain per item
-    // is the pipeline's period).  If the next packed stage has not landed yet the pending item is published at once.
-    uint32_t pend = 0xFFFFFFFFu;
-    auto flush = [&]() {
-      if (pend != 0xFFFFFFFFu) {
-        publish(pend);
-        pend = 0xFFFFFFFFu;
-      }
-    };
     int pT = tile0, pc0 = 0;
     int2 um_next = load_chunk(pT, pc0);
     for (int T = tile0; T < p.tiles; T += tstride) {
@@ -270,11 +259,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           const uint32_t ps = (q + (uint32_t)j) % GT_PST;
           {
             GT_T0();
-            const uint32_t fpb = bar(GT_B_FULL_P + ps), fpp = ((q + (uint32_t)j) / GT_PST) & 1;
-            if (!mbar_test_wait(fpb, fpp)) {
-              flush();
-              mbar_wait_parked(fpb, fpp);
-            }
+            mbar_wait_parked(bar(GT_B_FULL_P + ps), ((q + (uint32_t)j) / GT_PST) & 1);
             GT_ACC(6);
           }
           const uint32_t pw = sP + ps * GT_P_STAGE, pt = pw + TILE_BYTES;
@@ -290,7 +275,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             const uint32_t landed = zero_after(fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]) ^ fold4(w2[0]) ^ fold4(w2[1]));
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps) + landed);
-            flush();
             wait_stage(idx);
             uint32_t o[32];
 #pragma unroll
@@ -298,7 +282,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             tmem_st32(lane_base + (uint32_t)((idx & 3) * GT_A_COLS), o);
 #pragma unroll
             for (int c = 0; c < 2; ++c) expand_to_smem(su, wrow, wc0 + (uint32_t)c, w2[c]);
-            pend = idx;
+            publish(idx);
             if (has) {
               // ---- residual item: the cell's packed rows straight from global memory -> the next stage's B buffer; this
               //      thread = channel `row`; a k-half that holds a block is written for all 128 channels (zeros where the
@@ -317,7 +301,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
                   r4[h][1] = __ldg(reinterpret_cast<const uint4*>(src + 1024));
                 }
               }
-              flush();
               wait_stage(idx + 1);
               const uint32_t su2 = sU + ((idx + 1) & 3) * GT_U_STAGE;
 #pragma unroll
@@ -326,7 +309,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
                 expand_to_smem(su2, row, (uint32_t)(2 * h), r4[h][0]);
                 expand_to_smem(su2, row, (uint32_t)(2 * h + 1), r4[h][1]);
               }
-              pend = idx + 1;
+              publish(idx + 1);
             }
           } else {
             // ---- base item: one weight row (0..63), four chunks -> shared memory ----
@@ -336,15 +319,13 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             const uint32_t landed = zero_after(fold4(v4[0]) ^ fold4(v4[1]) ^ fold4(v4[2]) ^ fold4(v4[3]));
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(GT_B_EMPTY_P + ps) + landed);
-            flush();
             wait_stage(idx);
 #pragma unroll
             for (int c = 0; c < 4; ++c) expand_to_smem(su, wrow, (uint32_t)c, v4[c]);
-            pend = idx;
+            publish(idx);
             if (has) {   // nothing to expand for a residual item: keep the stage's arrival count in step
-              flush();
               wait_stage(idx + 1);
-              pend = idx + 1;
+              publish(idx + 1);
             }
           }
         }
@@ -352,7 +333,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         q += (uint32_t)nk;
       }
     }
-    flush();
   };
 
   if (warp < GT_WARP_E0) {
