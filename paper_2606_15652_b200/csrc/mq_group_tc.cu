@@ -446,7 +446,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     // ===================== epilogue warps (4..11): drain every K-step's sums into fp32 running sums =====================
     // A thread owns ONE token (its TMEM lane) and 64 channels (columns): the group scale s_a[t, g] is a register, the
     // channel scales are applied once per tile.  Register budget (160 per thread after the split): 64 running sums + two
-    // batches of 32 + two dozen scalars; whether a K-step owns a cell is fetched from global memory one K-step ahead.
+    // batches of 32 + two dozen scalars; which K-steps own a cell comes from the metadata words kept in the lanes.
     GT_REGS_INC();
     griddep_wait();   // the group scales and Y are ordered after the previous kernel in the stream
     const int half = (warp - GT_WARP_E0) >> 2;        // which 64 channels of the tile; TMEM lane quadrant = warp % 4
