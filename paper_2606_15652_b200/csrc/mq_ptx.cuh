@@ -69,7 +69,7 @@ __device__ __forceinline__ bool mbar_try_wait_parked(uint32_t bar, uint32_t pari
 __device__ __forceinline__ void mbar_wait_parked(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait_parked(bar, parity)) {
-    if (++spins > (1u << 20)) __trap();
+    if (++spins > (1u << 25)) __trap();   // (a parked round lasts 0.1-20 us: seconds at least)
   }
 }
 
