@@ -541,6 +541,9 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       const bool slow = flag == tile_no + 1u;
       const uint32_t tc_half = tc + (uint32_t)(half * 64 * 4);
       request_base(kq);   // (no load is left in flight across the tile's output stage)
+      // (the K-step loops once per kind of tile, regular / irregular channel scales: no test per K-step)
+      auto k_loops = [&](auto slow_c) {
+      constexpr bool SLOW = decltype(slow_c)::value;
       for (int c0 = 0; c0 < KS; c0 += 32) {
         const int2 um = um_next;
         next_chunk(pT, pc0);
@@ -565,7 +568,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           for (int i4 = 0; i4 < 8; ++i4) {
             float cs[4] = {0.f, 0.f, 0.f, 0.f};
             if (MODE != 0) {
-              const uint4 c4 = gt_lds128(tc_half + (uint32_t)(((MODE == 1 ? 2 : (slow ? 3 : 1)) * BN) * 4) + (uint32_t)((b * 32 + i4 * 4) * 4));
+              const uint4 c4 = gt_lds128(tc_half + (uint32_t)(((MODE == 1 ? 2 : (SLOW ? 3 : 1)) * BN) * 4) + (uint32_t)((b * 32 + i4 * 4) * 4));
               cs[0] = __uint_as_float(c4.x);
               cs[1] = __uint_as_float(c4.y);
               cs[2] = __uint_as_float(c4.z);
@@ -600,7 +603,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
         landed(a[0]);
         issue((uint32_t)(buf * BN) + 32u, a[1]);
         tie(a[0]);
-        if (!slow) add32(a[0], 0, std::integral_constant<int, 0>{}, p.dbg0); else add32(a[0], 0, std::integral_constant<int, 1>{}, p.dbg0);
+        add32(a[0], 0, std::integral_constant<int, SLOW ? 1 : 0>{}, p.dbg0);
         landed(a[1]);
         if (!has) {
           hand_back();
@@ -609,7 +612,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           issue((uint32_t)GT_ACC1_COL, a[0]);
         }
         tie(a[1]);
-        if (!slow) add32(a[1], 1, std::integral_constant<int, 0>{}, p.dbg0); else add32(a[1], 1, std::integral_constant<int, 1>{}, p.dbg0);
+        add32(a[1], 1, std::integral_constant<int, SLOW ? 1 : 0>{}, p.dbg0);
         // ---- residual sums of a K-step that owns a cell (a pass of its own: inside the base pass the compiler if-converts
         //      the cell test and EVERY element pays for it) ----
         if (has) {
@@ -634,6 +637,8 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
 #endif
       }
       }
+      };
+      if (slow) k_loops(std::true_type{}); else k_loops(std::false_type{});
       // the tile's sums are complete: times the channel constant, one rounding to the 16-bit output.  A thread owns 64
       // consecutive channels of one token: 128 contiguous bytes of Y, stored as eight 16-byte pieces
       {
