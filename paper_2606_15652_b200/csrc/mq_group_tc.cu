@@ -73,7 +73,12 @@ constexpr int GT_OFF_MISC = GT_OFF_BAR + GT_NUM_BARS * 8 + 8;     // [0] tmem ba
 // per-tile channel constants, double-buffered by tile parity: [2]{[{fin, rho, bscale, s_r}][128] floats, flag word}
 constexpr int GT_OFF_TC = (GT_OFF_MISC + 16 + 15) / 16 * 16;
 constexpr int GT_TC_BYTES = 4 * BN * 4 + 16;
-constexpr int GT_SMEM_BYTES = GT_OFF_TC + 2 * GT_TC_BYTES + 1024;  // + slack for the 1024-byte alignment
+// output staging, private to an epilogue warp: [32 tokens][64 B of 16-bit outputs + 16 B pad] (half of a thread's 64
+// channels at a time), so that global memory sees 64-byte row pieces from neighbouring lanes instead of 32 separate rows
+constexpr int GT_YS_ROW = 80;
+constexpr int GT_YS_WARP = 32 * GT_YS_ROW;
+constexpr int GT_OFF_YS = (GT_OFF_TC + 2 * GT_TC_BYTES + 15) / 16 * 16;
+constexpr int GT_SMEM_BYTES = GT_OFF_YS + GT_EWARPS * GT_YS_WARP + 1024;  // + slack for the 1024-byte alignment
 static_assert(GT_SMEM_BYTES <= 232448, "shared memory budget");
 static_assert(GT_A_COL0 + GT_UST * GT_A_COLS == 512, "tensor memory budget");
 static_assert(GT_OFF_P % 1024 == 0 && GT_P_STAGE % 1024 == 0 && GT_U_STAGE % 1024 == 0, "swizzle atoms need 1024-byte alignment");
@@ -516,6 +521,16 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       tc_fence_after();
       issue((k & 1) * (uint32_t)BN, a[0]);
     };
+    // the channel scales of a tile are requested one tile ahead (threads 0..127 of the epilogue group: one channel each)
+    float sw_nx = 0.f, sr_nx = 0.f;
+    auto request_scales = [&](int Tn) {
+      if (et < BN && Tn < p.tiles) {
+        const int nn = (Tn / p.TT) * BN + et;
+        asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(sw_nx) : "l"(p.sw + nn));
+        asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(sr_nx) : "l"(p.sr + nn));
+      }
+    };
+    request_scales(tile0);
     for (int T = tile0; T < p.tiles; T += tstride, ++tile_no) {
       const int n0 = (T / p.TT) * BN;
       // Per-tile channel constants in shared memory (double-buffered by tile parity, one barrier per tile).  The running
@@ -523,8 +538,9 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       // at the end: two instructions per base sum (I2F, FFMA).  A tile that holds a channel with s_w = 0 (or a ratio that
       // is not finite) keeps its sums in units of 1 and pays a third instruction (bscale = s_w, rho = s_r, fin = 1/256).
       const uint32_t tc = sTC + (tile_no & 1u) * (uint32_t)GT_TC_BYTES;
+      const float sw_raw = sw_nx, sr_raw = sr_nx;
+      request_scales(T + tstride);
       if (et < BN) {
-        const float sw_raw = __ldg(p.sw + n0 + et), sr_raw = __ldg(p.sr + n0 + et);
         const float ratio = __fdiv_rn(sr_raw, sw_raw);
         const bool odd = sw_raw == 0.f || !(fabsf(ratio) <= 3.0e38f);
         asm volatile("st.shared.f32 [%0], %1;" ::"r"(tc + 4u * (uint32_t)et), "f"(sw_raw * 0.00390625f) : "memory");          // fin (regular tile)
@@ -640,44 +656,74 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       };
       if (slow) k_loops(std::true_type{}); else k_loops(std::false_type{});
       // the tile's sums are complete: times the channel constant, one rounding to the 16-bit output.  A thread owns 64
-      // consecutive channels of one token: 128 contiguous bytes of Y, stored as eight 16-byte pieces
+      // consecutive channels of one token (128 contiguous bytes of Y).  32 channels at a time go through the warp's
+      // staging rows, so that a store instruction writes 64-byte pieces of 8 rows (4 neighbouring lanes per row) instead
+      // of 16 bytes of 32 rows; rows that are not 16-byte aligned take the direct 2-byte path
       {
 #ifdef GT_TRACE
         const long long gt_t0 = clock64();
 #endif
-        const int t = (T % p.TT) * GT_BT + trow;
-        uint8_t* yrow = reinterpret_cast<uint8_t*>(p.Y) + ((size_t)t * p.ldy + n0 + half * 64) * 2;
+        const int t_w0 = (T % p.TT) * GT_BT + (warp & 3) * 32;   // first token of this warp
         const bool vec = ((p.ldy & 7) == 0) && ((reinterpret_cast<uintptr_t>(p.Y) & 15) == 0);   // rows 16-byte aligned
+        const uint32_t ys = smem_base + (uint32_t)GT_OFF_YS + (uint32_t)((warp - GT_WARP_E0) * GT_YS_WARP);
+        auto tile_out = [&](auto bf_c) {
+          constexpr bool BF = decltype(bf_c)::value;
 #pragma unroll
-        for (int i8 = 0; i8 < 8; ++i8) {
-          uint32_t w4[4];
+          for (int h = 0; h < 2; ++h) {   // channels 32 h .. 32 h + 31 of this thread's 64
 #pragma unroll
-          for (int h4 = 0; h4 < 2; ++h4) {
-            const uint4 c4 = gt_lds128(tc_half + (uint32_t)((i8 * 8 + h4 * 4) * 4));   // fin of four channels
-            const float fin[4] = {__uint_as_float(c4.x), __uint_as_float(c4.y), __uint_as_float(c4.z), __uint_as_float(c4.w)};
+            for (int k = 0; k < 4; ++k) {
+              uint32_t w4[4];
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
-              const int i = i8 * 8 + h4 * 4 + 2 * e;
-              const float v0 = y[i] * (slow ? 0.00390625f : fin[2 * e]), v1 = y[i + 1] * (slow ? 0.00390625f : fin[2 * e + 1]);
-              const uint32_t lo = p.y_bf16 ? (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v0)) : (uint32_t)__half_as_ushort(__float2half_rn(v0));
-              const uint32_t hi = p.y_bf16 ? (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(v1)) : (uint32_t)__half_as_ushort(__float2half_rn(v1));
-              w4[h4 * 2 + e] = lo | (hi << 16);
-              y[i] = 0.f;
-              y[i + 1] = 0.f;
-            }
-          }
-          if (t < p.M) {
-            if (vec) {
-              *reinterpret_cast<uint4*>(yrow + i8 * 16) = make_uint4(w4[0], w4[1], w4[2], w4[3]);
-            } else {
+              for (int h4 = 0; h4 < 2; ++h4) {
+                const int i0 = 32 * h + 8 * k + 4 * h4;
+                float fin[4] = {0.00390625f, 0.00390625f, 0.00390625f, 0.00390625f};
+                if (!slow) {
+                  const uint4 c4 = gt_lds128(tc_half + (uint32_t)(i0 * 4));   // fin of four channels
+                  fin[0] = __uint_as_float(c4.x);
+                  fin[1] = __uint_as_float(c4.y);
+                  fin[2] = __uint_as_float(c4.z);
+                  fin[3] = __uint_as_float(c4.w);
+                }
 #pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                reinterpret_cast<uint16_t*>(yrow + i8 * 16)[2 * k] = (uint16_t)(w4[k] & 0xFFFF);
-                reinterpret_cast<uint16_t*>(yrow + i8 * 16)[2 * k + 1] = (uint16_t)(w4[k] >> 16);
+                for (int e = 0; e < 2; ++e) {
+                  const int i = i0 + 2 * e;
+                  const float v0 = y[i] * fin[2 * e], v1 = y[i + 1] * fin[2 * e + 1];
+                  if (BF) {   // one rounding each (round to nearest even), packed {v0 low, v1 high}
+                    const __nv_bfloat162 pk = __floats2bfloat162_rn(v0, v1);
+                    w4[h4 * 2 + e] = *reinterpret_cast<const uint32_t*>(&pk);
+                  } else {
+                    const __half2 pk = __floats2half2_rn(v0, v1);
+                    w4[h4 * 2 + e] = *reinterpret_cast<const uint32_t*>(&pk);
+                  }
+                  y[i] = 0.f;
+                  y[i + 1] = 0.f;
+                }
+              }
+              if (vec) {
+                gt_sts128(ys + (uint32_t)(lane * GT_YS_ROW + k * 16), w4);
+              } else if (t_w0 + lane < p.M) {
+                uint16_t* dst = reinterpret_cast<uint16_t*>(p.Y) + (size_t)(t_w0 + lane) * p.ldy + n0 + half * 64 + 32 * h + 8 * k;
+#pragma unroll
+                for (int q2 = 0; q2 < 4; ++q2) {
+                  dst[2 * q2] = (uint16_t)(w4[q2] & 0xFFFF);
+                  dst[2 * q2 + 1] = (uint16_t)(w4[q2] >> 16);
+                }
               }
             }
+            if (vec) {
+              __syncwarp();
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const int r = (lane >> 2) + 8 * i, c = lane & 3;   // row r of the warp's 32 tokens, 16-byte piece c of its 64 bytes
+                const uint4 v = gt_lds128(ys + (uint32_t)(r * GT_YS_ROW + c * 16));
+                if (t_w0 + r < p.M)
+                  *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(p.Y) + ((size_t)(t_w0 + r) * p.ldy + n0 + half * 64 + 32 * h + 8 * c) * 2) = v;
+              }
+              __syncwarp();
+            }
           }
-        }
+        };
+        if (p.y_bf16) tile_out(std::true_type{}); else tile_out(std::false_type{});
 #ifdef GT_TRACE
         gt_tile += clock64() - gt_t0;
 #endif
