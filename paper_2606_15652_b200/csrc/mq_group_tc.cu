@@ -12,15 +12,15 @@
 // K-step), and the channel scales, which do not change, are applied once per tile.  (The first version had channels
 // in the lanes: every thread then needed the 64 group scales of its tokens from shared memory in every K-step, 64 KB
 // per K-step through the shared-memory pipe, plus a block-wide barrier per K-step to publish them.)
-//   * the base accumulator is double-buffered PER K-STEP: the MMAs of K-step k+1 run into the other 128 columns while
-//     the epilogue warps read the sums of K-step k (tcgen05.ld), convert them and add them to fp32 running sums held in
-//     registers; the residual accumulator is single-buffered and handed over per CELL (cells are rare);
+//   * three accumulator buffers of 128 columns are taken in rotation by base items (a K-step) and residual items (a
+//     cell) alike, in the MMA warp's order: the MMAs of the next two items run while the epilogue warps read the sums of
+//     the current one (tcgen05.ld), convert them and add them to fp32 running sums held in registers;
 //   * the running sums are kept in units of s_w: y = sum_g s_a acc0_g + (s_a rho) acc1_g, rho = s_r / s_w, and
 //     Y = (s_w / 256) y at the end of the tile (the operands are x16): two instructions per base sum (I2F, FFMA).  A tile
 //     with a channel whose s_w is 0 (or whose ratio is not finite) keeps units of 1 instead (a third instruction);
 //   * eight epilogue warps (two per TMEM lane quadrant, 64 channels each) keep 64 fp32 sums per thread for the whole
 //     tile and store them as 128 contiguous bytes of the token's Y row.
-// Tensor memory (512 columns): acc0 2 x 128 | acc1 128 | A operand ring 4 x 32.  Roles (16 warps = 512 threads in four
+// Tensor memory (512 columns): accumulators 3 x 128 | A operand ring 4 x 32.  Roles (16 warps = 512 threads in four
 // warp groups; the block starts with 128 registers per thread and setmaxnreg moves 32 per thread from the other groups
 // to the epilogue: 160 there (64 sums + two batches of 32 columns in flight), 96 elsewhere; one CTA per SM):
 //   warp 0 producer (TMA) | warp 1 MMA issuer | warps 2-3 weight unpack (rows 0..63 -> shared memory) |
@@ -57,7 +57,7 @@ constexpr int GT_REGS_EPI = 160, GT_REGS_REST = 96;   // registers per thread af
 static_assert(GT_WARP_E0 == 4 && GT_WARP_T0 == 12 && GT_WARPS == 16, "roles fill whole warp groups");
 constexpr int GT_THREADS = 32 * GT_WARPS;         // 512: the largest block that still gets 128 registers per thread
 constexpr int GT_A_COLS = BK / 4;                 // 32 TMEM columns hold 128 int8 per lane (one K-step)
-constexpr int GT_ACC1_COL = 2 * GT_BT;
+constexpr int GT_NACC = 3;                        // accumulator buffers of 128 columns, taken in rotation by base and residual items alike
 constexpr int GT_A_COL0 = 3 * GT_BT;
 constexpr int GT_PST = 8;                         // packed (P) stages of one K-step
 constexpr int GT_U_STAGE = BN * BK;               // int8 weight sub-tile of one K-step (16 KB), the B operand
@@ -68,7 +68,7 @@ constexpr int GT_OFF_P = GT_OFF_U + GT_UST * GT_U_STAGE;
 constexpr int GT_OFF_BAR = GT_OFF_P + GT_PST * GT_P_STAGE;
 // barriers: FULL_P[8] EMPTY_P[8] FULL_U[4] EMPTY_U[4] GFULL[2] GEMPTY[2] A1E
 constexpr int GT_B_FULL_P = 0, GT_B_EMPTY_P = GT_PST, GT_B_FULL_U = 2 * GT_PST, GT_B_EMPTY_U = GT_B_FULL_U + GT_UST,
-              GT_B_GFULL = GT_B_EMPTY_U + GT_UST, GT_B_GEMPTY = GT_B_GFULL + 2, GT_B_A1E = GT_B_GEMPTY + 2, GT_NUM_BARS = GT_B_A1E + 1;
+              GT_B_GFULL = GT_B_EMPTY_U + GT_UST, GT_B_GEMPTY = GT_B_GFULL + GT_NACC, GT_NUM_BARS = GT_B_GEMPTY + GT_NACC;
 constexpr int GT_OFF_MISC = GT_OFF_BAR + GT_NUM_BARS * 8 + 8;     // [0] tmem base
 // per-tile channel constants, double-buffered by tile parity: [2]{[{fin, rho, bscale, s_r}][128] floats, flag word}
 constexpr int GT_OFF_TC = (GT_OFF_MISC + 16 + 15) / 16 * 16;
@@ -169,11 +169,10 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       mbar_init(bar(GT_B_FULL_U + i), GT_WWARPS + GT_TWARPS);
       mbar_init(bar(GT_B_EMPTY_U + i), 1);
     }
-    for (int i = 0; i < 2; ++i) {
-      mbar_init(bar(GT_B_GFULL + i), 1);             // tcgen05.commit after the K-step's MMAs
+    for (int i = 0; i < GT_NACC; ++i) {
+      mbar_init(bar(GT_B_GFULL + i), 1);             // tcgen05.commit after the item's MMAs
       mbar_init(bar(GT_B_GEMPTY + i), GT_EWARPS);    // every epilogue warp has read its part of the buffer
     }
-    mbar_init(bar(GT_B_A1E), GT_EWARPS);
     fence_mbar_init();
     for (int i = 0; i < 2; ++i) asm volatile("st.shared.u32 [%0], %1;" ::"r"(sTC + (uint32_t)(i * GT_TC_BYTES + 4 * BN * 4)), "r"(0u) : "memory");
   }
@@ -363,7 +362,14 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     } else if (warp == 1) {
       // ===================== MMA issuer: warp-uniform control, one elected lane issues =====================
       constexpr uint32_t IDESC = make_idesc_i8(GT_BT, BN);   // M = 128 tokens (A, tensor memory), N = 128 channels (B, shared memory)
-      uint32_t item = 0, kq = 0, cq = 0;   // operand-ring items, K-steps and cells so far
+      uint32_t item = 0, kq = 0;   // operand-ring items and K-steps so far
+    uint32_t ab = 0, aph = 0;    // accumulator buffer of the next item (item % 3) and the parity of its use count
+    auto next_acc = [&]() {
+      if (++ab == GT_NACC) {
+        ab = 0;
+        aph ^= 1;
+      }
+    };
       bool pre_ok = false;                 // the barrier of the item about to be processed was already seen complete
       // the operand stage of item i: FULL_U[i & 3], phase (i >> 2) & 1; the next item's barrier is polled once BEFORE this
       // item's MMAs are issued, so that the round trip hides under the tensor pipe's work
@@ -387,36 +393,35 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
           const int nk = min(32, KS - c0);
           for (int j = 0; j < nk; ++j, ++kq) {
             const bool has = (bits >> j) & 1;
-            const int us = (int)(item & 3), buf = (int)(kq & 1);
+            const int us = (int)(item & 3);
             acquire();
             {
               GT_T0();
-              mbar_wait(bar(GT_B_GEMPTY + buf), ((kq >> 1) & 1) ^ 1);   // the epilogue has read the sums of K-step kq - 2
+              mbar_wait(bar(GT_B_GEMPTY + (int)ab), aph ^ 1);   // the epilogue has read the sums this buffer held three items ago
               GT_ACC(1);
             }
             tc_fence_after();
-            const uint32_t d0 = tmem_base + (uint32_t)(buf * GT_BT);
+            const uint32_t d0 = tmem_base + ab * (uint32_t)BN;
             const uint32_t at = tmem_base + (uint32_t)(GT_A_COL0 + us * GT_A_COLS);
             const uint64_t dt = make_desc_sw128(sU + us * GT_U_STAGE);
             if (elect_one()) {
   #pragma unroll
               for (int k = 0; k < 4; ++k) mma_i8_ts(d0, at + (uint32_t)(k * 8), dt + (uint64_t)(k * 2), IDESC, k == 0 ? 0u : 1u);   // a fresh sum per group
-              if (!has) {
-                tc_commit(bar(GT_B_EMPTY_U + us));
-                tc_commit(bar(GT_B_GFULL + buf));
-              }
+              if (!has) tc_commit(bar(GT_B_EMPTY_U + us));
+              tc_commit(bar(GT_B_GFULL + (int)ab));
             }
             __syncwarp();
             ++item;
+            next_acc();
             if (has) {
               // residual cell of this K-step: its weights in the next stage's B buffer, the tokens of this K-step's
               // stage (the paper's re-use of the activation tile), second accumulator, also a fresh sum
               const uint32_t mask = (uint32_t)__shfl_sync(0xffffffffu, um.x, j) & 0xF;
               const int us2 = (int)(item & 3);
               acquire();
-              mbar_wait_parked(bar(GT_B_A1E), (cq & 1) ^ 1);   // the epilogue has read the previous cell's sums
+              mbar_wait(bar(GT_B_GEMPTY + (int)ab), aph ^ 1);
               tc_fence_after();
-              const uint32_t d1 = tmem_base + (uint32_t)GT_ACC1_COL;
+              const uint32_t d1 = tmem_base + ab * (uint32_t)BN;
               const uint64_t dt2 = make_desc_sw128(sU + us2 * GT_U_STAGE);
               if (elect_one()) {
                 uint32_t on = 0;
@@ -431,11 +436,11 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
                   }
                 tc_commit(bar(GT_B_EMPTY_U + us2));
                 tc_commit(bar(GT_B_EMPTY_U + us));
-                tc_commit(bar(GT_B_GFULL + buf));   // both accumulators of the K-step are complete
+                tc_commit(bar(GT_B_GFULL + (int)ab));
               }
               __syncwarp();
               ++item;
-              ++cq;
+              next_acc();
             }
           }
         }
@@ -461,9 +466,9 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
     // otherwise it re-derives them from %tid and the shared-memory window at every use (special-register reads, shifts,
     // uniform-register moves: a third of the loop's time went there) instead of keeping six registers.
     uint32_t acc0_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(half * 64);
-    uint32_t b_gfull = bar(GT_B_GFULL), b_gempty = bar(GT_B_GEMPTY), b_a1e = bar(GT_B_A1E);
+    uint32_t b_gfull = bar(GT_B_GFULL), b_gempty = bar(GT_B_GEMPTY);
     uint32_t lane0 = lane == 0 ? 1u : 0u;
-    asm volatile("" : "+r"(acc0_addr), "+r"(b_gfull), "+r"(b_gempty), "+r"(b_a1e), "+r"(lane0));
+    asm volatile("" : "+r"(acc0_addr), "+r"(b_gfull), "+r"(b_gempty), "+r"(lane0));
     float y[64];
 #pragma unroll
     for (int i = 0; i < 64; ++i) y[i] = 0.f;
@@ -514,12 +519,15 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       gt_tie16(v);
       gt_tie16(v + 16);
     };
-    auto request_base = [&](uint32_t k) {   // first batch of K-step k's base sums -> a[0]
+    // accumulator buffer of the item being drained (base and residual items take the three buffers in rotation, in the
+    // MMA warp's order) and the parity of its use count
+    uint32_t eb = 0, eph = 0;
+    auto request_item = [&]() {   // first batch of the item in buffer eb -> a[0]
       GT_T0();
-      mbar_wait(b_gfull + 8u * (k & 1u), (k >> 1) & 1);
+      mbar_wait(b_gfull + 8u * eb, eph);
       GT_ACC(3);
       tc_fence_after();
-      issue((k & 1) * (uint32_t)BN, a[0]);
+      issue(eb * (uint32_t)BN, a[0]);
     };
     // the channel scales of a tile are requested one tile ahead (threads 0..127 of the epilogue group: one channel each)
     float sw_nx = 0.f, sr_nx = 0.f;
@@ -556,7 +564,7 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       asm volatile("ld.shared.u32 %0, [%1];" : "=r"(flag) : "r"(tc + 4u * (uint32_t)(4 * BN)));
       const bool slow = flag == tile_no + 1u;
       const uint32_t tc_half = tc + (uint32_t)(half * 64 * 4);
-      request_base(kq);   // (no load is left in flight across the tile's output stage)
+      request_item();   // (no load is left in flight across the tile's output stage)
       // (the K-step loops once per kind of tile, regular / irregular channel scales: no test per K-step)
       auto k_loops = [&](auto slow_c) {
       constexpr bool SLOW = decltype(slow_c)::value;
@@ -569,7 +577,6 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
       for (int j = 0; j < nk; ++j, ++kq) {
         const int ks = c0 + j;
         const bool has = (bits >> j) & 1;
-        const int buf = (int)(kq & 1);
         // s_a[this token, this K-step's group], requested one K-step ago; the next one is requested now, into the same
         // register (nothing may touch that register before the next K-step: a copy right behind the load would wait for it)
         const float sa = sa_nxt;
@@ -607,38 +614,35 @@ __global__ void __launch_bounds__(GT_THREADS, 1) mq_group_tc_kernel(const __grid
             }
           }
         };
-        auto hand_back = [&]() {   // this warp's part of the K-step's accumulators is in registers: back to the MMA warp
+        auto hand_back = [&]() {   // this warp's part of the item's sums is in registers: the buffer goes back to the MMA warp
           tc_fence_before();
           __syncwarp();
-          if (lane0) {
-            mbar_arrive(b_gempty + 8u * (uint32_t)buf);
-            if (has) mbar_arrive(b_a1e);
+          if (lane0) mbar_arrive(b_gempty + 8u * eb);
+          if (++eb == GT_NACC) {
+            eb = 0;
+            eph ^= 1;
           }
         };
         // ---- base sums (a[0] was requested during the previous pass) ----
         landed(a[0]);
-        issue((uint32_t)(buf * BN) + 32u, a[1]);
+        issue(eb * (uint32_t)BN + 32u, a[1]);
         tie(a[0]);
         add32(a[0], 0, std::integral_constant<int, SLOW ? 1 : 0>{}, p.dbg0);
         landed(a[1]);
-        if (!has) {
-          hand_back();
-          if (ks + 1 < KS) request_base(kq + 1);
-        } else {
-          issue((uint32_t)GT_ACC1_COL, a[0]);
-        }
+        hand_back();
+        if (has || ks + 1 < KS) request_item();   // the K-step's residual item, or the next K-step's base item
         tie(a[1]);
         add32(a[1], 1, std::integral_constant<int, SLOW ? 1 : 0>{}, p.dbg0);
         // ---- residual sums of a K-step that owns a cell (a pass of its own: inside the base pass the compiler if-converts
         //      the cell test and EVERY element pays for it) ----
         if (has) {
           landed(a[0]);
-          issue((uint32_t)GT_ACC1_COL + 32u, a[1]);
+          issue(eb * (uint32_t)BN + 32u, a[1]);
           tie(a[0]);
           add32(a[0], 0, std::integral_constant<int, 2>{}, p.dbg1);
           landed(a[1]);
           hand_back();
-          if (ks + 1 < KS) request_base(kq + 1);
+          if (ks + 1 < KS) request_item();
           tie(a[1]);
           add32(a[1], 1, std::integral_constant<int, 2>{}, p.dbg1);
         } else if (DBG && p.dbg1) {
